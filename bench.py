@@ -1,0 +1,362 @@
+#!/usr/bin/env python
+"""bench.py — headline benchmark of the hq hot path on B200.
+
+Metric (BASELINE.json): batch-1 decode tokens/s of the 1B bf16 model (as a fraction of the HBM
+roofline), with envelope-prefill TTFT next to it.  Workload = BASELINE.json configs[1]: 256-token
+random prompt, then 128 greedy decode steps.  One bench "step" = one whole query (kv_reset, prefill,
+128 decode steps).  See DESIGN.md "Measurement" for the byte model behind the roofline object.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl hq|reference]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 \
+        --master-port P bench.py --gpus N --steps K --warmup W
+
+N > 1 runs N independent replicas (no collective on the data path).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+PROMPT_LEN, DECODE_STEPS = 256, 128
+METRIC, UNIT = "decode_tokens_per_s_batch1_1b_bf16", "tokens/s"
+WORKLOAD = "configs[1]: 1B Llama-style bf16, batch 1, 256-token random prompt, 128 greedy decode steps"
+FALLBACK_HBM_GBS = 6650.0  # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
+
+
+def weight_bytes(s) -> int:
+    return 2 * s.n_params
+
+
+def bytes_per_token(s, ctx: int, batch: int = 1) -> int:
+    """Algorithmic HBM bytes of one decode step: weights once + embedding row +
+    KV read of ctx cached tokens and write of one; 2*Hkv*hd*2 B*L per cached token."""
+    kv_tok = 2 * s.n_kv_heads * s.head_dim * 2 * s.n_layers
+    return weight_bytes(s) + batch * 2 * s.hidden + batch * (ctx + 1) * kv_tok
+
+
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy)"
+        except Exception:
+            pass
+    return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def ncu_traffic():
+    """dram bytes per launch of the dominant kernel from the committed ncu --set full summary."""
+    p = os.path.join(ROOT, "profiles", "roofline_traffic.json")
+    if os.path.exists(p):
+        try:
+            return json.load(open(p)).get("gateup_gemv_dram_bytes_per_launch")
+        except Exception:
+            return None
+    return None
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons during the timed region (NVML; nvidia-smi fields)."""
+
+    def __init__(self, index: int):
+        super().__init__(daemon=True)
+        self.index, self.samples, self.reasons, self.max_mhz = index, [], set(), None
+        self._stop_evt = threading.Event()
+        self.ok = False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+            self.ok = True
+        except Exception:
+            self.ok = False
+
+    def run(self):
+        if not self.ok:
+            return
+        nv = self.nv
+        names = {
+            getattr(nv, "nvmlClocksThrottleReasonHwSlowdown", 0x8): "hw_slowdown",
+            getattr(nv, "nvmlClocksThrottleReasonHwThermalSlowdown", 0x40): "hw_thermal_slowdown",
+            getattr(nv, "nvmlClocksThrottleReasonSwThermalSlowdown", 0x20): "sw_thermal_slowdown",
+            getattr(nv, "nvmlClocksThrottleReasonSwPowerCap", 0x4): "sw_power_cap",
+        }
+        while not self._stop_evt.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, name in names.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(0.05)
+
+    def stop(self):
+        self._stop_evt.set()
+        self.join(timeout=2)
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons)}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+def oracle_sample(weights, s, prompt_len=16, steps=24):
+    """cpu_baseline: the oracle as it stands on the host cores, on a bounded sample of the workload."""
+    import datagen
+    import oracle
+    om = oracle.Model.from_datagen(weights, max_seq=prompt_len + steps + 1)
+    prompt = datagen.tokens(1001, s.vocab, prompt_len)
+    t0 = time.perf_counter()
+    _, lg = om.forward(prompt, logits="last")
+    t1 = time.perf_counter()
+    tok = oracle.argmax(lg)
+    for _ in range(steps):
+        _, lg = om.forward([tok], logits="last")
+        tok = oracle.argmax(lg)
+    t2 = time.perf_counter()
+    return {"value": steps / (t2 - t1), "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+            "sample": f"same 1B weights; {prompt_len}-token prompt (prefill {t1 - t0:.2f} s, "
+                      f"{prompt_len / (t1 - t0):.1f} tok/s) then {steps} greedy decode steps "
+                      f"({(t2 - t1) / steps * 1e3:.0f} ms/token)"}
+
+
+def run_reference(args):
+    """--impl reference: the oracle, as it stands, on the host cores (rank 0 only)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import datagen
+    import oracle
+    s = datagen.ONE_B
+    w = datagen.make_weights(s)
+    prompt_len, steps = 8, 8  # bounded sample of the workload per bench step
+    om = oracle.Model.from_datagen(w, max_seq=prompt_len + steps + 1)
+    prompt = datagen.tokens(1001, s.vocab, prompt_len)
+
+    def one():
+        om.reset()
+        t0 = time.perf_counter()
+        _, lg = om.forward(prompt, logits="last")
+        t1 = time.perf_counter()
+        tok = oracle.argmax(lg)
+        for _ in range(steps):
+            _, lg = om.forward([tok], logits="last")
+            tok = oracle.argmax(lg)
+        return t1 - t0, time.perf_counter() - t1
+
+    for _ in range(args.warmup):
+        one()
+    tp = td = 0.0
+    for _ in range(args.steps):
+        a, b = one()
+        tp += a
+        td += b
+    value = args.steps * steps / td
+    sample = (f"per step: {prompt_len}-token prompt + {steps} greedy decode steps of the same 1B weights "
+              f"(bounded sample of configs[1])")
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": (tp + td) / args.steps * 1e3,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": {"workload": WORKLOAD, "sample": sample},
+            "ttft_ms": tp / args.steps * 1e3,
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+                             "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="hq", choices=["hq", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg")
+    ap.add_argument("--profile", type=int, default=0, metavar="N",
+                    help="ncu helper: one prefill + N decode steps of the bench workload, no timing")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import datagen
+    import paper_2606_12154_b200 as hq
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        torch.cuda.set_device(local_rank)
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))
+    dev = torch.device(f"cuda:{local_rank}")
+    torch.cuda.set_device(dev)
+
+    s = datagen.ONE_B
+    weights = datagen.make_weights(s)
+    max_seq = PROMPT_LEN + DECODE_STEPS + 32
+    gm = hq.Model.from_bf16_bits(s, weights.embedding, weights.final_norm, weights.layers, max_seq=max_seq,
+                                 device=str(dev))
+    prompt = datagen.tokens(1001, s.vocab, PROMPT_LEN)
+    stream = gm.stream       # the stream libhq launches on (CUDA events must be recorded there)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+
+    def query(events=None):
+        """One bench step on the device-resident path: async greedy decode, tokens stay on the GPU."""
+        gm.kv_reset()
+        if events:
+            events[0].record(stream)
+        gm.prefill(prompt, want_token=False)
+        if events:
+            events[1].record(stream)
+        gm.decode_run(DECODE_STEPS, want_tokens=False)
+        if events:
+            events[2].record(stream)
+
+    if args.profile:
+        gm.kv_reset()
+        gm.prefill(prompt, want_token=False)
+        gm.sync()
+        before = gm.kernel_count() + 86      # + launches made by hq_model_create
+        gm.decode_run(args.profile, want_tokens=False)
+        gm.sync()
+        print(json.dumps({"profile": True, "launches_before_decode": before,
+                          "decode_launches": gm.kernel_count() + 86 - before}), flush=True)
+        return
+
+    for _ in range(max(args.warmup, 3)):
+        query()
+    barrier()
+
+    # ---- timed region: K whole queries, device timed -------------------------------------------------
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    evs = [[ev(), ev(), ev()] for _ in range(args.steps)]
+    k0 = gm.kernel_count()
+    barrier()
+    t_start, t_end = ev(), ev()
+    t_start.record(stream)
+    for i in range(args.steps):
+        query(evs[i])
+    t_end.record(stream)
+    barrier()
+    clocks = sampler.stop()
+    launches = gm.kernel_count() - k0
+    total_ms = t_start.elapsed_time(t_end)
+    prefill_ms = [e[0].elapsed_time(e[1]) for e in evs]
+    decode_ms = [e[1].elapsed_time(e[2]) for e in evs]
+
+    # ---- e2e: same metric through the C ABI with HOST buffers, streaming one token per call ------------
+    first = np.empty(1, dtype=np.int32)
+    out = np.empty(1, dtype=np.int32)
+    e2e_decode_s, e2e_ttft_s = [], []
+    for _ in range(max(1, min(args.steps, 3))):
+        gm.kv_reset()
+        gm.sync()
+        t0 = time.perf_counter()
+        gm.prefill(prompt, want_token=True)                   # H2D prompt, D2H first token, sync
+        t1 = time.perf_counter()
+        for _ in range(DECODE_STEPS):
+            gm.decode_step(want_token=True, out=out)          # D2H 4 bytes + sync every token
+        t2 = time.perf_counter()
+        e2e_ttft_s.append(t1 - t0)
+        e2e_decode_s.append(t2 - t1)
+    del first
+
+    # ---- dominant kernel, timed alone over layers cycling (weights streamed > L2) ----------------------
+    reps = 16 * 8
+    gm.bench_kernel(0, 32)
+    torch.cuda.synchronize(dev)
+    a, b = ev(), ev()
+    a.record(stream)
+    gu_bytes = gm.bench_kernel(0, reps)
+    b.record(stream)
+    torch.cuda.synchronize(dev)
+    gu_ms = a.elapsed_time(b) / reps
+    kernels = {}
+    for which, name in ((1, "lm_head"), (2, "qkv"), (3, "o_proj"), (4, "down"), (5, "attn_decode")):
+        r = 16 if which == 1 else reps
+        gm.bench_kernel(which, 8)
+        a, b = ev(), ev()
+        a.record(stream)
+        nbytes = gm.bench_kernel(which, r)
+        b.record(stream)
+        torch.cuda.synchronize(dev)
+        ms = a.elapsed_time(b) / r
+        kernels[name] = {"us": ms * 1e3, "GBps": nbytes / ms / 1e6}
+    kernels["gate_up"] = {"us": gu_ms * 1e3, "GBps": gu_bytes / gu_ms / 1e6}
+
+    # ---- aggregate over ranks (max time) -----------------------------------------------------------------
+    dec_total_ms = float(sum(decode_ms))
+    if dist is not None:
+        t = torch.tensor([dec_total_ms, total_ms, float(np.mean(prefill_ms))], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dec_total_ms, total_ms, ttft = [float(v) for v in t.tolist()]
+        ln = torch.tensor([launches], device=dev, dtype=torch.int64)
+        dist.all_reduce(ln)
+        launches = int(ln.item())
+    else:
+        ttft = float(np.mean(prefill_ms))
+
+    if rank == 0:
+        peak, peak_src = measured_peak()
+        tokens_total = world * args.steps * DECODE_STEPS
+        value = tokens_total / (dec_total_ms * 1e-3)
+        ms_per_token = dec_total_ms / (args.steps * DECODE_STEPS)
+        ctx_mid = PROMPT_LEN + DECODE_STEPS // 2
+        bpt = bytes_per_token(s, ctx_mid)
+        step_gbs = bpt / (ms_per_token * 1e-3) / 1e9
+        achieved = gu_bytes / (gu_ms * 1e-3) / 1e9
+        e2e_value = world * DECODE_STEPS / float(np.mean(e2e_decode_s))
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "bf16 weights/KV, f32 accumulate", "data": "synthetic",
+            "config": {"workload": WORKLOAD, "l2": "inputs larger than L2 (2.47 GB of weights per token vs 126 MB)",
+                       "multi_gpu": "independent replicas, no collective"},
+            "ttft_ms": ttft, "ms_per_token": ms_per_token, "clocks": clocks, "gpu_launches": launches,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": PROMPT_LEN * 4,
+                    "d2h_bytes_per_step": (DECODE_STEPS + 1) * 4,
+                    "ttft_ms": float(np.mean(e2e_ttft_s)) * 1e3,
+                    "how": "hq_prefill(host tokens -> host first token) then 128 x hq_decode_step(host token out), "
+                           "host wall clock, one sync + 4-byte D2H per token"},
+            "roofline": {"bound": "hbm", "kernel": "gemv_kernel<gate/up + SwiGLU> (43% of bytes per token)",
+                         "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                         "traffic": ncu_traffic(), "peak_source": peak_src,
+                         "bytes_per_launch": gu_bytes, "us_per_launch": gu_ms * 1e3},
+            "step_roofline": {"bytes_per_token": bpt, "achieved_GBps": step_gbs, "frac_of_measured": step_gbs / peak,
+                              "frac_of_8TBps_spec": step_gbs / 8000.0},
+            "kernels_alone": kernels,
+        }
+        if not args.no_cpu_baseline:
+            line["cpu_baseline"] = oracle_sample(weights, s)
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

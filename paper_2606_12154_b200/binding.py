@@ -1,0 +1,251 @@
+"""ctypes binding of include/hq.h — argument marshalling only; every step runs in libhq's kernels.
+
+PyTorch is used for device memory (weights, workspace, outputs) and the CUDA stream, nothing else.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Dict, List, Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libhq.so")
+
+FLAG_CAPTURE_HIDDEN = 1
+FLAG_NO_GRAPH = 2
+FLAG_NO_PDL = 4
+
+HQ_OK, HQ_ERR_INVALID_ARG, HQ_ERR_CAPACITY, HQ_ERR_STATE, HQ_ERR_CUDA, HQ_ERR_UNSUPPORTED = 0, -1, -2, -3, -4, -5
+_CODE_NAMES = {-1: "HQ_ERR_INVALID_ARG", -2: "HQ_ERR_CAPACITY", -3: "HQ_ERR_STATE", -4: "HQ_ERR_CUDA",
+               -5: "HQ_ERR_UNSUPPORTED"}
+
+# every symbol include/hq.h declares (tests check the header and the library against this list)
+DECLARED_SYMBOLS = (
+    "hq_workspace_bytes", "hq_model_create", "hq_model_destroy", "hq_prefill", "hq_decode_step",
+    "hq_decode_run", "hq_decode_logits", "hq_get_hidden", "hq_sync", "hq_seq_len", "hq_kv_reset",
+    "hq_kernel_count", "hq_bench_kernel", "hq_last_error", "hq_version",
+)
+
+
+class HQError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"{_CODE_NAMES.get(code, code)}: {msg}")
+        self.code = code
+
+
+class Config(ctypes.Structure):
+    _fields_ = [("n_layers", ctypes.c_int32), ("hidden", ctypes.c_int32), ("n_heads", ctypes.c_int32),
+                ("n_kv_heads", ctypes.c_int32), ("head_dim", ctypes.c_int32), ("ffn", ctypes.c_int32),
+                ("vocab", ctypes.c_int32), ("rms_eps", ctypes.c_float), ("rope_theta", ctypes.c_float),
+                ("max_batch", ctypes.c_int32), ("max_seq", ctypes.c_int32), ("weight_dtype", ctypes.c_int32),
+                ("flags", ctypes.c_uint32)]
+
+
+_vpp = ctypes.POINTER(ctypes.c_void_p)
+
+
+class Weights(ctypes.Structure):
+    _fields_ = [("tok_embedding", ctypes.c_void_p), ("attn_norm", _vpp), ("wq", _vpp), ("wk", _vpp),
+                ("wv", _vpp), ("wo", _vpp), ("ffn_norm", _vpp), ("w_gate", _vpp), ("w_up", _vpp),
+                ("w_down", _vpp), ("final_norm", ctypes.c_void_p), ("lm_head", ctypes.c_void_p)]
+
+
+_lib = None
+
+
+def load_library(path: Optional[str] = None):
+    """Load libhq.so (in-tree).  Fails loudly when it has not been built: there is no fallback."""
+    global _lib
+    if _lib is not None and path is None:
+        return _lib
+    p = path or _LIB_PATH
+    if not os.path.exists(p):
+        raise ImportError(f"{p} is missing: build it with `python -m paper_2606_12154_b200.build` "
+                          "(or __graft_entry__.build()); hq has no CPU or PyTorch fallback")
+    l = ctypes.CDLL(p)
+    vp, i32, i64 = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64
+    l.hq_workspace_bytes.restype = ctypes.c_size_t
+    l.hq_workspace_bytes.argtypes = [ctypes.POINTER(Config)]
+    l.hq_model_create.restype = i32
+    l.hq_model_create.argtypes = [ctypes.POINTER(Config), ctypes.POINTER(Weights), vp, ctypes.c_size_t, vp,
+                                  ctypes.POINTER(vp)]
+    l.hq_model_destroy.restype = None
+    l.hq_model_destroy.argtypes = [vp]
+    l.hq_prefill.restype = i32
+    l.hq_prefill.argtypes = [vp, vp, i32, i32, vp, vp]
+    l.hq_decode_step.restype = i32
+    l.hq_decode_step.argtypes = [vp, vp, vp]
+    l.hq_decode_run.restype = i32
+    l.hq_decode_run.argtypes = [vp, i32, vp]
+    l.hq_decode_logits.restype = i32
+    l.hq_decode_logits.argtypes = [vp, vp]
+    l.hq_get_hidden.restype = i32
+    l.hq_get_hidden.argtypes = [vp, i32, vp]
+    l.hq_sync.restype = i32
+    l.hq_sync.argtypes = [vp]
+    l.hq_seq_len.restype = i32
+    l.hq_seq_len.argtypes = [vp, ctypes.POINTER(i32)]
+    l.hq_kv_reset.restype = i32
+    l.hq_kv_reset.argtypes = [vp]
+    l.hq_kernel_count.restype = i64
+    l.hq_kernel_count.argtypes = [vp]
+    l.hq_bench_kernel.restype = i32
+    l.hq_bench_kernel.argtypes = [vp, i32, i32, ctypes.POINTER(i64)]
+    l.hq_last_error.restype = ctypes.c_char_p
+    l.hq_last_error.argtypes = []
+    l.hq_version.restype = ctypes.c_char_p
+    l.hq_version.argtypes = []
+    if path is None:
+        _lib = l
+    return l
+
+
+def _check(rc: int):
+    if rc != HQ_OK:
+        raise HQError(rc, load_library().hq_last_error().decode())
+
+
+def version() -> str:
+    return load_library().hq_version().decode()
+
+
+def make_config(*, n_layers, hidden, n_heads, n_kv_heads, head_dim, ffn, vocab, rms_eps, rope_theta,
+                max_batch=1, max_seq=4352, flags=0) -> Config:
+    return Config(n_layers, hidden, n_heads, n_kv_heads, head_dim, ffn, vocab, rms_eps, rope_theta,
+                  max_batch, max_seq, 0, flags)
+
+
+def workspace_bytes(cfg: Config) -> int:
+    return int(load_library().hq_workspace_bytes(ctypes.byref(cfg)))
+
+
+LAYER_TENSORS = ("attn_norm", "wq", "wk", "wv", "wo", "ffn_norm", "w_gate", "w_up", "w_down")
+
+
+class Model:
+    """Owns the torch device tensors (weights, workspace) and the opaque hq_model handle.
+
+    Method names follow the C ABI: prefill, decode_step, decode_run, decode_logits, get_hidden,
+    sync, seq_len, kv_reset, kernel_count, bench_kernel.
+    """
+
+    def __init__(self, cfg: Config, embedding, final_norm, layers: Sequence[Dict[str, "object"]],
+                 lm_head=None, stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise HQError(HQ_ERR_CUDA, "no CUDA device: hq has no CPU fallback")
+        self._torch = torch
+        self._lib = load_library()
+        self.cfg = cfg
+        self.device = embedding.device
+        for t in [embedding, final_norm] + [l[k] for l in layers for k in LAYER_TENSORS]:
+            if t.dtype != torch.bfloat16 or not t.is_cuda or not t.is_contiguous():
+                raise HQError(HQ_ERR_INVALID_ARG, "weights must be contiguous CUDA bfloat16 tensors")
+        self._keep = [embedding, final_norm, layers, lm_head]
+        # a dedicated stream: CUDA graphs cannot be captured on the legacy default stream
+        self.stream = stream if stream is not None else torch.cuda.Stream(self.device)
+        torch.cuda.synchronize(self.device)     # weight uploads on the current stream are done
+        nbytes = workspace_bytes(cfg)
+        if nbytes == 0:
+            _check(HQ_ERR_INVALID_ARG)
+        self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        arrays = {}
+        for k in LAYER_TENSORS:
+            arr = (ctypes.c_void_p * cfg.n_layers)(*[layers[l][k].data_ptr() for l in range(cfg.n_layers)])
+            arrays[k] = arr
+        head = embedding if lm_head is None else lm_head
+        w = Weights(embedding.data_ptr(), *[ctypes.cast(arrays[k], _vpp) for k in LAYER_TENSORS],
+                    final_norm.data_ptr(), head.data_ptr())
+        h = ctypes.c_void_p()
+        _check(self._lib.hq_model_create(ctypes.byref(cfg), ctypes.byref(w), self.workspace.data_ptr(),
+                                         nbytes, self.stream.cuda_stream, ctypes.byref(h)))
+        self._h = h
+        self.vocab, self.hidden, self.n_layers = cfg.vocab, cfg.hidden, cfg.n_layers
+
+    # -- construction helper: bf16 bit patterns (numpy uint16) -> device tensors ---------------------
+    @classmethod
+    def from_bf16_bits(cls, shape, embedding_bits: np.ndarray, final_norm_bits: np.ndarray,
+                       layer_bits: List[Dict[str, np.ndarray]], *, max_batch=1, max_seq=4352, flags=0,
+                       device="cuda:0", stream=None) -> "Model":
+        import torch
+
+        def up(a: np.ndarray):
+            t = torch.from_numpy(np.ascontiguousarray(a).view(np.int16)).to(device)
+            return t.view(torch.bfloat16)
+
+        cfg = make_config(n_layers=shape.n_layers, hidden=shape.hidden, n_heads=shape.n_heads,
+                          n_kv_heads=shape.n_kv_heads, head_dim=shape.head_dim, ffn=shape.ffn,
+                          vocab=shape.vocab, rms_eps=shape.rms_eps, rope_theta=shape.rope_theta,
+                          max_batch=max_batch, max_seq=max_seq, flags=flags)
+        layers = [{k: up(l[k]) for k in LAYER_TENSORS} for l in layer_bits]
+        return cls(cfg, up(embedding_bits), up(final_norm_bits), layers, stream=stream)
+
+    def close(self):
+        h, self._h = getattr(self, "_h", None), None
+        if h:
+            self._lib.hq_model_destroy(h)
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- the C ABI, one method per call -------------------------------------------------------------
+    def prefill(self, tokens, logits=None, want_token: bool = True):
+        """tokens: int array [batch, n_tokens] (or [n_tokens]) on the HOST.  Returns first tokens or None."""
+        toks = np.ascontiguousarray(tokens, dtype=np.int32)
+        if toks.ndim == 1:
+            toks = toks[None, :]
+        batch, n = toks.shape
+        out = np.empty(batch, dtype=np.int32) if want_token else None
+        _check(self._lib.hq_prefill(self._h, toks.ctypes.data, batch, n,
+                                    logits.data_ptr() if logits is not None else None,
+                                    out.ctypes.data if want_token else None))
+        return out
+
+    def decode_step(self, tokens_in=None, want_token: bool = True, out: Optional[np.ndarray] = None):
+        tin = None if tokens_in is None else np.ascontiguousarray(tokens_in, dtype=np.int32).reshape(-1)
+        if want_token and out is None:
+            out = np.empty(max(1, self.cfg.max_batch), dtype=np.int32)
+        _check(self._lib.hq_decode_step(self._h, tin.ctypes.data if tin is not None else None,
+                                        out.ctypes.data if want_token else None))
+        return out if want_token else None
+
+    def decode_run(self, n_steps: int, want_tokens: bool = True, batch: int = 1):
+        out = np.empty((n_steps, batch), dtype=np.int32) if want_tokens else None
+        _check(self._lib.hq_decode_run(self._h, n_steps, out.ctypes.data if want_tokens else None))
+        return out
+
+    def decode_logits(self, batch: int = 1):
+        t = self._torch.empty((batch, self.vocab), dtype=self._torch.float32, device=self.device)
+        _check(self._lib.hq_decode_logits(self._h, t.data_ptr()))
+        self.sync()      # diagnostics: the copy ran on self.stream, the caller reads on another
+        return t
+
+    def get_hidden(self, layer: int, batch: int = 1):
+        t = self._torch.empty((batch, self.hidden), dtype=self._torch.float32, device=self.device)
+        _check(self._lib.hq_get_hidden(self._h, layer, t.data_ptr()))
+        self.sync()
+        return t
+
+    def sync(self):
+        _check(self._lib.hq_sync(self._h))
+
+    def seq_len(self) -> int:
+        v = ctypes.c_int32()
+        _check(self._lib.hq_seq_len(self._h, ctypes.byref(v)))
+        return v.value
+
+    def kv_reset(self):
+        _check(self._lib.hq_kv_reset(self._h))
+
+    def kernel_count(self) -> int:
+        return int(self._lib.hq_kernel_count(self._h))
+
+    def bench_kernel(self, which: int, reps: int) -> int:
+        b = ctypes.c_int64()
+        _check(self._lib.hq_bench_kernel(self._h, which, reps, ctypes.byref(b)))
+        return b.value

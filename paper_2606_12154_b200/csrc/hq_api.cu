@@ -1,0 +1,486 @@
+// hq_api.cu — the C ABI of include/hq.h: argument checking, workspace carve-up, step scheduling,
+// CUDA-graph capture.  Every step of the path runs in the kernels of hq_decode.cu / hq_prefill.cu;
+// there is no CPU fallback anywhere in this file.
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <new>
+
+#include "hq_internal.h"
+
+using namespace hq;
+
+struct hq_model : public hq_model_impl {};
+
+static thread_local char g_err[512] = "";
+
+static int32_t fail(int32_t code, const char *fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define HQ_CUDA(call)                                                                                  \
+    do {                                                                                               \
+        cudaError_t e__ = (call);                                                                      \
+        if (e__ != cudaSuccess)                                                                        \
+            return fail(HQ_ERR_CUDA, "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e__), __FILE__, \
+                        __LINE__);                                                                     \
+    } while (0)
+
+extern "C" const char *hq_last_error(void) { return g_err; }
+extern "C" const char *hq_version(void) { return "hq 0.1 sm_100a"; }
+
+// ---- workspace layout ---------------------------------------------------------------------------------
+static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+static bool config_ok(const hq_config *c, const char **why) {
+#define BAD(msg) do { *why = msg; return false; } while (0)
+    if (!c) BAD("cfg is NULL");
+    if (c->n_layers <= 0 || c->hidden <= 0 || c->n_heads <= 0 || c->n_kv_heads <= 0 || c->ffn <= 0 ||
+        c->vocab <= 0 || c->max_batch <= 0 || c->max_seq <= 0)
+        BAD("non-positive dimension");
+    if (c->weight_dtype != HQ_BF16) BAD("weight_dtype must be HQ_BF16");
+    return true;
+#undef BAD
+}
+
+static bool config_supported(const hq_config *c, const char **why) {
+#define BAD(msg) do { *why = msg; return false; } while (0)
+    if (c->head_dim != kHeadDim) BAD("head_dim must be 64");
+    if (c->n_heads % c->n_kv_heads != 0) BAD("n_heads must be a multiple of n_kv_heads");
+    if (c->n_heads / c->n_kv_heads > 8) BAD("GQA group size must be <= 8");
+    if (!gemv_shape_supported(c->hidden) || !gemv_shape_supported(c->ffn) ||
+        !gemv_shape_supported(c->n_heads * c->head_dim))
+        BAD("hidden, ffn and n_heads*head_dim must be multiples of 8 and <= 8192");
+    if (c->vocab % 2 != 0 || c->hidden % 2 != 0) BAD("vocab and hidden must be even");
+    if (c->max_batch > 32) BAD("max_batch must be <= 32");
+    return true;
+#undef BAD
+}
+
+// Walks the layout; when base != NULL also assigns the pointers.
+static size_t carve(const hq_config *c, char *base, Buffers *b) {
+    size_t off = 0;
+    auto take = [&](size_t bytes) -> char * {
+        char *p = base ? base + off : nullptr;
+        off = align_up(off + bytes, 256);
+        return p;
+    };
+    const size_t B = c->max_batch, L = c->n_layers, T = c->max_seq, d = c->hidden;
+    const size_t H = c->n_heads, Hkv = c->n_kv_heads, F = c->ffn, V = c->vocab;
+    const size_t kv_elems = L * B * Hkv * T * kHeadDim;
+    Buffers tmp;
+    Buffers &o = b ? *b : tmp;
+    o.kcache = (kv_t *)take(kv_elems * sizeof(kv_t));
+    o.vcache = (kv_t *)take(kv_elems * sizeof(kv_t));
+    o.rope = (float2 *)take(T * 32 * sizeof(float2));
+    o.pos = (int *)take(sizeof(int));
+    o.cur_tok = (int *)take(B * sizeof(int));
+    o.tok_hist = (int *)take((T + 1) * B * sizeof(int));
+    o.best = (unsigned long long *)take(B * sizeof(unsigned long long));
+    o.counter = (unsigned int *)take(sizeof(unsigned int));
+    o.x = (float *)take(B * d * sizeof(float));
+    o.q = (float *)take(B * H * kHeadDim * sizeof(float));
+    o.part_o = (float *)take(B * H * kMaxSplits * kHeadDim * sizeof(float));
+    o.part_ml = (float2 *)take(B * H * kMaxSplits * sizeof(float2));
+    o.act = (float *)take(B * F * sizeof(float));
+    o.logits = (float *)take(B * V * sizeof(float));
+    o.hidden = (float *)take((c->flags & HQ_FLAG_CAPTURE_HIDDEN) ? L * B * d * sizeof(float) : 0);
+    o.prompt = (int *)take(B * T * sizeof(int));
+    return off;
+}
+
+extern "C" size_t hq_workspace_bytes(const hq_config *cfg) {
+    const char *why = "";
+    if (!config_ok(cfg, &why)) {
+        fail(HQ_ERR_INVALID_ARG, "hq_workspace_bytes: %s", why);
+        return 0;
+    }
+    return carve(cfg, nullptr, nullptr);
+}
+
+// ---- one decode step: A1..A9 ------------------------------------------------------------------------
+// tok_src: device pointer to the token fed at this step.  with_head = false skips A9 and advances
+// the position with a one-thread kernel instead (used while walking a prompt token by token).
+static cudaError_t enqueue_step(hq_model *m, const int *tok_src, bool with_head, int *n_launched) {
+    const hq_config &c = m->cfg;
+    const LaunchCtx lc{m->stream, m->use_pdl, m->n_sms};
+    const Buffers &b = m->b;
+    const int qdim = c.n_heads * kHeadDim;
+    const size_t layer_kv = (size_t)c.max_batch * c.n_kv_heads * c.max_seq * kHeadDim;
+    cudaError_t e;
+    int n = 0;
+#define STEP(call) do { e = (call); if (e != cudaSuccess) return e; ++n; } while (0)
+    STEP(launch_embed(lc, m->emb, tok_src, b.x, c.hidden, 1));
+    for (int l = 0; l < c.n_layers; ++l) {
+        const LayerW &w = m->layers[l];
+        GemvParams p = {};
+        // A2+A3+A4: RMSNorm -> QKV GEMV -> RoPE + KV append
+        p.w0 = w.wq; p.w1 = w.wk; p.w2 = w.wv; p.gain = w.attn_norm; p.xin = b.x; p.K = c.hidden;
+        p.n_units = (c.n_heads + 2 * c.n_kv_heads) * 32; p.eps = c.rms_eps; p.out = b.q;
+        p.kc = b.kcache + l * layer_kv; p.vc = b.vcache + l * layer_kv; p.rope = b.rope; p.pos = b.pos;
+        p.n_heads = c.n_heads; p.n_kv_heads = c.n_kv_heads; p.max_seq = c.max_seq;
+        STEP(launch_gemv(lc, GEMV_QKV, XIN_NORM, p));
+        // A5: split-KV flash-decode
+        AttnDecodeParams a = {b.q, p.kc, p.vc, b.part_o, b.part_ml, b.pos, c.n_heads, c.n_kv_heads, c.max_seq};
+        STEP(launch_attn_decode(lc, a, 1));
+        // A6: merge splits -> O GEMV -> residual
+        GemvParams po = {};
+        po.w0 = w.wo; po.xin = b.part_o; po.part_ml = b.part_ml; po.K = qdim; po.n_units = c.hidden / 2;
+        po.out = b.x; po.pos = b.pos;
+        STEP(launch_gemv(lc, GEMV_RESID, XIN_ATTN, po));
+        // A2+A7: RMSNorm -> gate/up GEMV -> SwiGLU
+        GemvParams pg = {};
+        pg.w0 = w.w_gate; pg.w1 = w.w_up; pg.gain = w.ffn_norm; pg.xin = b.x; pg.K = c.hidden;
+        pg.n_units = c.ffn; pg.eps = c.rms_eps; pg.out = b.act;
+        STEP(launch_gemv(lc, GEMV_GATEUP, XIN_NORM, pg));
+        // A8: down GEMV -> residual
+        GemvParams pd = {};
+        pd.w0 = w.w_down; pd.xin = b.act; pd.K = c.ffn; pd.n_units = c.hidden / 2; pd.out = b.x;
+        STEP(launch_gemv(lc, GEMV_RESID, XIN_PLAIN, pd));
+        if (c.flags & HQ_FLAG_CAPTURE_HIDDEN) {
+            e = cudaMemcpyAsync(b.hidden + (size_t)l * c.max_batch * c.hidden, b.x, c.hidden * sizeof(float),
+                                cudaMemcpyDeviceToDevice, m->stream);
+            if (e != cudaSuccess) return e;
+        }
+    }
+    if (with_head) {
+        // A9: final norm -> LM head GEMV -> logits + argmax + step bookkeeping
+        GemvParams ph = {};
+        ph.w0 = m->lm_head; ph.gain = m->final_norm; ph.xin = b.x; ph.K = c.hidden; ph.n_units = c.vocab / 2;
+        ph.eps = c.rms_eps; ph.out = b.logits; ph.pos = b.pos; ph.best = b.best; ph.counter = b.counter;
+        ph.cur_tok = b.cur_tok; ph.tok_hist = b.tok_hist; ph.pos_rw = b.pos; ph.pos_inc = 1;
+        STEP(launch_gemv(lc, GEMV_LMHEAD, XIN_NORM, ph));
+    } else {
+        STEP(launch_advance(lc, b.pos, 1));
+    }
+#undef STEP
+    if (n_launched) *n_launched = n;
+    return cudaSuccess;
+}
+
+static cudaError_t capture_step_graph(hq_model *m) {
+    cudaError_t e = cudaStreamBeginCapture(m->stream, cudaStreamCaptureModeThreadLocal);
+    if (e != cudaSuccess) return e;
+    int n = 0;
+    cudaError_t e_step = enqueue_step(m, m->b.cur_tok, true, &n);
+    cudaGraph_t g = nullptr;
+    e = cudaStreamEndCapture(m->stream, &g);
+    if (e_step != cudaSuccess) { if (g) cudaGraphDestroy(g); return e_step; }
+    if (e != cudaSuccess) return e;
+    e = cudaGraphInstantiate(&m->step_graph, g, 0);
+    cudaGraphDestroy(g);
+    if (e != cudaSuccess) { m->step_graph = nullptr; return e; }
+    m->kernels_per_step = n;
+    return cudaSuccess;
+}
+
+// ---- create / destroy ---------------------------------------------------------------------------------
+extern "C" int32_t hq_model_create(const hq_config *cfg, const hq_weights *w, void *workspace, size_t ws_bytes,
+                                   void *cuda_stream, hq_model **out) {
+    const char *why = "";
+    if (!out) return fail(HQ_ERR_INVALID_ARG, "hq_model_create: out is NULL");
+    *out = nullptr;
+    if (!config_ok(cfg, &why)) return fail(HQ_ERR_INVALID_ARG, "hq_model_create: %s", why);
+    if (!config_supported(cfg, &why)) return fail(HQ_ERR_UNSUPPORTED, "hq_model_create: %s", why);
+    if (!w || !workspace) return fail(HQ_ERR_INVALID_ARG, "hq_model_create: weights or workspace is NULL");
+    if (!w->tok_embedding || !w->final_norm || !w->lm_head || !w->attn_norm || !w->wq || !w->wk || !w->wv ||
+        !w->wo || !w->ffn_norm || !w->w_gate || !w->w_up || !w->w_down)
+        return fail(HQ_ERR_INVALID_ARG, "hq_model_create: a weight pointer is NULL");
+    for (int l = 0; l < cfg->n_layers; ++l)
+        if (!w->attn_norm[l] || !w->wq[l] || !w->wk[l] || !w->wv[l] || !w->wo[l] || !w->ffn_norm[l] ||
+            !w->w_gate[l] || !w->w_up[l] || !w->w_down[l])
+            return fail(HQ_ERR_INVALID_ARG, "hq_model_create: a weight pointer of layer %d is NULL", l);
+    if (((uintptr_t)workspace & 255) != 0) return fail(HQ_ERR_INVALID_ARG, "hq_model_create: workspace not 256-byte aligned");
+    const size_t need = carve(cfg, nullptr, nullptr);
+    if (ws_bytes < need)
+        return fail(HQ_ERR_CAPACITY, "hq_model_create: workspace %zu bytes < %zu needed", ws_bytes, need);
+
+    int dev = 0;
+    HQ_CUDA(cudaGetDevice(&dev));
+    cudaDeviceProp prop;
+    HQ_CUDA(cudaGetDeviceProperties(&prop, dev));
+    if (prop.major != 10)
+        return fail(HQ_ERR_UNSUPPORTED, "hq_model_create: needs compute capability 10.x (sm_100a), found %d.%d",
+                    prop.major, prop.minor);
+
+    hq_model *m = new (std::nothrow) hq_model();
+    if (!m) return fail(HQ_ERR_INVALID_ARG, "hq_model_create: out of host memory");
+    m->cfg = *cfg;
+    m->stream = (cudaStream_t)cuda_stream;
+    m->n_sms = prop.multiProcessorCount;
+    m->emb = (const bf16 *)w->tok_embedding;
+    m->final_norm = (const bf16 *)w->final_norm;
+    m->lm_head = (const bf16 *)w->lm_head;
+    m->layers.resize(cfg->n_layers);
+    for (int l = 0; l < cfg->n_layers; ++l) {
+        LayerW &lw = m->layers[l];
+        lw.attn_norm = (const bf16 *)w->attn_norm[l]; lw.wq = (const bf16 *)w->wq[l];
+        lw.wk = (const bf16 *)w->wk[l]; lw.wv = (const bf16 *)w->wv[l]; lw.wo = (const bf16 *)w->wo[l];
+        lw.ffn_norm = (const bf16 *)w->ffn_norm[l]; lw.w_gate = (const bf16 *)w->w_gate[l];
+        lw.w_up = (const bf16 *)w->w_up[l]; lw.w_down = (const bf16 *)w->w_down[l];
+    }
+    carve(cfg, (char *)workspace, &m->b);
+    m->use_pdl = !(cfg->flags & HQ_FLAG_NO_PDL) && !getenv("HQ_NO_PDL");
+
+    // RoPE table in double on the host (reading 7): angle = pos * theta^(-2i/64)
+    {
+        std::vector<float2> tab((size_t)cfg->max_seq * 32);
+        for (int p = 0; p < cfg->max_seq; ++p)
+            for (int i = 0; i < 32; ++i) {
+                const double phi = (double)p * pow((double)cfg->rope_theta, -2.0 * i / (double)kHeadDim);
+                tab[(size_t)p * 32 + i] = make_float2((float)cos(phi), (float)sin(phi));
+            }
+        cudaError_t e = cudaMemcpyAsync(m->b.rope, tab.data(), tab.size() * sizeof(float2), cudaMemcpyHostToDevice, m->stream);
+        if (e == cudaSuccess) e = launch_set_state(LaunchCtx{m->stream, false, m->n_sms}, m->b.pos, 0, m->b.best,
+                                                   m->b.counter, cfg->max_batch);
+        if (e == cudaSuccess) e = launch_zero_tokens(LaunchCtx{m->stream, false, m->n_sms}, m->b.cur_tok, cfg->max_batch);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(m->stream);
+        if (e != cudaSuccess) {
+            delete m;
+            return fail(HQ_ERR_CUDA, "hq_model_create: state init failed: %s", cudaGetErrorString(e));
+        }
+    }
+
+    // A stream capture cannot start on the legacy default stream: without a real stream the decode
+    // step is launched kernel by kernel.
+    if (!(cfg->flags & HQ_FLAG_NO_GRAPH) && !getenv("HQ_NO_GRAPH") && m->stream != nullptr) {
+        // One eager step first so that every kernel is loaded before the capture (lazy module
+        // loading is not allowed while capturing); its side effects are reset right after.
+        cudaError_t e = enqueue_step(m, m->b.cur_tok, true, nullptr);
+        if (e == cudaSuccess) e = launch_set_state(LaunchCtx{m->stream, false, m->n_sms}, m->b.pos, 0, m->b.best,
+                                                   m->b.counter, cfg->max_batch);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(m->stream);
+        if (e == cudaSuccess) e = capture_step_graph(m);
+        if (e != cudaSuccess && m->use_pdl) {  // retry without programmatic edges
+            cudaGetLastError();
+            m->use_pdl = false;
+            e = capture_step_graph(m);
+        }
+        if (e != cudaSuccess) {
+            cudaGetLastError();
+            delete m;
+            return fail(HQ_ERR_CUDA, "hq_model_create: graph capture failed: %s", cudaGetErrorString(e));
+        }
+    }
+    *out = m;
+    return HQ_OK;
+}
+
+extern "C" void hq_model_destroy(hq_model *m) {
+    if (!m) return;
+    if (m->step_graph) cudaGraphExecDestroy(m->step_graph);
+    delete m;
+}
+
+// ---- state --------------------------------------------------------------------------------------------
+extern "C" int32_t hq_sync(hq_model *m) {
+    if (!m) return fail(HQ_ERR_INVALID_ARG, "hq_sync: model is NULL");
+    HQ_CUDA(cudaStreamSynchronize(m->stream));
+    return HQ_OK;
+}
+
+extern "C" int32_t hq_seq_len(const hq_model *m, int32_t *out) {
+    if (!m || !out) return fail(HQ_ERR_INVALID_ARG, "hq_seq_len: NULL argument");
+    *out = m->seq_len;
+    return HQ_OK;
+}
+
+extern "C" int32_t hq_kv_reset(hq_model *m) {
+    if (!m) return fail(HQ_ERR_INVALID_ARG, "hq_kv_reset: model is NULL");
+    HQ_CUDA(launch_set_state(LaunchCtx{m->stream, false, m->n_sms}, m->b.pos, 0, m->b.best, m->b.counter,
+                             m->cfg.max_batch));
+    m->kernel_count += 1;
+    m->seq_len = 0;
+    m->batch = 0;
+    m->have_token = false;
+    return HQ_OK;
+}
+
+extern "C" int64_t hq_kernel_count(const hq_model *m) { return m ? m->kernel_count : 0; }
+
+// ---- prefill -----------------------------------------------------------------------------------------
+extern "C" int32_t hq_prefill(hq_model *m, const int32_t *tokens_host, int32_t batch, int32_t n_tokens,
+                              float *logits_dev, int32_t *first_token_host) {
+    if (!m || !tokens_host) return fail(HQ_ERR_INVALID_ARG, "hq_prefill: NULL argument");
+    if (batch <= 0 || n_tokens <= 0) return fail(HQ_ERR_INVALID_ARG, "hq_prefill: batch and n_tokens must be > 0");
+    const hq_config &c = m->cfg;
+    if (batch > c.max_batch) return fail(HQ_ERR_CAPACITY, "hq_prefill: batch %d > max_batch %d", batch, c.max_batch);
+    if (m->batch != 0 && batch != m->batch)
+        return fail(HQ_ERR_STATE, "hq_prefill: active batch is %d, got %d (hq_kv_reset first)", m->batch, batch);
+    if ((long long)m->seq_len + n_tokens > c.max_seq)
+        return fail(HQ_ERR_CAPACITY, "hq_prefill: seq_len %d + %d tokens > max_seq %d", m->seq_len, n_tokens, c.max_seq);
+    for (long long i = 0; i < (long long)batch * n_tokens; ++i)
+        if (tokens_host[i] < 0 || tokens_host[i] >= c.vocab)
+            return fail(HQ_ERR_INVALID_ARG, "hq_prefill: token %d at index %lld outside [0, %d)", tokens_host[i], i, c.vocab);
+    if (batch != 1) return fail(HQ_ERR_UNSUPPORTED, "hq_prefill: batch > 1 is not implemented yet");
+
+    HQ_CUDA(cudaMemcpyAsync(m->b.prompt, tokens_host, (size_t)n_tokens * sizeof(int), cudaMemcpyHostToDevice, m->stream));
+    for (int t = 0; t < n_tokens; ++t) {
+        int n = 0;
+        HQ_CUDA(enqueue_step(m, m->b.prompt + t, t == n_tokens - 1, &n));
+        m->kernel_count += n;
+    }
+    m->batch = batch;
+    m->seq_len += n_tokens;
+    m->have_token = true;
+    if (logits_dev)
+        HQ_CUDA(cudaMemcpyAsync(logits_dev, m->b.logits, (size_t)batch * c.vocab * sizeof(float),
+                                cudaMemcpyDeviceToDevice, m->stream));
+    if (first_token_host) {
+        HQ_CUDA(cudaMemcpyAsync(first_token_host, m->b.cur_tok, batch * sizeof(int), cudaMemcpyDeviceToHost, m->stream));
+        HQ_CUDA(cudaStreamSynchronize(m->stream));
+    }
+    return HQ_OK;
+}
+
+// ---- decode ------------------------------------------------------------------------------------------
+static int32_t decode_precheck(hq_model *m, const char *who, int n_steps) {
+    if (!m) return fail(HQ_ERR_INVALID_ARG, "%s: model is NULL", who);
+    if (m->batch == 0) return fail(HQ_ERR_STATE, "%s: no active sequence (call hq_prefill first)", who);
+    if ((long long)m->seq_len + n_steps > m->cfg.max_seq)
+        return fail(HQ_ERR_CAPACITY, "%s: seq_len %d + %d > max_seq %d", who, m->seq_len, n_steps, m->cfg.max_seq);
+    return HQ_OK;
+}
+
+static int32_t launch_one_step(hq_model *m) {
+    if (m->step_graph) {
+        HQ_CUDA(cudaGraphLaunch(m->step_graph, m->stream));
+        m->kernel_count += m->kernels_per_step;
+    } else {
+        int n = 0;
+        HQ_CUDA(enqueue_step(m, m->b.cur_tok, true, &n));
+        m->kernel_count += n;
+    }
+    m->seq_len += 1;
+    return HQ_OK;
+}
+
+extern "C" int32_t hq_decode_step(hq_model *m, const int32_t *tokens_in_host, int32_t *tokens_out_host) {
+    int32_t rc = decode_precheck(m, "hq_decode_step", 1);
+    if (rc != HQ_OK) return rc;
+    if (tokens_in_host) {
+        for (int b = 0; b < m->batch; ++b)
+            if (tokens_in_host[b] < 0 || tokens_in_host[b] >= m->cfg.vocab)
+                return fail(HQ_ERR_INVALID_ARG, "hq_decode_step: token %d outside [0, %d)", tokens_in_host[b], m->cfg.vocab);
+        HQ_CUDA(cudaMemcpyAsync(m->b.cur_tok, tokens_in_host, m->batch * sizeof(int), cudaMemcpyHostToDevice, m->stream));
+    } else if (!m->have_token) {
+        return fail(HQ_ERR_STATE, "hq_decode_step: no device-resident token to feed");
+    }
+    rc = launch_one_step(m);
+    if (rc != HQ_OK) return rc;
+    m->have_token = true;
+    if (tokens_out_host) {
+        HQ_CUDA(cudaMemcpyAsync(tokens_out_host, m->b.cur_tok, m->batch * sizeof(int), cudaMemcpyDeviceToHost, m->stream));
+        HQ_CUDA(cudaStreamSynchronize(m->stream));
+    }
+    return HQ_OK;
+}
+
+extern "C" int32_t hq_decode_run(hq_model *m, int32_t n_steps, int32_t *tokens_out_host) {
+    if (n_steps <= 0) return fail(HQ_ERR_INVALID_ARG, "hq_decode_run: n_steps must be > 0");
+    int32_t rc = decode_precheck(m, "hq_decode_run", n_steps);
+    if (rc != HQ_OK) return rc;
+    if (!m->have_token) return fail(HQ_ERR_STATE, "hq_decode_run: no device-resident token to feed");
+    const int first = m->seq_len + 1;
+    for (int i = 0; i < n_steps; ++i) {
+        rc = launch_one_step(m);
+        if (rc != HQ_OK) return rc;
+    }
+    if (tokens_out_host) {
+        HQ_CUDA(cudaMemcpyAsync(tokens_out_host, m->b.tok_hist + (size_t)first * m->batch,
+                                (size_t)n_steps * m->batch * sizeof(int), cudaMemcpyDeviceToHost, m->stream));
+        HQ_CUDA(cudaStreamSynchronize(m->stream));
+    }
+    return HQ_OK;
+}
+
+extern "C" int32_t hq_decode_logits(hq_model *m, float *logits_dev) {
+    if (!m || !logits_dev) return fail(HQ_ERR_INVALID_ARG, "hq_decode_logits: NULL argument");
+    if (m->batch == 0) return fail(HQ_ERR_STATE, "hq_decode_logits: nothing has been evaluated yet");
+    HQ_CUDA(cudaMemcpyAsync(logits_dev, m->b.logits, (size_t)m->batch * m->cfg.vocab * sizeof(float),
+                            cudaMemcpyDeviceToDevice, m->stream));
+    return HQ_OK;
+}
+
+extern "C" int32_t hq_get_hidden(hq_model *m, int32_t layer, float *hidden_dev) {
+    if (!m || !hidden_dev) return fail(HQ_ERR_INVALID_ARG, "hq_get_hidden: NULL argument");
+    if (!(m->cfg.flags & HQ_FLAG_CAPTURE_HIDDEN)) return fail(HQ_ERR_STATE, "hq_get_hidden: model created without HQ_FLAG_CAPTURE_HIDDEN");
+    if (layer < 0 || layer >= m->cfg.n_layers) return fail(HQ_ERR_INVALID_ARG, "hq_get_hidden: layer %d outside [0, %d)", layer, m->cfg.n_layers);
+    if (m->batch == 0) return fail(HQ_ERR_STATE, "hq_get_hidden: nothing has been evaluated yet");
+    HQ_CUDA(cudaMemcpyAsync(hidden_dev, m->b.hidden + (size_t)layer * m->cfg.max_batch * m->cfg.hidden,
+                            (size_t)m->batch * m->cfg.hidden * sizeof(float), cudaMemcpyDeviceToDevice, m->stream));
+    return HQ_OK;
+}
+
+// ---- measurement hook ---------------------------------------------------------------------------------
+extern "C" int32_t hq_bench_kernel(hq_model *m, int32_t which, int32_t reps, int64_t *bytes_per_launch) {
+    if (!m || reps <= 0) return fail(HQ_ERR_INVALID_ARG, "hq_bench_kernel: bad argument");
+    if (m->batch == 0 || m->seq_len == 0) return fail(HQ_ERR_STATE, "hq_bench_kernel: needs a prefilled cache");
+    if (m->seq_len >= m->cfg.max_seq) return fail(HQ_ERR_CAPACITY, "hq_bench_kernel: cache is full");
+    const hq_config &c = m->cfg;
+    const LaunchCtx lc{m->stream, m->use_pdl, m->n_sms};
+    const Buffers &b = m->b;
+    const size_t layer_kv = (size_t)c.max_batch * c.n_kv_heads * c.max_seq * kHeadDim;
+    const int qdim = c.n_heads * kHeadDim;
+    int64_t bytes = 0;
+    for (int r = 0; r < reps; ++r) {
+        const int l = r % c.n_layers;
+        const LayerW &w = m->layers[l];
+        GemvParams p = {};
+        switch (which) {
+            case 0:
+                p.w0 = w.w_gate; p.w1 = w.w_up; p.gain = w.ffn_norm; p.xin = b.x; p.K = c.hidden; p.n_units = c.ffn;
+                p.eps = c.rms_eps; p.out = b.act;
+                HQ_CUDA(launch_gemv(lc, GEMV_GATEUP, XIN_NORM, p));
+                bytes = 2ll * 2 * c.ffn * c.hidden;
+                break;
+            case 1:
+                // LM head without state side effects: pos_inc = 0, token/history writes go to scratch slots
+                p.w0 = m->lm_head; p.gain = m->final_norm; p.xin = b.x; p.K = c.hidden; p.n_units = c.vocab / 2;
+                p.eps = c.rms_eps; p.out = b.logits; p.pos = b.pos; p.best = b.best; p.counter = b.counter;
+                p.cur_tok = b.cur_tok; p.tok_hist = b.tok_hist; p.pos_rw = b.pos; p.pos_inc = 0;
+                HQ_CUDA(launch_gemv(lc, GEMV_LMHEAD, XIN_NORM, p));
+                bytes = 2ll * c.vocab * c.hidden;
+                break;
+            case 2:
+                // QKV: rewrites the K/V row at the current position with garbage from the scratch x
+                p.w0 = w.wq; p.w1 = w.wk; p.w2 = w.wv; p.gain = w.attn_norm; p.xin = b.x; p.K = c.hidden;
+                p.n_units = (c.n_heads + 2 * c.n_kv_heads) * 32; p.eps = c.rms_eps; p.out = b.q;
+                p.kc = b.kcache + l * layer_kv; p.vc = b.vcache + l * layer_kv; p.rope = b.rope; p.pos = b.pos;
+                p.n_heads = c.n_heads; p.n_kv_heads = c.n_kv_heads; p.max_seq = c.max_seq;
+                HQ_CUDA(launch_gemv(lc, GEMV_QKV, XIN_NORM, p));
+                bytes = 2ll * (c.n_heads + 2 * c.n_kv_heads) * kHeadDim * c.hidden;
+                break;
+            case 3:
+                p.w0 = w.wo; p.xin = b.part_o; p.part_ml = b.part_ml; p.K = qdim; p.n_units = c.hidden / 2;
+                p.out = b.x; p.pos = b.pos;
+                HQ_CUDA(launch_gemv(lc, GEMV_RESID, XIN_ATTN, p));
+                bytes = 2ll * c.hidden * qdim;
+                break;
+            case 4:
+                p.w0 = w.w_down; p.xin = b.act; p.K = c.ffn; p.n_units = c.hidden / 2; p.out = b.x;
+                HQ_CUDA(launch_gemv(lc, GEMV_RESID, XIN_PLAIN, p));
+                bytes = 2ll * c.hidden * c.ffn;
+                break;
+            case 5: {
+                AttnDecodeParams a = {b.q, b.kcache + l * layer_kv, b.vcache + l * layer_kv, b.part_o, b.part_ml,
+                                      b.pos, c.n_heads, c.n_kv_heads, c.max_seq};
+                HQ_CUDA(launch_attn_decode(lc, a, 1));
+                bytes = 2ll * 2 * c.n_kv_heads * kHeadDim * (m->seq_len + 1);
+                break;
+            }
+            default:
+                return fail(HQ_ERR_INVALID_ARG, "hq_bench_kernel: unknown kernel %d", which);
+        }
+        m->kernel_count += 1;
+    }
+    if (bytes_per_launch) *bytes_per_launch = bytes;
+    return HQ_OK;
+}

@@ -1,0 +1,128 @@
+// hq_internal.h — host-side model object and launcher prototypes shared by the libhq TUs.
+#pragma once
+#include <cuda_bf16.h>
+#include <cuda_fp16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/hq.h"
+
+namespace hq {
+
+typedef __nv_bfloat16 bf16;
+// KV cache element type.  fp16, not bf16: same 2 bytes, 3 more mantissa bits.  With bf16 the
+// cache rounding alone costs 0.008 of the 0.01 per-layer hidden-state tolerance on the 1B
+// random-weight model; K/V magnitudes here are O(1..10), far from
+// the fp16 range limit.
+typedef __half kv_t;
+
+constexpr int kHeadDim = 64;        // only head_dim the kernels implement
+constexpr int kMaxSplits = 16;      // split-KV partials per head (decode attention)
+constexpr int kMinSplitLen = 64;    // do not split contexts shorter than this per split
+constexpr int kGemvThreads = 256;
+
+struct LayerW {
+    const bf16 *attn_norm, *wq, *wk, *wv, *wo, *ffn_norm, *w_gate, *w_up, *w_down;
+};
+
+// Device buffers carved from the caller's workspace (see hq_api.cu carve()).
+struct Buffers {
+    kv_t *kcache = nullptr, *vcache = nullptr;  // [L][B][Hkv][Tmax][64] fp16
+    float2 *rope = nullptr;                     // [Tmax][32] (cos, sin), built on the host in double
+    // decode state / activations (fp32)
+    int *pos = nullptr;                         // cached positions (device resident, graph safe)
+    int *cur_tok = nullptr;                     // [B] token to feed next
+    int *tok_hist = nullptr;                    // [Tmax+1][B] emitted tokens, index = pos at emission
+    unsigned long long *best = nullptr;         // [B] packed argmax
+    unsigned int *counter = nullptr;            // last-CTA ticket
+    float *x = nullptr;                         // [B][d] residual stream
+    float *q = nullptr;                         // [B][H*64]
+    float *part_o = nullptr;                    // [B][H][kMaxSplits][64]
+    float2 *part_ml = nullptr;                  // [B][H][kMaxSplits] (m, l)
+    float *act = nullptr;                       // [B][F]
+    float *logits = nullptr;                    // [B][V]
+    float *hidden = nullptr;                    // [L][B][d] (capture flag)
+    int *prompt = nullptr;                      // [B][Tmax] staged prompt tokens
+};
+
+struct hq_model_impl {
+    hq_config cfg;
+    std::vector<LayerW> layers;
+    const bf16 *emb = nullptr, *final_norm = nullptr, *lm_head = nullptr;
+    cudaStream_t stream = nullptr;
+    Buffers b;
+    int n_sms = 148;
+    int batch = 0;      // active batch (0 = none)
+    int seq_len = 0;    // host mirror of *b.pos
+    bool have_token = false;
+    cudaGraphExec_t step_graph = nullptr;
+    long long kernel_count = 0;
+    int kernels_per_step = 0;
+    bool use_pdl = true;
+};
+
+// ---- parameter blocks --------------------------------------------------------------------------------
+enum GemvMode { GEMV_QKV = 0, GEMV_GATEUP = 1, GEMV_RESID = 2, GEMV_LMHEAD = 3 };
+enum GemvInput { XIN_NORM = 0, XIN_PLAIN = 1, XIN_ATTN = 2 };
+
+struct GemvParams {
+    // weights: QKV uses w0=wq, w1=wk, w2=wv; GATEUP w0=gate, w1=up; RESID/LMHEAD w0
+    const bf16 *w0, *w1, *w2;
+    const bf16 *gain;        // XIN_NORM
+    const float *xin;        // XIN_NORM: residual x [K]; XIN_PLAIN: act [K]; XIN_ATTN: part_o
+    const float2 *part_ml;   // XIN_ATTN
+    int K;                   // input features
+    int n_units;             // work units (2 output rows each)
+    float eps;
+    // outputs
+    float *out;              // QKV: q [H*64]; GATEUP: act [F]; RESID: x (read-modify-write); LMHEAD: logits
+    kv_t *kc, *vc;           // QKV: this layer's cache base for sequence 0
+    const float2 *rope;
+    const int *pos;          // device-resident position
+    int n_heads, n_kv_heads, max_seq;
+    // LMHEAD
+    unsigned long long *best;
+    unsigned int *counter;
+    int *cur_tok, *tok_hist;
+    int *pos_rw;
+    int pos_inc;
+};
+
+struct AttnDecodeParams {
+    const float *q;          // [H*64]
+    const kv_t *kc, *vc;     // layer base
+    float *part_o;
+    float2 *part_ml;
+    const int *pos;
+    int n_heads, n_kv_heads, max_seq;
+};
+
+// split policy shared by the attention kernel and the O-proj prologue (host + device)
+__host__ __device__ inline int attn_num_splits(int n_ctx) {
+    int s = (n_ctx + kMinSplitLen - 1) / kMinSplitLen;
+    return s < 1 ? 1 : (s > kMaxSplits ? kMaxSplits : s);
+}
+__host__ __device__ inline int attn_split_len(int n_ctx, int n_splits) {
+    int c = (n_ctx + n_splits - 1) / n_splits;
+    return (c + 15) & ~15;  // 16-position granules
+}
+
+// ---- launchers (hq_decode.cu) ------------------------------------------------------------------------
+struct LaunchCtx {
+    cudaStream_t stream;
+    bool pdl;
+    int n_sms;
+};
+cudaError_t launch_embed(const LaunchCtx &c, const bf16 *emb, const int *tok, float *x, int hidden, int batch);
+cudaError_t launch_gemv(const LaunchCtx &c, GemvMode mode, GemvInput xin, const GemvParams &p);
+cudaError_t launch_attn_decode(const LaunchCtx &c, const AttnDecodeParams &p, int batch);
+cudaError_t launch_advance(const LaunchCtx &c, int *pos, int inc);
+cudaError_t launch_set_state(const LaunchCtx &c, int *pos, int pos_value, unsigned long long *best,
+                             unsigned int *counter, int batch);
+cudaError_t launch_zero_tokens(const LaunchCtx &c, int *cur_tok, int batch);
+bool gemv_shape_supported(int K);
+
+}  // namespace hq
