@@ -22,8 +22,8 @@
  *  - Weight matrices are bf16, nn.Linear layout [out_features, in_features], row-major, rows
  *    16-byte aligned.  Norm gains are bf16 [hidden].  Activations inside the library: fp32
  *    residual stream, fp32 accumulators/softmax/norm statistics, fp16 KV cache (2 bytes per element,
- *    32,768 B per cached token for the 1B shape), bf16 tensor-core
- *    operands (prefill / batched decode only).
+ *    32,768 B per cached token for the 1B shape), on the tensor cores (prefill / batched decode only) bf16
+ *    weight operands x activation operands split into two bf16 planes hi + lo (16 mantissa bits).
  *  - Sequences of a batch advance in lock step (equal lengths), as in every BASELINE.json config.
  */
 #ifndef HQ_H_
@@ -90,6 +90,7 @@ size_t hq_workspace_bytes(const hq_config *cfg);
  * >= hq_workspace_bytes).  cuda_stream is a cudaStream_t (NULL = legacy default stream).
  * Supported shapes: head_dim == 64, n_heads % n_kv_heads == 0 with group size <= 8, hidden and
  * ffn multiples of 8 and <= 8192, max_batch <= 32; anything else returns HQ_ERR_UNSUPPORTED.
+ * batch 1 decodes with the GEMV kernels; batch > 1 and prompts of >= 8 tokens run on the tcgen05 GEMM path.
  * Requires compute capability 10.x. */
 int32_t hq_model_create(const hq_config *cfg, const hq_weights *weights, void *workspace_dev,
                         size_t workspace_bytes, void *cuda_stream, hq_model **out);
@@ -143,6 +144,16 @@ int32_t hq_kv_reset(hq_model *m);
  * bytes_per_launch (HOST, may be NULL) receives the algorithmic HBM bytes of one launch. */
 int64_t hq_kernel_count(const hq_model *m);
 int32_t hq_bench_kernel(hq_model *m, int32_t which, int32_t reps, int64_t *bytes_per_launch);
+
+/* Diagnostics: the tcgen05 GEMM of the prefill / batched-decode path on its own (unit tests).
+ * All pointers DEVICE.  w, w2: bf16 [n_rows][k]; x: bf16 [2][n_tokens][k], the activation as two planes
+ * x = hi + lo (hi = bf16(x), lo = bf16(x - hi)); token_tile in {32,64,128,256}.
+ *   mode 0: out fp32 [n_tokens][n_rows]  = x w^T   (splits > 1: out must be zeroed, partials add atomically)
+ *   mode 1: out fp32 [n_tokens][n_rows] += x w^T   (residual epilogue)
+ *   mode 2: out bf16 [2][n_tokens][n_rows] = hi/lo planes of silu(x w^T) * (x w2^T)   (SwiGLU epilogue)
+ * Asynchronous on cuda_stream. */
+int32_t hq_debug_gemm(void *cuda_stream, int32_t mode, const void *w_dev, const void *w2_dev, const void *x_dev,
+                      void *out_dev, int32_t n_rows, int32_t k, int32_t n_tokens, int32_t token_tile, int32_t splits);
 
 /* Thread-local message of the last failing call on this thread; static storage, never NULL. */
 const char *hq_last_error(void);

@@ -25,7 +25,7 @@ _CODE_NAMES = {-1: "HQ_ERR_INVALID_ARG", -2: "HQ_ERR_CAPACITY", -3: "HQ_ERR_STAT
 DECLARED_SYMBOLS = (
     "hq_workspace_bytes", "hq_model_create", "hq_model_destroy", "hq_prefill", "hq_decode_step",
     "hq_decode_run", "hq_decode_logits", "hq_get_hidden", "hq_sync", "hq_seq_len", "hq_kv_reset",
-    "hq_kernel_count", "hq_bench_kernel", "hq_last_error", "hq_version",
+    "hq_kernel_count", "hq_bench_kernel", "hq_debug_gemm", "hq_last_error", "hq_version",
 )
 
 
@@ -93,6 +93,8 @@ def load_library(path: Optional[str] = None):
     l.hq_kernel_count.argtypes = [vp]
     l.hq_bench_kernel.restype = i32
     l.hq_bench_kernel.argtypes = [vp, i32, i32, ctypes.POINTER(i64)]
+    l.hq_debug_gemm.restype = i32
+    l.hq_debug_gemm.argtypes = [vp, i32, vp, vp, vp, vp, i32, i32, i32, i32, i32]
     l.hq_last_error.restype = ctypes.c_char_p
     l.hq_last_error.argtypes = []
     l.hq_version.restype = ctypes.c_char_p
@@ -249,3 +251,13 @@ class Model:
         b = ctypes.c_int64()
         _check(self._lib.hq_bench_kernel(self._h, which, reps, ctypes.byref(b)))
         return b.value
+
+
+def debug_gemm(mode: int, w, x, out, *, w2=None, token_tile: int = 128, splits: int = 1, stream=None):
+    """hq_debug_gemm on torch CUDA tensors: bf16 w [N,K], bf16 x planes [2,T,K] (hi, lo); out fp32 [T,N],
+    or bf16 planes [2,T,N] for mode 2."""
+    import torch
+    st = stream if stream is not None else torch.cuda.current_stream(w.device)
+    n_rows, k = w.shape
+    _check(load_library().hq_debug_gemm(st.cuda_stream, mode, w.data_ptr(), w2.data_ptr() if w2 is not None else None,
+                                        x.data_ptr(), out.data_ptr(), n_rows, k, x.shape[1], token_tile, splits))

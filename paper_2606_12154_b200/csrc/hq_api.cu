@@ -64,6 +64,14 @@ static bool config_supported(const hq_config *c, const char **why) {
 #undef BAD
 }
 
+// Row capacity of one row-batched pass (tokens of all sequences together), a multiple of 256.
+static size_t pass_rows(const hq_config *c) {
+    size_t r = (size_t)c->max_batch * c->max_seq;
+    if (r > 2048) r = 2048;
+    if (r < (size_t)c->max_batch) r = c->max_batch;
+    return (r + 255) / 256 * 256;
+}
+
 // Walks the layout; when base != NULL also assigns the pointers.
 static size_t carve(const hq_config *c, char *base, Buffers *b) {
     size_t off = 0;
@@ -93,6 +101,16 @@ static size_t carve(const hq_config *c, char *base, Buffers *b) {
     o.logits = (float *)take(B * V * sizeof(float));
     o.hidden = (float *)take((c->flags & HQ_FLAG_CAPTURE_HIDDEN) ? L * B * d * sizeof(float) : 0);
     o.prompt = (int *)take(B * T * sizeof(int));
+    const size_t R = pass_rows(c), qdim = H * kHeadDim, qkvd = (H + 2 * Hkv) * kHeadDim;
+    o.pf_tok = (int *)take(R * sizeof(int));
+    o.last_idx = (int *)take(B * sizeof(int));
+    o.xs = (float *)take(R * d * sizeof(float));
+    o.hn = (act_t *)take(2 * R * d * sizeof(act_t));
+    o.qkv = (float *)take(R * qkvd * sizeof(float));
+    o.q16 = (__half *)take(R * qdim * sizeof(__half));
+    o.ao = (act_t *)take(2 * R * qdim * sizeof(act_t));
+    o.actb = (act_t *)take(2 * R * F * sizeof(act_t));
+    o.hn_last = (act_t *)take(2 * 32 * d * sizeof(act_t));
     return off;
 }
 
@@ -181,6 +199,156 @@ static cudaError_t capture_step_graph(hq_model *m) {
     return cudaSuccess;
 }
 
+// ---- row-batched (tensor-core) path: envelope prefill passes and batched decode steps ---------------
+static int tile_index(int rows) { return rows <= 32 ? 0 : rows <= 64 ? 1 : rows <= 128 ? 2 : 3; }
+
+// split-K so that about one CTA per SM streams weights; at least 4 K blocks per split
+static int pick_splits(const hq_model *m, int n_rows, int rows, int NT, int K) {
+    const int tiles = ((n_rows + 127) / 128) * ((rows + NT - 1) / NT);
+    int s = m->n_sms / (tiles > 0 ? tiles : 1);
+    const int kb = (K + 63) / 64;
+    if (s > kb / 4) s = kb / 4;
+    return s < 1 ? 1 : s;
+}
+
+// All layers for `rows` = batch * Tc token rows already embedded in b.xs; positions start at *b.pos.
+// decode = true: Tc == 1, attention over the cache with the split-KV decode kernel.
+static cudaError_t enqueue_rows_layers(hq_model *m, int batch, int Tc, bool decode, bool capture_hidden, int *n_launched) {
+    const hq_config &c = m->cfg;
+    const LaunchCtx lc{m->stream, m->use_pdl, m->n_sms};
+    const Buffers &b = m->b;
+    const int rows = batch * Tc, ti = tile_index(rows), NT = kTokenTiles[ti];
+    const int d = c.hidden, qdim = c.n_heads * kHeadDim, kvdim = c.n_kv_heads * kHeadDim, qkvd = qdim + 2 * kvdim;
+    const size_t layer_kv = (size_t)c.max_batch * c.n_kv_heads * c.max_seq * kHeadDim;
+    const int R = m->pf_rows;                                  // lo plane sits R rows below the hi plane
+    const size_t lo_d = (size_t)R * d, lo_q = (size_t)R * qdim, lo_f = (size_t)R * c.ffn;
+    cudaError_t e;
+    int n = 0;
+#define STEP(call) do { e = (call); if (e != cudaSuccess) return e; ++n; } while (0)
+    for (int l = 0; l < c.n_layers; ++l) {
+        const LayerW &w = m->layers[l];
+        const LayerMaps &mp = m->maps[l];
+        kv_t *kc = b.kcache + l * layer_kv, *vc = b.vcache + l * layer_kv;
+        STEP(launch_rmsnorm_rows(lc, b.xs, w.attn_norm, b.hn, lo_d, d, c.rms_eps, rows, nullptr, d));
+        // P1: QKV GEMMs (three weight pointers, no repack) into one fp32 [rows][qkvd] buffer
+        const int sq = pick_splits(m, qkvd, rows, NT, d);
+        if (sq > 1) {
+            e = cudaMemsetAsync(b.qkv, 0, (size_t)rows * qkvd * sizeof(float), m->stream);
+            if (e != cudaSuccess) return e;
+        }
+        STEP(launch_gemm(lc, EPI_STORE, mp.wq, nullptr, m->map_hn[ti], R, qdim, d, rows, NT, sq, b.qkv, nullptr, 0, qkvd));
+        STEP(launch_gemm(lc, EPI_STORE, mp.wk, nullptr, m->map_hn[ti], R, kvdim, d, rows, NT, sq, b.qkv + qdim, nullptr, 0, qkvd));
+        STEP(launch_gemm(lc, EPI_STORE, mp.wv, nullptr, m->map_hn[ti], R, kvdim, d, rows, NT, sq, b.qkv + qdim + kvdim, nullptr, 0, qkvd));
+        // P4: RoPE + KV append
+        STEP(launch_rope_append(lc, b.qkv, b.q16, decode ? b.q : nullptr, kc, vc, b.rope, b.pos, rows, Tc, c.n_heads,
+                                c.n_kv_heads, c.max_seq));
+        if (decode) {
+            // B2: split-KV decode attention per sequence, then merge
+            AttnDecodeParams a = {b.q, kc, vc, b.part_o, b.part_ml, b.pos, c.n_heads, c.n_kv_heads, c.max_seq};
+            STEP(launch_attn_decode(lc, a, batch));
+            STEP(launch_attn_combine(lc, b.part_o, b.part_ml, b.ao, lo_q, b.pos, batch, c.n_heads));
+        } else {
+            // P2: causal flash attention
+            STEP(launch_flash_prefill(lc, b.q16, kc, vc, b.ao, lo_q, b.pos, batch, Tc, c.n_heads, c.n_kv_heads, c.max_seq));
+        }
+        STEP(launch_gemm(lc, EPI_RESID, mp.wo, nullptr, m->map_ao[ti], R, d, qdim, rows, NT,
+                         pick_splits(m, d, rows, NT, qdim), b.xs, nullptr, 0, d));
+        STEP(launch_rmsnorm_rows(lc, b.xs, w.ffn_norm, b.hn, lo_d, d, c.rms_eps, rows, nullptr, d));
+        STEP(launch_gemm(lc, EPI_SWIGLU, mp.w_gate, &mp.w_up, m->map_hn[ti], R, c.ffn, d, rows, NT, 1, nullptr, b.actb,
+                         lo_f, c.ffn));
+        STEP(launch_gemm(lc, EPI_RESID, mp.w_down, nullptr, m->map_actb[ti], R, d, c.ffn, rows, NT,
+                         pick_splits(m, d, rows, NT, c.ffn), b.xs, nullptr, 0, d));
+        if (capture_hidden) {
+            // residual of the last position of every sequence -> hidden[l][b]
+            e = cudaMemcpy2DAsync(b.hidden + (size_t)l * c.max_batch * d, d * sizeof(float),
+                                  b.xs + (size_t)(Tc - 1) * d, (size_t)Tc * d * sizeof(float), d * sizeof(float), batch,
+                                  cudaMemcpyDeviceToDevice, m->stream);
+            if (e != cudaSuccess) return e;
+        }
+    }
+#undef STEP
+    if (n_launched) *n_launched += n;
+    return cudaSuccess;
+}
+
+// LM head for the last row of every sequence: final norm -> GEMM (weights read once for all
+// sequences) -> fp32 logits [batch][vocab] -> argmax + step bookkeeping (pos += pos_inc).
+static cudaError_t enqueue_rows_head(hq_model *m, int batch, int Tc, int pos_inc, int *n_launched) {
+    const hq_config &c = m->cfg;
+    const LaunchCtx lc{m->stream, m->use_pdl, m->n_sms};
+    const Buffers &b = m->b;
+    cudaError_t e;
+    int n = 0;
+#define STEP(call) do { e = (call); if (e != cudaSuccess) return e; ++n; } while (0)
+    // rows (Tc-1), (2Tc-1), ... : stride Tc rows starting at row Tc-1
+    STEP(launch_rmsnorm_rows(lc, b.xs + (size_t)(Tc - 1) * c.hidden, m->final_norm, b.hn_last, (size_t)32 * c.hidden,
+                             c.hidden, c.rms_eps, batch, nullptr, Tc * c.hidden));
+    STEP(launch_gemm(lc, EPI_STORE, m->map_lm_head, nullptr, m->map_hn_last, 32, c.vocab, c.hidden, batch, 32, 1, b.logits,
+                     nullptr, 0, c.vocab));
+    STEP(launch_argmax_rows(lc, b.logits, c.vocab, batch, b.cur_tok, b.tok_hist, b.pos, pos_inc, b.counter));
+#undef STEP
+    if (n_launched) *n_launched += n;
+    return cudaSuccess;
+}
+
+// one batched decode step (B1 + B2): embed -> layers -> head
+static cudaError_t enqueue_batch_step(hq_model *m, int batch, int *n_launched) {
+    const LaunchCtx lc{m->stream, m->use_pdl, m->n_sms};
+    int n = 0;
+    cudaError_t e = launch_embed_rows(lc, m->emb, m->b.cur_tok, m->b.xs, m->cfg.hidden, batch);
+    if (e != cudaSuccess) return e;
+    ++n;
+    e = enqueue_rows_layers(m, batch, 1, true, (m->cfg.flags & HQ_FLAG_CAPTURE_HIDDEN) != 0, &n);
+    if (e != cudaSuccess) return e;
+    e = enqueue_rows_head(m, batch, 1, 1, &n);
+    if (e != cudaSuccess) return e;
+    if (n_launched) *n_launched = n;
+    return cudaSuccess;
+}
+
+static cudaError_t capture_batch_graph(hq_model *m, int batch) {
+    if (m->batch_graph) { cudaGraphExecDestroy(m->batch_graph); m->batch_graph = nullptr; m->batch_graph_b = 0; }
+    cudaError_t e = cudaStreamBeginCapture(m->stream, cudaStreamCaptureModeThreadLocal);
+    if (e != cudaSuccess) return e;
+    int n = 0;
+    cudaError_t e_step = enqueue_batch_step(m, batch, &n);
+    cudaGraph_t g = nullptr;
+    e = cudaStreamEndCapture(m->stream, &g);
+    if (e_step != cudaSuccess) { if (g) cudaGraphDestroy(g); return e_step; }
+    if (e != cudaSuccess) return e;
+    e = cudaGraphInstantiate(&m->batch_graph, g, 0);
+    cudaGraphDestroy(g);
+    if (e != cudaSuccess) { m->batch_graph = nullptr; return e; }
+    m->batch_graph_b = batch;
+    m->batch_graph_kernels = n;
+    return cudaSuccess;
+}
+
+static bool build_tensor_maps(hq_model *m) {
+    const hq_config &c = m->cfg;
+    const Buffers &b = m->b;
+    const uint64_t d = c.hidden, qdim = (uint64_t)c.n_heads * kHeadDim, kvdim = (uint64_t)c.n_kv_heads * kHeadDim, F = c.ffn;
+    m->maps.resize(c.n_layers);
+    bool ok = true;
+    for (int l = 0; l < c.n_layers; ++l) {
+        const LayerW &w = m->layers[l];
+        LayerMaps &mp = m->maps[l];
+        ok = ok && make_tensor_map_16b(&mp.wq, w.wq, qdim, d, 128) && make_tensor_map_16b(&mp.wk, w.wk, kvdim, d, 128) &&
+             make_tensor_map_16b(&mp.wv, w.wv, kvdim, d, 128) && make_tensor_map_16b(&mp.wo, w.wo, d, qdim, 128) &&
+             make_tensor_map_16b(&mp.w_gate, w.w_gate, F, d, 128) && make_tensor_map_16b(&mp.w_up, w.w_up, F, d, 128) &&
+             make_tensor_map_16b(&mp.w_down, w.w_down, d, F, 128);
+    }
+    ok = ok && make_tensor_map_16b(&m->map_lm_head, m->lm_head, c.vocab, d, 128);
+    for (int i = 0; i < 4; ++i) {
+        const uint32_t nt = kTokenTiles[i];
+        ok = ok && make_tensor_map_16b(&m->map_hn[i], b.hn, 2 * (uint64_t)m->pf_rows, d, nt) &&
+             make_tensor_map_16b(&m->map_ao[i], b.ao, 2 * (uint64_t)m->pf_rows, qdim, nt) &&
+             make_tensor_map_16b(&m->map_actb[i], b.actb, 2 * (uint64_t)m->pf_rows, F, nt);
+    }
+    ok = ok && make_tensor_map_16b(&m->map_hn_last, b.hn_last, 64, d, 32);
+    return ok;
+}
+
 // ---- create / destroy ---------------------------------------------------------------------------------
 extern "C" int32_t hq_model_create(const hq_config *cfg, const hq_weights *w, void *workspace, size_t ws_bytes,
                                    void *cuda_stream, hq_model **out) {
@@ -227,6 +395,11 @@ extern "C" int32_t hq_model_create(const hq_config *cfg, const hq_weights *w, vo
         lw.w_up = (const bf16 *)w->w_up[l]; lw.w_down = (const bf16 *)w->w_down[l];
     }
     carve(cfg, (char *)workspace, &m->b);
+    m->pf_rows = (int)pass_rows(cfg);
+    if (!build_tensor_maps(m)) {
+        delete m;
+        return fail(HQ_ERR_CUDA, "hq_model_create: cuTensorMapEncodeTiled failed (driver entry point or bad alignment)");
+    }
     m->use_pdl = !(cfg->flags & HQ_FLAG_NO_PDL) && !getenv("HQ_NO_PDL");
 
     // RoPE table in double on the host (reading 7): angle = pos * theta^(-2i/64)
@@ -276,6 +449,7 @@ extern "C" int32_t hq_model_create(const hq_config *cfg, const hq_weights *w, vo
 extern "C" void hq_model_destroy(hq_model *m) {
     if (!m) return;
     if (m->step_graph) cudaGraphExecDestroy(m->step_graph);
+    if (m->batch_graph) cudaGraphExecDestroy(m->batch_graph);
     delete m;
 }
 
@@ -319,13 +493,34 @@ extern "C" int32_t hq_prefill(hq_model *m, const int32_t *tokens_host, int32_t b
     for (long long i = 0; i < (long long)batch * n_tokens; ++i)
         if (tokens_host[i] < 0 || tokens_host[i] >= c.vocab)
             return fail(HQ_ERR_INVALID_ARG, "hq_prefill: token %d at index %lld outside [0, %d)", tokens_host[i], i, c.vocab);
-    if (batch != 1) return fail(HQ_ERR_UNSUPPORTED, "hq_prefill: batch > 1 is not implemented yet");
-
-    HQ_CUDA(cudaMemcpyAsync(m->b.prompt, tokens_host, (size_t)n_tokens * sizeof(int), cudaMemcpyHostToDevice, m->stream));
-    for (int t = 0; t < n_tokens; ++t) {
-        int n = 0;
-        HQ_CUDA(enqueue_step(m, m->b.prompt + t, t == n_tokens - 1, &n));
-        m->kernel_count += n;
+    const LaunchCtx lc{m->stream, m->use_pdl, m->n_sms};
+    const bool capture = (c.flags & HQ_FLAG_CAPTURE_HIDDEN) != 0;
+    if (batch == 1 && (n_tokens < 8 || getenv("HQ_PREFILL_GEMV"))) {
+        // very short appends: walk the tokens with the batch-1 decode kernels
+        HQ_CUDA(cudaMemcpyAsync(m->b.prompt, tokens_host, (size_t)n_tokens * sizeof(int), cudaMemcpyHostToDevice, m->stream));
+        for (int t = 0; t < n_tokens; ++t) {
+            int n = 0;
+            HQ_CUDA(enqueue_step(m, m->b.prompt + t, t == n_tokens - 1, &n));
+            m->kernel_count += n;
+        }
+    } else {
+        // tensor-core passes of at most pf_rows token rows (all sequences together)
+        const int tc_max = m->pf_rows / batch;
+        for (int t0 = 0; t0 < n_tokens; t0 += tc_max) {
+            const int Tc = n_tokens - t0 < tc_max ? n_tokens - t0 : tc_max;
+            const bool last = t0 + Tc == n_tokens;
+            // rows m = b * Tc + t  <-  tokens_host[b][t0 + t]
+            HQ_CUDA(cudaMemcpy2DAsync(m->b.pf_tok, (size_t)Tc * sizeof(int), tokens_host + t0, (size_t)n_tokens * sizeof(int),
+                                      (size_t)Tc * sizeof(int), batch, cudaMemcpyHostToDevice, m->stream));
+            int n = 0;
+            HQ_CUDA(launch_embed_rows(lc, m->emb, m->b.pf_tok, m->b.xs, c.hidden, batch * Tc));
+            ++n;
+            HQ_CUDA(enqueue_rows_layers(m, batch, Tc, false, capture && last, &n));
+            HQ_CUDA(launch_advance(lc, m->b.pos, Tc));
+            ++n;
+            if (last) HQ_CUDA(enqueue_rows_head(m, batch, Tc, 0, &n));
+            m->kernel_count += n;
+        }
     }
     m->batch = batch;
     m->seq_len += n_tokens;
@@ -350,7 +545,24 @@ static int32_t decode_precheck(hq_model *m, const char *who, int n_steps) {
 }
 
 static int32_t launch_one_step(hq_model *m) {
-    if (m->step_graph) {
+    if (m->batch > 1) {
+        // batched decode (B1/B2): tensor-core GEMMs, weights read once per step for all sequences.
+        // The first step of a batch size runs eagerly (loads every kernel), the second captures a graph.
+        const bool want_graph = !(m->cfg.flags & HQ_FLAG_NO_GRAPH) && !getenv("HQ_NO_GRAPH") && m->stream != nullptr;
+        if (want_graph && m->batch_graph_b != m->batch && m->batch_eager_b == m->batch) {
+            cudaError_t e = capture_batch_graph(m, m->batch);
+            if (e != cudaSuccess) { cudaGetLastError(); m->batch_eager_b = -1; }   // stay eager
+        }
+        if (m->batch_graph && m->batch_graph_b == m->batch) {
+            HQ_CUDA(cudaGraphLaunch(m->batch_graph, m->stream));
+            m->kernel_count += m->batch_graph_kernels;
+        } else {
+            int n = 0;
+            HQ_CUDA(enqueue_batch_step(m, m->batch, &n));
+            m->kernel_count += n;
+            if (m->batch_eager_b != -1) m->batch_eager_b = m->batch;
+        }
+    } else if (m->step_graph) {
         HQ_CUDA(cudaGraphLaunch(m->step_graph, m->stream));
         m->kernel_count += m->kernels_per_step;
     } else {
@@ -482,5 +694,27 @@ extern "C" int32_t hq_bench_kernel(hq_model *m, int32_t which, int32_t reps, int
         m->kernel_count += 1;
     }
     if (bytes_per_launch) *bytes_per_launch = bytes;
+    return HQ_OK;
+}
+
+// ---- diagnostics: the tensor-core GEMM on its own ------------------------------------------------------
+extern "C" int32_t hq_debug_gemm(void *cuda_stream, int32_t mode, const void *w_dev, const void *w2_dev,
+                                 const void *x_dev, void *out_dev, int32_t n_rows, int32_t k, int32_t n_tokens,
+                                 int32_t token_tile, int32_t splits) {
+    if (!w_dev || !x_dev || !out_dev || n_rows <= 0 || k <= 0 || n_tokens <= 0)
+        return fail(HQ_ERR_INVALID_ARG, "hq_debug_gemm: bad argument");
+    if (mode < 0 || mode > 2 || (mode == 2 && !w2_dev)) return fail(HQ_ERR_INVALID_ARG, "hq_debug_gemm: bad mode");
+    if (token_tile != 32 && token_tile != 64 && token_tile != 128 && token_tile != 256)
+        return fail(HQ_ERR_INVALID_ARG, "hq_debug_gemm: token_tile must be 32, 64, 128 or 256");
+    if (k % 8 != 0) return fail(HQ_ERR_UNSUPPORTED, "hq_debug_gemm: k must be a multiple of 8");
+    TensorMap mw, mw2, mx;
+    // x_dev holds the hi plane [n_tokens][k] followed by the lo plane [n_tokens][k]
+    if (!make_tensor_map_16b(&mw, w_dev, n_rows, k, 128) || !make_tensor_map_16b(&mx, x_dev, 2 * (uint64_t)n_tokens, k, token_tile) ||
+        (mode == 2 && !make_tensor_map_16b(&mw2, w2_dev, n_rows, k, 128)))
+        return fail(HQ_ERR_CUDA, "hq_debug_gemm: cuTensorMapEncodeTiled failed");
+    const LaunchCtx lc{(cudaStream_t)cuda_stream, false, 148};
+    HQ_CUDA(launch_gemm(lc, (GemmEpilogue)mode, mw, mode == 2 ? &mw2 : nullptr, mx, n_tokens, n_rows, k, n_tokens, token_tile,
+                        mode == 2 ? 1 : splits, mode == 2 ? nullptr : (float *)out_dev, mode == 2 ? (act_t *)out_dev : nullptr,
+                        (size_t)n_tokens * n_rows, n_rows));
     return HQ_OK;
 }

@@ -1,0 +1,328 @@
+// hq_gemm.cu — tcgen05 / TMEM / TMA GEMM for envelope prefill and batched decode.
+//
+//   D[n, t] = sum_k W[n, k] * X[t, k]        W: bf16 weights [N, K] (nn.Linear layout, K-major)
+//                                            X: activations [T, K] (K-major) as two bf16 planes hi + lo (act_t)
+// "Swap-AB": the weight tile is the UMMA A operand (M = 128 weight rows), the token tile is the
+// B operand (UMMA N = NT tokens, 32..256), so the accumulator D lives in TMEM with one weight row
+// per lane and one token per column, and every weight byte is streamed from HBM exactly once per
+// token tile.  Both operands are staged by TMA (cp.async.bulk.tensor, SWIZZLE_128B, 64-element
+// K blocks) into an mbarrier ring; one elected thread issues tcgen05.mma; four epilogue warps
+// read TMEM with tcgen05.ld and apply the fused epilogue:
+//   EPI_STORE   out_f32[t][n]  = D            (split-K: atomic add into a zeroed buffer)
+//   EPI_RESID   x[t][n]       += D            (residual add; split-K partials add atomically)
+//   EPI_SWIGLU  act[t][f]      = hi/lo bf16 of silu(D_gate) * D_up   two accumulators, two weight maps
+// Warp roles (192 threads): warp 0 TMA producer, warp 1 TMEM owner + MMA issuer, warps 2-5 epilogue.
+#include <cuda.h>
+
+#include "hq_common.cuh"
+#include "hq_internal.h"
+
+namespace hq {
+
+constexpr int kGemmThreads = 192;
+constexpr int kBlockM = 128;  // weight rows per CTA (UMMA M)
+constexpr int kBlockK = 64;   // bf16 elements per K block = 128 bytes = one swizzle row
+
+// ---- PTX wrappers --------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbarrier_init(uint64_t *bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbarrier_expect_tx(uint64_t *bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbarrier_wait(uint64_t *bar, uint32_t parity) {
+    asm volatile(
+        "{\n\t.reg .pred P1;\n\tLAB_WAIT:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n\t"
+        "@P1 bra DONE;\n\tbra LAB_WAIT;\n\tDONE:\n\t}" ::"r"(smem_u32(bar)),
+        "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void tma_load_2d(const CUtensorMap *map, uint64_t *bar, void *smem_dst, int c0, int c1) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];" ::"r"(
+            smem_u32(smem_dst)),
+        "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1)
+        : "memory");
+}
+__device__ __forceinline__ void tcgen05_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tcgen05_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tcgen05_commit(uint64_t *bar) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+// D[tmem] (+)= A[smem desc] * B[smem desc]
+__device__ __forceinline__ void umma_bf16(uint32_t tmem_d, uint64_t desc_a, uint64_t desc_b, uint32_t idesc, uint32_t accumulate) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}" ::"r"(tmem_d),
+        "l"(desc_a), "l"(desc_b), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+// 32 lanes x 32 columns of fp32: thread (lane) gets 32 consecutive columns of its own TMEM lane
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+        "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]),
+          "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]), "=r"(v[16]),
+          "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]), "=r"(v[24]),
+          "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+        : "r"(taddr));
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+}
+
+// K-major, SWIZZLE_128B shared-memory matrix descriptor: rows of 128 bytes, 8-row groups 1024 bytes
+// apart (stride byte offset); leading byte offset unused for swizzled K-major; descriptor version 1.
+__device__ __forceinline__ uint64_t make_smem_desc(uint32_t smem_addr) {
+    uint64_t d = 0;
+    d |= (uint64_t)((smem_addr & 0x3FFFF) >> 4);        // start address, bits [0,14)
+    d |= (uint64_t)(1024 >> 4) << 32;                   // stride byte offset, bits [32,46)
+    d |= (uint64_t)1 << 46;                             // version = 1 (sm_100)
+    d |= (uint64_t)2 << 61;                             // layout type SWIZZLE_128B
+    return d;
+}
+// kind::f16 instruction descriptor: D fp32 (bits 4-5 = 1), A and B bf16 (bits 7-9 and 10-12 = 1; the two
+// formats must match: a bf16 x fp16 descriptor raises an illegal-instruction fault on sm_100a), both K-major
+// (bits 15, 16 = 0), N >> 3 at bits 17-22, M >> 4 at bits 24-28
+__host__ __device__ inline uint32_t make_idesc(int n) {
+    return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(kBlockM >> 4) << 24);
+}
+
+template <int MODE>
+__global__ void __launch_bounds__(kGemmThreads, 1)
+gemm_tc_kernel(const __grid_constant__ CUtensorMap map_w, const __grid_constant__ CUtensorMap map_w2,
+               const __grid_constant__ CUtensorMap map_x, const GemmParams p) {
+    extern __shared__ __align__(1024) uint8_t smem_raw[];
+    constexpr int NACC = (MODE == EPI_SWIGLU) ? 2 : 1;
+    const int NT = p.NT;
+    const uint32_t a_bytes = kBlockM * kBlockK * 2;          // 16 KB per weight tile
+    const uint32_t b_bytes = (uint32_t)NT * kBlockK * 2;      // one plane (hi or lo) of the token tile
+    const uint32_t stage_bytes = NACC * a_bytes + 2 * b_bytes;
+    const int stages = p.stages;
+
+    uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+    uint64_t *full_bar = reinterpret_cast<uint64_t *>(smem + (size_t)stages * stage_bytes);
+    uint64_t *empty_bar = full_bar + stages;
+    uint64_t *acc_bar = empty_bar + stages;
+    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(acc_bar + 1);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int n0 = blockIdx.x * kBlockM;           // first weight row of this CTA
+    const int t0 = blockIdx.y * NT;                // first token of this CTA
+    const int kb0 = blockIdx.z * p.k_blocks_per_split;
+    const int kb1 = min(kb0 + p.k_blocks_per_split, p.k_blocks);
+    const int nkb = kb1 - kb0;
+    const uint32_t tmem_cols = (NACC * NT <= 32) ? 32 : (NACC * NT <= 64) ? 64 : (NACC * NT <= 128) ? 128
+                               : (NACC * NT <= 256) ? 256 : 512;
+
+    if (warp == 0 && lane == 0) {
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&map_w) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&map_x) : "memory");
+        if (NACC == 2) asm volatile("prefetch.tensormap [%0];" ::"l"(&map_w2) : "memory");
+        for (int s = 0; s < stages; ++s) {
+            mbarrier_init(&full_bar[s], 1);
+            mbarrier_init(&empty_bar[s], 1);
+        }
+        mbarrier_init(acc_bar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 1) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "r"(tmem_cols) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    tcgen05_fence_before();
+    __syncthreads();
+    tcgen05_fence_after();
+    const uint32_t tmem_base = *tmem_slot;
+
+    pdl_launch_dependents();
+    pdl_wait();   // activations (and, for atomics/residual, the output buffer) come from earlier kernels
+
+    if (warp == 0) {
+        // ===== TMA producer =====
+        if (lane == 0) {
+            for (int i = 0; i < nkb; ++i) {
+                const int s = i % stages;
+                const uint32_t ph = (i / stages) & 1;
+                mbarrier_wait(&empty_bar[s], ph ^ 1);
+                uint8_t *st = smem + (size_t)s * stage_bytes;
+                mbarrier_expect_tx(&full_bar[s], stage_bytes);
+                const int kc = (kb0 + i) * kBlockK;
+                tma_load_2d(&map_w, &full_bar[s], st, kc, n0);
+                if (NACC == 2) tma_load_2d(&map_w2, &full_bar[s], st + a_bytes, kc, n0);
+                tma_load_2d(&map_x, &full_bar[s], st + NACC * a_bytes, kc, t0);
+                tma_load_2d(&map_x, &full_bar[s], st + NACC * a_bytes + b_bytes, kc, p.x_lo_row + t0);
+            }
+        }
+    } else if (warp == 1) {
+        // ===== MMA issuer (one elected thread) =====
+        if (lane == 0) {
+            const uint32_t idesc = make_idesc(NT);
+            for (int i = 0; i < nkb; ++i) {
+                const int s = i % stages;
+                const uint32_t ph = (i / stages) & 1;
+                mbarrier_wait(&full_bar[s], ph);
+                tcgen05_fence_after();
+                const uint32_t a_addr = smem_u32(smem + (size_t)s * stage_bytes);
+                const uint32_t b_addr = a_addr + NACC * a_bytes;
+                const uint64_t da = make_smem_desc(a_addr), db = make_smem_desc(b_addr);
+                const uint64_t da2 = make_smem_desc(a_addr + a_bytes), dbl = make_smem_desc(b_addr + b_bytes);
+#pragma unroll
+                for (int k = 0; k < kBlockK / 16; ++k) {
+                    const uint32_t acc = (i > 0 || k > 0) ? 1u : 0u;
+                    // advance 16 elements = 32 bytes inside the 128-byte swizzle row: +2 in the >>4 address field
+                    umma_bf16(tmem_base, da + 2 * k, db + 2 * k, idesc, acc);       // W * x_hi
+                    umma_bf16(tmem_base, da + 2 * k, dbl + 2 * k, idesc, 1u);       // W * x_lo
+                    if (NACC == 2) {
+                        umma_bf16(tmem_base + NT, da2 + 2 * k, db + 2 * k, idesc, acc);
+                        umma_bf16(tmem_base + NT, da2 + 2 * k, dbl + 2 * k, idesc, 1u);
+                    }
+                }
+                tcgen05_commit(&empty_bar[s]);   // frees the smem stage when these MMAs retire
+            }
+            tcgen05_commit(acc_bar);             // accumulator complete
+        }
+    } else {
+        // ===== epilogue: warp w owns TMEM lanes 32*(w%4) .. +31 =====
+        const int q = warp & 3;
+        const int n = n0 + 32 * q + lane;
+        mbarrier_wait(acc_bar, 0);
+        tcgen05_fence_after();
+        const uint32_t lane_addr = tmem_base + ((uint32_t)(32 * q) << 16);
+        const bool row_ok = n < p.n_rows;
+        for (int c = 0; c < NT; c += 32) {
+            uint32_t v[32];
+            tmem_ld32(lane_addr + c, v);
+            if (MODE == EPI_SWIGLU) {
+                uint32_t u[32];
+                tmem_ld32(lane_addr + NT + c, u);
+                if (row_ok) {
+#pragma unroll
+                    for (int j = 0; j < 32; ++j) {
+                        const int t = t0 + c + j;
+                        if (t < p.T) {
+                            act_t hi, lo;
+                            split_bf16(silu_f(__uint_as_float(v[j])) * __uint_as_float(u[j]), hi, lo);
+                            p.out_act[(size_t)t * p.ld_out + n] = hi;
+                            p.out_act[p.out_lo_offset + (size_t)t * p.ld_out + n] = lo;
+                        }
+                    }
+                }
+            } else if (row_ok) {
+#pragma unroll
+                for (int j = 0; j < 32; ++j) {
+                    const int t = t0 + c + j;
+                    if (t < p.T) {
+                        float *dst = p.out_f32 + (size_t)t * p.ld_out + n;
+                        const float val = __uint_as_float(v[j]);
+                        if (p.atomic) atomicAdd(dst, val);
+                        else if (MODE == EPI_RESID) *dst = __ldcg(dst) + val;
+                        else *dst = val;
+                    }
+                }
+            }
+        }
+        tcgen05_fence_before();
+    }
+    __syncthreads();
+    if (warp == 1) {
+        tcgen05_fence_after();
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(tmem_cols) : "memory");
+    }
+}
+
+// ---- host side -----------------------------------------------------------------------------------------
+typedef CUresult (*PFN_encodeTiled)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                    const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static PFN_encodeTiled get_encode() {
+    static PFN_encodeTiled fn = nullptr;
+    if (!fn) {
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = (PFN_encodeTiled)p;
+    }
+    return fn;
+}
+
+// 2-D tensor of 16-bit elements [rows][cols] row-major, box = box_rows x 64 columns, 128-byte swizzle
+// (weights, and the stacked hi/lo planes of an activation buffer).
+bool make_tensor_map_16b(TensorMap *out, const void *base, uint64_t rows, uint64_t cols, uint32_t box_rows) {
+    PFN_encodeTiled enc = get_encode();
+    if (!enc) return false;
+    static_assert(sizeof(TensorMap) == sizeof(CUtensorMap), "TensorMap must mirror CUtensorMap");
+    cuuint64_t dims[2] = {cols, rows};
+    cuuint64_t strides[1] = {cols * 2};
+    cuuint32_t box[2] = {(cuuint32_t)kBlockK, box_rows};
+    cuuint32_t estr[2] = {1, 1};
+    CUresult r = enc(reinterpret_cast<CUtensorMap *>(out), CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void *>(base),
+                     dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                     CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS;
+}
+
+static const int kSmemBudget = 200 * 1024;
+
+template <int MODE>
+static cudaError_t launch_mode(const LaunchCtx &c, const TensorMap &w, const TensorMap &w2, const TensorMap &x,
+                               GemmParams p, int n_tiles, int t_tiles, int splits) {
+    const int nacc = (MODE == EPI_SWIGLU) ? 2 : 1;
+    const int stage_bytes = nacc * kBlockM * kBlockK * 2 + 2 * p.NT * kBlockK * 2;
+    int stages = kSmemBudget / stage_bytes;
+    if (stages > 8) stages = 8;
+    if (stages > p.k_blocks_per_split) stages = p.k_blocks_per_split < 2 ? 2 : p.k_blocks_per_split;
+    p.stages = stages;
+    const size_t smem = (size_t)stages * stage_bytes + 1024 + (2 * stages + 1) * 8 + 16;
+    static bool attr_done = false;
+    if (!attr_done) {
+        cudaError_t e = cudaFuncSetAttribute(gemm_tc_kernel<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+        if (e != cudaSuccess) return e;
+        attr_done = true;
+    }
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(n_tiles, t_tiles, splits);
+    cfg.blockDim = dim3(kGemmThreads);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = c.stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = c.pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, gemm_tc_kernel<MODE>, *reinterpret_cast<const CUtensorMap *>(&w),
+                              *reinterpret_cast<const CUtensorMap *>(&w2), *reinterpret_cast<const CUtensorMap *>(&x), p);
+}
+
+// n_rows: weight rows (output features; for EPI_SWIGLU the ffn size), K: reduction size (multiple of 64),
+// T: valid tokens, NT: token tile (32/64/128/256).  splits > 1 requires atomic accumulation (EPI_STORE into a
+// zeroed buffer, EPI_RESID always legal).
+cudaError_t launch_gemm(const LaunchCtx &c, GemmEpilogue mode, const TensorMap &w, const TensorMap *w2,
+                        const TensorMap &x, int x_lo_row, int n_rows, int K, int T, int NT, int splits, float *out_f32,
+                        act_t *out_act, size_t out_lo_offset, int ld_out) {
+    // K need not be a multiple of 64: TMA zero-fills the out-of-range tail of the last K block
+    if (K % 8 != 0 || NT % 32 != 0 || NT < 32 || NT > 256 || T <= 0) return cudaErrorInvalidValue;
+    const int kblocks = (K + kBlockK - 1) / kBlockK;
+    if (splits < 1) splits = 1;
+    if (splits > kblocks) splits = kblocks;
+    GemmParams p = {};
+    p.K = K; p.n_rows = n_rows; p.T = T; p.NT = NT; p.k_blocks = kblocks;
+    p.k_blocks_per_split = (kblocks + splits - 1) / splits;
+    splits = (kblocks + p.k_blocks_per_split - 1) / p.k_blocks_per_split;
+    p.out_f32 = out_f32; p.out_act = out_act; p.out_lo_offset = out_lo_offset; p.x_lo_row = x_lo_row; p.ld_out = ld_out; p.atomic = splits > 1 ? 1 : 0;
+    const int n_tiles = (n_rows + kBlockM - 1) / kBlockM, t_tiles = (T + NT - 1) / NT;
+    switch (mode) {
+        case EPI_STORE: return launch_mode<EPI_STORE>(c, w, w, x, p, n_tiles, t_tiles, splits);
+        case EPI_RESID: return launch_mode<EPI_RESID>(c, w, w, x, p, n_tiles, t_tiles, splits);
+        case EPI_SWIGLU:
+            if (splits != 1 || !w2) return cudaErrorInvalidValue;
+            return launch_mode<EPI_SWIGLU>(c, w, *w2, x, p, n_tiles, t_tiles, 1);
+    }
+    return cudaErrorInvalidValue;
+}
+
+}  // namespace hq

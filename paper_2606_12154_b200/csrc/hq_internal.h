@@ -18,11 +18,20 @@ typedef __nv_bfloat16 bf16;
 // random-weight model; K/V magnitudes here are O(1..10), far from
 // the fp16 range limit.
 typedef __half kv_t;
+// Activation operands of the tensor-core GEMMs are bf16 like the weights (tcgen05 kind::f16 rejects
+// mixed fp16 x bf16 operands: illegal instruction on sm_100a), but a single bf16 rounding of the
+// activations drifts the per-layer hidden state of the 1B model past the 1e-2 tolerance by layer 5
+// (measured 1.04e-2).  So every activation operand is stored as TWO bf16 planes, x = hi + lo with
+// hi = bf16(x), lo = bf16(x - hi) (16 mantissa bits), and every K step issues two MMAs into the same
+// accumulator.  Plane layout: [2][rows][K], lo plane `rows` rows below the hi plane.
+typedef __nv_bfloat16 act_t;
 
 constexpr int kHeadDim = 64;        // only head_dim the kernels implement
 constexpr int kMaxSplits = 16;      // split-KV partials per head (decode attention)
 constexpr int kMinSplitLen = 64;    // do not split contexts shorter than this per split
 constexpr int kGemvThreads = 256;
+
+struct alignas(64) TensorMap { uint64_t opaque[16]; };   // mirrors CUtensorMap (driver type, 128 bytes)
 
 struct LayerW {
     const bf16 *attn_norm, *wq, *wk, *wv, *wo, *ffn_norm, *w_gate, *w_up, *w_down;
@@ -46,7 +55,20 @@ struct Buffers {
     float *logits = nullptr;                    // [B][V]
     float *hidden = nullptr;                    // [L][B][d] (capture flag)
     int *prompt = nullptr;                      // [B][Tmax] staged prompt tokens
+    // row-batched (tensor-core) path: rows m = b * Tc + t of one pass, at most pf_rows of them
+    int *pf_tok = nullptr;                      // [pf_rows]
+    int *last_idx = nullptr;                    // [B] row of the last position of every sequence
+    float *xs = nullptr;                        // [pf_rows][d] residual stream
+    act_t *hn = nullptr;                        // [2][pf_rows][d] normalised hidden (GEMM operand, hi/lo)
+    float *qkv = nullptr;                       // [pf_rows][(H+2Hkv)*64]
+    __half *q16 = nullptr;                      // [pf_rows][H*64] rotated queries
+    act_t *ao = nullptr;                        // [2][pf_rows][H*64] attention output (GEMM operand, hi/lo)
+    act_t *actb = nullptr;                      // [2][pf_rows][F] SwiGLU output (GEMM operand, hi/lo)
+    act_t *hn_last = nullptr;                   // [2][32][d] normalised last rows (LM-head operand, hi/lo)
 };
+
+constexpr int kTokenTiles[4] = {32, 64, 128, 256};
+struct LayerMaps { TensorMap wq, wk, wv, wo, w_gate, w_up, w_down; };
 
 struct hq_model_impl {
     hq_config cfg;
@@ -62,6 +84,13 @@ struct hq_model_impl {
     long long kernel_count = 0;
     int kernels_per_step = 0;
     bool use_pdl = true;
+    // tensor-core path
+    int pf_rows = 0;                            // row capacity of one pass
+    std::vector<LayerMaps> maps;
+    TensorMap map_lm_head;
+    TensorMap map_hn[4], map_ao[4], map_actb[4], map_hn_last;   // activation maps per token tile
+    cudaGraphExec_t batch_graph = nullptr;      // batched decode step (captured for batch_graph_b)
+    int batch_graph_b = 0, batch_graph_kernels = 0, batch_eager_b = 0;
 };
 
 // ---- parameter blocks --------------------------------------------------------------------------------
@@ -110,12 +139,43 @@ __host__ __device__ inline int attn_split_len(int n_ctx, int n_splits) {
     return (c + 15) & ~15;  // 16-position granules
 }
 
-// ---- launchers (hq_decode.cu) ------------------------------------------------------------------------
 struct LaunchCtx {
     cudaStream_t stream;
     bool pdl;
     int n_sms;
 };
+
+// ---- tensor-core GEMM (hq_gemm.cu) -------------------------------------------------------------------
+enum GemmEpilogue { EPI_STORE = 0, EPI_RESID = 1, EPI_SWIGLU = 2 };
+struct GemmParams {
+    int K, n_rows, T, NT, k_blocks, k_blocks_per_split, stages;
+    float *out_f32;
+    act_t *out_act;     // hi plane; lo plane at out_act + out_lo_offset
+    size_t out_lo_offset;
+    int ld_out;
+    int atomic;
+    int x_lo_row;       // row offset of the lo plane inside the activation tensor map
+};
+bool make_tensor_map_16b(TensorMap *out, const void *base, uint64_t rows, uint64_t cols, uint32_t box_rows);
+cudaError_t launch_gemm(const LaunchCtx &c, GemmEpilogue mode, const TensorMap &w, const TensorMap *w2,
+                        const TensorMap &x, int x_lo_row, int n_rows, int K, int T, int NT, int splits, float *out_f32,
+                        act_t *out_act, size_t out_lo_offset, int ld_out);
+
+// ---- row-batched kernels (hq_prefill.cu) -------------------------------------------------------------
+cudaError_t launch_embed_rows(const LaunchCtx &c, const bf16 *emb, const int *tok, float *x, int hidden, int rows);
+cudaError_t launch_rmsnorm_rows(const LaunchCtx &c, const float *x, const bf16 *gain, act_t *out, size_t lo_offset,
+                                int hidden, float eps, int rows, const int *row_index, int x_stride_rows);
+cudaError_t launch_rope_append(const LaunchCtx &c, const float *qkv, __half *q16, float *q32, kv_t *kc, kv_t *vc,
+                               const float2 *rope, const int *pos, int rows, int Tc, int n_heads, int n_kv_heads,
+                               int max_seq);
+cudaError_t launch_flash_prefill(const LaunchCtx &c, const __half *q16, const kv_t *kc, const kv_t *vc, act_t *out,
+                                 size_t lo_offset, const int *pos, int batch, int Tc, int n_heads, int n_kv_heads, int max_seq);
+cudaError_t launch_attn_combine(const LaunchCtx &c, const float *part_o, const float2 *part_ml, act_t *out,
+                                size_t lo_offset, const int *pos, int batch, int n_heads);
+cudaError_t launch_argmax_rows(const LaunchCtx &c, const float *logits, int vocab, int batch, int *cur_tok,
+                               int *tok_hist, int *pos, int pos_inc, unsigned int *counter);
+
+// ---- launchers (hq_decode.cu) ------------------------------------------------------------------------
 cudaError_t launch_embed(const LaunchCtx &c, const bf16 *emb, const int *tok, float *x, int hidden, int batch);
 cudaError_t launch_gemv(const LaunchCtx &c, GemvMode mode, GemvInput xin, const GemvParams &p);
 cudaError_t launch_attn_decode(const LaunchCtx &c, const AttnDecodeParams &p, int batch);

@@ -1,0 +1,423 @@
+// hq_prefill.cu — row-batched kernels around the tcgen05 GEMMs: envelope prefill (SURVEY.md §8(a)
+// P2-P4) and batched decode (B1-B2).  "Rows" are tokens m = b * Tc + t of the current pass.
+//   embed_rows      x[m] = float(E[tok[m]])                                          (A1 for many rows)
+//   rmsnorm_rows    hn[m] = hi/lo bf16 of x[m] * rsqrt(mean(x[m]^2) + eps) * g       (tensor-core operand)
+//   rope_append     qkv fp32 -> RoPE(q) as fp16 (+ fp32 copy for decode), RoPE(k), v -> fp16 KV cache   (P4)
+//   flash_prefill   causal GQA flash attention, mma.sync m16n8k16 fp16, fp32 online softmax           (P2)
+//   attn_combine    merge split-KV partials of the decode attention -> o hi/lo bf16                         (B2)
+//   argmax_rows     greedy token per sequence from fp32 logits + device-resident step state           (A9/B1)
+#include "hq_common.cuh"
+#include "hq_internal.h"
+
+namespace hq {
+
+// =====================================================================================================
+__global__ void __launch_bounds__(256) embed_rows_kernel(const bf16 *__restrict__ emb, const int *tok,
+                                                         float *__restrict__ x, int hidden) {
+    pdl_launch_dependents();
+    pdl_wait();
+    const int m = blockIdx.x;
+    const bf16 *row = emb + (size_t)ld_act(tok + m) * hidden;
+    for (int c = threadIdx.x; c < (hidden >> 3); c += blockDim.x) {
+        const uint4 w = ld_weight16(row + c * 8);
+        float4 *dst = reinterpret_cast<float4 *>(x + (size_t)m * hidden + c * 8);
+        dst[0] = make_float4(bf16lo(w.x), bf16hi(w.x), bf16lo(w.y), bf16hi(w.y));
+        dst[1] = make_float4(bf16lo(w.z), bf16hi(w.z), bf16lo(w.w), bf16hi(w.w));
+    }
+}
+
+// one CTA per row; x row stays in L1/L2 between the two passes
+__global__ void __launch_bounds__(256) rmsnorm_rows_kernel(const float *x, const bf16 *__restrict__ gain,
+                                                           act_t *__restrict__ out, size_t lo_offset, int hidden,
+                                                           float eps, const int *row_index, int x_stride_rows) {
+    pdl_launch_dependents();
+    pdl_wait();
+    __shared__ float red[8];
+    const int m = blockIdx.x;
+    // row_index (optional) gathers rows (e.g. last position of every sequence)
+    const size_t src = row_index ? (size_t)row_index[m] : (size_t)m;
+    const float *xr = x + src * x_stride_rows;
+    float ss = 0.f;
+    for (int c = threadIdx.x; c < (hidden >> 2); c += blockDim.x) {
+        const float4 v = ld_act4(xr + c * 4);
+        ss += v.x * v.x + v.y * v.y + v.z * v.z + v.w * v.w;
+    }
+    ss = warp_sum(ss);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = ss;
+    __syncthreads();
+    float tot = 0.f;
+#pragma unroll
+    for (int w = 0; w < 8; ++w) tot += red[w];
+    const float inv = 1.0f / sqrtf(tot / (float)hidden + eps);
+    for (int c = threadIdx.x; c < (hidden >> 2); c += blockDim.x) {
+        const float4 v = ld_act4(xr + c * 4);
+        const uint2 g = *reinterpret_cast<const uint2 *>(gain + c * 4);
+        uint2 oh, ol;
+        split_bf16x2(v.x * inv * bf16lo(g.x), v.y * inv * bf16hi(g.x), oh.x, ol.x);
+        split_bf16x2(v.z * inv * bf16lo(g.y), v.w * inv * bf16hi(g.y), oh.y, ol.y);
+        *reinterpret_cast<uint2 *>(out + (size_t)m * hidden + c * 4) = oh;
+        *reinterpret_cast<uint2 *>(out + lo_offset + (size_t)m * hidden + c * 4) = ol;
+    }
+}
+
+// qkv fp32 [M][(H + 2 Hkv) * 64] -> q (fp16 [M][H*64], optional fp32 copy), K/V cache rows.
+// grid (M), block 256: thread handles (head-any hh, i) pairs in a loop.
+__global__ void __launch_bounds__(256) rope_append_kernel(const float *qkv, __half *q16, float *q32, kv_t *kc, kv_t *vc,
+                                                          const float2 *__restrict__ rope, const int *pos_ptr, int Tc,
+                                                          int n_heads, int n_kv_heads, int max_seq) {
+    pdl_launch_dependents();
+    pdl_wait();
+    const int m = blockIdx.x;
+    const int b = m / Tc, t = m % Tc;
+    const int pos = ld_act(pos_ptr) + t;
+    const int nh = n_heads + 2 * n_kv_heads;
+    const float *src = qkv + (size_t)m * nh * kHeadDim;
+    for (int idx = threadIdx.x; idx < nh * 32; idx += blockDim.x) {
+        const int hh = idx >> 5, i = idx & 31;
+        const float a = ld_act(src + hh * kHeadDim + i), c = ld_act(src + hh * kHeadDim + i + 32);
+        if (hh < n_heads + n_kv_heads) {
+            const float2 cs = rope[(size_t)pos * 32 + i];
+            const float ra = a * cs.x - c * cs.y, rc = c * cs.x + a * cs.y;
+            if (hh < n_heads) {
+                const size_t o = ((size_t)m * n_heads + hh) * kHeadDim + i;
+                q16[o] = __float2half_rn(ra);
+                q16[o + 32] = __float2half_rn(rc);
+                if (q32) { q32[o] = ra; q32[o + 32] = rc; }
+            } else {
+                kv_t *dst = kc + (((size_t)b * n_kv_heads + (hh - n_heads)) * max_seq + pos) * kHeadDim;
+                dst[i] = __float2half_rn(ra);
+                dst[i + 32] = __float2half_rn(rc);
+            }
+        } else {
+            kv_t *dst = vc + (((size_t)b * n_kv_heads + (hh - n_heads - n_kv_heads)) * max_seq + pos) * kHeadDim;
+            dst[i] = __float2half_rn(a);
+            dst[i + 32] = __float2half_rn(c);
+        }
+    }
+}
+
+// =====================================================================================================
+// P2: causal flash attention for a pass of Tc query positions per sequence starting at position p0.
+// grid (ceil(Tc/64), H, B), 128 threads: warp w owns query rows 16w..16w+15 of the 64-row tile.
+// =====================================================================================================
+constexpr int kFaTile = 64;
+
+__device__ __forceinline__ void cp_async16(void *smem_dst, const void *gmem_src, bool valid) {
+    const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
+    const int sz = valid ? 16 : 0;   // src-size 0 -> zero fill
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(d), "l"(gmem_src), "r"(sz) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+__device__ __forceinline__ void ldmatrix_x4(uint32_t (&r)[4], const void *smem) {
+    const uint32_t a = (uint32_t)__cvta_generic_to_shared(smem);
+    asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(a));
+}
+__device__ __forceinline__ void ldmatrix_x4_trans(uint32_t (&r)[4], const void *smem) {
+    const uint32_t a = (uint32_t)__cvta_generic_to_shared(smem);
+    asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(a));
+}
+__device__ __forceinline__ void mma_f16(float (&d)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1) {
+    asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+                 : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
+                 : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
+}
+// element (row, col) of a [64][64] fp16 tile with 16-byte chunks XOR-swizzled by the row
+__device__ __forceinline__ __half *tile_ptr(__half *tile, int row, int col) {
+    return tile + row * 64 + ((((col >> 3) ^ (row & 7)) << 3) | (col & 7));
+}
+__device__ __forceinline__ uint32_t pack_half2(float a, float b) {
+    __half2 h = __floats2half2_rn(a, b);
+    return *reinterpret_cast<uint32_t *>(&h);
+}
+
+__global__ void __launch_bounds__(128) flash_prefill_kernel(const __half *q16, const kv_t *kc, const kv_t *vc,
+                                                            act_t *out, size_t lo_offset, const int *pos_ptr, int Tc,
+                                                            int n_heads,
+                                                            int n_kv_heads, int max_seq) {
+    __shared__ __align__(128) __half Qs[kFaTile * 64];
+    __shared__ __align__(128) __half Ks[2][kFaTile * 64];
+    __shared__ __align__(128) __half Vs[2][kFaTile * 64];
+    pdl_launch_dependents();
+    pdl_wait();
+
+    const int qt = blockIdx.x, h = blockIdx.y, b = blockIdx.z;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int g = lane >> 2, tig = lane & 3;
+    const int p0 = ld_act(pos_ptr);
+    const int kvh = h / (n_heads / n_kv_heads);
+    const int q_lo = qt * kFaTile;                        // first local query of the tile
+    const int q_hi = min(Tc, q_lo + kFaTile);             // one past the last valid local query
+    const int n_keys = p0 + q_hi;                         // keys 0 .. n_keys-1 can be visible
+    const int n_kt = (n_keys + kFaTile - 1) / kFaTile;
+    const kv_t *kg = kc + ((size_t)b * n_kv_heads + kvh) * max_seq * kHeadDim;
+    const kv_t *vg = vc + ((size_t)b * n_kv_heads + kvh) * max_seq * kHeadDim;
+
+    auto load_kv = [&](int buf, int kt) {
+        for (int c = threadIdx.x; c < kFaTile * 8; c += 128) {
+            const int r = c >> 3, ch = c & 7;
+            const int key = kt * kFaTile + r;
+            const bool ok = key < n_keys;
+            const size_t off = (size_t)(ok ? key : 0) * kHeadDim + ch * 8;
+            cp_async16(tile_ptr(Ks[buf], r, ch * 8), kg + off, ok);
+            cp_async16(tile_ptr(Vs[buf], r, ch * 8), vg + off, ok);
+        }
+    };
+    // Q tile
+    for (int c = threadIdx.x; c < kFaTile * 8; c += 128) {
+        const int r = c >> 3, ch = c & 7;
+        const bool ok = q_lo + r < Tc;
+        const size_t m = (size_t)b * Tc + (ok ? q_lo + r : 0);
+        cp_async16(tile_ptr(Qs, r, ch * 8), q16 + (m * n_heads + h) * kHeadDim + ch * 8, ok);
+    }
+    load_kv(0, 0);
+    cp_async_commit();
+    cp_async_wait<0>();
+    __syncthreads();
+
+    // Q fragments: 4 k-steps (dims 16kk..16kk+15) for rows 16*warp .. +15
+    uint32_t qf[4][4];
+#pragma unroll
+    for (int kk = 0; kk < 4; ++kk)
+        ldmatrix_x4(qf[kk], tile_ptr(Qs, 16 * warp + (lane & 15), kk * 16 + (lane >> 4) * 8));
+
+    float o[8][4];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) { o[j][0] = o[j][1] = o[j][2] = o[j][3] = 0.f; }
+    float m_run[2] = {-INFINITY, -INFINITY}, l_run[2] = {0.f, 0.f};
+    const float sl2 = 0.125f * 1.4426950408889634f;       // softmax scale * log2(e)
+    const int qpos0 = p0 + q_lo + 16 * warp + g;           // global position of fragment row g (row g+8: +8)
+
+    for (int kt = 0; kt < n_kt; ++kt) {
+        const int buf = kt & 1;
+        if (kt + 1 < n_kt) load_kv(buf ^ 1, kt + 1);
+        cp_async_commit();
+        // S = Q K^T for 64 keys: 8 n-tiles of 8 keys
+        float s[8][4];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) { s[j][0] = s[j][1] = s[j][2] = s[j][3] = 0.f; }
+#pragma unroll
+        for (int kk = 0; kk < 4; ++kk) {
+#pragma unroll
+            for (int jp = 0; jp < 4; ++jp) {   // pairs of n-tiles
+                uint32_t kf[4];
+                const int mi = lane >> 3;
+                ldmatrix_x4(kf, tile_ptr(Ks[buf], jp * 16 + (mi >> 1) * 8 + (lane & 7), kk * 16 + (mi & 1) * 8));
+                mma_f16(s[2 * jp], qf[kk], kf[0], kf[1]);
+                mma_f16(s[2 * jp + 1], qf[kk], kf[2], kf[3]);
+            }
+        }
+        // causal mask + online softmax (rows g and g+8 of this warp's 16)
+        const int key0 = kt * kFaTile;
+        float mx[2] = {m_run[0], m_run[1]};
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                const int key = key0 + j * 8 + tig * 2 + (e & 1);
+                const int qp = qpos0 + (e >> 1) * 8;
+                if (key > qp) s[j][e] = -INFINITY;
+                mx[e >> 1] = fmaxf(mx[e >> 1], s[j][e]);
+            }
+        }
+#pragma unroll
+        for (int r = 0; r < 2; ++r) {
+            mx[r] = fmaxf(mx[r], __shfl_xor_sync(0xffffffffu, mx[r], 1));
+            mx[r] = fmaxf(mx[r], __shfl_xor_sync(0xffffffffu, mx[r], 2));
+        }
+        float corr[2], rs[2] = {0.f, 0.f};
+#pragma unroll
+        for (int r = 0; r < 2; ++r) {
+            // a fully masked row (padding rows beyond Tc) keeps m = -inf: use 0 to avoid inf - inf
+            const float mref = (mx[r] == -INFINITY) ? 0.f : mx[r];
+            corr[r] = exp2f((m_run[r] - mref) * sl2);
+            m_run[r] = mx[r];
+            mx[r] = mref;
+        }
+        uint32_t pf[4][4];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            const float p0v = exp2f((s[j][0] - mx[0]) * sl2), p1v = exp2f((s[j][1] - mx[0]) * sl2);
+            const float p2v = exp2f((s[j][2] - mx[1]) * sl2), p3v = exp2f((s[j][3] - mx[1]) * sl2);
+            rs[0] += p0v + p1v;
+            rs[1] += p2v + p3v;
+            pf[j >> 1][(j & 1) * 2 + 0] = pack_half2(p0v, p1v);
+            pf[j >> 1][(j & 1) * 2 + 1] = pack_half2(p2v, p3v);
+        }
+#pragma unroll
+        for (int r = 0; r < 2; ++r) {
+            rs[r] += __shfl_xor_sync(0xffffffffu, rs[r], 1);
+            rs[r] += __shfl_xor_sync(0xffffffffu, rs[r], 2);
+            l_run[r] = l_run[r] * corr[r] + rs[r];
+        }
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            o[j][0] *= corr[0]; o[j][1] *= corr[0]; o[j][2] *= corr[1]; o[j][3] *= corr[1];
+        }
+        // O += P V : k-steps over keys (16 each), n-tiles over dims
+#pragma unroll
+        for (int kk = 0; kk < 4; ++kk) {
+#pragma unroll
+            for (int jp = 0; jp < 4; ++jp) {
+                uint32_t vf[4];
+                const int mi = lane >> 3;
+                ldmatrix_x4_trans(vf, tile_ptr(Vs[buf], kk * 16 + (mi & 1) * 8 + (lane & 7), jp * 16 + (mi >> 1) * 8));
+                mma_f16(o[2 * jp], pf[kk], vf[0], vf[1]);
+                mma_f16(o[2 * jp + 1], pf[kk], vf[2], vf[3]);
+            }
+        }
+        cp_async_wait<0>();
+        __syncthreads();
+    }
+
+    // normalise and store o as hi/lo bf16 planes [m][H*64]
+#pragma unroll
+    for (int r = 0; r < 2; ++r) {
+        const int ql = q_lo + 16 * warp + g + r * 8;
+        if (ql < Tc) {
+            const float inv = 1.0f / l_run[r];
+            act_t *dst = out + (((size_t)b * Tc + ql) * n_heads + h) * kHeadDim;
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                uint32_t vh, vl;
+                split_bf16x2(o[j][2 * r] * inv, o[j][2 * r + 1] * inv, vh, vl);
+                *reinterpret_cast<uint32_t *>(dst + j * 8 + tig * 2) = vh;
+                *reinterpret_cast<uint32_t *>(dst + lo_offset + j * 8 + tig * 2) = vl;
+            }
+        }
+    }
+}
+
+// =====================================================================================================
+// B2: merge split-KV partials -> o bf16 [B][H*64].  grid (B), block = H*8 threads... generic loop.
+// =====================================================================================================
+__global__ void __launch_bounds__(256) attn_combine_kernel(const float *part_o, const float2 *part_ml, act_t *out,
+                                                           size_t lo_offset, const int *pos_ptr, int n_heads) {
+    pdl_launch_dependents();
+    pdl_wait();
+    const int b = blockIdx.x;
+    const int n_ctx = ld_act(pos_ptr) + 1;
+    const int ns = attn_num_splits(n_ctx);
+    for (int chunk = threadIdx.x; chunk < n_heads * 8; chunk += blockDim.x) {
+        const int head = chunk >> 3, d0 = (chunk & 7) * 8;
+        const size_t hb = (size_t)b * n_heads + head;
+        const float2 *ml = part_ml + hb * kMaxSplits;
+        float M = -INFINITY;
+        for (int s = 0; s < ns; ++s) M = fmaxf(M, __ldcg(&ml[s]).x);
+        float acc[8] = {0, 0, 0, 0, 0, 0, 0, 0}, denom = 0.f;
+        for (int s = 0; s < ns; ++s) {
+            const float2 v = __ldcg(&ml[s]);
+            const float w = __expf(v.x - M);
+            denom += w * v.y;
+            const float *po = part_o + (hb * kMaxSplits + s) * kHeadDim + d0;
+            const float4 a = ld_act4(po), c = ld_act4(po + 4);
+            acc[0] += w * a.x; acc[1] += w * a.y; acc[2] += w * a.z; acc[3] += w * a.w;
+            acc[4] += w * c.x; acc[5] += w * c.y; acc[6] += w * c.z; acc[7] += w * c.w;
+        }
+        const float inv = 1.0f / denom;
+        act_t *dst = out + hb * kHeadDim + d0;
+#pragma unroll
+        for (int i = 0; i < 8; i += 2) {
+            uint32_t vh, vl;
+            split_bf16x2(acc[i] * inv, acc[i + 1] * inv, vh, vl);
+            *reinterpret_cast<uint32_t *>(dst + i) = vh;
+            *reinterpret_cast<uint32_t *>(dst + lo_offset + i) = vl;
+        }
+    }
+}
+
+// =====================================================================================================
+// greedy argmax per sequence over fp32 logits [B][V] (lowest index on ties) + step bookkeeping.
+// grid (B), block 1024.  The last block to finish advances the shared position.
+// =====================================================================================================
+__global__ void __launch_bounds__(1024) argmax_rows_kernel(const float *logits, int vocab, int batch, int *cur_tok,
+                                                           int *tok_hist, int *pos, int pos_inc, unsigned int *counter) {
+    pdl_launch_dependents();
+    pdl_wait();
+    __shared__ unsigned long long red[32];
+    const int b = blockIdx.x;
+    const float *row = logits + (size_t)b * vocab;
+    unsigned long long best = 0ull;
+    for (int i = threadIdx.x; i < vocab; i += blockDim.x) {
+        const unsigned long long k = pack_argmax(ld_act(row + i), i);
+        best = best > k ? best : k;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        const unsigned long long other = __shfl_xor_sync(0xffffffffu, best, o);
+        best = best > other ? best : other;
+    }
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = best;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        best = red[threadIdx.x];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            const unsigned long long other = __shfl_xor_sync(0xffffffffu, best, o);
+            best = best > other ? best : other;
+        }
+        if (threadIdx.x == 0) {
+            const int p = ld_act(pos);
+            const int tok = unpack_argmax_idx(best);
+            cur_tok[b] = tok;
+            tok_hist[(size_t)(p + pos_inc) * batch + b] = tok;
+            __threadfence();
+            const unsigned int ticket = atomicAdd(counter, 1u);
+            if (ticket == (unsigned int)batch - 1) {
+                *pos = p + pos_inc;
+                *counter = 0u;
+            }
+        }
+    }
+}
+
+// ---- launchers ------------------------------------------------------------------------------------------
+template <typename... KArgs, typename... Args>
+static cudaError_t launch_k(const LaunchCtx &c, void (*kernel)(KArgs...), dim3 grid, dim3 block, Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.stream = c.stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = c.pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
+
+cudaError_t launch_embed_rows(const LaunchCtx &c, const bf16 *emb, const int *tok, float *x, int hidden, int rows) {
+    return launch_k(c, embed_rows_kernel, dim3(rows), dim3(256), emb, tok, x, hidden);
+}
+cudaError_t launch_rmsnorm_rows(const LaunchCtx &c, const float *x, const bf16 *gain, act_t *out, size_t lo_offset,
+                                int hidden, float eps, int rows, const int *row_index, int x_stride_rows) {
+    return launch_k(c, rmsnorm_rows_kernel, dim3(rows), dim3(256), x, gain, out, lo_offset, hidden, eps, row_index,
+                    x_stride_rows);
+}
+cudaError_t launch_rope_append(const LaunchCtx &c, const float *qkv, __half *q16, float *q32, kv_t *kc, kv_t *vc,
+                               const float2 *rope, const int *pos, int rows, int Tc, int n_heads, int n_kv_heads,
+                               int max_seq) {
+    return launch_k(c, rope_append_kernel, dim3(rows), dim3(256), qkv, q16, q32, kc, vc, rope, pos, Tc, n_heads,
+                    n_kv_heads, max_seq);
+}
+cudaError_t launch_flash_prefill(const LaunchCtx &c, const __half *q16, const kv_t *kc, const kv_t *vc, act_t *out,
+                                 size_t lo_offset, const int *pos, int batch, int Tc, int n_heads, int n_kv_heads,
+                                 int max_seq) {
+    return launch_k(c, flash_prefill_kernel, dim3((Tc + kFaTile - 1) / kFaTile, n_heads, batch), dim3(128), q16, kc, vc,
+                    out, lo_offset, pos, Tc, n_heads, n_kv_heads, max_seq);
+}
+cudaError_t launch_attn_combine(const LaunchCtx &c, const float *part_o, const float2 *part_ml, act_t *out,
+                                size_t lo_offset, const int *pos, int batch, int n_heads) {
+    return launch_k(c, attn_combine_kernel, dim3(batch), dim3(256), part_o, part_ml, out, lo_offset, pos, n_heads);
+}
+cudaError_t launch_argmax_rows(const LaunchCtx &c, const float *logits, int vocab, int batch, int *cur_tok,
+                               int *tok_hist, int *pos, int pos_inc, unsigned int *counter) {
+    return launch_k(c, argmax_rows_kernel, dim3(batch), dim3(1024), logits, vocab, batch, cur_tok, tok_hist, pos,
+                    pos_inc, counter);
+}
+
+}  // namespace hq

@@ -175,3 +175,82 @@ def test_1b_config1_teacher_forced(one_b_weights):
     frac = float((ref["margins"] > MARGIN).mean())
     print("1b config[1] parity:", stats, "positions with margin>0.1: %.2f" % frac)
     assert stats["argmax_checked"] >= 16
+
+
+# ---------------------------------------------------------------------------------------------------
+# batched serving (configs[3] shape on the tiny model): tensor-core prefill + batched decode
+# ---------------------------------------------------------------------------------------------------
+def run_batched(gm, weights, prompts, n_steps, max_seq, check_every=1):
+    """Every sequence is run alone through the oracle (reading 17); the GPU runs them as one batch,
+    teacher-forced with the oracle's tokens.  Returns worst errors."""
+    B, T = prompts.shape
+    refs = []
+    for b in range(B):
+        om = oracle.Model.from_datagen(weights, max_seq=max_seq)
+        refs.append(om.greedy(prompts[b], n_steps, hidden="last"))
+    stats = {"hidden": 0.0, "logits": 0.0, "argmax_checked": 0}
+    L = weights.shape.n_layers
+
+    def check(i, toks):
+        lg = gm.decode_logits(batch=B).cpu().numpy()
+        hid = [gm.get_hidden(l, batch=B).cpu().numpy() for l in range(L)]
+        for b in range(B):
+            e = rel_l2(lg[b], refs[b]["logits"][i])
+            stats["logits"] = max(stats["logits"], e)
+            assert e <= TOL_LOGITS, f"seq {b} pos {i}: logits rel-L2 {e:.3e}"
+            for l in range(L):
+                e = rel_l2(hid[l][b], refs[b]["hidden"][i][l])
+                stats["hidden"] = max(stats["hidden"], e)
+                assert e <= TOL_HIDDEN, f"seq {b} pos {i} layer {l}: hidden rel-L2 {e:.3e}"
+            if refs[b]["margins"][i] > MARGIN:
+                assert int(toks[b]) == int(refs[b]["tokens"][i]), f"seq {b} pos {i}"
+                stats["argmax_checked"] += 1
+
+    first = gm.prefill(prompts)
+    check(0, first)
+    for i in range(1, n_steps + 1):
+        out = gm.decode_step(tokens_in=[int(refs[b]["tokens"][i - 1]) for b in range(B)])
+        if i % check_every == 0 or i == n_steps:
+            check(i, out[:B])
+    assert gm.seq_len() == T + n_steps
+    return refs, stats
+
+
+def test_tiny_batched_prefill_and_decode(tiny_weights):
+    B, T, steps = 3, 24, 10
+    prompts = datagen.tokens(1003, datagen.TINY.vocab, B * T).reshape(B, T)
+    gm = gpu_model(tiny_weights, max_seq=64, max_batch=4)
+    refs, stats = run_batched(gm, tiny_weights, prompts, steps, 64)
+    print("tiny batched parity:", stats)
+    assert stats["argmax_checked"] >= B * 4
+
+
+def test_tiny_batch_invariance(tiny_weights):
+    """Sequence 0's logits do not depend on its neighbours beyond rounding (reading 17)."""
+    T = 20
+    prompts = datagen.tokens(1004, datagen.TINY.vocab, 4 * T).reshape(4, T)
+    gm = gpu_model(tiny_weights, max_seq=64, max_batch=4)
+    gm.prefill(prompts)
+    gm.decode_run(3, batch=4)
+    a = gm.decode_logits(batch=4)[0].cpu().numpy()
+    gm.kv_reset()
+    other = prompts.copy()
+    other[1:] = prompts[1:][::-1]
+    gm.prefill(other[:2])
+    gm.decode_run(3, batch=2)
+    b = gm.decode_logits(batch=2)[0].cpu().numpy()
+    assert rel_l2(a, b) < 1e-4
+
+
+def test_tiny_chunked_prefill_matches_single_pass(tiny_weights):
+    toks = datagen.tokens(1005, datagen.TINY.vocab, 60)
+    gm = gpu_model(tiny_weights, max_seq=64)
+    gm.prefill(toks)
+    a = gm.decode_logits()[0].cpu().numpy()
+    gm.kv_reset()
+    gm.prefill(toks[:17]); gm.prefill(toks[17:20]); gm.prefill(toks[20:])   # tensor-core, GEMV, tensor-core
+    b = gm.decode_logits()[0].cpu().numpy()
+    assert rel_l2(b, a) < 2e-3
+    om = oracle.Model.from_datagen(tiny_weights, max_seq=64)
+    _, lg = om.forward(toks, logits="last")
+    assert rel_l2(a, lg) <= TOL_LOGITS and rel_l2(b, lg) <= TOL_LOGITS
