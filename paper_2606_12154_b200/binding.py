@@ -16,6 +16,7 @@ _LIB_PATH = os.path.join(_HERE, "libhq.so")
 FLAG_CAPTURE_HIDDEN = 1
 FLAG_NO_GRAPH = 2
 FLAG_NO_PDL = 4
+FLAG_NO_MEGA = 8
 
 HQ_OK, HQ_ERR_INVALID_ARG, HQ_ERR_CAPACITY, HQ_ERR_STATE, HQ_ERR_CUDA, HQ_ERR_UNSUPPORTED = 0, -1, -2, -3, -4, -5
 _CODE_NAMES = {-1: "HQ_ERR_INVALID_ARG", -2: "HQ_ERR_CAPACITY", -3: "HQ_ERR_STATE", -4: "HQ_ERR_CUDA",

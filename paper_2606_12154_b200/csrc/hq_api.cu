@@ -60,6 +60,7 @@ static bool config_supported(const hq_config *c, const char **why) {
         BAD("hidden, ffn and n_heads*head_dim must be multiples of 8 and <= 8192");
     if (c->vocab % 2 != 0 || c->hidden % 2 != 0) BAD("vocab and hidden must be even");
     if (c->max_batch > 32) BAD("max_batch must be <= 32");
+    if (c->n_kv_heads > 56) BAD("n_kv_heads must be <= 56");
     return true;
 #undef BAD
 }
@@ -111,6 +112,12 @@ static size_t carve(const hq_config *c, char *base, Buffers *b) {
     o.ao = (act_t *)take(2 * R * qdim * sizeof(act_t));
     o.actb = (act_t *)take(2 * R * F * sizeof(act_t));
     o.hn_last = (act_t *)take(2 * 32 * d * sizeof(act_t));
+    o.mk_layers = (LayerW *)take(L * sizeof(LayerW));
+    o.mk_qkv = (float *)take(qkvd * sizeof(float));
+    o.mk_attn_out = (float *)take(qdim * sizeof(float));
+    o.mk_part_o = (float *)take(H * kMkMaxParts * kHeadDim * sizeof(float));
+    o.mk_part_ml = (float2 *)take(H * kMkMaxParts * sizeof(float2));
+    o.mk_sync = (unsigned int *)take(64 * sizeof(unsigned int));
     return off;
 }
 
@@ -126,10 +133,36 @@ extern "C" size_t hq_workspace_bytes(const hq_config *cfg) {
 // ---- one decode step: A1..A9 ------------------------------------------------------------------------
 // tok_src: device pointer to the token fed at this step.  with_head = false skips A9 and advances
 // the position with a one-thread kernel instead (used while walking a prompt token by token).
+static MegaParams mega_params(const hq_model *m, const int *tok_src, int n_steps, bool with_head) {
+    const hq_config &c = m->cfg;
+    const Buffers &b = m->b;
+    MegaParams p = {};
+    p.n_layers = c.n_layers; p.hidden = c.hidden; p.n_heads = c.n_heads; p.n_kv_heads = c.n_kv_heads; p.ffn = c.ffn;
+    p.vocab = c.vocab; p.max_seq = c.max_seq; p.eps = c.rms_eps;
+    p.emb = m->emb; p.final_norm = m->final_norm; p.lm_head = m->lm_head; p.layers = b.mk_layers; p.rope = b.rope;
+    p.kc = b.kcache; p.vc = b.vcache;
+    p.layer_kv = (size_t)c.max_batch * c.n_kv_heads * c.max_seq * kHeadDim;
+    p.pos = b.pos; p.cur_tok = b.cur_tok; p.tok_hist = b.tok_hist; p.tok_src = tok_src; p.best = b.best;
+    p.bar = b.mk_sync; p.exit_ticket = b.mk_sync + 1; p.head_ticket = b.mk_sync + 2; p.err = (int *)(b.mk_sync + 3);
+    p.kv_ticket = b.mk_sync + 8;
+    p.x = b.x; p.qkv = b.mk_qkv; p.attn_out = b.mk_attn_out; p.act = b.act; p.logits = b.logits;
+    p.part_o = b.mk_part_o; p.part_ml = b.mk_part_ml;
+    p.hidden_out = (c.flags & HQ_FLAG_CAPTURE_HIDDEN) ? b.hidden : nullptr;
+    p.hidden_stride = (size_t)c.max_batch * c.hidden;
+    p.n_steps = n_steps; p.with_head = with_head ? 1 : 0;
+    return p;
+}
+
 static cudaError_t enqueue_step(hq_model *m, const int *tok_src, bool with_head, int *n_launched) {
     const hq_config &c = m->cfg;
     const LaunchCtx lc{m->stream, m->use_pdl, m->n_sms};
     const Buffers &b = m->b;
+    if (m->use_mega) {
+        // A1-A9 in one persistent launch (hq_mega.cu)
+        cudaError_t em = launch_mega(lc, mega_params(m, tok_src, 1, with_head), m->mega_coop);
+        if (em == cudaSuccess && n_launched) *n_launched = 1;
+        return em;
+    }
     const int qdim = c.n_heads * kHeadDim;
     const size_t layer_kv = (size_t)c.max_batch * c.n_kv_heads * c.max_seq * kHeadDim;
     cudaError_t e;
@@ -401,6 +434,16 @@ extern "C" int32_t hq_model_create(const hq_config *cfg, const hq_weights *w, vo
         return fail(HQ_ERR_CUDA, "hq_model_create: cuTensorMapEncodeTiled failed (driver entry point or bad alignment)");
     }
     m->use_pdl = !(cfg->flags & HQ_FLAG_NO_PDL) && !getenv("HQ_NO_PDL");
+    m->use_mega = !(cfg->flags & HQ_FLAG_NO_MEGA) && !getenv("HQ_NO_MEGA") && mega_shape_supported(*cfg);
+    {
+        cudaError_t e = cudaMemcpyAsync(m->b.mk_layers, m->layers.data(), m->layers.size() * sizeof(LayerW),
+                                        cudaMemcpyHostToDevice, m->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(m->stream);
+        if (e != cudaSuccess) {
+            delete m;
+            return fail(HQ_ERR_CUDA, "hq_model_create: layer table upload failed: %s", cudaGetErrorString(e));
+        }
+    }
 
     // RoPE table in double on the host (reading 7): angle = pos * theta^(-2i/64)
     {
@@ -412,7 +455,7 @@ extern "C" int32_t hq_model_create(const hq_config *cfg, const hq_weights *w, vo
             }
         cudaError_t e = cudaMemcpyAsync(m->b.rope, tab.data(), tab.size() * sizeof(float2), cudaMemcpyHostToDevice, m->stream);
         if (e == cudaSuccess) e = launch_set_state(LaunchCtx{m->stream, false, m->n_sms}, m->b.pos, 0, m->b.best,
-                                                   m->b.counter, cfg->max_batch);
+                                                   m->b.counter, cfg->max_batch, m->b.mk_sync);
         if (e == cudaSuccess) e = launch_zero_tokens(LaunchCtx{m->stream, false, m->n_sms}, m->b.cur_tok, cfg->max_batch);
         if (e == cudaSuccess) e = cudaStreamSynchronize(m->stream);
         if (e != cudaSuccess) {
@@ -428,9 +471,14 @@ extern "C" int32_t hq_model_create(const hq_config *cfg, const hq_weights *w, vo
         // loading is not allowed while capturing); its side effects are reset right after.
         cudaError_t e = enqueue_step(m, m->b.cur_tok, true, nullptr);
         if (e == cudaSuccess) e = launch_set_state(LaunchCtx{m->stream, false, m->n_sms}, m->b.pos, 0, m->b.best,
-                                                   m->b.counter, cfg->max_batch);
+                                                   m->b.counter, cfg->max_batch, m->b.mk_sync);
         if (e == cudaSuccess) e = cudaStreamSynchronize(m->stream);
         if (e == cudaSuccess) e = capture_step_graph(m);
+        if (e != cudaSuccess && m->use_mega && m->mega_coop) {  // retry as a plain launch (grid = #SMs is co-resident)
+            cudaGetLastError();
+            m->mega_coop = false;
+            e = capture_step_graph(m);
+        }
         if (e != cudaSuccess && m->use_pdl) {  // retry without programmatic edges
             cudaGetLastError();
             m->use_pdl = false;
@@ -469,7 +517,7 @@ extern "C" int32_t hq_seq_len(const hq_model *m, int32_t *out) {
 extern "C" int32_t hq_kv_reset(hq_model *m) {
     if (!m) return fail(HQ_ERR_INVALID_ARG, "hq_kv_reset: model is NULL");
     HQ_CUDA(launch_set_state(LaunchCtx{m->stream, false, m->n_sms}, m->b.pos, 0, m->b.best, m->b.counter,
-                             m->cfg.max_batch));
+                             m->cfg.max_batch, m->b.mk_sync));
     m->kernel_count += 1;
     m->seq_len = 0;
     m->batch = 0;
@@ -601,9 +649,16 @@ extern "C" int32_t hq_decode_run(hq_model *m, int32_t n_steps, int32_t *tokens_o
     if (rc != HQ_OK) return rc;
     if (!m->have_token) return fail(HQ_ERR_STATE, "hq_decode_run: no device-resident token to feed");
     const int first = m->seq_len + 1;
-    for (int i = 0; i < n_steps; ++i) {
-        rc = launch_one_step(m);
-        if (rc != HQ_OK) return rc;
+    if (m->use_mega && m->batch == 1) {
+        // the persistent kernel loops over the tokens itself: no launch gap, the weight stream never stops
+        HQ_CUDA(launch_mega(LaunchCtx{m->stream, false, m->n_sms}, mega_params(m, m->b.cur_tok, n_steps, true), m->mega_coop));
+        m->kernel_count += 1;
+        m->seq_len += n_steps;
+    } else {
+        for (int i = 0; i < n_steps; ++i) {
+            rc = launch_one_step(m);
+            if (rc != HQ_OK) return rc;
+        }
     }
     if (tokens_out_host) {
         HQ_CUDA(cudaMemcpyAsync(tokens_out_host, m->b.tok_hist + (size_t)first * m->batch,

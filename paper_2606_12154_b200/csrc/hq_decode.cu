@@ -44,12 +44,13 @@ __global__ void advance_kernel(int *pos, int inc) {
 }
 
 __global__ void set_state_kernel(int *pos, int pos_value, unsigned long long *best, unsigned int *counter,
-                                 int batch) {
+                                 int batch, unsigned int *mk_sync) {
     if (threadIdx.x == 0) {
         *pos = pos_value;
         *counter = 0u;
     }
     if ((int)threadIdx.x < batch) best[threadIdx.x] = 0ull;
+    for (int i = threadIdx.x; i < 64; i += blockDim.x) mk_sync[i] = 0u;   // barrier, tickets, error flag
 }
 
 __global__ void zero_tokens_kernel(int *cur_tok, int batch) {
@@ -427,10 +428,10 @@ cudaError_t launch_advance(const LaunchCtx &c, int *pos, int inc) {
 }
 
 cudaError_t launch_set_state(const LaunchCtx &c, int *pos, int pos_value, unsigned long long *best,
-                             unsigned int *counter, int batch) {
+                             unsigned int *counter, int batch, unsigned int *mk_sync) {
     LaunchCtx nc = c;
     nc.pdl = false;
-    return launch_k(nc, set_state_kernel, dim3(1), dim3(32), pos, pos_value, best, counter, batch);
+    return launch_k(nc, set_state_kernel, dim3(1), dim3(32), pos, pos_value, best, counter, batch, mk_sync);
 }
 
 cudaError_t launch_zero_tokens(const LaunchCtx &c, int *cur_tok, int batch) {

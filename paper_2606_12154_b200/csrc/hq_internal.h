@@ -30,6 +30,11 @@ constexpr int kHeadDim = 64;        // only head_dim the kernels implement
 constexpr int kMaxSplits = 16;      // split-KV partials per head (decode attention)
 constexpr int kMinSplitLen = 64;    // do not split contexts shorter than this per split
 constexpr int kGemvThreads = 256;
+// persistent decode kernel (hq_mega.cu)
+constexpr int kMkStageBytes = 32768;  // one ring stage: 2, 4 or 8 weight rows
+constexpr int kMkStages = 6;          // ring depth: 192 KB of weights in flight per SM
+constexpr int kMkMaxSplits = 16;      // context splits per KV head
+constexpr int kMkMaxParts = 128;      // attention partials per head = splits x sub-splits (<= 16 x 8)
 
 struct alignas(64) TensorMap { uint64_t opaque[16]; };   // mirrors CUtensorMap (driver type, 128 bytes)
 
@@ -65,6 +70,13 @@ struct Buffers {
     act_t *ao = nullptr;                        // [2][pf_rows][H*64] attention output (GEMM operand, hi/lo)
     act_t *actb = nullptr;                      // [2][pf_rows][F] SwiGLU output (GEMM operand, hi/lo)
     act_t *hn_last = nullptr;                   // [2][32][d] normalised last rows (LM-head operand, hi/lo)
+    // persistent decode kernel (batch 1)
+    struct LayerW *mk_layers = nullptr;         // [L] device copy of the per-layer weight pointers
+    float *mk_qkv = nullptr;                    // [(H+2Hkv)*64] RoPE'd q, RoPE'd k, v of the current token
+    float *mk_attn_out = nullptr;               // [H*64] merged attention output
+    float *mk_part_o = nullptr;                 // [H][kMkMaxParts][64]
+    float2 *mk_part_ml = nullptr;               // [H][kMkMaxParts]
+    unsigned int *mk_sync = nullptr;            // [0] grid barrier, [1] exit ticket, [2] head ticket, [3] error, [8..] per-KV-head tickets
 };
 
 constexpr int kTokenTiles[4] = {32, 64, 128, 256};
@@ -91,6 +103,8 @@ struct hq_model_impl {
     TensorMap map_hn[4], map_ao[4], map_actb[4], map_hn_last;   // activation maps per token tile
     cudaGraphExec_t batch_graph = nullptr;      // batched decode step (captured for batch_graph_b)
     int batch_graph_b = 0, batch_graph_kernels = 0, batch_eager_b = 0;
+    bool use_mega = false;                      // batch-1 decode runs in the persistent kernel
+    bool mega_coop = true;                      // launched with the cooperative attribute
 };
 
 // ---- parameter blocks --------------------------------------------------------------------------------
@@ -145,6 +159,32 @@ struct LaunchCtx {
     int n_sms;
 };
 
+// ---- persistent decode kernel (hq_mega.cu) ------------------------------------------------------------
+struct MegaParams {
+    int n_layers, hidden, n_heads, n_kv_heads, ffn, vocab, max_seq;
+    float eps;
+    const bf16 *emb, *final_norm, *lm_head;
+    const LayerW *layers;        // device array [n_layers]
+    const float2 *rope;
+    kv_t *kc, *vc;               // sequence 0 of layer 0
+    size_t layer_kv;             // elements per layer
+    // device-resident step state
+    int *pos, *cur_tok, *tok_hist;
+    const int *tok_src;          // token fed at the first step (later steps feed cur_tok)
+    unsigned long long *best;
+    unsigned int *bar, *exit_ticket, *head_ticket, *kv_ticket;
+    int *err;
+    // activations (fp32)
+    float *x, *qkv, *attn_out, *act, *logits, *part_o;
+    float2 *part_ml;
+    float *hidden_out;           // NULL or [n_layers][hidden_stride] residual after every layer
+    size_t hidden_stride;
+    int n_steps, with_head;
+};
+size_t mega_smem_bytes();
+bool mega_shape_supported(const hq_config &c);
+cudaError_t launch_mega(const LaunchCtx &c, const MegaParams &p, bool cooperative);
+
 // ---- tensor-core GEMM (hq_gemm.cu) -------------------------------------------------------------------
 enum GemmEpilogue { EPI_STORE = 0, EPI_RESID = 1, EPI_SWIGLU = 2 };
 struct GemmParams {
@@ -181,7 +221,7 @@ cudaError_t launch_gemv(const LaunchCtx &c, GemvMode mode, GemvInput xin, const 
 cudaError_t launch_attn_decode(const LaunchCtx &c, const AttnDecodeParams &p, int batch);
 cudaError_t launch_advance(const LaunchCtx &c, int *pos, int inc);
 cudaError_t launch_set_state(const LaunchCtx &c, int *pos, int pos_value, unsigned long long *best,
-                             unsigned int *counter, int batch);
+                             unsigned int *counter, int batch, unsigned int *mk_sync);
 cudaError_t launch_zero_tokens(const LaunchCtx &c, int *cur_tok, int batch);
 bool gemv_shape_supported(int K);
 

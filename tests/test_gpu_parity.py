@@ -18,9 +18,13 @@ def rel_l2(got, want):
     return float(np.linalg.norm(got - want) / np.linalg.norm(want))
 
 
-def gpu_model(weights, max_seq, flags=None, max_batch=1):
+def gpu_model(weights, max_seq, flags=None, max_batch=1, no_mega=False):
+    """no_mega=True: batch-1 decode as one kernel per step of the path (hq_decode.cu) instead of the
+    persistent kernel (hq_mega.cu); both must meet the same tolerances."""
     import paper_2606_12154_b200 as hq
     f = hq.FLAG_CAPTURE_HIDDEN if flags is None else flags
+    if no_mega:
+        f |= hq.FLAG_NO_MEGA
     return hq.Model.from_bf16_bits(weights.shape, weights.embedding, weights.final_norm, weights.layers,
                                    max_seq=max_seq, max_batch=max_batch, flags=f)
 
@@ -61,17 +65,19 @@ def run_teacher_forced(gm, om, prompt, n_steps, check_every=1):
 # ---------------------------------------------------------------------------------------------------
 # configs[0]: tiny model, 32-token prompt, 16 greedy steps
 # ---------------------------------------------------------------------------------------------------
-def test_tiny_prefill_and_decode(tiny_weights, tiny_tokens):
-    gm = gpu_model(tiny_weights, max_seq=64)
+@pytest.mark.parametrize("no_mega", [False, True])
+def test_tiny_prefill_and_decode(tiny_weights, tiny_tokens, no_mega):
+    gm = gpu_model(tiny_weights, max_seq=64, no_mega=no_mega)
     om = oracle.Model.from_datagen(tiny_weights, max_seq=64)
     ref, stats = run_teacher_forced(gm, om, tiny_tokens, 16)
     assert stats["argmax_checked"] >= 8
     print("tiny parity:", stats)
 
 
-def test_tiny_every_prompt_position(tiny_weights, tiny_tokens):
+@pytest.mark.parametrize("no_mega", [False, True])
+def test_tiny_every_prompt_position(tiny_weights, tiny_tokens, no_mega):
     """configs[0] additionally compares all prompt positions (chunked prefill, one token at a time)."""
-    gm = gpu_model(tiny_weights, max_seq=64)
+    gm = gpu_model(tiny_weights, max_seq=64, no_mega=no_mega)
     om = oracle.Model.from_datagen(tiny_weights, max_seq=64)
     hid, lg = om.forward(tiny_tokens, hidden="all", logits="all")
     stats = {}
@@ -89,18 +95,24 @@ def test_tiny_free_running_matches_teacher_forced(tiny_weights, tiny_tokens):
     import paper_2606_12154_b200 as hq
     om = oracle.Model.from_datagen(tiny_weights, max_seq=64)
     ref = om.greedy(tiny_tokens, 16)
-    outs = []
-    for flags in (0, hq.FLAG_NO_GRAPH, hq.FLAG_NO_PDL, hq.FLAG_NO_GRAPH | hq.FLAG_NO_PDL):
-        gm = gpu_model(tiny_weights, max_seq=64, flags=flags)
-        first = gm.prefill(tiny_tokens)
-        toks = gm.decode_run(16)[:, 0]
-        lg = gm.decode_logits()[0].cpu().numpy()
-        outs.append((int(first[0]), toks.copy(), lg))
-    for o in outs[1:]:
-        assert o[0] == outs[0][0] and np.array_equal(o[1], outs[0][1]) and np.array_equal(o[2], outs[0][2])
-    got = np.concatenate([[outs[0][0]], outs[0][1]])
-    if ref["margins"].min() > MARGIN:
-        assert np.array_equal(got, ref["tokens"])
+    for family in (0, hq.FLAG_NO_MEGA):
+        outs = []
+        for flags in (0, hq.FLAG_NO_GRAPH, hq.FLAG_NO_PDL, hq.FLAG_NO_GRAPH | hq.FLAG_NO_PDL):
+            gm = gpu_model(tiny_weights, max_seq=64, flags=flags | family)
+            first = gm.prefill(tiny_tokens)
+            toks = gm.decode_run(16)[:, 0]
+            lg = gm.decode_logits()[0].cpu().numpy()
+            outs.append((int(first[0]), toks.copy(), lg))
+            # streaming one step per call emits the same tokens as the single multi-step call
+            gm.kv_reset()
+            gm.prefill(tiny_tokens)
+            one_by_one = np.array([int(gm.decode_step()[0]) for _ in range(16)])
+            assert np.array_equal(one_by_one, toks) and np.array_equal(gm.decode_logits()[0].cpu().numpy(), lg)
+        for o in outs[1:]:
+            assert o[0] == outs[0][0] and np.array_equal(o[1], outs[0][1]) and np.array_equal(o[2], outs[0][2])
+        got = np.concatenate([[outs[0][0]], outs[0][1]])
+        if ref["margins"].min() > MARGIN:
+            assert np.array_equal(got, ref["tokens"])
 
 
 def test_tiny_kv_reset_and_reuse(tiny_weights, tiny_tokens):
@@ -116,18 +128,23 @@ def test_tiny_kv_reset_and_reuse(tiny_weights, tiny_tokens):
     assert np.array_equal(a, b) and np.array_equal(la, lb)
 
 
-def test_tiny_ragged_lengths(tiny_weights):
-    """Context lengths around the 16/32/64/128 tile and split boundaries of the attention kernel."""
-    toks = datagen.tokens(4242, datagen.TINY.vocab, 200)
+@pytest.mark.parametrize("no_mega", [False, True])
+def test_tiny_ragged_lengths(tiny_weights, no_mega):
+    """Context lengths around the 16/32/64/128 tile and split boundaries of the attention kernels: the
+    prompt goes through prefill, then ONE decode step attends over n+1 positions (decode attention)."""
+    toks = datagen.tokens(4242, datagen.TINY.vocab, 202)
     om = oracle.Model.from_datagen(tiny_weights, max_seq=256)
     _, lg = om.forward(toks, logits="all")
-    gm = gpu_model(tiny_weights, max_seq=256)
+    gm = gpu_model(tiny_weights, max_seq=256, no_mega=no_mega)
     checked = 0
     for n in (1, 2, 15, 16, 17, 31, 33, 63, 64, 65, 127, 128, 129, 191, 200):
         gm.kv_reset()
         gm.prefill(toks[:n])
         e = rel_l2(gm.decode_logits()[0].cpu().numpy(), lg[n - 1])
         assert e <= TOL_LOGITS, f"prompt length {n}: logits rel-L2 {e:.3e}"
+        gm.decode_step(tokens_in=[int(toks[n])])
+        e = rel_l2(gm.decode_logits()[0].cpu().numpy(), lg[n])
+        assert e <= TOL_LOGITS, f"decode at context {n + 1}: logits rel-L2 {e:.3e}"
         checked += 1
     assert checked == 15
 
@@ -166,10 +183,11 @@ def one_b_weights():
     return datagen.make_weights(datagen.ONE_B)
 
 
-def test_1b_config1_teacher_forced(one_b_weights):
+@pytest.mark.parametrize("no_mega", [False, True])
+def test_1b_config1_teacher_forced(one_b_weights, no_mega):
     s = datagen.ONE_B
     prompt = datagen.tokens(1001, s.vocab, 256)
-    gm = gpu_model(one_b_weights, max_seq=512)
+    gm = gpu_model(one_b_weights, max_seq=512, no_mega=no_mega)
     om = oracle.Model.from_datagen(one_b_weights, max_seq=512)
     ref, stats = run_teacher_forced(gm, om, prompt, 128, check_every=8)
     frac = float((ref["margins"] > MARGIN).mean())
