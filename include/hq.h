@@ -158,6 +158,15 @@ int32_t hq_bench_kernel(hq_model *m, int32_t which, int32_t reps, int64_t *bytes
 int32_t hq_debug_gemm(void *cuda_stream, int32_t mode, const void *w_dev, const void *w2_dev, const void *x_dev,
                       void *out_dev, int32_t n_rows, int32_t k, int32_t n_tokens, int32_t token_tile, int32_t splits);
 
+/* Diagnostics: timeline of the persistent batch-1 decode kernel.  trace_dev: DEVICE uint64 [n_ctas][cap] (n_ctas =
+ * number of SMs), or NULL to switch tracing off.  While set, thread 0 of every CTA stores the GPU global timer (ns)
+ * at the start of the launch, after every weight phase, after the attention phase and after every grid barrier, in
+ * program order (per layer: QKV, barrier, attention, barrier, O, barrier, gate/up, barrier, down, barrier; then LM
+ * head, barrier), for every step of every later launch, restarting at index 0 each launch; stamps beyond cap are
+ * dropped.  The buffer is BORROWED until tracing is switched off.  Takes effect for direct launches (hq_decode_run);
+ * a captured single-step graph keeps the setting it was captured with. */
+int32_t hq_debug_trace(hq_model *m, uint64_t *trace_dev, int32_t cap);
+
 /* Thread-local message of the last failing call on this thread; static storage, never NULL. */
 const char *hq_last_error(void);
 

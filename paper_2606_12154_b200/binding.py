@@ -26,7 +26,7 @@ _CODE_NAMES = {-1: "HQ_ERR_INVALID_ARG", -2: "HQ_ERR_CAPACITY", -3: "HQ_ERR_STAT
 DECLARED_SYMBOLS = (
     "hq_workspace_bytes", "hq_model_create", "hq_model_destroy", "hq_prefill", "hq_decode_step",
     "hq_decode_run", "hq_decode_logits", "hq_get_hidden", "hq_sync", "hq_seq_len", "hq_kv_reset",
-    "hq_kernel_count", "hq_bench_kernel", "hq_debug_gemm", "hq_last_error", "hq_version",
+    "hq_kernel_count", "hq_bench_kernel", "hq_debug_gemm", "hq_debug_trace", "hq_last_error", "hq_version",
 )
 
 
@@ -96,6 +96,8 @@ def load_library(path: Optional[str] = None):
     l.hq_bench_kernel.argtypes = [vp, i32, i32, ctypes.POINTER(i64)]
     l.hq_debug_gemm.restype = i32
     l.hq_debug_gemm.argtypes = [vp, i32, vp, vp, vp, vp, i32, i32, i32, i32, i32]
+    l.hq_debug_trace.restype = i32
+    l.hq_debug_trace.argtypes = [vp, vp, i32]
     l.hq_last_error.restype = ctypes.c_char_p
     l.hq_last_error.argtypes = []
     l.hq_version.restype = ctypes.c_char_p
@@ -247,6 +249,18 @@ class Model:
 
     def kernel_count(self) -> int:
         return int(self._lib.hq_kernel_count(self._h))
+
+    def debug_trace(self, cap: int = 0):
+        """Switch the persistent kernel's timeline on (cap > 0: returns the uint64 [n_sms][cap] device tensor the
+        next hq_decode_run launches fill) or off (cap == 0)."""
+        if cap <= 0:
+            _check(self._lib.hq_debug_trace(self._h, None, 0))
+            self._trace = None
+            return None
+        n_sms = self._torch.cuda.get_device_properties(self.device).multi_processor_count
+        self._trace = self._torch.zeros((n_sms, cap), dtype=self._torch.int64, device=self.device)
+        _check(self._lib.hq_debug_trace(self._h, self._trace.data_ptr(), cap))
+        return self._trace
 
     def bench_kernel(self, which: int, reps: int) -> int:
         b = ctypes.c_int64()

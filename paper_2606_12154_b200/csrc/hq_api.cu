@@ -142,9 +142,11 @@ static MegaParams mega_params(const hq_model *m, const int *tok_src, int n_steps
     p.emb = m->emb; p.final_norm = m->final_norm; p.lm_head = m->lm_head; p.layers = b.mk_layers; p.rope = b.rope;
     p.kc = b.kcache; p.vc = b.vcache;
     p.layer_kv = (size_t)c.max_batch * c.n_kv_heads * c.max_seq * kHeadDim;
-    p.pos = b.pos; p.cur_tok = b.cur_tok; p.tok_hist = b.tok_hist; p.tok_src = tok_src; p.best = b.best;
-    p.bar = b.mk_sync; p.exit_ticket = b.mk_sync + 1; p.head_ticket = b.mk_sync + 2; p.err = (int *)(b.mk_sync + 3);
+    p.pos = b.pos; p.cur_tok = b.cur_tok; p.tok_hist = b.tok_hist; p.tok_src = tok_src;
+    p.best2 = (unsigned long long *)(b.mk_sync + 4);
+    p.bar = b.mk_sync; p.exit_ticket = b.mk_sync + 1; p.err = (int *)(b.mk_sync + 3);
     p.kv_ticket = b.mk_sync + 8;
+    p.trace = m->trace; p.trace_cap = m->trace_cap;
     p.x = b.x; p.qkv = b.mk_qkv; p.attn_out = b.mk_attn_out; p.act = b.act; p.logits = b.logits;
     p.part_o = b.mk_part_o; p.part_ml = b.mk_part_ml;
     p.hidden_out = (c.flags & HQ_FLAG_CAPTURE_HIDDEN) ? b.hidden : nullptr;
@@ -434,7 +436,7 @@ extern "C" int32_t hq_model_create(const hq_config *cfg, const hq_weights *w, vo
         return fail(HQ_ERR_CUDA, "hq_model_create: cuTensorMapEncodeTiled failed (driver entry point or bad alignment)");
     }
     m->use_pdl = !(cfg->flags & HQ_FLAG_NO_PDL) && !getenv("HQ_NO_PDL");
-    m->use_mega = !(cfg->flags & HQ_FLAG_NO_MEGA) && !getenv("HQ_NO_MEGA") && mega_shape_supported(*cfg);
+    m->use_mega = !(cfg->flags & HQ_FLAG_NO_MEGA) && !getenv("HQ_NO_MEGA") && mega_shape_supported(*cfg, m->n_sms);
     {
         cudaError_t e = cudaMemcpyAsync(m->b.mk_layers, m->layers.data(), m->layers.size() * sizeof(LayerW),
                                         cudaMemcpyHostToDevice, m->stream);
@@ -749,6 +751,13 @@ extern "C" int32_t hq_bench_kernel(hq_model *m, int32_t which, int32_t reps, int
         m->kernel_count += 1;
     }
     if (bytes_per_launch) *bytes_per_launch = bytes;
+    return HQ_OK;
+}
+
+extern "C" int32_t hq_debug_trace(hq_model *m, uint64_t *trace_dev, int32_t cap) {
+    if (!m || cap < 0 || (trace_dev && cap == 0)) return fail(HQ_ERR_INVALID_ARG, "hq_debug_trace: bad argument");
+    m->trace = (unsigned long long *)trace_dev;
+    m->trace_cap = trace_dev ? cap : 0;
     return HQ_OK;
 }
 

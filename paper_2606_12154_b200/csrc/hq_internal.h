@@ -31,10 +31,11 @@ constexpr int kMaxSplits = 16;      // split-KV partials per head (decode attent
 constexpr int kMinSplitLen = 64;    // do not split contexts shorter than this per split
 constexpr int kGemvThreads = 256;
 // persistent decode kernel (hq_mega.cu)
-constexpr int kMkStageBytes = 32768;  // one ring stage: 2, 4 or 8 weight rows
-constexpr int kMkStages = 6;          // ring depth: 192 KB of weights in flight per SM
-constexpr int kMkMaxSplits = 16;      // context splits per KV head
-constexpr int kMkMaxParts = 128;      // attention partials per head = splits x sub-splits (<= 16 x 8)
+constexpr int kMkSliceChunks = 256;   // 16-byte chunks of one row slice (2048 bf16): what one warp keeps of x in registers
+constexpr int kMkStageBytes = 65536;  // one ring stage: 16 slices = 8 / S units of two rows
+constexpr int kMkStages = 3;          // ring depth: 192 KB of weights in flight per SM
+constexpr int kMkMaxSplits = 32;      // context splits per KV head
+constexpr int kMkMaxParts = 128;      // attention partial slots per head in the workspace (>= kMkMaxSplits)
 
 struct alignas(64) TensorMap { uint64_t opaque[16]; };   // mirrors CUtensorMap (driver type, 128 bytes)
 
@@ -76,7 +77,7 @@ struct Buffers {
     float *mk_attn_out = nullptr;               // [H*64] merged attention output
     float *mk_part_o = nullptr;                 // [H][kMkMaxParts][64]
     float2 *mk_part_ml = nullptr;               // [H][kMkMaxParts]
-    unsigned int *mk_sync = nullptr;            // [0] grid barrier, [1] exit ticket, [2] head ticket, [3] error, [8..] per-KV-head tickets
+    unsigned int *mk_sync = nullptr;            // [0] grid barrier, [1] exit ticket, [3] error, [4..7] two packed-argmax slots, [8..63] per-KV-head tickets
 };
 
 constexpr int kTokenTiles[4] = {32, 64, 128, 256};
@@ -105,6 +106,8 @@ struct hq_model_impl {
     int batch_graph_b = 0, batch_graph_kernels = 0, batch_eager_b = 0;
     bool use_mega = false;                      // batch-1 decode runs in the persistent kernel
     bool mega_coop = true;                      // launched with the cooperative attribute
+    unsigned long long *trace = nullptr;        // hq_debug_trace: device buffer [n_sms][trace_cap] or NULL
+    int trace_cap = 0;
 };
 
 // ---- parameter blocks --------------------------------------------------------------------------------
@@ -171,9 +174,11 @@ struct MegaParams {
     // device-resident step state
     int *pos, *cur_tok, *tok_hist;
     const int *tok_src;          // token fed at the first step (later steps feed cur_tok)
-    unsigned long long *best;
-    unsigned int *bar, *exit_ticket, *head_ticket, *kv_ticket;
+    unsigned long long *best2;   // [2] packed argmax of the step, slots alternate; zero between launches
+    unsigned int *bar, *exit_ticket, *kv_ticket;
     int *err;
+    unsigned long long *trace;   // NULL or [grid][trace_cap] global-timer stamps (hq_debug_trace)
+    int trace_cap;
     // activations (fp32)
     float *x, *qkv, *attn_out, *act, *logits, *part_o;
     float2 *part_ml;
@@ -182,7 +187,7 @@ struct MegaParams {
     int n_steps, with_head;
 };
 size_t mega_smem_bytes();
-bool mega_shape_supported(const hq_config &c);
+bool mega_shape_supported(const hq_config &c, int n_sms);
 cudaError_t launch_mega(const LaunchCtx &c, const MegaParams &p, bool cooperative);
 
 // ---- tensor-core GEMM (hq_gemm.cu) -------------------------------------------------------------------

@@ -6,21 +6,25 @@
 // stream never stops:
 //   * grid = one CTA per SM, 9 warps.  Warp 8 is the PRODUCER: one elected thread walks the static schedule
 //     (layer, phase, this CTA's rows) and streams every weight row with cp.async.bulk (TMA bulk copy,
-//     mbarrier complete_tx) into a ring of kMkStages x 32 KB shared-memory stages.  Weights are immutable, so
-//     the producer runs ahead of the phase barriers — while the consumers wait for the other SMs, do the
+//     mbarrier complete_tx) into a ring of kMkStages x 64 KB shared-memory stages.  Weights are immutable, so
+//     the producer runs ahead of the phase barriers: while the consumers wait for the other SMs, do the
 //     attention, or reduce, the next phases' rows are already landing.
-//   * warps 0-7 are CONSUMERS: the (normalised) input vector of the phase lives in registers, a stage holds
-//     R = 2, 4 or 8 rows (a "unit" = 2 rows: RoPE pair / gate+up pair / two adjacent rows), 8/R warps per row,
-//     conflict-free 16-byte shared loads, fp32 FMA, warp-shuffle reduction, fused epilogues (RoPE, SwiGLU,
-//     residual add, logits + packed argmax).
-//   * phases are separated by a grid barrier (one release-add + acquire-poll on a global counter): per layer
+//   * warps 0-7 are CONSUMERS and never synchronise with one another inside a weight phase.  A stage holds
+//     8/S "units" (a unit = two rows: RoPE pair (i, i+32) / gate+up pair / two adjacent rows); a row is cut
+//     into S slices of <= 2048 elements and warp w owns slice w % S of unit w / S, so the slice of the
+//     (normalised) input vector it needs stays in 64 registers for the whole phase.  Per stage and warp: two
+//     conflict-free 16-byte shared loads per chunk, fp32 FMA, one 6-shuffle reduction for both rows, one
+//     mbarrier arrive, and the fused epilogue (RoPE + KV append, SwiGLU, logits + packed argmax) from lane 0.
+//     Only the residual projections (O, down) park their per-slice partials in shared memory and finish after
+//     one CTA barrier at the end of the phase.
+//   * phases are separated by a grid barrier (red.release + ld.acquire poll on a global counter): per layer
 //     QKV | attention | O | gate/up | down, then the LM head.  The token and the position stay on the device;
 //     the kernel loops over n_steps tokens (hq_decode_run) so there is no launch gap between tokens either.
-//   * attention: work item = (KV head, split); warp = (query head of the group, sub-split); LANE = POSITION:
-//     every lane runs its own online softmax over its positions (K/V rows are one 128-byte line each, read
-//     with 256-bit loads), then the 32 lane states are merged with a transposed butterfly.  The last CTA of a
-//     KV head (ticket) merges the split partials, so the O phase reads a plain vector.  The new K/V row is
-//     appended by the CTA that owns the last split, from the fp32 scratch the QKV phase wrote.
+//   * attention: work item = (KV head, context split); warp = (query head of the group, sub-split); LANE =
+//     POSITION: every lane runs its own online softmax over its positions (K/V rows are one 128-byte line each,
+//     read with 256-bit loads), then the 32 lane states are merged with a transposed butterfly, the sub-splits
+//     through shared memory, and the splits by the last CTA of the KV head (ticket), so the O phase reads a
+//     plain vector.
 #include "hq_common.cuh"
 #include "hq_internal.h"
 
@@ -29,6 +33,7 @@ namespace hq {
 constexpr int kMkConsumerWarps = 8;
 constexpr int kMkConsumers = 32 * kMkConsumerWarps;
 constexpr int kMkThreads = kMkConsumers + 32;
+constexpr int kMkPartRows = 64;                   // residual rows of one CTA in one phase (2 * units)
 constexpr long long kSpinCycles = 6000000000ll;   // ~3 s of SM clocks: a lost arrival traps instead of hanging the GPU
 
 enum { PH_QKV = 0, PH_O = 1, PH_GATEUP = 2, PH_DOWN = 3, PH_HEAD = 4 };
@@ -82,23 +87,32 @@ __device__ __forceinline__ unsigned ld_acquire_u32(const unsigned *p) {
 __device__ __forceinline__ void red_release_add(unsigned *p, unsigned v) {
     asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
-// one 128-byte K or V row (64 fp16) of a cache position: read-only for the life of the kernel
+__device__ __forceinline__ unsigned long long mk_globaltimer() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+// one 128-byte K or V row (64 fp16) of a cache position.  Plain (coherent-after-acquire) loads: the row of the
+// current position was written in this launch, before the grid barrier that precedes the attention phase.
 struct KvRow { uint4 v[8]; };
 __device__ __forceinline__ void ld_kv_row(KvRow &r, const kv_t *p) {
 #pragma unroll
     for (int j = 0; j < 4; ++j)
-        asm volatile("ld.global.nc.v8.u32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+        asm volatile("ld.global.v8.u32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
                      : "=r"(r.v[2 * j].x), "=r"(r.v[2 * j].y), "=r"(r.v[2 * j].z), "=r"(r.v[2 * j].w),
                        "=r"(r.v[2 * j + 1].x), "=r"(r.v[2 * j + 1].y), "=r"(r.v[2 * j + 1].z), "=r"(r.v[2 * j + 1].w)
-                     : "l"(p + 16 * j));
+                     : "l"(p + 16 * j)
+                     : "memory");
 }
 __device__ __forceinline__ float2 h2f(uint32_t u) { return __half22float2(*reinterpret_cast<const __half2 *>(&u)); }
 
 // ---- static schedule shared by producer and consumers -----------------------------------------------------
 struct PhaseGeom {
     int K, row_bytes;
+    int S, log2S;      // K-slices per row (1, 2, 4 or 8): S warps share a unit
+    int cps;           // 16-byte chunks per slice (<= 256)
+    int ups;           // units per stage = 8 / S; a stage holds 2*ups rows
     int u0, u1;        // this CTA's units [u0, u1)
-    int ups;           // units per stage (1, 2 or 4): a stage holds 2*ups rows
     int n_stages;
 };
 
@@ -122,11 +136,15 @@ __device__ __forceinline__ PhaseGeom phase_geom(const MegaParams &p, int ph) {
     PhaseGeom g;
     g.K = phase_k(p, ph);
     g.row_bytes = g.K * 2;
+    const int chunks = g.K >> 3;
+    g.S = 1;
+    g.log2S = 0;
+    while ((chunks + g.S - 1) / g.S > kMkSliceChunks) { g.S <<= 1; ++g.log2S; }
+    g.cps = (chunks + g.S - 1) / g.S;
+    g.ups = kMkConsumerWarps >> g.log2S;
     const int n = phase_units(p, ph), per = n / gridDim.x, rem = n % gridDim.x, b = blockIdx.x;
     g.u0 = b * per + min(b, rem);
     g.u1 = g.u0 + per + (b < rem ? 1 : 0);
-    const int fit = kMkStageBytes / (2 * g.row_bytes);
-    g.ups = fit >= 4 ? 4 : (fit >= 2 ? 2 : 1);
     g.n_stages = (g.u1 - g.u0 + g.ups - 1) / g.ups;
     return g;
 }
@@ -152,21 +170,13 @@ __device__ __forceinline__ void unit_row_ptrs(const MegaParams &p, const LayerW 
     }
 }
 
-// attention split policy (device only; a function of the context length and the grid)
-__device__ __forceinline__ int mk_num_splits(const MegaParams &p, int n_ctx) {
-    int ns_max = (int)gridDim.x / p.n_kv_heads;
-    ns_max = ns_max < 1 ? 1 : (ns_max > kMkMaxSplits ? kMkMaxSplits : ns_max);
-    const int want = (n_ctx + 15) >> 4;   // at least 16 positions per split
-    return want < ns_max ? want : ns_max;
-}
-
 struct MkShared {
     uint64_t full[kMkStages], empty[kMkStages];
-    float partial[2][kMkConsumerWarps];
+    float part[kMkPartRows][kMkConsumerWarps];   // residual phases: [row of this CTA][slice] partial sums
     float2 rope[32];
-    float q[8][kHeadDim];                 // pre-scaled queries of the group
-    alignas(16) __half knew[kHeadDim];    // this step's K/V row of the KV head, fp16-rounded
-    alignas(16) __half vnew[kHeadDim];
+    float q[8][kHeadDim];                        // pre-scaled queries of the group
+    float mrg[kMkConsumerWarps][kHeadDim + 2];   // attention: sub-split states (o[64], m, l)
+    unsigned long long wbest[kMkConsumerWarps];  // LM head: per-warp packed argmax
     int flag;
 };
 
@@ -205,53 +215,57 @@ struct MkCtx {
     unsigned bar_target; // thread 0: arrivals expected at the next grid barrier
     int pos, tok;
     int layer;
+    int ti;              // trace cursor (thread 0)
     unsigned long long best;
 };
 
+// optional timeline (hq_debug_trace): every CTA's thread 0 stamps the global timer at each phase boundary
+__device__ __forceinline__ void mk_trace(const MegaParams &p, MkCtx &c) {
+    if (p.trace && threadIdx.x == 0) {
+        if (c.ti < p.trace_cap) p.trace[(size_t)blockIdx.x * p.trace_cap + c.ti] = mk_globaltimer();
+        ++c.ti;
+    }
+}
+
+// Grid barrier.  bar.sync orders every consumer's global stores of the phase before thread 0's gpu-scope
+// release (cumulativity); the acquire poll + bar.sync orders the other CTAs' stores before every consumer's
+// later loads.
 __device__ __forceinline__ void grid_barrier(const MegaParams &p, MkCtx &c) {
-    consumer_sync();   // every consumer's global stores of this phase are issued
+    consumer_sync();
     if (threadIdx.x == 0) {
         c.bar_target += gridDim.x;
-        __threadfence();
         red_release_add(p.bar, 1u);
+        mk_trace(p, c);
         const long long t0 = clock64();
         unsigned spins = 0;
         while ((int)(ld_acquire_u32(p.bar) - c.bar_target) < 0)
             if ((++spins & 1023u) == 0 && clock64() - t0 > kSpinCycles) mk_fail(p.err, 2);
-        __threadfence();
     }
     consumer_sync();
+    mk_trace(p, c);
 }
 
-// residual stream value i: the embedding row of the token before layer 0's O projection, x afterwards
-__device__ __forceinline__ float2 resid2(const MegaParams &p, const MkCtx &c, bool from_emb, int i) {
-    if (from_emb) {
-        const uint32_t u = __ldg(reinterpret_cast<const uint32_t *>(p.emb + (size_t)c.tok * p.hidden + i));
-        return make_float2(bf16lo(u), bf16hi(u));
-    }
-    return __ldcg(reinterpret_cast<const float2 *>(p.x + i));
-}
-
-// Phase input vector -> registers.  Lane owns chunks (8 elements) ks*cpw + j*32 + lane, j < NCH, of the row.
+// Phase input slice -> registers.  Lane owns chunks (8 elements) c0 + j*32 + lane, j < NCH, of the row.
+// Phases with a fused RMSNorm (A2) have S == 1 (hidden <= 2048): the warp holds the whole vector, so the sum of
+// squares is one warp reduction, recomputed by every warp (deterministic, no atomics).
 template <int NCH>
-__device__ __forceinline__ void load_x(const MegaParams &p, const MkCtx &c, int ph, int K, int wpr, float (&xr)[NCH][8]) {
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int chunks = K >> 3, cpw = (chunks + wpr - 1) / wpr, ks = warp % wpr;
-    const int c_end = min(chunks, (ks + 1) * cpw);
+__device__ __forceinline__ void load_x(const MegaParams &p, const MkCtx &c, int ph, int K, int c0, int my_chunks,
+                                       float (&xr)[NCH][8]) {
+    const int lane = threadIdx.x & 31;
     const bool norm = (ph == PH_QKV || ph == PH_GATEUP || ph == PH_HEAD);
     const bool from_emb = (ph == PH_QKV && c.layer == 0);
     const float *src = ph == PH_O ? p.attn_out : (ph == PH_DOWN ? p.act : p.x);
     float ss = 0.f;
 #pragma unroll
     for (int j = 0; j < NCH; ++j) {
-        const int ch = ks * cpw + j * 32 + lane;
-        if (ch < c_end) {
+        const int ch = j * 32 + lane;
+        if (ch < my_chunks) {
             if (from_emb) {
-                const uint4 e = __ldg(reinterpret_cast<const uint4 *>(p.emb + (size_t)c.tok * p.hidden) + ch);
+                const uint4 e = __ldg(reinterpret_cast<const uint4 *>(p.emb + (size_t)c.tok * p.hidden) + c0 + ch);
                 xr[j][0] = bf16lo(e.x); xr[j][1] = bf16hi(e.x); xr[j][2] = bf16lo(e.y); xr[j][3] = bf16hi(e.y);
                 xr[j][4] = bf16lo(e.z); xr[j][5] = bf16hi(e.z); xr[j][6] = bf16lo(e.w); xr[j][7] = bf16hi(e.w);
             } else {
-                const float4 a = ld_act4(src + ch * 8), b = ld_act4(src + ch * 8 + 4);
+                const float4 a = ld_act4(src + (size_t)(c0 + ch) * 8), b = ld_act4(src + (size_t)(c0 + ch) * 8 + 4);
                 xr[j][0] = a.x; xr[j][1] = a.y; xr[j][2] = a.z; xr[j][3] = a.w;
                 xr[j][4] = b.x; xr[j][5] = b.y; xr[j][6] = b.z; xr[j][7] = b.w;
             }
@@ -259,144 +273,164 @@ __device__ __forceinline__ void load_x(const MegaParams &p, const MkCtx &c, int 
 #pragma unroll
             for (int i = 0; i < 8; ++i) xr[j][i] = 0.f;
         }
-#pragma unroll
-        for (int i = 0; i < 8; ++i) ss = fmaf(xr[j][i], xr[j][i], ss);
     }
     if (norm) {
-        // fused RMSNorm (A2): every warp recomputes sum(x^2) of the L2-resident vector (deterministic)
-        if (wpr == 1) {
-            ss = warp_sum(ss);
-        } else {
-            ss = 0.f;
-            for (int ch = lane; ch < chunks; ch += 32) {
-                float v[8];
-                if (from_emb) {
-                    const uint4 e = __ldg(reinterpret_cast<const uint4 *>(p.emb + (size_t)c.tok * p.hidden) + ch);
-                    v[0] = bf16lo(e.x); v[1] = bf16hi(e.x); v[2] = bf16lo(e.y); v[3] = bf16hi(e.y);
-                    v[4] = bf16lo(e.z); v[5] = bf16hi(e.z); v[6] = bf16lo(e.w); v[7] = bf16hi(e.w);
-                } else {
-                    const float4 a = ld_act4(src + ch * 8), b = ld_act4(src + ch * 8 + 4);
-                    v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w; v[4] = b.x; v[5] = b.y; v[6] = b.z; v[7] = b.w;
-                }
-#pragma unroll
-                for (int i = 0; i < 8; ++i) ss = fmaf(v[i], v[i], ss);
-            }
-            ss = warp_sum(ss);
-        }
-        const float inv = 1.0f / sqrtf(ss / (float)K + p.eps);
         const bf16 *gain = ph == PH_QKV ? p.layers[c.layer].attn_norm : (ph == PH_GATEUP ? p.layers[c.layer].ffn_norm : p.final_norm);
+        uint4 gq[NCH];
 #pragma unroll
         for (int j = 0; j < NCH; ++j) {
-            const int ch = ks * cpw + j * 32 + lane;
-            if (ch < c_end) {
-                const uint4 gq = __ldg(reinterpret_cast<const uint4 *>(gain) + ch);
-                const uint32_t gg[4] = {gq.x, gq.y, gq.z, gq.w};
+            const int ch = j * 32 + lane;
+            gq[j] = ch < my_chunks ? __ldg(reinterpret_cast<const uint4 *>(gain) + c0 + ch) : make_uint4(0, 0, 0, 0);
 #pragma unroll
-                for (int i = 0; i < 4; ++i) {
-                    xr[j][2 * i] *= inv * bf16lo(gg[i]);
-                    xr[j][2 * i + 1] *= inv * bf16hi(gg[i]);
-                }
+            for (int i = 0; i < 8; ++i) ss = fmaf(xr[j][i], xr[j][i], ss);
+        }
+        ss = warp_sum(ss);
+        const float inv = 1.0f / sqrtf(ss / (float)K + p.eps);
+#pragma unroll
+        for (int j = 0; j < NCH; ++j) {
+            const uint32_t gg[4] = {gq[j].x, gq[j].y, gq[j].z, gq[j].w};
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                xr[j][2 * i] *= inv * bf16lo(gg[i]);
+                xr[j][2 * i + 1] *= inv * bf16hi(gg[i]);
             }
         }
     }
 }
 
-// One weight phase on the consumer side: input vector -> registers, then stage by stage.
+// fused epilogue of one finished unit (two row totals a, b) of a phase whose rows are whole in one warp
+__device__ __forceinline__ void finish_unit(const MegaParams &p, MkCtx &c, int ph, int u, float a, float b, const MkShared &sh) {
+    if (ph == PH_QKV) {
+        // A4: RoPE on q and k heads (pair (i, i+32)), q -> scratch, k/v -> cache row of this position (fp16)
+        const int hh = u >> 5, i = u & 31;
+        if (hh < p.n_heads) {
+            const float2 cs = sh.rope[i];
+            p.qkv[hh * kHeadDim + i] = a * cs.x - b * cs.y;
+            p.qkv[hh * kHeadDim + i + 32] = b * cs.x + a * cs.y;
+        } else {
+            const bool is_k = hh < p.n_heads + p.n_kv_heads;
+            const int kvh = hh - p.n_heads - (is_k ? 0 : p.n_kv_heads);
+            float o0 = a, o1 = b;
+            if (is_k) {
+                const float2 cs = sh.rope[i];
+                o0 = a * cs.x - b * cs.y;
+                o1 = b * cs.x + a * cs.y;
+            }
+            kv_t *row = (is_k ? p.kc : p.vc) + (size_t)c.layer * p.layer_kv + ((size_t)kvh * p.max_seq + c.pos) * kHeadDim;
+            row[i] = __float2half_rn(o0);
+            row[i + 32] = __float2half_rn(o1);
+        }
+    } else if (ph == PH_GATEUP) {
+        p.act[u] = silu_f(a) * b;   // A7: fused SwiGLU
+    } else {
+        // A9: logits + running packed argmax (lowest index wins ties)
+        *reinterpret_cast<float2 *>(p.logits + 2 * u) = make_float2(a, b);
+        unsigned long long ka = pack_argmax(a, 2 * u), kb = pack_argmax(b, 2 * u + 1);
+        ka = ka > kb ? ka : kb;
+        c.best = c.best > ka ? c.best : ka;
+    }
+}
+
+// One weight phase on the consumer side: input slice -> registers, then stage by stage, no CTA-wide sync.
 template <int NCH>
 __device__ __forceinline__ void consume_phase(const MegaParams &p, MkCtx &c, int ph, const PhaseGeom &geo, const uint8_t *ring,
                                               MkShared &sh) {
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int R = 2 * geo.ups, wpr = kMkConsumerWarps / R;
-    const int chunks = geo.K >> 3, cpw = (chunks + wpr - 1) / wpr;
-    const int row = warp / wpr, ks = warp % wpr;
-    const int my_chunks = min(chunks, (ks + 1) * cpw) - ks * cpw;   // may be <= 0 for a ragged tail slice
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int slice = warp & (geo.S - 1), pair = warp >> geo.log2S;
+    const int chunks = geo.K >> 3, c0 = slice * geo.cps;
+    const int my_chunks = min(chunks, c0 + geo.cps) - c0;   // may be <= 0 for a ragged tail slice
+    const bool resid = (ph == PH_O || ph == PH_DOWN);
+
+    // A6/A8: the threads that will finish the residual rows fetch the old values now
+    float rold = 0.f;
+    const int n_rows_cta = 2 * (geo.u1 - geo.u0);
+    if (resid && tid < n_rows_cta) {
+        const int r = 2 * geo.u0 + tid;
+        rold = (ph == PH_O && c.layer == 0) ? __bfloat162float(p.emb[(size_t)c.tok * p.hidden + r]) : ld_act(p.x + r);
+    }
 
     float xr[NCH][8];
-    load_x<NCH>(p, c, ph, geo.K, wpr, xr);
-    const bool from_emb = (ph == PH_O && c.layer == 0);
-    const bool resid = (ph == PH_O || ph == PH_DOWN);
+    load_x<NCH>(p, c, ph, geo.K, c0, my_chunks, xr);
+    mk_trace(p, c);
 
     for (int s = 0; s < geo.n_stages; ++s, ++c.g) {
         const int slot = c.g % kMkStages;
         const uint32_t par = (c.g / kMkStages) & 1;
         const int ub = geo.u0 + s * geo.ups;
         const int nu = min(geo.ups, geo.u1 - ub);
-        // epilogue lanes fetch the old residual values while the stage is computed
-        float2 rold = make_float2(0.f, 0.f);
-        const bool epi = (warp == 0 && lane < nu);
-        if (resid && epi) rold = resid2(p, c, from_emb, 2 * (ub + lane));
-
         mk_mbar_wait(&sh.full[slot], par, p.err);
-        float acc[NCH];
-#pragma unroll
-        for (int j = 0; j < NCH; ++j) acc[j] = 0.f;
-        if (row < 2 * nu) {
-            const uint4 *rp = reinterpret_cast<const uint4 *>(ring + (size_t)slot * kMkStageBytes + (size_t)row * geo.row_bytes) +
-                              ks * cpw;
+        if (s == 0) mk_trace(p, c);
+        float a0 = 0.f, a1 = 0.f, b0 = 0.f, b1 = 0.f;
+        if (pair < nu) {
+            const uint4 *r0 = reinterpret_cast<const uint4 *>(ring + (size_t)slot * kMkStageBytes + (size_t)(2 * pair) * geo.row_bytes) + c0;
+            const uint4 *r1 = r0 + (geo.row_bytes >> 4);
 #pragma unroll
             for (int j = 0; j < NCH; ++j) {
                 const int ch = j * 32 + lane;
-                if (ch < my_chunks) acc[j] = dot8(rp[ch], xr[j], 0.f);
-            }
-        }
-        float tot = acc[0];
-#pragma unroll
-        for (int j = 1; j < NCH; ++j) tot += acc[j];
-        tot = warp_sum(tot);
-        if (lane == 0) {
-            sh.partial[s & 1][warp] = tot;
-            mk_mbar_arrive(&sh.empty[slot]);   // warp_sum ordered every lane's shared loads before this
-        }
-        consumer_sync();
-        if (epi) {
-            const int u = ub + lane;
-            float a = 0.f, b = 0.f;
-            for (int k = 0; k < wpr; ++k) {
-                a += sh.partial[s & 1][(2 * lane) * wpr + k];
-                b += sh.partial[s & 1][(2 * lane + 1) * wpr + k];
-            }
-            if (ph == PH_QKV) {
-                const int hh = u >> 5, i = u & 31;
-                float o0 = a, o1 = b;
-                if (hh < p.n_heads + p.n_kv_heads) {
-                    const float2 cs = sh.rope[i];
-                    o0 = a * cs.x - b * cs.y;
-                    o1 = b * cs.x + a * cs.y;
+                if (ch < my_chunks) {
+                    if (j & 1) { a1 = dot8(r0[ch], xr[j], a1); b1 = dot8(r1[ch], xr[j], b1); }
+                    else { a0 = dot8(r0[ch], xr[j], a0); b0 = dot8(r1[ch], xr[j], b0); }
                 }
-                p.qkv[hh * kHeadDim + i] = o0;
-                p.qkv[hh * kHeadDim + i + 32] = o1;
-            } else if (ph == PH_GATEUP) {
-                p.act[u] = silu_f(a) * b;
-            } else if (resid) {
-                *reinterpret_cast<float2 *>(p.x + 2 * u) = make_float2(rold.x + a, rold.y + b);
-            } else {
-                *reinterpret_cast<float2 *>(p.logits + 2 * u) = make_float2(a, b);
-                unsigned long long ka = pack_argmax(a, 2 * u), kb = pack_argmax(b, 2 * u + 1);
-                ka = ka > kb ? ka : kb;
-                c.best = c.best > ka ? c.best : ka;
             }
         }
+        float a = a0 + a1, b = b0 + b1;
+        // both row totals with 6 shuffles: halves swap rows, 4 butterfly steps, one exchange
+        const bool up = (lane & 16) != 0;
+        float v = (up ? b : a) + __shfl_xor_sync(0xffffffffu, up ? a : b, 16);
+#pragma unroll
+        for (int o = 8; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        const float w = __shfl_xor_sync(0xffffffffu, v, 16);   // lane 0: v = row a total, w = row b total
+        if (lane == 0) {
+            mk_mbar_arrive(&sh.empty[slot]);   // the shuffles ordered every lane's shared loads before this
+            if (pair < nu) {
+                if (resid) {
+                    const int rl = 2 * (s * geo.ups + pair);
+                    sh.part[rl][slice] = v;
+                    sh.part[rl + 1][slice] = w;
+                } else {
+                    finish_unit(p, c, ph, ub + pair, v, w, sh);
+                }
+            }
+        }
+    }
+    if (resid) {
+        consumer_sync();
+        if (tid < n_rows_cta) {
+            float t = rold;
+            for (int k = 0; k < geo.S; ++k) t += sh.part[tid][k];
+            p.x[2 * geo.u0 + tid] = t;
+        }
+        // sh.part is next written after the grid barrier that follows every residual phase
     }
 }
 
 __device__ __forceinline__ void run_phase(const MegaParams &p, MkCtx &c, int ph, const uint8_t *ring, MkShared &sh) {
     const PhaseGeom geo = phase_geom(p, ph);
-    const int wpr = kMkConsumerWarps / (2 * geo.ups);
-    const int cpw = ((geo.K >> 3) + wpr - 1) / wpr;
-    const int nch = (cpw + 31) / 32;
+    const int nch = (geo.cps + 31) / 32;
     if (nch <= 1) consume_phase<1>(p, c, ph, geo, ring, sh);
     else if (nch <= 2) consume_phase<2>(p, c, ph, geo, ring, sh);
     else if (nch <= 4) consume_phase<4>(p, c, ph, geo, ring, sh);
     else consume_phase<8>(p, c, ph, geo, ring, sh);
+    mk_trace(p, c);
 }
 
 // ---- A5: attention phase ---------------------------------------------------------------------------------------
+// attention split policy (device only; a function of the context length and the grid): one 32-position
+// iteration per warp while the grid has CTAs to spare, then longer splits
+__device__ __forceinline__ int mk_num_splits(const MegaParams &p, int n_ctx, int nsub) {
+    int ns_max = (int)gridDim.x / p.n_kv_heads;
+    ns_max = ns_max < 1 ? 1 : (ns_max > kMkMaxSplits ? kMkMaxSplits : ns_max);
+    const int per = 32 * nsub;
+    const int want = (n_ctx + per - 1) / per;
+    return want < ns_max ? want : ns_max;
+}
+
 __device__ void attention_phase(const MegaParams &p, MkCtx &c, MkShared &sh) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int G = p.n_heads / p.n_kv_heads;
     const int nsub = kMkConsumerWarps / G;
     const int n_ctx = c.pos + 1;
-    const int ns = mk_num_splits(p, n_ctx);
+    const int ns = mk_num_splits(p, n_ctx, nsub);
     const int len = (n_ctx + ns - 1) / ns;
     const int items = p.n_kv_heads * ns;
     const size_t layer_off = (size_t)c.layer * p.layer_kv;
@@ -404,23 +438,18 @@ __device__ void attention_phase(const MegaParams &p, MkCtx &c, MkShared &sh) {
     for (int item = blockIdx.x; item < items; item += gridDim.x) {
         const int kvh = item / ns, split = item % ns;
         const int s0 = split * len, s1 = min(n_ctx, s0 + len);
-        const bool owns_new = (split == ns - 1);
-        // stage the group's queries (pre-scaled by 1/sqrt(64) = 0.125, exact) and the new K/V row
+        // stage the group's queries, pre-scaled by 1/sqrt(64) = 0.125 (exact)
         for (int i = tid; i < G * kHeadDim; i += kMkConsumers)
             sh.q[i >> 6][i & 63] = 0.125f * ld_act(p.qkv + (size_t)(kvh * G) * kHeadDim + i);
-        if (owns_new && tid < 2 * kHeadDim) {
-            const int i = tid & 63;
-            const int hh = p.n_heads + (tid < kHeadDim ? 0 : p.n_kv_heads) + kvh;
-            const __half hv = __float2half_rn(ld_act(p.qkv + (size_t)hh * kHeadDim + i));
-            kv_t *cache = (tid < kHeadDim ? p.kc : p.vc) + layer_off + ((size_t)kvh * p.max_seq + c.pos) * kHeadDim;
-            (tid < kHeadDim ? sh.knew : sh.vnew)[i] = hv;
-            cache[i] = hv;   // KV append (A4): read again only by later steps
-        }
         consumer_sync();
+        if (item == (int)blockIdx.x) mk_trace(p, c);
 
-        if (warp < G * nsub) {
-            const int g = warp % G, sub = warp / G;
-            const int head = kvh * G + g;
+        const bool active = warp < G * nsub;
+        const int g = warp % G, sub = warp / G;
+        const int head = kvh * G + g;
+        const int r = warp_row_of_lane<32>(lane);   // the output dims (r, 32 + r) this lane holds after the merge
+        float M = -INFINITY, l_tot = 0.f, o_lo = 0.f, o_hi = 0.f;
+        if (active) {
             const int sub_len = (s1 - s0 + nsub - 1) / nsub;
             const int w0 = s0 + sub * sub_len, w1 = min(s1, w0 + sub_len);
             const kv_t *kg = p.kc + layer_off + (size_t)kvh * p.max_seq * kHeadDim;
@@ -432,16 +461,8 @@ __device__ void attention_phase(const MegaParams &p, MkCtx &c, MkShared &sh) {
             for (int d = 0; d < kHeadDim; ++d) o[d] = 0.f;
             for (int t = w0 + lane; t < w1; t += 32) {
                 KvRow kr, vr;
-                if (t == c.pos) {
-#pragma unroll
-                    for (int j = 0; j < 8; ++j) {
-                        kr.v[j] = reinterpret_cast<const uint4 *>(sh.knew)[j];
-                        vr.v[j] = reinterpret_cast<const uint4 *>(sh.vnew)[j];
-                    }
-                } else {
-                    ld_kv_row(kr, kg + (size_t)t * kHeadDim);
-                    ld_kv_row(vr, vg + (size_t)t * kHeadDim);
-                }
+                ld_kv_row(kr, kg + (size_t)t * kHeadDim);
+                ld_kv_row(vr, vg + (size_t)t * kHeadDim);
                 float s = 0.f, s2 = 0.f;
 #pragma unroll
                 for (int j = 0; j < 8; ++j) {
@@ -472,52 +493,81 @@ __device__ void attention_phase(const MegaParams &p, MkCtx &c, MkShared &sh) {
                 m = m_new;
             }
             // merge the 32 lane states: common max, rescale, transposed butterfly over the 64 dims
-            const float M = warp_max(m);
+            M = warp_max(m);
             const float sc = (m == -INFINITY) ? 0.f : __expf(m - M);
-            const float l_tot = warp_sum(l * sc);
+            l_tot = warp_sum(l * sc);
 #pragma unroll
             for (int d = 0; d < kHeadDim; ++d) o[d] *= sc;
             float(&h0)[32] = *reinterpret_cast<float(*)[32]>(&o[0]);
             float(&h1)[32] = *reinterpret_cast<float(*)[32]>(&o[32]);
             warp_reduce_rows<32>(h0, lane);
             warp_reduce_rows<32>(h1, lane);
-            const int r = warp_row_of_lane<32>(lane);
-            const size_t pidx = (size_t)head * kMkMaxParts + split * nsub + sub;
-            p.part_o[pidx * kHeadDim + r] = h0[0];
-            p.part_o[pidx * kHeadDim + 32 + r] = h1[0];
-            if (lane == 0) p.part_ml[pidx] = make_float2(M, l_tot);
+            o_lo = h0[0];
+            o_hi = h1[0];
+            if (sub > 0) {   // park the state for the sub-split 0 warp of this head
+                sh.mrg[warp][r] = o_lo;
+                sh.mrg[warp][32 + r] = o_hi;
+                if (lane == 0) { sh.mrg[warp][kHeadDim] = M; sh.mrg[warp][kHeadDim + 1] = l_tot; }
+            }
         }
-        // the last CTA of this KV head merges the split partials (fixed slot order: deterministic)
-        consumer_sync();
-        if (tid == 0) {
-            __threadfence();
-            const unsigned t = atomicAdd(p.kv_ticket + kvh, 1u);
-            sh.flag = (t == (unsigned)ns - 1u);
-            if (sh.flag) {
-                p.kv_ticket[kvh] = 0u;
+        if (nsub > 1) consumer_sync();
+        if (active && sub == 0) {
+            for (int k = 1; k < nsub; ++k) {
+                const float *o2 = sh.mrg[k * G + g];
+                const float M2 = o2[kHeadDim], l2 = o2[kHeadDim + 1];
+                const float Mn = fmaxf(M, M2);
+                const float wa = (M == -INFINITY) ? 0.f : __expf(M - Mn), wb = (M2 == -INFINITY) ? 0.f : __expf(M2 - Mn);
+                l_tot = l_tot * wa + l2 * wb;
+                o_lo = o_lo * wa + o2[r] * wb;
+                o_hi = o_hi * wa + o2[32 + r] * wb;
+                M = Mn;
+            }
+            if (ns == 1) {   // the whole context in one CTA: final
+                const float inv = 1.0f / l_tot;
+                p.attn_out[head * kHeadDim + r] = o_lo * inv;
+                p.attn_out[head * kHeadDim + 32 + r] = o_hi * inv;
+            } else {
+                const size_t pidx = (size_t)head * kMkMaxSplits + split;
+                p.part_o[pidx * kHeadDim + r] = o_lo;
+                p.part_o[pidx * kHeadDim + 32 + r] = o_hi;
+                if (lane == 0) p.part_ml[pidx] = make_float2(M, l_tot);
+            }
+        }
+        if (item == (int)blockIdx.x) mk_trace(p, c);
+        if (ns > 1) {
+            // the last CTA of this KV head merges the split partials (fixed slot order: deterministic)
+            consumer_sync();
+            if (tid == 0) {
                 __threadfence();
-            }
-        }
-        consumer_sync();
-        if (sh.flag) {
-            const int n_parts = ns * nsub;
-            for (int i = tid; i < G * kHeadDim; i += kMkConsumers) {
-                const int head = kvh * G + (i >> 6), d = i & 63;
-                const float2 *ml = p.part_ml + (size_t)head * kMkMaxParts;
-                float M = -INFINITY;
-                for (int s = 0; s < n_parts; ++s) M = fmaxf(M, __ldcg(&ml[s]).x);
-                float acc = 0.f, den = 0.f;
-                for (int s = 0; s < n_parts; ++s) {
-                    const float2 v = __ldcg(&ml[s]);
-                    const float wgt = (v.x == -INFINITY) ? 0.f : __expf(v.x - M);
-                    den = fmaf(wgt, v.y, den);
-                    acc = fmaf(wgt, __ldcg(p.part_o + ((size_t)head * kMkMaxParts + s) * kHeadDim + d), acc);
+                const unsigned t = atomicAdd(p.kv_ticket + kvh, 1u);
+                sh.flag = (t == (unsigned)ns - 1u);
+                if (sh.flag) {
+                    p.kv_ticket[kvh] = 0u;
+                    __threadfence();
                 }
-                p.attn_out[head * kHeadDim + d] = acc / den;
+            }
+            consumer_sync();
+            if (sh.flag) {
+                for (int i = tid; i < G * kHeadDim; i += kMkConsumers) {
+                    const int hd = kvh * G + (i >> 6), d = i & 63;
+                    const float2 *ml = p.part_ml + (size_t)hd * kMkMaxSplits;
+                    float Mx = -INFINITY;
+                    for (int s = 0; s < ns; ++s) Mx = fmaxf(Mx, __ldcg(&ml[s]).x);
+                    float acc = 0.f, den = 0.f;
+                    for (int s = 0; s < ns; ++s) {
+                        const float2 v = __ldcg(&ml[s]);
+                        const float wgt = (v.x == -INFINITY) ? 0.f : __expf(v.x - Mx);
+                        den = fmaf(wgt, v.y, den);
+                        acc = fmaf(wgt, __ldcg(p.part_o + ((size_t)hd * kMkMaxSplits + s) * kHeadDim + d), acc);
+                    }
+                    p.attn_out[hd * kHeadDim + d] = acc / den;
+                }
             }
         }
-        consumer_sync();   // sh.q / sh.flag are reused by the next item
+        consumer_sync();   // sh.q / sh.mrg / sh.flag are reused by the next item
     }
+    if ((int)blockIdx.x >= items) { mk_trace(p, c); mk_trace(p, c); }
+    mk_trace(p, c);
 }
 
 // ---- the kernel -----------------------------------------------------------------------------------------------
@@ -545,9 +595,11 @@ __global__ void __launch_bounds__(kMkThreads, 1) mega_decode_kernel(const __grid
     c.g = 0;
     c.bar_target = 0;
     c.best = 0ull;
+    c.ti = 0;
+    c.pos = ld_act(p.pos);
+    c.tok = ld_act(p.tok_src);
+    mk_trace(p, c);
     for (int step = 0; step < p.n_steps; ++step) {
-        c.pos = ld_act(p.pos);
-        c.tok = ld_act(step == 0 ? p.tok_src : p.cur_tok);
         if (tid < 32) sh.rope[tid] = p.rope[(size_t)c.pos * 32 + tid];
         consumer_sync();
         for (c.layer = 0; c.layer < p.n_layers; ++c.layer) {
@@ -566,37 +618,35 @@ __global__ void __launch_bounds__(kMkThreads, 1) mega_decode_kernel(const __grid
                     p.hidden_out[(size_t)c.layer * p.hidden_stride + i] = ld_act(p.x + i);
         }
         if (p.with_head) {
+            // A9: every CTA folds its best (logit, index) into the step's slot with one packed 64-bit atomicMax
+            // before the barrier; after it every CTA reads the winner = the next token.  Two slots alternate so
+            // the one not in use can be cleared without a further barrier.
             c.best = 0ull;
             run_phase(p, c, PH_HEAD, ring, sh);
-            // fused argmax (A9): per-CTA best -> one packed 64-bit atomicMax; the last CTA publishes the token
-            if (warp == 0) {
-                unsigned long long b = c.best;
-#pragma unroll
-                for (int o = 16; o > 0; o >>= 1) {
-                    const unsigned long long other = __shfl_xor_sync(0xffffffffu, b, o);
-                    b = b > other ? b : other;
-                }
-                if (tid == 0) {
-                    if (b) atomicMax(p.best, b);
-                    __threadfence();
-                    const unsigned t = atomicAdd(p.head_ticket, 1u);
-                    if (t == gridDim.x - 1) {
-                        __threadfence();
-                        const unsigned long long win = atomicExch(p.best, 0ull);
-                        const int tok = unpack_argmax_idx(win);
-                        *p.cur_tok = tok;
-                        p.tok_hist[c.pos + 1] = tok;
-                        *p.pos = c.pos + 1;
-                        *p.head_ticket = 0u;
-                    }
-                }
+            unsigned long long *slot = p.best2 + (step & 1);
+            if ((tid & 31) == 0) sh.wbest[warp] = c.best;   // lane 0 ran every epilogue of its warp
+            consumer_sync();
+            if (tid == 0) {
+                unsigned long long b = sh.wbest[0];
+                for (int k = 1; k < kMkConsumerWarps; ++k) b = b > sh.wbest[k] ? b : sh.wbest[k];
+                if (b) atomicMax(slot, b);
             }
-            if (step + 1 < p.n_steps) grid_barrier(p, c);   // the next step reads the token and the position
-        } else if (blockIdx.x == 0 && tid == 0) {
-            *p.pos = c.pos + 1;   // every CTA read the position before the first barrier of this step
+            grid_barrier(p, c);
+            const unsigned long long win = __ldcg(slot);
+            c.tok = unpack_argmax_idx(win);
+            if (blockIdx.x == 0 && tid == 0) {
+                *p.cur_tok = c.tok;
+                p.tok_hist[c.pos + 1] = c.tok;
+                *p.pos = c.pos + 1;
+                p.best2[(step + 1) & 1] = 0ull;   // last read two barriers ago, next written after >= 1 more
+            }
+        } else {
+            if (blockIdx.x == 0 && tid == 0) *p.pos = c.pos + 1;
+            c.tok = 0;   // without the head the kernel runs one step (hq_prefill token walk)
         }
+        c.pos += 1;
     }
-    // leave the barrier counter at zero for the next launch: the last CTA out resets it
+    // leave the barrier counter and the argmax slots at zero for the next launch: the last CTA out resets them
     consumer_sync();
     if (tid == 0) {
         __threadfence();
@@ -604,6 +654,8 @@ __global__ void __launch_bounds__(kMkThreads, 1) mega_decode_kernel(const __grid
         if (t == gridDim.x - 1) {
             *p.bar = 0u;
             *p.exit_ticket = 0u;
+            p.best2[0] = 0ull;
+            p.best2[1] = 0ull;
         }
     }
 }
@@ -611,12 +663,14 @@ __global__ void __launch_bounds__(kMkThreads, 1) mega_decode_kernel(const __grid
 // ---- host side ---------------------------------------------------------------------------------------------------
 size_t mega_smem_bytes() { return (size_t)kMkStages * kMkStageBytes + sizeof(MkShared) + 128; }
 
-bool mega_shape_supported(const hq_config &c) {
-    // a unit (two rows) must fit one stage; the group must fit the consumer warps
-    const int kmax = c.ffn > c.hidden ? c.ffn : c.hidden;
+bool mega_shape_supported(const hq_config &c, int n_sms) {
+    // RMSNorm phases keep the whole vector in one warp (hidden <= 2048); residual phases cut K into <= 8 slices;
+    // the residual rows of one CTA must fit the partial buffer; the group must fit the consumer warps
     const int q = c.n_heads * c.head_dim;
-    return 2 * 2 * (kmax > q ? kmax : q) <= kMkStageBytes && c.n_heads / c.n_kv_heads <= kMkConsumerWarps &&
-           c.hidden % 8 == 0 && c.ffn % 8 == 0 && c.vocab % 2 == 0;
+    const int units_cta = (c.hidden / 2 + n_sms - 1) / n_sms;
+    return c.hidden <= 8 * kMkSliceChunks && q <= 64 * kMkSliceChunks && c.ffn <= 64 * kMkSliceChunks &&
+           2 * units_cta <= kMkPartRows && c.n_heads / c.n_kv_heads <= kMkConsumerWarps && c.hidden % 8 == 0 &&
+           c.ffn % 8 == 0 && c.vocab % 2 == 0 && n_sms >= 1;
 }
 
 cudaError_t launch_mega(const LaunchCtx &c, const MegaParams &p, bool cooperative) {
