@@ -152,6 +152,7 @@ static MegaParams mega_params(const hq_model *m, const int *tok_src, int n_steps
     p.hidden_out = (c.flags & HQ_FLAG_CAPTURE_HIDDEN) ? b.hidden : nullptr;
     p.hidden_stride = (size_t)c.max_batch * c.hidden;
     p.n_steps = n_steps; p.with_head = with_head ? 1 : 0;
+    p.prefetch_stages = m->mega_prefetch;
     return p;
 }
 
@@ -436,6 +437,7 @@ extern "C" int32_t hq_model_create(const hq_config *cfg, const hq_weights *w, vo
         return fail(HQ_ERR_CUDA, "hq_model_create: cuTensorMapEncodeTiled failed (driver entry point or bad alignment)");
     }
     m->use_pdl = !(cfg->flags & HQ_FLAG_NO_PDL) && !getenv("HQ_NO_PDL");
+    if (const char *pf = getenv("HQ_MEGA_PREFETCH")) m->mega_prefetch = atoi(pf) < 0 ? 0 : (atoi(pf) > 64 ? 64 : atoi(pf));
     m->use_mega = !(cfg->flags & HQ_FLAG_NO_MEGA) && !getenv("HQ_NO_MEGA") && mega_shape_supported(*cfg, m->n_sms);
     {
         cudaError_t e = cudaMemcpyAsync(m->b.mk_layers, m->layers.data(), m->layers.size() * sizeof(LayerW),

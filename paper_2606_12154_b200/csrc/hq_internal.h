@@ -34,6 +34,7 @@ constexpr int kGemvThreads = 256;
 constexpr int kMkSliceChunks = 256;   // 16-byte chunks of one row slice (2048 bf16): what one warp keeps of x in registers
 constexpr int kMkStageBytes = 65536;  // one ring stage: 16 slices = 8 / S units of two rows
 constexpr int kMkStages = 3;          // ring depth: 192 KB of weights in flight per SM
+constexpr int kMkPrefetchStages = 0;  // default L2 look-ahead of the producer beyond the ring (HQ_MEGA_PREFETCH overrides)
 constexpr int kMkMaxSplits = 32;      // context splits per KV head
 constexpr int kMkMaxParts = 128;      // attention partial slots per head in the workspace (>= kMkMaxSplits)
 
@@ -106,6 +107,7 @@ struct hq_model_impl {
     int batch_graph_b = 0, batch_graph_kernels = 0, batch_eager_b = 0;
     bool use_mega = false;                      // batch-1 decode runs in the persistent kernel
     bool mega_coop = true;                      // launched with the cooperative attribute
+    int mega_prefetch = kMkPrefetchStages;      // L2 look-ahead of the persistent kernel's producer (ring stages)
     unsigned long long *trace = nullptr;        // hq_debug_trace: device buffer [n_sms][trace_cap] or NULL
     int trace_cap = 0;
 };
@@ -185,6 +187,7 @@ struct MegaParams {
     float *hidden_out;           // NULL or [n_layers][hidden_stride] residual after every layer
     size_t hidden_stride;
     int n_steps, with_head;
+    int prefetch_stages;         // producer: L2 look-ahead beyond the ring, in ring stages (0 = off)
 };
 size_t mega_smem_bytes();
 bool mega_shape_supported(const hq_config &c, int n_sms);

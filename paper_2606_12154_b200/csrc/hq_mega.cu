@@ -33,7 +33,8 @@ namespace hq {
 constexpr int kMkConsumerWarps = 8;
 constexpr int kMkConsumers = 32 * kMkConsumerWarps;
 constexpr int kMkThreads = kMkConsumers + 32;
-constexpr int kMkPartRows = 64;                   // residual rows of one CTA in one phase (2 * units)
+constexpr int kMkPartRows = 64;
+constexpr int kMkStagedK = 8 * kMkConsumers;      // 2048: one 8-element chunk per consumer thread                   // residual rows of one CTA in one phase (2 * units)
 constexpr long long kSpinCycles = 6000000000ll;   // ~3 s of SM clocks: a lost arrival traps instead of hanging the GPU
 
 enum { PH_QKV = 0, PH_O = 1, PH_GATEUP = 2, PH_DOWN = 3, PH_HEAD = 4 };
@@ -77,6 +78,23 @@ __device__ __forceinline__ void mk_bulk_g2s(void *smem_dst, const void *gmem_src
                      mk_smem_u32(smem_dst)),
                  "l"(gmem_src), "r"(bytes), "r"(mk_smem_u32(bar))
                  : "memory");
+}
+// weights are read once per token: mark their L2 lines evict-first so that the activations, the attention partials and
+// the KV cache (re-read every token) stay resident in the 126 MB L2
+__device__ __forceinline__ uint64_t mk_policy_evict_first() {
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+__device__ __forceinline__ void mk_bulk_g2s_hint(void *smem_dst, const void *gmem_src, uint32_t bytes, uint64_t *bar, uint64_t pol) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(
+                     mk_smem_u32(smem_dst)),
+                 "l"(gmem_src), "r"(bytes), "r"(mk_smem_u32(bar)), "l"(pol)
+                 : "memory");
+}
+// fire-and-forget HBM -> L2 prefetch of a weight row (no completion tracking: the later bulk copy just hits L2)
+__device__ __forceinline__ void mk_bulk_prefetch_l2(const void *gmem_src, uint32_t bytes, uint64_t pol) {
+    asm volatile("cp.async.bulk.prefetch.L2.global.L2::cache_hint [%0], %1, %2;" ::"l"(gmem_src), "r"(bytes), "l"(pol) : "memory");
 }
 __device__ __forceinline__ void consumer_sync() { asm volatile("bar.sync 1, %0;" ::"n"(kMkConsumers) : "memory"); }
 __device__ __forceinline__ unsigned ld_acquire_u32(const unsigned *p) {
@@ -172,40 +190,86 @@ __device__ __forceinline__ void unit_row_ptrs(const MegaParams &p, const LayerW 
 
 struct MkShared {
     uint64_t full[kMkStages], empty[kMkStages];
+    alignas(16) float xs[kMkStagedK];            // phase input staged once per CTA (phases with K <= kMkStagedK)
     float part[kMkPartRows][kMkConsumerWarps];   // residual phases: [row of this CTA][slice] partial sums
     float2 rope[32];
-    float q[8][kHeadDim];                        // pre-scaled queries of the group
+    alignas(16) float q[kMkConsumerWarps][kHeadDim];   // per warp: pre-scaled query of its head
     float mrg[kMkConsumerWarps][kHeadDim + 2];   // attention: sub-split states (o[64], m, l)
+    float red[kMkConsumerWarps];                 // RMSNorm: per-warp sum of squares
     unsigned long long wbest[kMkConsumerWarps];  // LM head: per-warp packed argmax
-    int flag;
 };
 
 // ---- producer ----------------------------------------------------------------------------------------------
+// Position in this CTA's static stage schedule: (step, phase index, stage of the phase).
+struct MkCursor {
+    int step, pi, s, ph, layer;
+    PhaseGeom geo;
+    bool done;
+};
+__device__ __forceinline__ void cursor_load_phase(const MegaParams &p, MkCursor &c) {
+    const int n_ph = p.n_layers * 4 + (p.with_head ? 1 : 0);
+    for (;;) {   // skip phases in which this CTA owns no unit
+        if (c.pi == n_ph) { c.pi = 0; ++c.step; }
+        if (c.step >= p.n_steps) { c.done = true; return; }
+        c.layer = c.pi >> 2;
+        c.ph = c.layer < p.n_layers ? (c.pi & 3) : PH_HEAD;
+        c.geo = phase_geom(p, c.ph);
+        if (c.geo.n_stages > 0) return;
+        ++c.pi;
+    }
+}
+__device__ __forceinline__ void cursor_init(const MegaParams &p, MkCursor &c) {
+    c.step = 0; c.pi = 0; c.s = 0; c.done = false;
+    cursor_load_phase(p, c);
+}
+__device__ __forceinline__ void cursor_next(const MegaParams &p, MkCursor &c) {
+    if (++c.s == c.geo.n_stages) { c.s = 0; ++c.pi; cursor_load_phase(p, c); }
+}
+
+// One elected thread.  Two cursors walk the same schedule: `ld` fills the shared-memory ring (TMA bulk copies, mbarrier
+// complete_tx), `pf` runs p.prefetch_stages stages ahead of it and only pulls the rows HBM -> L2.  The ring alone holds
+// ~4 us of streaming; the dependent chain down -> QKV -> attention -> O of a layer is longer than that, so without the
+// L2 look-ahead the HBM pipe would idle while the consumers sit in grid barriers.
 __device__ void mk_producer(const MegaParams &p, uint8_t *ring, MkShared &sh) {
-    unsigned g = 0;   // stages produced so far
-    for (int step = 0; step < p.n_steps; ++step) {
-        const int n_ph = p.n_layers * 4 + (p.with_head ? 1 : 0);
-        for (int pi = 0; pi < n_ph; ++pi) {
-            const int layer = pi >> 2;
-            const int ph = layer < p.n_layers ? (pi & 3) : PH_HEAD;
-            const LayerW &w = p.layers[layer < p.n_layers ? layer : 0];
-            const PhaseGeom geo = phase_geom(p, ph);
-            for (int s = 0; s < geo.n_stages; ++s, ++g) {
-                const int slot = g % kMkStages;
-                const uint32_t par = (g / kMkStages) & 1;
-                mk_mbar_wait(&sh.empty[slot], par ^ 1, p.err);
-                const int ub = geo.u0 + s * geo.ups;
-                const int nu = min(geo.ups, geo.u1 - ub);
-                mk_mbar_expect_tx(&sh.full[slot], (uint32_t)(2 * nu * geo.row_bytes));
-                uint8_t *dst = ring + (size_t)slot * kMkStageBytes;
+    const uint64_t pol = mk_policy_evict_first();
+    MkCursor ld, pf;
+    cursor_init(p, ld);
+    pf = ld;
+    int ahead = 0;   // stages pf is ahead of ld
+    unsigned g = 0;  // stages produced so far
+    while (!ld.done) {
+        while (!pf.done && ahead < p.prefetch_stages) {
+            if (ahead > 0) {   // distance 0 would duplicate the bulk copy issued right below
+                const LayerW &w = p.layers[pf.layer < p.n_layers ? pf.layer : 0];
+                const int ub = pf.geo.u0 + pf.s * pf.geo.ups;
+                const int nu = min(pf.geo.ups, pf.geo.u1 - ub);
                 for (int j = 0; j < nu; ++j) {
                     const bf16 *ra, *rb;
-                    unit_row_ptrs(p, w, ph, geo.K, ub + j, ra, rb);
-                    mk_bulk_g2s(dst + (size_t)(2 * j) * geo.row_bytes, ra, geo.row_bytes, &sh.full[slot]);
-                    mk_bulk_g2s(dst + (size_t)(2 * j + 1) * geo.row_bytes, rb, geo.row_bytes, &sh.full[slot]);
+                    unit_row_ptrs(p, w, pf.ph, pf.geo.K, ub + j, ra, rb);
+                    mk_bulk_prefetch_l2(ra, pf.geo.row_bytes, pol);
+                    mk_bulk_prefetch_l2(rb, pf.geo.row_bytes, pol);
                 }
             }
+            cursor_next(p, pf);
+            ++ahead;
         }
+        const int slot = g % kMkStages;
+        const uint32_t par = (g / kMkStages) & 1;
+        mk_mbar_wait(&sh.empty[slot], par ^ 1, p.err);
+        const LayerW &w = p.layers[ld.layer < p.n_layers ? ld.layer : 0];
+        const int ub = ld.geo.u0 + ld.s * ld.geo.ups;
+        const int nu = min(ld.geo.ups, ld.geo.u1 - ub);
+        mk_mbar_expect_tx(&sh.full[slot], (uint32_t)(2 * nu * ld.geo.row_bytes));
+        uint8_t *dst = ring + (size_t)slot * kMkStageBytes;
+        for (int j = 0; j < nu; ++j) {
+            const bf16 *ra, *rb;
+            unit_row_ptrs(p, w, ld.ph, ld.geo.K, ub + j, ra, rb);
+            mk_bulk_g2s_hint(dst + (size_t)(2 * j) * ld.geo.row_bytes, ra, ld.geo.row_bytes, &sh.full[slot], pol);
+            mk_bulk_g2s_hint(dst + (size_t)(2 * j + 1) * ld.geo.row_bytes, rb, ld.geo.row_bytes, &sh.full[slot], pol);
+        }
+        cursor_next(p, ld);
+        ++g;
+        if (ahead > 0) --ahead;
     }
 }
 
@@ -245,55 +309,127 @@ __device__ __forceinline__ void grid_barrier(const MegaParams &p, MkCtx &c) {
     mk_trace(p, c);
 }
 
+// attention split policy (device only; a function of the context length and the grid): one 32-position
+// iteration per warp while the grid has CTAs to spare, then longer splits.  n_kv_heads * splits <= gridDim.x, so
+// every CTA owns at most one (KV head, split) item.
+__device__ __forceinline__ int mk_num_splits(const MegaParams &p, int n_ctx, int nsub) {
+    int ns_max = (int)gridDim.x / p.n_kv_heads;
+    ns_max = ns_max < 1 ? 1 : (ns_max > kMkMaxSplits ? kMkMaxSplits : ns_max);
+    const int per = 32 * nsub;
+    const int want = (n_ctx + per - 1) / per;
+    return want < ns_max ? want : ns_max;
+}
+
+// Phase input, K <= kMkStagedK: the CTA reads the vector from L2 ONCE (thread t owns elements [8t, 8t+8)), applies the
+// fused prologue, and leaves it in shared memory for its 8 warps.  (Every warp fetching its own copy made all 1184
+// warps of the chip hit the same 64 L2 lines at once: 4-5 us per phase, profiles/r01_mega_timeline.md.)
+//   QKV, gate/up, LM head: A2 RMSNorm (sum of squares reduced across the CTA, deterministic), gain multiply
+//   O:                     A5 merge of the split-KV partials (m, l, o) written by the attention phase
+//   down (small models):   plain copy
+__device__ __forceinline__ void stage_input(const MegaParams &p, const MkCtx &c, int ph, int K, MkShared &sh) {
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const bool has = tid * 8 < K;
+    float v[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) v[i] = 0.f;
+    if (ph == PH_O) {
+        if (has) {
+            const int G = p.n_heads / p.n_kv_heads;
+            const int ns = mk_num_splits(p, c.pos + 1, kMkConsumerWarps / G);
+            const int h = tid >> 3, d0 = (tid & 7) * 8;
+            const float2 *ml = p.part_ml + (size_t)h * kMkMaxSplits;
+            const float *po = p.part_o + (size_t)h * kMkMaxSplits * kHeadDim + d0;
+            float Mx = -INFINITY;
+            for (int s = 0; s < ns; ++s) Mx = fmaxf(Mx, __ldcg(&ml[s]).x);
+            float den = 0.f;
+            for (int s = 0; s < ns; ++s) {
+                const float2 m = __ldcg(&ml[s]);
+                const float wgt = (m.x == -INFINITY) ? 0.f : __expf(m.x - Mx);
+                const float4 a = ld_act4(po + (size_t)s * kHeadDim), b = ld_act4(po + (size_t)s * kHeadDim + 4);
+                den = fmaf(wgt, m.y, den);
+                v[0] = fmaf(wgt, a.x, v[0]); v[1] = fmaf(wgt, a.y, v[1]); v[2] = fmaf(wgt, a.z, v[2]); v[3] = fmaf(wgt, a.w, v[3]);
+                v[4] = fmaf(wgt, b.x, v[4]); v[5] = fmaf(wgt, b.y, v[5]); v[6] = fmaf(wgt, b.z, v[6]); v[7] = fmaf(wgt, b.w, v[7]);
+            }
+            const float inv = 1.0f / den;
+#pragma unroll
+            for (int i = 0; i < 8; ++i) v[i] *= inv;
+        }
+    } else if (ph == PH_DOWN) {
+        if (has) {
+            const float4 a = ld_act4(p.act + (size_t)tid * 8), b = ld_act4(p.act + (size_t)tid * 8 + 4);
+            v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w; v[4] = b.x; v[5] = b.y; v[6] = b.z; v[7] = b.w;
+        }
+    } else {
+        const bf16 *gain = ph == PH_QKV ? p.layers[c.layer].attn_norm : (ph == PH_GATEUP ? p.layers[c.layer].ffn_norm : p.final_norm);
+        uint4 gq = make_uint4(0, 0, 0, 0);
+        if (has) {
+            gq = __ldg(reinterpret_cast<const uint4 *>(gain) + tid);
+            if (ph == PH_QKV && c.layer == 0) {   // A1: the residual stream starts as the embedding row
+                const uint4 e = __ldg(reinterpret_cast<const uint4 *>(p.emb + (size_t)c.tok * p.hidden) + tid);
+                v[0] = bf16lo(e.x); v[1] = bf16hi(e.x); v[2] = bf16lo(e.y); v[3] = bf16hi(e.y);
+                v[4] = bf16lo(e.z); v[5] = bf16hi(e.z); v[6] = bf16lo(e.w); v[7] = bf16hi(e.w);
+            } else {
+                const float4 a = ld_act4(p.x + (size_t)tid * 8), b = ld_act4(p.x + (size_t)tid * 8 + 4);
+                v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w; v[4] = b.x; v[5] = b.y; v[6] = b.z; v[7] = b.w;
+            }
+        }
+        float ss = 0.f;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) ss = fmaf(v[i], v[i], ss);
+        ss = warp_sum(ss);
+        if (lane == 0) sh.red[warp] = ss;
+        consumer_sync();
+        float tot = 0.f;
+#pragma unroll
+        for (int k = 0; k < kMkConsumerWarps; ++k) tot += sh.red[k];
+        const float inv = 1.0f / sqrtf(tot / (float)K + p.eps);
+        const uint32_t gg[4] = {gq.x, gq.y, gq.z, gq.w};
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            v[2 * i] *= inv * bf16lo(gg[i]);
+            v[2 * i + 1] *= inv * bf16hi(gg[i]);
+        }
+    }
+    if (has) {
+        float4 *dst = reinterpret_cast<float4 *>(sh.xs + tid * 8);
+        dst[0] = make_float4(v[0], v[1], v[2], v[3]);
+        dst[1] = make_float4(v[4], v[5], v[6], v[7]);
+    }
+    consumer_sync();
+}
+
 // Phase input slice -> registers.  Lane owns chunks (8 elements) c0 + j*32 + lane, j < NCH, of the row.
-// Phases with a fused RMSNorm (A2) have S == 1 (hidden <= 2048): the warp holds the whole vector, so the sum of
-// squares is one warp reduction, recomputed by every warp (deterministic, no atomics).
 template <int NCH>
-__device__ __forceinline__ void load_x(const MegaParams &p, const MkCtx &c, int ph, int K, int c0, int my_chunks,
-                                       float (&xr)[NCH][8]) {
+__device__ __forceinline__ void load_x_staged(const MkShared &sh, int my_chunks, float (&xr)[NCH][8]) {
     const int lane = threadIdx.x & 31;
-    const bool norm = (ph == PH_QKV || ph == PH_GATEUP || ph == PH_HEAD);
-    const bool from_emb = (ph == PH_QKV && c.layer == 0);
-    const float *src = ph == PH_O ? p.attn_out : (ph == PH_DOWN ? p.act : p.x);
-    float ss = 0.f;
+    const float4 *xs4 = reinterpret_cast<const float4 *>(sh.xs);
 #pragma unroll
     for (int j = 0; j < NCH; ++j) {
         const int ch = j * 32 + lane;
         if (ch < my_chunks) {
-            if (from_emb) {
-                const uint4 e = __ldg(reinterpret_cast<const uint4 *>(p.emb + (size_t)c.tok * p.hidden) + c0 + ch);
-                xr[j][0] = bf16lo(e.x); xr[j][1] = bf16hi(e.x); xr[j][2] = bf16lo(e.y); xr[j][3] = bf16hi(e.y);
-                xr[j][4] = bf16lo(e.z); xr[j][5] = bf16hi(e.z); xr[j][6] = bf16lo(e.w); xr[j][7] = bf16hi(e.w);
-            } else {
-                const float4 a = ld_act4(src + (size_t)(c0 + ch) * 8), b = ld_act4(src + (size_t)(c0 + ch) * 8 + 4);
-                xr[j][0] = a.x; xr[j][1] = a.y; xr[j][2] = a.z; xr[j][3] = a.w;
-                xr[j][4] = b.x; xr[j][5] = b.y; xr[j][6] = b.z; xr[j][7] = b.w;
-            }
+            const float4 a = xs4[2 * ch], b = xs4[2 * ch + 1];
+            xr[j][0] = a.x; xr[j][1] = a.y; xr[j][2] = a.z; xr[j][3] = a.w;
+            xr[j][4] = b.x; xr[j][5] = b.y; xr[j][6] = b.z; xr[j][7] = b.w;
         } else {
 #pragma unroll
             for (int i = 0; i < 8; ++i) xr[j][i] = 0.f;
         }
     }
-    if (norm) {
-        const bf16 *gain = ph == PH_QKV ? p.layers[c.layer].attn_norm : (ph == PH_GATEUP ? p.layers[c.layer].ffn_norm : p.final_norm);
-        uint4 gq[NCH];
+}
+// K > kMkStagedK (the down projection of the 1B model, K = 8192): every warp reads its own slice from L2
+template <int NCH>
+__device__ __forceinline__ void load_x_direct(const float *src, int c0, int my_chunks, float (&xr)[NCH][8]) {
+    const int lane = threadIdx.x & 31;
 #pragma unroll
-        for (int j = 0; j < NCH; ++j) {
-            const int ch = j * 32 + lane;
-            gq[j] = ch < my_chunks ? __ldg(reinterpret_cast<const uint4 *>(gain) + c0 + ch) : make_uint4(0, 0, 0, 0);
+    for (int j = 0; j < NCH; ++j) {
+        const int ch = j * 32 + lane;
+        if (ch < my_chunks) {
+            const float4 a = ld_act4(src + (size_t)(c0 + ch) * 8), b = ld_act4(src + (size_t)(c0 + ch) * 8 + 4);
+            xr[j][0] = a.x; xr[j][1] = a.y; xr[j][2] = a.z; xr[j][3] = a.w;
+            xr[j][4] = b.x; xr[j][5] = b.y; xr[j][6] = b.z; xr[j][7] = b.w;
+        } else {
 #pragma unroll
-            for (int i = 0; i < 8; ++i) ss = fmaf(xr[j][i], xr[j][i], ss);
-        }
-        ss = warp_sum(ss);
-        const float inv = 1.0f / sqrtf(ss / (float)K + p.eps);
-#pragma unroll
-        for (int j = 0; j < NCH; ++j) {
-            const uint32_t gg[4] = {gq[j].x, gq[j].y, gq[j].z, gq[j].w};
-#pragma unroll
-            for (int i = 0; i < 4; ++i) {
-                xr[j][2 * i] *= inv * bf16lo(gg[i]);
-                xr[j][2 * i + 1] *= inv * bf16hi(gg[i]);
-            }
+            for (int i = 0; i < 8; ++i) xr[j][i] = 0.f;
         }
     }
 }
@@ -350,7 +486,12 @@ __device__ __forceinline__ void consume_phase(const MegaParams &p, MkCtx &c, int
     }
 
     float xr[NCH][8];
-    load_x<NCH>(p, c, ph, geo.K, c0, my_chunks, xr);
+    if (geo.K <= kMkStagedK) {   // S == 1: the warp holds the whole vector
+        stage_input(p, c, ph, geo.K, sh);
+        load_x_staged<NCH>(sh, my_chunks, xr);
+    } else {
+        load_x_direct<NCH>(p.act, c0, my_chunks, xr);   // only the down projection has K > kMkStagedK
+    }
     mk_trace(p, c);
 
     for (int s = 0; s < geo.n_stages; ++s, ++c.g) {
@@ -415,159 +556,138 @@ __device__ __forceinline__ void run_phase(const MegaParams &p, MkCtx &c, int ph,
 }
 
 // ---- A5: attention phase ---------------------------------------------------------------------------------------
-// attention split policy (device only; a function of the context length and the grid): one 32-position
-// iteration per warp while the grid has CTAs to spare, then longer splits
-__device__ __forceinline__ int mk_num_splits(const MegaParams &p, int n_ctx, int nsub) {
-    int ns_max = (int)gridDim.x / p.n_kv_heads;
-    ns_max = ns_max < 1 ? 1 : (ns_max > kMkMaxSplits ? kMkMaxSplits : ns_max);
-    const int per = 32 * nsub;
-    const int want = (n_ctx + per - 1) / per;
-    return want < ns_max ? want : ns_max;
-}
-
-__device__ void attention_phase(const MegaParams &p, MkCtx &c, MkShared &sh) {
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int G = p.n_heads / p.n_kv_heads;
-    const int nsub = kMkConsumerWarps / G;
+// Work item of a CTA = (KV head, context split); warp = (query head of the group, sub-split); LANE = POSITION.
+// attn_prefetch runs BEFORE the grid barrier that ends the QKV phase: the K/V rows of earlier positions do not depend
+// on this step's projections, so their HBM/L2 latency overlaps the barrier.  Only the row of the current position
+// (written by the QKV phase of this step) has to wait.
+struct AttnItem {
+    int kvh, split, g, sub, w1, t0;
+    bool has_item, active, pre;
+};
+__device__ __forceinline__ void attn_prefetch(const MegaParams &p, const MkCtx &c, AttnItem &it, KvRow &kr, KvRow &vr) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int G = p.n_heads / p.n_kv_heads, nsub = kMkConsumerWarps / G;
     const int n_ctx = c.pos + 1;
     const int ns = mk_num_splits(p, n_ctx, nsub);
     const int len = (n_ctx + ns - 1) / ns;
-    const int items = p.n_kv_heads * ns;
-    const size_t layer_off = (size_t)c.layer * p.layer_kv;
+    it.has_item = (int)blockIdx.x < p.n_kv_heads * ns;
+    it.kvh = (int)blockIdx.x / ns;
+    it.split = (int)blockIdx.x % ns;
+    it.g = warp % G;
+    it.sub = warp / G;
+    it.active = it.has_item && warp < G * nsub;
+    const int s0 = it.split * len, s1 = min(n_ctx, s0 + len);
+    const int sub_len = (max(s1 - s0, 0) + nsub - 1) / nsub;
+    const int w0 = s0 + it.sub * sub_len;
+    it.w1 = min(s1, w0 + sub_len);
+    it.t0 = w0 + lane;
+    it.pre = it.active && it.t0 < it.w1 && it.t0 < c.pos;
+    if (it.pre) {
+        const size_t off = (size_t)c.layer * p.layer_kv + ((size_t)it.kvh * p.max_seq + it.t0) * kHeadDim;
+        ld_kv_row(kr, p.kc + off);
+        ld_kv_row(vr, p.vc + off);
+    }
+}
 
-    for (int item = blockIdx.x; item < items; item += gridDim.x) {
-        const int kvh = item / ns, split = item % ns;
-        const int s0 = split * len, s1 = min(n_ctx, s0 + len);
-        // stage the group's queries, pre-scaled by 1/sqrt(64) = 0.125 (exact)
-        for (int i = tid; i < G * kHeadDim; i += kMkConsumers)
-            sh.q[i >> 6][i & 63] = 0.125f * ld_act(p.qkv + (size_t)(kvh * G) * kHeadDim + i);
-        consumer_sync();
-        if (item == (int)blockIdx.x) mk_trace(p, c);
-
-        const bool active = warp < G * nsub;
-        const int g = warp % G, sub = warp / G;
-        const int head = kvh * G + g;
-        const int r = warp_row_of_lane<32>(lane);   // the output dims (r, 32 + r) this lane holds after the merge
-        float M = -INFINITY, l_tot = 0.f, o_lo = 0.f, o_hi = 0.f;
-        if (active) {
-            const int sub_len = (s1 - s0 + nsub - 1) / nsub;
-            const int w0 = s0 + sub * sub_len, w1 = min(s1, w0 + sub_len);
-            const kv_t *kg = p.kc + layer_off + (size_t)kvh * p.max_seq * kHeadDim;
-            const kv_t *vg = p.vc + layer_off + (size_t)kvh * p.max_seq * kHeadDim;
-            const float4 *q4 = reinterpret_cast<const float4 *>(sh.q[g]);
-
-            float m = -INFINITY, l = 0.f, o[kHeadDim];
+__device__ void attention_phase(const MegaParams &p, MkCtx &c, MkShared &sh, const AttnItem &it, KvRow &kr, KvRow &vr) {
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    if (!it.has_item) { mk_trace(p, c); mk_trace(p, c); mk_trace(p, c); return; }
+    const int G = p.n_heads / p.n_kv_heads, nsub = kMkConsumerWarps / G;
+    const int head = it.kvh * G + it.g;
+    const int r = warp_row_of_lane<32>(lane);   // the output dims (r, 32 + r) this lane holds after the merge
+    float M = -INFINITY, l_tot = 0.f, o_lo = 0.f, o_hi = 0.f;
+    if (it.active) {
+        // the warp's query, pre-scaled by 1/sqrt(64) = 0.125 (exact), broadcast-read from shared memory below
+        if (lane < 16) {
+            float4 qv = ld_act4(p.qkv + (size_t)head * kHeadDim + lane * 4);
+            qv.x *= 0.125f; qv.y *= 0.125f; qv.z *= 0.125f; qv.w *= 0.125f;
+            reinterpret_cast<float4 *>(sh.q[warp])[lane] = qv;
+        }
+        __syncwarp();
+    }
+    mk_trace(p, c);
+    if (it.active) {
+        const kv_t *kg = p.kc + (size_t)c.layer * p.layer_kv + (size_t)it.kvh * p.max_seq * kHeadDim;
+        const kv_t *vg = p.vc + (size_t)c.layer * p.layer_kv + (size_t)it.kvh * p.max_seq * kHeadDim;
+        const float4 *q4 = reinterpret_cast<const float4 *>(sh.q[warp]);
+        float m = -INFINITY, l = 0.f, o[kHeadDim];
 #pragma unroll
-            for (int d = 0; d < kHeadDim; ++d) o[d] = 0.f;
-            for (int t = w0 + lane; t < w1; t += 32) {
-                KvRow kr, vr;
+        for (int d = 0; d < kHeadDim; ++d) o[d] = 0.f;
+        bool loaded = it.pre;
+        for (int t = it.t0; t < it.w1; t += 32) {
+            if (!loaded) {
                 ld_kv_row(kr, kg + (size_t)t * kHeadDim);
                 ld_kv_row(vr, vg + (size_t)t * kHeadDim);
-                float s = 0.f, s2 = 0.f;
+            }
+            loaded = false;
+            float s = 0.f, s2 = 0.f;
 #pragma unroll
-                for (int j = 0; j < 8; ++j) {
-                    const float4 qa = q4[2 * j], qb = q4[2 * j + 1];
-                    const float2 k0 = h2f(kr.v[j].x), k1 = h2f(kr.v[j].y), k2 = h2f(kr.v[j].z), k3 = h2f(kr.v[j].w);
-                    s = fmaf(qa.x, k0.x, s); s2 = fmaf(qa.y, k0.y, s2);
-                    s = fmaf(qa.z, k1.x, s); s2 = fmaf(qa.w, k1.y, s2);
-                    s = fmaf(qb.x, k2.x, s); s2 = fmaf(qb.y, k2.y, s2);
-                    s = fmaf(qb.z, k3.x, s); s2 = fmaf(qb.w, k3.y, s2);
-                }
-                s += s2;
-                const float m_new = fmaxf(m, s);
-                const float corr = __expf(m - m_new);   // m = -inf the first time -> 0
-                const float pr = __expf(s - m_new);
-                l = l * corr + pr;
+            for (int j = 0; j < 8; ++j) {
+                const float4 qa = q4[2 * j], qb = q4[2 * j + 1];
+                const float2 k0 = h2f(kr.v[j].x), k1 = h2f(kr.v[j].y), k2 = h2f(kr.v[j].z), k3 = h2f(kr.v[j].w);
+                s = fmaf(qa.x, k0.x, s); s2 = fmaf(qa.y, k0.y, s2);
+                s = fmaf(qa.z, k1.x, s); s2 = fmaf(qa.w, k1.y, s2);
+                s = fmaf(qb.x, k2.x, s); s2 = fmaf(qb.y, k2.y, s2);
+                s = fmaf(qb.z, k3.x, s); s2 = fmaf(qb.w, k3.y, s2);
+            }
+            s += s2;
+            const float m_new = fmaxf(m, s);
+            const float corr = __expf(m - m_new);   // m = -inf the first time -> 0
+            const float pr = __expf(s - m_new);
+            l = l * corr + pr;
 #pragma unroll
-                for (int j = 0; j < 8; ++j) {
-                    const float2 v0 = h2f(vr.v[j].x), v1 = h2f(vr.v[j].y), v2 = h2f(vr.v[j].z), v3 = h2f(vr.v[j].w);
-                    o[8 * j + 0] = fmaf(pr, v0.x, o[8 * j + 0] * corr);
-                    o[8 * j + 1] = fmaf(pr, v0.y, o[8 * j + 1] * corr);
-                    o[8 * j + 2] = fmaf(pr, v1.x, o[8 * j + 2] * corr);
-                    o[8 * j + 3] = fmaf(pr, v1.y, o[8 * j + 3] * corr);
-                    o[8 * j + 4] = fmaf(pr, v2.x, o[8 * j + 4] * corr);
-                    o[8 * j + 5] = fmaf(pr, v2.y, o[8 * j + 5] * corr);
-                    o[8 * j + 6] = fmaf(pr, v3.x, o[8 * j + 6] * corr);
-                    o[8 * j + 7] = fmaf(pr, v3.y, o[8 * j + 7] * corr);
-                }
-                m = m_new;
+            for (int j = 0; j < 8; ++j) {
+                const float2 v0 = h2f(vr.v[j].x), v1 = h2f(vr.v[j].y), v2 = h2f(vr.v[j].z), v3 = h2f(vr.v[j].w);
+                o[8 * j + 0] = fmaf(pr, v0.x, o[8 * j + 0] * corr);
+                o[8 * j + 1] = fmaf(pr, v0.y, o[8 * j + 1] * corr);
+                o[8 * j + 2] = fmaf(pr, v1.x, o[8 * j + 2] * corr);
+                o[8 * j + 3] = fmaf(pr, v1.y, o[8 * j + 3] * corr);
+                o[8 * j + 4] = fmaf(pr, v2.x, o[8 * j + 4] * corr);
+                o[8 * j + 5] = fmaf(pr, v2.y, o[8 * j + 5] * corr);
+                o[8 * j + 6] = fmaf(pr, v3.x, o[8 * j + 6] * corr);
+                o[8 * j + 7] = fmaf(pr, v3.y, o[8 * j + 7] * corr);
             }
-            // merge the 32 lane states: common max, rescale, transposed butterfly over the 64 dims
-            M = warp_max(m);
-            const float sc = (m == -INFINITY) ? 0.f : __expf(m - M);
-            l_tot = warp_sum(l * sc);
+            m = m_new;
+        }
+        // merge the 32 lane states: common max, rescale, transposed butterfly over the 64 dims
+        M = warp_max(m);
+        const float sc = (m == -INFINITY) ? 0.f : __expf(m - M);
+        l_tot = warp_sum(l * sc);
 #pragma unroll
-            for (int d = 0; d < kHeadDim; ++d) o[d] *= sc;
-            float(&h0)[32] = *reinterpret_cast<float(*)[32]>(&o[0]);
-            float(&h1)[32] = *reinterpret_cast<float(*)[32]>(&o[32]);
-            warp_reduce_rows<32>(h0, lane);
-            warp_reduce_rows<32>(h1, lane);
-            o_lo = h0[0];
-            o_hi = h1[0];
-            if (sub > 0) {   // park the state for the sub-split 0 warp of this head
-                sh.mrg[warp][r] = o_lo;
-                sh.mrg[warp][32 + r] = o_hi;
-                if (lane == 0) { sh.mrg[warp][kHeadDim] = M; sh.mrg[warp][kHeadDim + 1] = l_tot; }
-            }
+        for (int d = 0; d < kHeadDim; ++d) o[d] *= sc;
+        float(&h0)[32] = *reinterpret_cast<float(*)[32]>(&o[0]);
+        float(&h1)[32] = *reinterpret_cast<float(*)[32]>(&o[32]);
+        warp_reduce_rows<32>(h0, lane);
+        warp_reduce_rows<32>(h1, lane);
+        o_lo = h0[0];
+        o_hi = h1[0];
+        if (it.sub > 0) {   // park the state for the sub-split 0 warp of this head
+            sh.mrg[warp][r] = o_lo;
+            sh.mrg[warp][32 + r] = o_hi;
+            if (lane == 0) { sh.mrg[warp][kHeadDim] = M; sh.mrg[warp][kHeadDim + 1] = l_tot; }
         }
-        if (nsub > 1) consumer_sync();
-        if (active && sub == 0) {
-            for (int k = 1; k < nsub; ++k) {
-                const float *o2 = sh.mrg[k * G + g];
-                const float M2 = o2[kHeadDim], l2 = o2[kHeadDim + 1];
-                const float Mn = fmaxf(M, M2);
-                const float wa = (M == -INFINITY) ? 0.f : __expf(M - Mn), wb = (M2 == -INFINITY) ? 0.f : __expf(M2 - Mn);
-                l_tot = l_tot * wa + l2 * wb;
-                o_lo = o_lo * wa + o2[r] * wb;
-                o_hi = o_hi * wa + o2[32 + r] * wb;
-                M = Mn;
-            }
-            if (ns == 1) {   // the whole context in one CTA: final
-                const float inv = 1.0f / l_tot;
-                p.attn_out[head * kHeadDim + r] = o_lo * inv;
-                p.attn_out[head * kHeadDim + 32 + r] = o_hi * inv;
-            } else {
-                const size_t pidx = (size_t)head * kMkMaxSplits + split;
-                p.part_o[pidx * kHeadDim + r] = o_lo;
-                p.part_o[pidx * kHeadDim + 32 + r] = o_hi;
-                if (lane == 0) p.part_ml[pidx] = make_float2(M, l_tot);
-            }
-        }
-        if (item == (int)blockIdx.x) mk_trace(p, c);
-        if (ns > 1) {
-            // the last CTA of this KV head merges the split partials (fixed slot order: deterministic)
-            consumer_sync();
-            if (tid == 0) {
-                __threadfence();
-                const unsigned t = atomicAdd(p.kv_ticket + kvh, 1u);
-                sh.flag = (t == (unsigned)ns - 1u);
-                if (sh.flag) {
-                    p.kv_ticket[kvh] = 0u;
-                    __threadfence();
-                }
-            }
-            consumer_sync();
-            if (sh.flag) {
-                for (int i = tid; i < G * kHeadDim; i += kMkConsumers) {
-                    const int hd = kvh * G + (i >> 6), d = i & 63;
-                    const float2 *ml = p.part_ml + (size_t)hd * kMkMaxSplits;
-                    float Mx = -INFINITY;
-                    for (int s = 0; s < ns; ++s) Mx = fmaxf(Mx, __ldcg(&ml[s]).x);
-                    float acc = 0.f, den = 0.f;
-                    for (int s = 0; s < ns; ++s) {
-                        const float2 v = __ldcg(&ml[s]);
-                        const float wgt = (v.x == -INFINITY) ? 0.f : __expf(v.x - Mx);
-                        den = fmaf(wgt, v.y, den);
-                        acc = fmaf(wgt, __ldcg(p.part_o + ((size_t)hd * kMkMaxSplits + s) * kHeadDim + d), acc);
-                    }
-                    p.attn_out[hd * kHeadDim + d] = acc / den;
-                }
-            }
-        }
-        consumer_sync();   // sh.q / sh.mrg / sh.flag are reused by the next item
     }
-    if ((int)blockIdx.x >= items) { mk_trace(p, c); mk_trace(p, c); }
+    if (nsub > 1) consumer_sync();
+    if (it.active && it.sub == 0) {
+        for (int k = 1; k < nsub; ++k) {
+            const float *o2 = sh.mrg[k * G + it.g];
+            const float M2 = o2[kHeadDim], l2 = o2[kHeadDim + 1];
+            const float Mn = fmaxf(M, M2);
+            const float wa = (M == -INFINITY) ? 0.f : __expf(M - Mn), wb = (M2 == -INFINITY) ? 0.f : __expf(M2 - Mn);
+            l_tot = l_tot * wa + l2 * wb;
+            o_lo = o_lo * wa + o2[r] * wb;
+            o_hi = o_hi * wa + o2[32 + r] * wb;
+            M = Mn;
+        }
+        // unnormalised split state; the O phase of every CTA merges the splits while it stages its input (stage_input)
+        const size_t pidx = (size_t)head * kMkMaxSplits + it.split;
+        p.part_o[pidx * kHeadDim + r] = o_lo;
+        p.part_o[pidx * kHeadDim + 32 + r] = o_hi;
+        if (lane == 0) p.part_ml[pidx] = make_float2(M, l_tot);
+    }
     mk_trace(p, c);
+    mk_trace(p, c);
+    // sh.q / sh.mrg are next written after two more grid barriers
 }
 
 // ---- the kernel -----------------------------------------------------------------------------------------------
@@ -604,8 +724,11 @@ __global__ void __launch_bounds__(kMkThreads, 1) mega_decode_kernel(const __grid
         consumer_sync();
         for (c.layer = 0; c.layer < p.n_layers; ++c.layer) {
             run_phase(p, c, PH_QKV, ring, sh);
+            AttnItem it;
+            KvRow kr, vr;
+            attn_prefetch(p, c, it, kr, vr);
             grid_barrier(p, c);
-            attention_phase(p, c, sh);
+            attention_phase(p, c, sh, it, kr, vr);
             grid_barrier(p, c);
             run_phase(p, c, PH_O, ring, sh);
             grid_barrier(p, c);
@@ -668,9 +791,9 @@ bool mega_shape_supported(const hq_config &c, int n_sms) {
     // the residual rows of one CTA must fit the partial buffer; the group must fit the consumer warps
     const int q = c.n_heads * c.head_dim;
     const int units_cta = (c.hidden / 2 + n_sms - 1) / n_sms;
-    return c.hidden <= 8 * kMkSliceChunks && q <= 64 * kMkSliceChunks && c.ffn <= 64 * kMkSliceChunks &&
+    return c.hidden <= kMkStagedK && q <= kMkStagedK && c.ffn <= 64 * kMkSliceChunks &&
            2 * units_cta <= kMkPartRows && c.n_heads / c.n_kv_heads <= kMkConsumerWarps && c.hidden % 8 == 0 &&
-           c.ffn % 8 == 0 && c.vocab % 2 == 0 && n_sms >= 1;
+           c.ffn % 8 == 0 && c.vocab % 2 == 0 && n_sms >= c.n_kv_heads;
 }
 
 cudaError_t launch_mega(const LaunchCtx &c, const MegaParams &p, bool cooperative) {
