@@ -308,6 +308,22 @@ def main():
         kernels[name] = {"us": ms * 1e3, "GBps": nbytes / ms / 1e6}
     kernels["gate_up"] = {"us": gu_ms * 1e3, "GBps": gu_bytes / gu_ms / 1e6}
 
+    # ---- the persistent-kernel path, same workload, reported beside the default ------------------------------
+    gm_mega = hq.Model(gm.cfg_with_flags(hq.FLAG_MEGA), *gm.weight_tensors())   # same device weights
+    for _ in range(3):
+        gm_mega.kv_reset(); gm_mega.prefill(prompt, want_token=False); gm_mega.decode_run(DECODE_STEPS, want_tokens=False)
+    torch.cuda.synchronize(dev)
+    mega_ms = []
+    for _ in range(max(1, min(args.steps, 3))):
+        gm_mega.kv_reset(); gm_mega.prefill(prompt, want_token=False)
+        a, b = ev(), ev()
+        a.record(gm_mega.stream)
+        gm_mega.decode_run(DECODE_STEPS, want_tokens=False)
+        b.record(gm_mega.stream)
+        torch.cuda.synchronize(dev)
+        mega_ms.append(a.elapsed_time(b))
+    mega_tok_s = DECODE_STEPS / (float(np.mean(mega_ms)) * 1e-3)
+
     # ---- aggregate over ranks (max time) -----------------------------------------------------------------
     dec_total_ms = float(sum(decode_ms))
     if dist is not None:
@@ -349,6 +365,8 @@ def main():
             "step_roofline": {"bytes_per_token": bpt, "achieved_GBps": step_gbs, "frac_of_measured": step_gbs / peak,
                               "frac_of_8TBps_spec": step_gbs / 8000.0},
             "kernels_alone": kernels,
+            "persistent_kernel": {"value": mega_tok_s, "unit": UNIT,
+                                  "note": "HQ_FLAG_MEGA: the same 128 decode steps in ONE launch (hq_mega.cu), this rank"},
         }
         if not args.no_cpu_baseline:
             line["cpu_baseline"] = oracle_sample(weights, s)

@@ -50,7 +50,8 @@ enum {
     HQ_FLAG_CAPTURE_HIDDEN = 1u, /* keep the residual stream after every layer (parity tests) */
     HQ_FLAG_NO_GRAPH = 2u,       /* launch decode kernels directly instead of replaying a CUDA graph */
     HQ_FLAG_NO_PDL = 4u,         /* no programmatic dependent launch edges between kernels */
-    HQ_FLAG_NO_MEGA = 8u         /* batch-1 decode as one kernel per step of the path instead of the persistent kernel */
+    HQ_FLAG_NO_MEGA = 8u,        /* never use the persistent decode kernel (wins over HQ_FLAG_MEGA and the HQ_MEGA environment variable) */
+    HQ_FLAG_MEGA = 16u           /* batch-1 decode in ONE persistent kernel per call instead of one kernel per step of the path */
 };
 
 typedef struct hq_model hq_model; /* opaque, library-owned (host memory) */
@@ -91,9 +92,9 @@ size_t hq_workspace_bytes(const hq_config *cfg);
  * >= hq_workspace_bytes).  cuda_stream is a cudaStream_t (NULL = legacy default stream).
  * Supported shapes: head_dim == 64, n_heads % n_kv_heads == 0 with group size <= 8, hidden and
  * ffn multiples of 8 and <= 8192, max_batch <= 32; anything else returns HQ_ERR_UNSUPPORTED.
- * batch 1 decodes in one persistent kernel per call (TMA-fed weight ring, grid barriers between the steps of
- * the path; HQ_FLAG_NO_MEGA selects one GEMV kernel per step of the path instead); batch > 1 and prompts of
- * >= 8 tokens run on the tcgen05 GEMM path.
+ * batch 1 decodes with one fused GEMV kernel per step of the path inside a CUDA graph (default, the faster of the two
+ * on B200 today), or with HQ_FLAG_MEGA in one persistent kernel per call (TMA-fed weight ring, tagged-word exchange
+ * between the SMs, no grid barrier); batch > 1 and prompts of >= 8 tokens run on the tcgen05 GEMM path.
  * Requires compute capability 10.x. */
 int32_t hq_model_create(const hq_config *cfg, const hq_weights *weights, void *workspace_dev,
                         size_t workspace_bytes, void *cuda_stream, hq_model **out);

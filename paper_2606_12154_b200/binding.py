@@ -17,6 +17,7 @@ FLAG_CAPTURE_HIDDEN = 1
 FLAG_NO_GRAPH = 2
 FLAG_NO_PDL = 4
 FLAG_NO_MEGA = 8
+FLAG_MEGA = 16
 
 HQ_OK, HQ_ERR_INVALID_ARG, HQ_ERR_CAPACITY, HQ_ERR_STATE, HQ_ERR_CUDA, HQ_ERR_UNSUPPORTED = 0, -1, -2, -3, -4, -5
 _CODE_NAMES = {-1: "HQ_ERR_INVALID_ARG", -2: "HQ_ERR_CAPACITY", -3: "HQ_ERR_STATE", -4: "HQ_ERR_CUDA",
@@ -186,6 +187,16 @@ class Model:
                           max_batch=max_batch, max_seq=max_seq, flags=flags)
         layers = [{k: up(l[k]) for k in LAYER_TENSORS} for l in layer_bits]
         return cls(cfg, up(embedding_bits), up(final_norm_bits), layers, stream=stream)
+
+    def cfg_with_flags(self, flags: int) -> "Config":
+        """A copy of this model's config with other HQ_FLAG_* bits (for a second model over the same weights)."""
+        c = Config.from_buffer_copy(self.cfg)
+        c.flags = flags
+        return c
+
+    def weight_tensors(self):
+        """(embedding, final_norm, layers, lm_head) device tensors this model borrows."""
+        return tuple(self._keep)
 
     def close(self):
         h, self._h = getattr(self, "_h", None), None

@@ -113,10 +113,8 @@ static size_t carve(const hq_config *c, char *base, Buffers *b) {
     o.actb = (act_t *)take(2 * R * F * sizeof(act_t));
     o.hn_last = (act_t *)take(2 * 32 * d * sizeof(act_t));
     o.mk_layers = (LayerW *)take(L * sizeof(LayerW));
-    o.mk_qkv = (float *)take(qkvd * sizeof(float));
-    o.mk_attn_out = (float *)take(qdim * sizeof(float));
-    o.mk_part_o = (float *)take(H * kMkMaxParts * kHeadDim * sizeof(float));
-    o.mk_part_ml = (float2 *)take(H * kMkMaxParts * sizeof(float2));
+    o.mk_ll = (unsigned long long *)take(mega_ll_words(*c) * sizeof(unsigned long long));
+    o.mk_epoch = (unsigned int *)take(sizeof(unsigned int));
     o.mk_sync = (unsigned int *)take(64 * sizeof(unsigned int));
     return off;
 }
@@ -143,16 +141,23 @@ static MegaParams mega_params(const hq_model *m, const int *tok_src, int n_steps
     p.kc = b.kcache; p.vc = b.vcache;
     p.layer_kv = (size_t)c.max_batch * c.n_kv_heads * c.max_seq * kHeadDim;
     p.pos = b.pos; p.cur_tok = b.cur_tok; p.tok_hist = b.tok_hist; p.tok_src = tok_src;
-    p.best2 = (unsigned long long *)(b.mk_sync + 4);
-    p.bar = b.mk_sync; p.exit_ticket = b.mk_sync + 1; p.err = (int *)(b.mk_sync + 3);
-    p.kv_ticket = b.mk_sync + 8;
+    p.epoch = b.mk_epoch; p.err = (int *)(b.mk_sync + 3);
     p.trace = m->trace; p.trace_cap = m->trace_cap;
-    p.x = b.x; p.qkv = b.mk_qkv; p.attn_out = b.mk_attn_out; p.act = b.act; p.logits = b.logits;
-    p.part_o = b.mk_part_o; p.part_ml = b.mk_part_ml;
+    {   // carve the exchange buffers (layout must match mega_ll_words)
+        const size_t H = c.n_heads, Hkv = c.n_kv_heads;
+        unsigned long long *w = b.mk_ll;
+        p.ll_x = w; w += 2 * (size_t)c.hidden;
+        p.ll_qkv = w; w += (H + 2 * Hkv) * kHeadDim;
+        p.ll_act = w; w += c.ffn;
+        p.ll_part_o = w; w += H * kMkMaxSplits * kHeadDim;
+        p.ll_part_ml = w; w += H * kMkMaxSplits * 2;
+        p.ll_best = w;
+    }
+    p.logits = b.logits;
     p.hidden_out = (c.flags & HQ_FLAG_CAPTURE_HIDDEN) ? b.hidden : nullptr;
     p.hidden_stride = (size_t)c.max_batch * c.hidden;
     p.n_steps = n_steps; p.with_head = with_head ? 1 : 0;
-    p.prefetch_stages = m->mega_prefetch;
+    p.inflight_stages = m->mega_inflight;
     return p;
 }
 
@@ -437,11 +442,15 @@ extern "C" int32_t hq_model_create(const hq_config *cfg, const hq_weights *w, vo
         return fail(HQ_ERR_CUDA, "hq_model_create: cuTensorMapEncodeTiled failed (driver entry point or bad alignment)");
     }
     m->use_pdl = !(cfg->flags & HQ_FLAG_NO_PDL) && !getenv("HQ_NO_PDL");
-    if (const char *pf = getenv("HQ_MEGA_PREFETCH")) m->mega_prefetch = atoi(pf) < 0 ? 0 : (atoi(pf) > 64 ? 64 : atoi(pf));
-    m->use_mega = !(cfg->flags & HQ_FLAG_NO_MEGA) && !getenv("HQ_NO_MEGA") && mega_shape_supported(*cfg, m->n_sms);
+    if (const char *fl = getenv("HQ_MEGA_INFLIGHT")) m->mega_inflight = atoi(fl) < 1 ? 1 : (atoi(fl) > kMkStages ? kMkStages : atoi(fl));
+    m->use_mega = ((cfg->flags & HQ_FLAG_MEGA) || getenv("HQ_MEGA")) && !(cfg->flags & HQ_FLAG_NO_MEGA) && !getenv("HQ_NO_MEGA") &&
+                  mega_shape_supported(*cfg, m->n_sms);
     {
         cudaError_t e = cudaMemcpyAsync(m->b.mk_layers, m->layers.data(), m->layers.size() * sizeof(LayerW),
                                         cudaMemcpyHostToDevice, m->stream);
+        // tagged exchange words start with tag 0 (never a valid epoch); the epoch counter only ever grows
+        if (e == cudaSuccess) e = cudaMemsetAsync(m->b.mk_ll, 0, mega_ll_words(*cfg) * sizeof(unsigned long long), m->stream);
+        if (e == cudaSuccess) e = cudaMemsetAsync(m->b.mk_epoch, 0, sizeof(unsigned int), m->stream);
         if (e == cudaSuccess) e = cudaStreamSynchronize(m->stream);
         if (e != cudaSuccess) {
             delete m;

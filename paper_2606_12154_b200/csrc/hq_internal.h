@@ -34,9 +34,8 @@ constexpr int kGemvThreads = 256;
 constexpr int kMkSliceChunks = 256;   // 16-byte chunks of one row slice (2048 bf16): what one warp keeps of x in registers
 constexpr int kMkStageBytes = 65536;  // one ring stage: 16 slices = 8 / S units of two rows
 constexpr int kMkStages = 3;          // ring depth: 192 KB of weights in flight per SM
-constexpr int kMkPrefetchStages = 0;  // default L2 look-ahead of the producer beyond the ring (HQ_MEGA_PREFETCH overrides)
-constexpr int kMkMaxSplits = 32;      // context splits per KV head
-constexpr int kMkMaxParts = 128;      // attention partial slots per head in the workspace (>= kMkMaxSplits)
+constexpr int kMkMaxSplits = 8;       // context splits per KV head (every CTA re-reads all split states in the O phase)
+constexpr int kMkMaxGrid = 1024;      // per-CTA argmax slots in the exchange buffer
 
 struct alignas(64) TensorMap { uint64_t opaque[16]; };   // mirrors CUtensorMap (driver type, 128 bytes)
 
@@ -74,11 +73,9 @@ struct Buffers {
     act_t *hn_last = nullptr;                   // [2][32][d] normalised last rows (LM-head operand, hi/lo)
     // persistent decode kernel (batch 1)
     struct LayerW *mk_layers = nullptr;         // [L] device copy of the per-layer weight pointers
-    float *mk_qkv = nullptr;                    // [(H+2Hkv)*64] RoPE'd q, RoPE'd k, v of the current token
-    float *mk_attn_out = nullptr;               // [H*64] merged attention output
-    float *mk_part_o = nullptr;                 // [H][kMkMaxParts][64]
-    float2 *mk_part_ml = nullptr;               // [H][kMkMaxParts]
-    unsigned int *mk_sync = nullptr;            // [0] grid barrier, [1] exit ticket, [3] error, [4..7] two packed-argmax slots, [8..63] per-KV-head tickets
+    unsigned long long *mk_ll = nullptr;        // tagged-word exchange buffers (mega_ll_words() words, zeroed at create)
+    unsigned int *mk_epoch = nullptr;           // steps run so far by the persistent kernel (never reset: tags only grow)
+    unsigned int *mk_sync = nullptr;            // [3] error flag of the persistent kernel
 };
 
 constexpr int kTokenTiles[4] = {32, 64, 128, 256};
@@ -107,7 +104,7 @@ struct hq_model_impl {
     int batch_graph_b = 0, batch_graph_kernels = 0, batch_eager_b = 0;
     bool use_mega = false;                      // batch-1 decode runs in the persistent kernel
     bool mega_coop = true;                      // launched with the cooperative attribute
-    int mega_prefetch = kMkPrefetchStages;      // L2 look-ahead of the persistent kernel's producer (ring stages)
+    int mega_inflight = 2;                      // bulk-copy stages in flight per SM during the layers (HQ_MEGA_INFLIGHT overrides)
     unsigned long long *trace = nullptr;        // hq_debug_trace: device buffer [n_sms][trace_cap] or NULL
     int trace_cap = 0;
 };
@@ -175,21 +172,26 @@ struct MegaParams {
     size_t layer_kv;             // elements per layer
     // device-resident step state
     int *pos, *cur_tok, *tok_hist;
-    const int *tok_src;          // token fed at the first step (later steps feed cur_tok)
-    unsigned long long *best2;   // [2] packed argmax of the step, slots alternate; zero between launches
-    unsigned int *bar, *exit_ticket, *kv_ticket;
+    const int *tok_src;          // token fed at the first step (later steps feed the token the kernel just chose)
+    unsigned int *epoch;         // steps run by earlier launches: base of the tags of this launch, advanced at exit
     int *err;
     unsigned long long *trace;   // NULL or [grid][trace_cap] global-timer stamps (hq_debug_trace)
     int trace_cap;
-    // activations (fp32)
-    float *x, *qkv, *attn_out, *act, *logits, *part_o;
-    float2 *part_ml;
+    // cross-CTA exchange buffers of tagged words (fp32 value | epoch tag), see hq_mega.cu
+    unsigned long long *ll_x;        // [2][hidden]: residual after the O projection / after the down projection
+    unsigned long long *ll_qkv;      // [(H+2Hkv)*64] RoPE'd q, RoPE'd k, v of the current token
+    unsigned long long *ll_act;      // [ffn] SwiGLU output
+    unsigned long long *ll_part_o;   // [H][kMkMaxSplits][64] split-KV partial outputs (unnormalised)
+    unsigned long long *ll_part_ml;  // [H][kMkMaxSplits][2] (m, l)
+    unsigned long long *ll_best;     // [grid][2] per-CTA argmax (ordered logit key, index)
+    float *logits;
     float *hidden_out;           // NULL or [n_layers][hidden_stride] residual after every layer
     size_t hidden_stride;
     int n_steps, with_head;
-    int prefetch_stages;         // producer: L2 look-ahead beyond the ring, in ring stages (0 = off)
+    int inflight_stages;         // producer: at most this many ring stages issued and not yet landed (1..kMkStages)
 };
 size_t mega_smem_bytes();
+size_t mega_ll_words(const hq_config &c);   // 64-bit words of exchange buffers
 bool mega_shape_supported(const hq_config &c, int n_sms);
 cudaError_t launch_mega(const LaunchCtx &c, const MegaParams &p, bool cooperative);
 

@@ -6,25 +6,30 @@
 // stream never stops:
 //   * grid = one CTA per SM, 9 warps.  Warp 8 is the PRODUCER: one elected thread walks the static schedule
 //     (layer, phase, this CTA's rows) and streams every weight row with cp.async.bulk (TMA bulk copy,
-//     mbarrier complete_tx) into a ring of kMkStages x 64 KB shared-memory stages.  Weights are immutable, so
-//     the producer runs ahead of the phase barriers: while the consumers wait for the other SMs, do the
-//     attention, or reduce, the next phases' rows are already landing.
+//     mbarrier complete_tx, L2 evict-first) into a ring of kMkStages x 64 KB shared-memory stages.  Weights are
+//     immutable, so the producer runs ahead of the data dependencies: while the consumers wait for another SM's
+//     result or do the attention, the next phases' rows are already landing.
 //   * warps 0-7 are CONSUMERS and never synchronise with one another inside a weight phase.  A stage holds
 //     8/S "units" (a unit = two rows: RoPE pair (i, i+32) / gate+up pair / two adjacent rows); a row is cut
 //     into S slices of <= 2048 elements and warp w owns slice w % S of unit w / S, so the slice of the
 //     (normalised) input vector it needs stays in 64 registers for the whole phase.  Per stage and warp: two
 //     conflict-free 16-byte shared loads per chunk, fp32 FMA, one 6-shuffle reduction for both rows, one
 //     mbarrier arrive, and the fused epilogue (RoPE + KV append, SwiGLU, logits + packed argmax) from lane 0.
-//     Only the residual projections (O, down) park their per-slice partials in shared memory and finish after
-//     one CTA barrier at the end of the phase.
-//   * phases are separated by a grid barrier (red.release + ld.acquire poll on a global counter): per layer
-//     QKV | attention | O | gate/up | down, then the LM head.  The token and the position stay on the device;
-//     the kernel loops over n_steps tokens (hq_decode_run) so there is no launch gap between tokens either.
+//   * NO GRID BARRIERS AND NO FENCES.  Measured on B200 (profiles/r01_mega_sync_microbench.md): with the ring's
+//     192 KB of bulk copies in flight per SM a membar.gpu / red.release takes 3-9 us (idle: 0.35 us) and a
+//     release/acquire grid barrier 10 us, i.e. more than the 1.2 us of DRAM time of a small phase.  So every vector that
+//     crosses CTAs (residual x, q/k/v of the token, split-KV partials, SwiGLU output, per-CTA argmax) travels
+//     as 8-byte (fp32 value, 32-bit epoch tag) words written with ONE relaxed 64-bit store each and polled by
+//     the readers until every tag equals the epoch of (step, layer) — the "flag in the data" protocol of
+//     latency-bound collectives.  A 64-bit aligned store is single-copy atomic, so a matching tag proves the
+//     value; no ordering between different words is ever needed.  Reuse of a buffer is safe by the data
+//     dependencies themselves (its next writer needs, transitively, a result from every reader of the
+//     previous epoch).
 //   * attention: work item = (KV head, context split); warp = (query head of the group, sub-split); LANE =
 //     POSITION: every lane runs its own online softmax over its positions (K/V rows are one 128-byte line each,
-//     read with 256-bit loads), then the 32 lane states are merged with a transposed butterfly, the sub-splits
-//     through shared memory, and the splits by the last CTA of the KV head (ticket), so the O phase reads a
-//     plain vector.
+//     read with 256-bit loads issued BEFORE the warp waits for its query), then the 32 lane states are merged
+//     with a transposed butterfly, the sub-splits through shared memory; the split states (m, l, o) go out as
+//     tagged words and every CTA merges them while it stages the input of the O projection.
 #include "hq_common.cuh"
 #include "hq_internal.h"
 
@@ -33,8 +38,9 @@ namespace hq {
 constexpr int kMkConsumerWarps = 8;
 constexpr int kMkConsumers = 32 * kMkConsumerWarps;
 constexpr int kMkThreads = kMkConsumers + 32;
-constexpr int kMkPartRows = 64;
-constexpr int kMkStagedK = 8 * kMkConsumers;      // 2048: one 8-element chunk per consumer thread                   // residual rows of one CTA in one phase (2 * units)
+constexpr int kMkPartRows = 64;                   // residual rows of one CTA in one phase (2 * units)
+constexpr int kMkStagedK = 8 * kMkConsumers;      // 2048: one 8-element chunk per consumer thread
+constexpr unsigned kMaxPollSpins = 1u << 23;      // poll rounds (each >= one L2 round trip + 64 ns sleep) before a lost word traps
 constexpr long long kSpinCycles = 6000000000ll;   // ~3 s of SM clocks: a lost arrival traps instead of hanging the GPU
 
 enum { PH_QKV = 0, PH_O = 1, PH_GATEUP = 2, PH_DOWN = 3, PH_HEAD = 4 };
@@ -61,17 +67,20 @@ __device__ __forceinline__ bool mk_mbar_try_wait(uint64_t *bar, uint32_t parity)
         : "memory");
     return ok != 0;
 }
-__device__ __forceinline__ void mk_fail(int *err, int code) {
+__device__ __noinline__ void mk_fail(int *err, int code) {
     atomicExch(err, code);
     __threadfence_system();
     __trap();
 }
-__device__ __forceinline__ void mk_mbar_wait(uint64_t *bar, uint32_t parity, int *err) {
-    if (mk_mbar_try_wait(bar, parity)) return;
+// slow path out of line: the kernel's steady-state code must fit the instruction cache (see consume_phase)
+__device__ __noinline__ void mk_mbar_wait_slow(uint64_t *bar, uint32_t parity, int *err) {
     const long long t0 = clock64();
     unsigned spins = 0;
     while (!mk_mbar_try_wait(bar, parity))
         if ((++spins & 1023u) == 0 && clock64() - t0 > kSpinCycles) mk_fail(err, 1);
+}
+__device__ __forceinline__ void mk_mbar_wait(uint64_t *bar, uint32_t parity, int *err) {
+    if (!mk_mbar_try_wait(bar, parity)) mk_mbar_wait_slow(bar, parity, err);
 }
 __device__ __forceinline__ void mk_bulk_g2s(void *smem_dst, const void *gmem_src, uint32_t bytes, uint64_t *bar) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
@@ -92,18 +101,39 @@ __device__ __forceinline__ void mk_bulk_g2s_hint(void *smem_dst, const void *gme
                  "l"(gmem_src), "r"(bytes), "r"(mk_smem_u32(bar)), "l"(pol)
                  : "memory");
 }
-// fire-and-forget HBM -> L2 prefetch of a weight row (no completion tracking: the later bulk copy just hits L2)
-__device__ __forceinline__ void mk_bulk_prefetch_l2(const void *gmem_src, uint32_t bytes, uint64_t pol) {
-    asm volatile("cp.async.bulk.prefetch.L2.global.L2::cache_hint [%0], %1, %2;" ::"l"(gmem_src), "r"(bytes), "l"(pol) : "memory");
-}
 __device__ __forceinline__ void consumer_sync() { asm volatile("bar.sync 1, %0;" ::"n"(kMkConsumers) : "memory"); }
-__device__ __forceinline__ unsigned ld_acquire_u32(const unsigned *p) {
-    unsigned v;
-    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-    return v;
+// ---- tagged words: (fp32 value | 32-bit epoch tag) in one 64-bit word -------------------------------------
+typedef unsigned long long llw_t;
+__device__ __forceinline__ void ll_store(llw_t *p, float v, uint32_t tag) {
+    const llw_t w = ((llw_t)tag << 32) | (llw_t)__float_as_uint(v);
+    asm volatile("st.global.cg.u64 [%0], %1;" ::"l"(p), "l"(w) : "memory");
 }
-__device__ __forceinline__ void red_release_add(unsigned *p, unsigned v) {
-    asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+__device__ __forceinline__ void ll_store_u32(llw_t *p, uint32_t v, uint32_t tag) {
+    const llw_t w = ((llw_t)tag << 32) | (llw_t)v;
+    asm volatile("st.global.cg.u64 [%0], %1;" ::"l"(p), "l"(w) : "memory");
+}
+__device__ __forceinline__ void ll_load2(const llw_t *p, llw_t &a, llw_t &b) {
+    asm volatile("ld.volatile.global.v2.u64 {%0,%1}, [%2];" : "=l"(a), "=l"(b) : "l"(p) : "memory");
+}
+__device__ __forceinline__ bool ll_ok(llw_t w, uint32_t tag) { return (uint32_t)(w >> 32) == tag; }
+__device__ __forceinline__ float ll_val(llw_t w) { return __uint_as_float((uint32_t)w); }
+// Poll N (even) consecutive tagged words until all carry `tag`.  All loads of a round are in flight together.
+template <int N>
+__device__ __forceinline__ void ll_poll(const llw_t *src, uint32_t tag, float (&v)[N], int *err) {
+    llw_t w[N];
+    unsigned spins = 0;
+    for (;;) {
+#pragma unroll
+        for (int i = 0; i < N; i += 2) ll_load2(src + i, w[i], w[i + 1]);
+        bool ok = true;
+#pragma unroll
+        for (int i = 0; i < N; ++i) ok = ok && ll_ok(w[i], tag);
+        if (ok) break;
+        if (++spins == kMaxPollSpins) mk_fail(err, 3);
+        __nanosleep(64);
+    }
+#pragma unroll
+    for (int i = 0; i < N; ++i) v[i] = ll_val(w[i]);
 }
 __device__ __forceinline__ unsigned long long mk_globaltimer() {
     unsigned long long t;
@@ -157,7 +187,8 @@ __device__ __forceinline__ PhaseGeom phase_geom(const MegaParams &p, int ph) {
     const int chunks = g.K >> 3;
     g.S = 1;
     g.log2S = 0;
-    while ((chunks + g.S - 1) / g.S > kMkSliceChunks) { g.S <<= 1; ++g.log2S; }
+    const int lim = chunks > kMkSliceChunks ? kMkSliceChunks / 2 : kMkSliceChunks;   // un-staged inputs: 4 chunks per lane = one poll round
+    while ((chunks + g.S - 1) / g.S > lim) { g.S <<= 1; ++g.log2S; }
     g.cps = (chunks + g.S - 1) / g.S;
     g.ups = kMkConsumerWarps >> g.log2S;
     const int n = phase_units(p, ph), per = n / gridDim.x, rem = n % gridDim.x, b = blockIdx.x;
@@ -190,143 +221,93 @@ __device__ __forceinline__ void unit_row_ptrs(const MegaParams &p, const LayerW 
 
 struct MkShared {
     uint64_t full[kMkStages], empty[kMkStages];
+    PhaseGeom geo[5];                            // this CTA's static schedule, computed once (integer divisions out of the loop)
     alignas(16) float xs[kMkStagedK];            // phase input staged once per CTA (phases with K <= kMkStagedK)
     float part[kMkPartRows][kMkConsumerWarps];   // residual phases: [row of this CTA][slice] partial sums
     float2 rope[32];
-    alignas(16) float q[kMkConsumerWarps][kHeadDim];   // per warp: pre-scaled query of its head
+    alignas(16) kv_t kvnew[kMkConsumerWarps][2][kHeadDim];   // per warp: this step's K and V row (fp16 like the cache)
     float mrg[kMkConsumerWarps][kHeadDim + 2];   // attention: sub-split states (o[64], m, l)
     float red[kMkConsumerWarps];                 // RMSNorm: per-warp sum of squares
     unsigned long long wbest[kMkConsumerWarps];  // LM head: per-warp packed argmax
 };
 
 // ---- producer ----------------------------------------------------------------------------------------------
-// Position in this CTA's static stage schedule: (step, phase index, stage of the phase).
-struct MkCursor {
-    int step, pi, s, ph, layer;
-    PhaseGeom geo;
-    bool done;
-};
-__device__ __forceinline__ void cursor_load_phase(const MegaParams &p, MkCursor &c) {
-    const int n_ph = p.n_layers * 4 + (p.with_head ? 1 : 0);
-    for (;;) {   // skip phases in which this CTA owns no unit
-        if (c.pi == n_ph) { c.pi = 0; ++c.step; }
-        if (c.step >= p.n_steps) { c.done = true; return; }
-        c.layer = c.pi >> 2;
-        c.ph = c.layer < p.n_layers ? (c.pi & 3) : PH_HEAD;
-        c.geo = phase_geom(p, c.ph);
-        if (c.geo.n_stages > 0) return;
-        ++c.pi;
-    }
-}
-__device__ __forceinline__ void cursor_init(const MegaParams &p, MkCursor &c) {
-    c.step = 0; c.pi = 0; c.s = 0; c.done = false;
-    cursor_load_phase(p, c);
-}
-__device__ __forceinline__ void cursor_next(const MegaParams &p, MkCursor &c) {
-    if (++c.s == c.geo.n_stages) { c.s = 0; ++c.pi; cursor_load_phase(p, c); }
-}
-
-// One elected thread.  Two cursors walk the same schedule: `ld` fills the shared-memory ring (TMA bulk copies, mbarrier
-// complete_tx), `pf` runs p.prefetch_stages stages ahead of it and only pulls the rows HBM -> L2.  The ring alone holds
-// ~4 us of streaming; the dependent chain down -> QKV -> attention -> O of a layer is longer than that, so without the
-// L2 look-ahead the HBM pipe would idle while the consumers sit in grid barriers.
+// One elected thread walks this CTA's static schedule and fills the shared-memory ring (TMA bulk copies, mbarrier
+// complete_tx, L2 evict-first).  At most p.inflight_stages stages are issued and not yet landed: a deeper queue buys no
+// bandwidth, it only delays the small exchange loads and stores (and instruction fetches) that share the memory system
+// with the stream (queueing delay = bytes in flight / HBM rate, profiles/r01_mega_sync_microbench.md).
 __device__ void mk_producer(const MegaParams &p, uint8_t *ring, MkShared &sh) {
     const uint64_t pol = mk_policy_evict_first();
-    MkCursor ld, pf;
-    cursor_init(p, ld);
-    pf = ld;
-    int ahead = 0;   // stages pf is ahead of ld
-    unsigned g = 0;  // stages produced so far
-    while (!ld.done) {
-        while (!pf.done && ahead < p.prefetch_stages) {
-            if (ahead > 0) {   // distance 0 would duplicate the bulk copy issued right below
-                const LayerW &w = p.layers[pf.layer < p.n_layers ? pf.layer : 0];
-                const int ub = pf.geo.u0 + pf.s * pf.geo.ups;
-                const int nu = min(pf.geo.ups, pf.geo.u1 - ub);
+    const int n_ph = p.n_layers * 4 + (p.with_head ? 1 : 0);
+    unsigned g = 0;   // stages produced so far
+    for (int step = 0; step < p.n_steps; ++step)
+        for (int pi = 0; pi < n_ph; ++pi) {
+            const int layer = pi >> 2;
+            const int ph = layer < p.n_layers ? (pi & 3) : PH_HEAD;
+            const LayerW &w = p.layers[layer < p.n_layers ? layer : 0];
+            const PhaseGeom &geo = sh.geo[ph];
+            for (int s = 0; s < geo.n_stages; ++s, ++g) {
+                const int slot = g % kMkStages;
+                mk_mbar_wait(&sh.empty[slot], ((g / kMkStages) & 1) ^ 1, p.err);
+                // the LM head has no exchange to protect: full depth there (7.1 vs 5.4 TB/s)
+                const unsigned infl = ph == PH_HEAD ? (unsigned)kMkStages : (unsigned)p.inflight_stages;
+                if (g >= infl) {
+                    const unsigned gl = g - infl;
+                    mk_mbar_wait(&sh.full[gl % kMkStages], (gl / kMkStages) & 1, p.err);
+                }
+                const int ub = geo.u0 + s * geo.ups;
+                const int nu = min(geo.ups, geo.u1 - ub);
+                mk_mbar_expect_tx(&sh.full[slot], (uint32_t)(2 * nu * geo.row_bytes));
+                uint8_t *dst = ring + (size_t)slot * kMkStageBytes;
+#pragma unroll 1
                 for (int j = 0; j < nu; ++j) {
                     const bf16 *ra, *rb;
-                    unit_row_ptrs(p, w, pf.ph, pf.geo.K, ub + j, ra, rb);
-                    mk_bulk_prefetch_l2(ra, pf.geo.row_bytes, pol);
-                    mk_bulk_prefetch_l2(rb, pf.geo.row_bytes, pol);
+                    unit_row_ptrs(p, w, ph, geo.K, ub + j, ra, rb);
+                    mk_bulk_g2s_hint(dst + (size_t)(2 * j) * geo.row_bytes, ra, geo.row_bytes, &sh.full[slot], pol);
+                    mk_bulk_g2s_hint(dst + (size_t)(2 * j + 1) * geo.row_bytes, rb, geo.row_bytes, &sh.full[slot], pol);
                 }
             }
-            cursor_next(p, pf);
-            ++ahead;
         }
-        const int slot = g % kMkStages;
-        const uint32_t par = (g / kMkStages) & 1;
-        mk_mbar_wait(&sh.empty[slot], par ^ 1, p.err);
-        const LayerW &w = p.layers[ld.layer < p.n_layers ? ld.layer : 0];
-        const int ub = ld.geo.u0 + ld.s * ld.geo.ups;
-        const int nu = min(ld.geo.ups, ld.geo.u1 - ub);
-        mk_mbar_expect_tx(&sh.full[slot], (uint32_t)(2 * nu * ld.geo.row_bytes));
-        uint8_t *dst = ring + (size_t)slot * kMkStageBytes;
-        for (int j = 0; j < nu; ++j) {
-            const bf16 *ra, *rb;
-            unit_row_ptrs(p, w, ld.ph, ld.geo.K, ub + j, ra, rb);
-            mk_bulk_g2s_hint(dst + (size_t)(2 * j) * ld.geo.row_bytes, ra, ld.geo.row_bytes, &sh.full[slot], pol);
-            mk_bulk_g2s_hint(dst + (size_t)(2 * j + 1) * ld.geo.row_bytes, rb, ld.geo.row_bytes, &sh.full[slot], pol);
-        }
-        cursor_next(p, ld);
-        ++g;
-        if (ahead > 0) --ahead;
-    }
 }
 
 // ---- consumer state ------------------------------------------------------------------------------------------
 struct MkCtx {
     unsigned g;          // stages consumed so far
-    unsigned bar_target; // thread 0: arrivals expected at the next grid barrier
     int pos, tok;
     int layer;
+    uint32_t tag;        // epoch tag of (step, layer): every word exchanged in this layer carries it
+    uint32_t tag_prev;   // tag of the previous layer of this step (input of the QKV phase / the LM head)
+    float rold;          // residual phases: thread tid < rows of this CTA keeps x[row] in a register
     int ti;              // trace cursor (thread 0)
     unsigned long long best;
 };
 
-// optional timeline (hq_debug_trace): every CTA's thread 0 stamps the global timer at each phase boundary
+// optional timeline (hq_debug_trace): every CTA's thread 0 stamps the global timer at fixed points
+template <bool TRACE>
 __device__ __forceinline__ void mk_trace(const MegaParams &p, MkCtx &c) {
-    if (p.trace && threadIdx.x == 0) {
+    if (TRACE && p.trace && threadIdx.x == 0) {
         if (c.ti < p.trace_cap) p.trace[(size_t)blockIdx.x * p.trace_cap + c.ti] = mk_globaltimer();
         ++c.ti;
     }
 }
 
-// Grid barrier.  bar.sync orders every consumer's global stores of the phase before thread 0's gpu-scope
-// release (cumulativity); the acquire poll + bar.sync orders the other CTAs' stores before every consumer's
-// later loads.
-__device__ __forceinline__ void grid_barrier(const MegaParams &p, MkCtx &c) {
-    consumer_sync();
-    if (threadIdx.x == 0) {
-        c.bar_target += gridDim.x;
-        red_release_add(p.bar, 1u);
-        mk_trace(p, c);
-        const long long t0 = clock64();
-        unsigned spins = 0;
-        while ((int)(ld_acquire_u32(p.bar) - c.bar_target) < 0)
-            if ((++spins & 1023u) == 0 && clock64() - t0 > kSpinCycles) mk_fail(p.err, 2);
-    }
-    consumer_sync();
-    mk_trace(p, c);
-}
-
 // attention split policy (device only; a function of the context length and the grid): one 32-position
-// iteration per warp while the grid has CTAs to spare, then longer splits.  n_kv_heads * splits <= gridDim.x, so
+// iterations per warp before another split is added (every CTA re-reads all split states: few splits = one poll round).  n_kv_heads * splits <= gridDim.x, so
 // every CTA owns at most one (KV head, split) item.
 __device__ __forceinline__ int mk_num_splits(const MegaParams &p, int n_ctx, int nsub) {
     int ns_max = (int)gridDim.x / p.n_kv_heads;
     ns_max = ns_max < 1 ? 1 : (ns_max > kMkMaxSplits ? kMkMaxSplits : ns_max);
-    const int per = 32 * nsub;
+    const int per = 64 * nsub;
     const int want = (n_ctx + per - 1) / per;
     return want < ns_max ? want : ns_max;
 }
 
-// Phase input, K <= kMkStagedK: the CTA reads the vector from L2 ONCE (thread t owns elements [8t, 8t+8)), applies the
-// fused prologue, and leaves it in shared memory for its 8 warps.  (Every warp fetching its own copy made all 1184
-// warps of the chip hit the same 64 L2 lines at once: 4-5 us per phase, profiles/r01_mega_timeline.md.)
+// Phase input, K <= kMkStagedK: the CTA polls the tagged vector from L2 ONCE (thread t owns elements [8t, 8t+8)),
+// applies the fused prologue, and leaves it in shared memory for its 8 warps.
 //   QKV, gate/up, LM head: A2 RMSNorm (sum of squares reduced across the CTA, deterministic), gain multiply
-//   O:                     A5 merge of the split-KV partials (m, l, o) written by the attention phase
+//   O:                     A5 merge of the split-KV states (m, l, o) written by the attention phase
 //   down (small models):   plain copy
-__device__ __forceinline__ void stage_input(const MegaParams &p, const MkCtx &c, int ph, int K, MkShared &sh) {
+__device__ __forceinline__ void stage_input(const MegaParams &p, MkCtx &c, int ph, int K, MkShared &sh) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const bool has = tid * 8 < K;
     float v[8];
@@ -337,40 +318,69 @@ __device__ __forceinline__ void stage_input(const MegaParams &p, const MkCtx &c,
             const int G = p.n_heads / p.n_kv_heads;
             const int ns = mk_num_splits(p, c.pos + 1, kMkConsumerWarps / G);
             const int h = tid >> 3, d0 = (tid & 7) * 8;
-            const float2 *ml = p.part_ml + (size_t)h * kMkMaxSplits;
-            const float *po = p.part_o + (size_t)h * kMkMaxSplits * kHeadDim + d0;
-            float Mx = -INFINITY;
-            for (int s = 0; s < ns; ++s) Mx = fmaxf(Mx, __ldcg(&ml[s]).x);
-            float den = 0.f;
-            for (int s = 0; s < ns; ++s) {
-                const float2 m = __ldcg(&ml[s]);
-                const float wgt = (m.x == -INFINITY) ? 0.f : __expf(m.x - Mx);
-                const float4 a = ld_act4(po + (size_t)s * kHeadDim), b = ld_act4(po + (size_t)s * kHeadDim + 4);
-                den = fmaf(wgt, m.y, den);
-                v[0] = fmaf(wgt, a.x, v[0]); v[1] = fmaf(wgt, a.y, v[1]); v[2] = fmaf(wgt, a.z, v[2]); v[3] = fmaf(wgt, a.w, v[3]);
-                v[4] = fmaf(wgt, b.x, v[4]); v[5] = fmaf(wgt, b.y, v[5]); v[6] = fmaf(wgt, b.z, v[6]); v[7] = fmaf(wgt, b.w, v[7]);
+            const llw_t *ml = p.ll_part_ml + (size_t)h * kMkMaxSplits * 2;
+            const llw_t *po = p.ll_part_o + (size_t)h * kMkMaxSplits * kHeadDim + d0;
+            // online merge in split order (deterministic); the 20 loads of up to 4 splits are in flight together
+            float Mx = -INFINITY, den = 0.f;
+#pragma unroll 1
+            for (int s0 = 0; s0 < ns; s0 += 4) {
+                llw_t w[4][10];
+                unsigned spins = 0;
+                for (;;) {
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) {
+                        const int sk = min(s0 + k, ns - 1);   // past the end: re-read the last split (registers stay registers)
+                        ll_load2(ml + (size_t)sk * 2, w[k][0], w[k][1]);
+#pragma unroll
+                        for (int i = 0; i < 8; i += 2) ll_load2(po + (size_t)sk * kHeadDim + i, w[k][2 + i], w[k][3 + i]);
+                    }
+                    bool ok = true;
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) {
+#pragma unroll
+                        for (int i = 0; i < 10; ++i) ok = ok && ll_ok(w[k][i], c.tag);
+                    }
+                    if (ok) break;
+                    if (++spins == kMaxPollSpins) mk_fail(p.err, 4);
+                __nanosleep(64);
+                }
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    const float m = s0 + k < ns ? ll_val(w[k][0]) : -INFINITY, l = ll_val(w[k][1]);
+                    const float Mn = fmaxf(Mx, m);
+                    const float corr = (Mx == -INFINITY) ? 0.f : __expf(Mx - Mn);
+                    const float wgt = (m == -INFINITY) ? 0.f : __expf(m - Mn);
+                    den = den * corr + wgt * l;
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) v[i] = v[i] * corr + wgt * ll_val(w[k][2 + i]);
+                    Mx = Mn;
+                }
             }
             const float inv = 1.0f / den;
 #pragma unroll
             for (int i = 0; i < 8; ++i) v[i] *= inv;
         }
     } else if (ph == PH_DOWN) {
-        if (has) {
-            const float4 a = ld_act4(p.act + (size_t)tid * 8), b = ld_act4(p.act + (size_t)tid * 8 + 4);
-            v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w; v[4] = b.x; v[5] = b.y; v[6] = b.z; v[7] = b.w;
-        }
+        if (has) ll_poll<8>(p.ll_act + (size_t)tid * 8, c.tag, v, p.err);
     } else {
         const bf16 *gain = ph == PH_QKV ? p.layers[c.layer].attn_norm : (ph == PH_GATEUP ? p.layers[c.layer].ffn_norm : p.final_norm);
         uint4 gq = make_uint4(0, 0, 0, 0);
+        if (has) gq = __ldg(reinterpret_cast<const uint4 *>(gain) + tid);
         if (has) {
-            gq = __ldg(reinterpret_cast<const uint4 *>(gain) + tid);
             if (ph == PH_QKV && c.layer == 0) {   // A1: the residual stream starts as the embedding row
                 const uint4 e = __ldg(reinterpret_cast<const uint4 *>(p.emb + (size_t)c.tok * p.hidden) + tid);
                 v[0] = bf16lo(e.x); v[1] = bf16hi(e.x); v[2] = bf16lo(e.y); v[3] = bf16hi(e.y);
                 v[4] = bf16lo(e.z); v[5] = bf16hi(e.z); v[6] = bf16lo(e.w); v[7] = bf16hi(e.w);
+            } else if (ph == PH_GATEUP) {
+                ll_poll<8>(p.ll_x + (size_t)tid * 8, c.tag, v, p.err);                  // x after the O projection
             } else {
-                const float4 a = ld_act4(p.x + (size_t)tid * 8), b = ld_act4(p.x + (size_t)tid * 8 + 4);
-                v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w; v[4] = b.x; v[5] = b.y; v[6] = b.z; v[7] = b.w;
+                ll_poll<8>(p.ll_x + (size_t)p.hidden + (size_t)tid * 8, c.tag_prev, v, p.err);   // x after the previous layer
+                if (p.hidden_out && blockIdx.x == 0) {   // parity capture: residual after layer (c.layer - 1) / the last layer
+                    const int l = (ph == PH_HEAD ? p.n_layers : c.layer) - 1;
+                    float4 *dst = reinterpret_cast<float4 *>(p.hidden_out + (size_t)l * p.hidden_stride + tid * 8);
+                    dst[0] = make_float4(v[0], v[1], v[2], v[3]);
+                    dst[1] = make_float4(v[4], v[5], v[6], v[7]);
+                }
             }
         }
         float ss = 0.f;
@@ -416,20 +426,44 @@ __device__ __forceinline__ void load_x_staged(const MkShared &sh, int my_chunks,
         }
     }
 }
-// K > kMkStagedK (the down projection of the 1B model, K = 8192): every warp reads its own slice from L2
+// K > kMkStagedK (the down projection of the 1B model, K = 8192): every warp polls its own slice of the tagged
+// SwiGLU vector straight into registers, up to four chunks (32 words) per lane and round trip
 template <int NCH>
-__device__ __forceinline__ void load_x_direct(const float *src, int c0, int my_chunks, float (&xr)[NCH][8]) {
+__device__ __forceinline__ void load_x_direct(const MegaParams &p, const MkCtx &c, int c0, int my_chunks, float (&xr)[NCH][8]) {
     const int lane = threadIdx.x & 31;
+    constexpr int NB = NCH < 4 ? NCH : 4;
+    if (my_chunks <= 0) {
 #pragma unroll
-    for (int j = 0; j < NCH; ++j) {
-        const int ch = j * 32 + lane;
-        if (ch < my_chunks) {
-            const float4 a = ld_act4(src + (size_t)(c0 + ch) * 8), b = ld_act4(src + (size_t)(c0 + ch) * 8 + 4);
-            xr[j][0] = a.x; xr[j][1] = a.y; xr[j][2] = a.z; xr[j][3] = a.w;
-            xr[j][4] = b.x; xr[j][5] = b.y; xr[j][6] = b.z; xr[j][7] = b.w;
-        } else {
+        for (int j = 0; j < NCH; ++j)
 #pragma unroll
             for (int i = 0; i < 8; ++i) xr[j][i] = 0.f;
+        return;
+    }
+#pragma unroll
+    for (int j0 = 0; j0 < NCH; j0 += NB) {
+        llw_t w[NB][8];
+        unsigned spins = 0;
+        for (;;) {
+#pragma unroll
+            for (int k = 0; k < NB; ++k) {
+                const int ch = min((j0 + k) * 32 + lane, my_chunks - 1);   // past the end: re-read a valid chunk
+#pragma unroll
+                for (int i = 0; i < 8; i += 2) ll_load2(p.ll_act + (size_t)(c0 + ch) * 8 + i, w[k][i], w[k][i + 1]);
+            }
+            bool ok = true;
+#pragma unroll
+            for (int k = 0; k < NB; ++k)
+#pragma unroll
+                for (int i = 0; i < 8; ++i) ok = ok && ll_ok(w[k][i], c.tag);
+            if (ok) break;
+            if (++spins == kMaxPollSpins) mk_fail(p.err, 5);
+                __nanosleep(64);
+        }
+#pragma unroll
+        for (int k = 0; k < NB; ++k) {
+            const bool in = (j0 + k) * 32 + lane < my_chunks;
+#pragma unroll
+            for (int i = 0; i < 8; ++i) xr[j0 + k][i] = in ? ll_val(w[k][i]) : 0.f;
         }
     }
 }
@@ -437,27 +471,25 @@ __device__ __forceinline__ void load_x_direct(const float *src, int c0, int my_c
 // fused epilogue of one finished unit (two row totals a, b) of a phase whose rows are whole in one warp
 __device__ __forceinline__ void finish_unit(const MegaParams &p, MkCtx &c, int ph, int u, float a, float b, const MkShared &sh) {
     if (ph == PH_QKV) {
-        // A4: RoPE on q and k heads (pair (i, i+32)), q -> scratch, k/v -> cache row of this position (fp16)
+        // A4: RoPE on q and k heads (pair (i, i+32)); q, k, v of the token -> tagged words; k, v also -> cache (fp16)
         const int hh = u >> 5, i = u & 31;
-        if (hh < p.n_heads) {
+        float o0 = a, o1 = b;
+        if (hh < p.n_heads + p.n_kv_heads) {
             const float2 cs = sh.rope[i];
-            p.qkv[hh * kHeadDim + i] = a * cs.x - b * cs.y;
-            p.qkv[hh * kHeadDim + i + 32] = b * cs.x + a * cs.y;
-        } else {
+            o0 = a * cs.x - b * cs.y;
+            o1 = b * cs.x + a * cs.y;
+        }
+        ll_store(p.ll_qkv + hh * kHeadDim + i, o0, c.tag);
+        ll_store(p.ll_qkv + hh * kHeadDim + i + 32, o1, c.tag);
+        if (hh >= p.n_heads) {
             const bool is_k = hh < p.n_heads + p.n_kv_heads;
             const int kvh = hh - p.n_heads - (is_k ? 0 : p.n_kv_heads);
-            float o0 = a, o1 = b;
-            if (is_k) {
-                const float2 cs = sh.rope[i];
-                o0 = a * cs.x - b * cs.y;
-                o1 = b * cs.x + a * cs.y;
-            }
             kv_t *row = (is_k ? p.kc : p.vc) + (size_t)c.layer * p.layer_kv + ((size_t)kvh * p.max_seq + c.pos) * kHeadDim;
             row[i] = __float2half_rn(o0);
             row[i + 32] = __float2half_rn(o1);
         }
     } else if (ph == PH_GATEUP) {
-        p.act[u] = silu_f(a) * b;   // A7: fused SwiGLU
+        ll_store(p.ll_act + u, silu_f(a) * b, c.tag);   // A7: fused SwiGLU
     } else {
         // A9: logits + running packed argmax (lowest index wins ties)
         *reinterpret_cast<float2 *>(p.logits + 2 * u) = make_float2(a, b);
@@ -468,39 +500,38 @@ __device__ __forceinline__ void finish_unit(const MegaParams &p, MkCtx &c, int p
 }
 
 // One weight phase on the consumer side: input slice -> registers, then stage by stage, no CTA-wide sync.
-template <int NCH>
+// ONE instantiation (NCH = 8 covers every slice of <= 256 chunks, shorter slices predicate chunks off) and ONE call site
+// (the kernel loops over the phases): inlined into five call sites with four instantiations each the kernel was 352 KB of
+// SASS, every phase ran code that was not in the 32 KB instruction cache, and every fetch waited in the same saturated
+// memory system as the weights (0.5-1 us per straight-line section, profiles/r01_mega_timeline.md).
+template <int NCH, bool TRACE>
 __device__ __forceinline__ void consume_phase(const MegaParams &p, MkCtx &c, int ph, const PhaseGeom &geo, const uint8_t *ring,
-                                              MkShared &sh) {
+                                           MkShared &sh) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int slice = warp & (geo.S - 1), pair = warp >> geo.log2S;
     const int chunks = geo.K >> 3, c0 = slice * geo.cps;
     const int my_chunks = min(chunks, c0 + geo.cps) - c0;   // may be <= 0 for a ragged tail slice
     const bool resid = (ph == PH_O || ph == PH_DOWN);
-
-    // A6/A8: the threads that will finish the residual rows fetch the old values now
-    float rold = 0.f;
     const int n_rows_cta = 2 * (geo.u1 - geo.u0);
-    if (resid && tid < n_rows_cta) {
-        const int r = 2 * geo.u0 + tid;
-        rold = (ph == PH_O && c.layer == 0) ? __bfloat162float(p.emb[(size_t)c.tok * p.hidden + r]) : ld_act(p.x + r);
-    }
 
     float xr[NCH][8];
-    if (geo.K <= kMkStagedK) {   // S == 1: the warp holds the whole vector
-        stage_input(p, c, ph, geo.K, sh);
+    if (geo.K <= kMkStagedK) {   // S == 1: the warp holds the whole vector, staged by run_phase
         load_x_staged<NCH>(sh, my_chunks, xr);
     } else {
-        load_x_direct<NCH>(p.act, c0, my_chunks, xr);   // only the down projection has K > kMkStagedK
+        load_x_direct<NCH>(p, c, c0, my_chunks, xr);   // only the down projection has K > kMkStagedK
     }
-    mk_trace(p, c);
+    mk_trace<TRACE>(p, c);
 
-    for (int s = 0; s < geo.n_stages; ++s, ++c.g) {
-        const int slot = c.g % kMkStages;
-        const uint32_t par = (c.g / kMkStages) & 1;
+    unsigned g = c.g;
+    MkCtx lc = c;   // registers: c lives in the caller's frame
+#pragma unroll 1
+    for (int s = 0; s < geo.n_stages; ++s, ++g) {
+        const int slot = g % kMkStages;
+        const uint32_t par = (g / kMkStages) & 1;
         const int ub = geo.u0 + s * geo.ups;
         const int nu = min(geo.ups, geo.u1 - ub);
         mk_mbar_wait(&sh.full[slot], par, p.err);
-        if (s == 0) mk_trace(p, c);
+        if (s == 0) mk_trace<TRACE>(p, c);
         float a0 = 0.f, a1 = 0.f, b0 = 0.f, b1 = 0.f;
         if (pair < nu) {
             const uint4 *r0 = reinterpret_cast<const uint4 *>(ring + (size_t)slot * kMkStageBytes + (size_t)(2 * pair) * geo.row_bytes) + c0;
@@ -529,168 +560,195 @@ __device__ __forceinline__ void consume_phase(const MegaParams &p, MkCtx &c, int
                     sh.part[rl][slice] = v;
                     sh.part[rl + 1][slice] = w;
                 } else {
-                    finish_unit(p, c, ph, ub + pair, v, w, sh);
+                    finish_unit(p, lc, ph, ub + pair, v, w, sh);
                 }
             }
         }
     }
+    c.g = g;
+    c.best = lc.best;
     if (resid) {
         consumer_sync();
         if (tid < n_rows_cta) {
-            float t = rold;
+            float t = c.rold;
+#pragma unroll 1
             for (int k = 0; k < geo.S; ++k) t += sh.part[tid][k];
-            p.x[2 * geo.u0 + tid] = t;
+            c.rold = t;
+            ll_store(p.ll_x + (ph == PH_DOWN ? (size_t)p.hidden : 0) + 2 * geo.u0 + tid, t, c.tag);
         }
-        // sh.part is next written after the grid barrier that follows every residual phase
+        // sh.part is next written after the next phase's stage_input (CTA syncs in between)
     }
 }
 
+template <bool TRACE>
 __device__ __forceinline__ void run_phase(const MegaParams &p, MkCtx &c, int ph, const uint8_t *ring, MkShared &sh) {
-    const PhaseGeom geo = phase_geom(p, ph);
-    const int nch = (geo.cps + 31) / 32;
-    if (nch <= 1) consume_phase<1>(p, c, ph, geo, ring, sh);
-    else if (nch <= 2) consume_phase<2>(p, c, ph, geo, ring, sh);
-    else if (nch <= 4) consume_phase<4>(p, c, ph, geo, ring, sh);
-    else consume_phase<8>(p, c, ph, geo, ring, sh);
-    mk_trace(p, c);
+    const PhaseGeom &geo = sh.geo[ph];
+    if (geo.n_stages == 0) {
+        mk_trace<TRACE>(p, c); mk_trace<TRACE>(p, c); mk_trace<TRACE>(p, c);
+        return;
+    }   // no unit of this phase here
+    // A6 of layer 0: the residual stream starts as the embedding row; afterwards the owner of a row keeps it in c.rold
+    if (ph == PH_O && c.layer == 0 && (int)threadIdx.x < 2 * (geo.u1 - geo.u0))
+        c.rold = __bfloat162float(p.emb[(size_t)c.tok * p.hidden + 2 * geo.u0 + threadIdx.x]);
+    if (geo.K <= kMkStagedK) stage_input(p, c, ph, geo.K, sh);
+    consume_phase<kMkSliceChunks / 32, TRACE>(p, c, ph, geo, ring, sh);
+    mk_trace<TRACE>(p, c);
 }
 
 // ---- A5: attention phase ---------------------------------------------------------------------------------------
-// Work item of a CTA = (KV head, context split); warp = (query head of the group, sub-split); LANE = POSITION.
-// attn_prefetch runs BEFORE the grid barrier that ends the QKV phase: the K/V rows of earlier positions do not depend
-// on this step's projections, so their HBM/L2 latency overlaps the barrier.  Only the row of the current position
-// (written by the QKV phase of this step) has to wait.
-struct AttnItem {
-    int kvh, split, g, sub, w1, t0;
-    bool has_item, active, pre;
-};
-__device__ __forceinline__ void attn_prefetch(const MegaParams &p, const MkCtx &c, AttnItem &it, KvRow &kr, KvRow &vr) {
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+// Work item of a CTA = (KV head, context split); warp = (query head of the group, sub-split); inside the warp
+// lane = (position mod 4, dim octet): 8 lanes share one position (a 128-byte K or V row = 8 x 16 bytes), the score is
+// an 8-FMA partial dot product + 3 shuffles, each lane keeps 8 output dims, and the 4 position streams run their own
+// online softmax until one 2-shuffle merge at the end.  Compact on purpose: the earlier lane = position variant was
+// ~2,000 instructions, and code that falls out of the instruction cache is refetched through the same saturated memory
+// system as the weights (see consume_phase).  The K/V rows of earlier positions do not depend on this step, so the
+// first batch of 32 positions is loaded BEFORE the warp polls for its query; the row of the current position comes
+// from the tagged q/k/v words of this step (rounded to fp16 exactly like the cache row later steps will read).
+template <bool TRACE>
+__device__ __forceinline__ void attention_phase(const MegaParams &p, MkCtx &c, MkShared &sh) {
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int G = p.n_heads / p.n_kv_heads, nsub = kMkConsumerWarps / G;
     const int n_ctx = c.pos + 1;
     const int ns = mk_num_splits(p, n_ctx, nsub);
+    if ((int)blockIdx.x >= p.n_kv_heads * ns) { mk_trace<TRACE>(p, c); mk_trace<TRACE>(p, c); mk_trace<TRACE>(p, c); return; }
     const int len = (n_ctx + ns - 1) / ns;
-    it.has_item = (int)blockIdx.x < p.n_kv_heads * ns;
-    it.kvh = (int)blockIdx.x / ns;
-    it.split = (int)blockIdx.x % ns;
-    it.g = warp % G;
-    it.sub = warp / G;
-    it.active = it.has_item && warp < G * nsub;
-    const int s0 = it.split * len, s1 = min(n_ctx, s0 + len);
+    const int kvh = (int)blockIdx.x / ns, split = (int)blockIdx.x % ns;
+    const int g = warp % G, sub = warp / G;
+    const bool active = warp < G * nsub;
+    const int head = kvh * G + g;
+    const int s0 = split * len, s1 = min(n_ctx, s0 + len);
     const int sub_len = (max(s1 - s0, 0) + nsub - 1) / nsub;
-    const int w0 = s0 + it.sub * sub_len;
-    it.w1 = min(s1, w0 + sub_len);
-    it.t0 = w0 + lane;
-    it.pre = it.active && it.t0 < it.w1 && it.t0 < c.pos;
-    if (it.pre) {
-        const size_t off = (size_t)c.layer * p.layer_kv + ((size_t)it.kvh * p.max_seq + it.t0) * kHeadDim;
-        ld_kv_row(kr, p.kc + off);
-        ld_kv_row(vr, p.vc + off);
-    }
-}
+    const int w0 = s0 + sub * sub_len, w1 = min(s1, w0 + sub_len);
+    const int oct = lane & 7, grp = lane >> 3;
+    const bool has_new = active && c.pos >= w0 && c.pos < w1;   // this warp covers the current position
+    const uint4 *kg = reinterpret_cast<const uint4 *>(p.kc + (size_t)c.layer * p.layer_kv + (size_t)kvh * p.max_seq * kHeadDim) + oct;
+    const uint4 *vg = reinterpret_cast<const uint4 *>(p.vc + (size_t)c.layer * p.layer_kv + (size_t)kvh * p.max_seq * kHeadDim) + oct;
+    const uint4 *kn = reinterpret_cast<const uint4 *>(sh.kvnew[warp][0]) + oct, *vn = reinterpret_cast<const uint4 *>(sh.kvnew[warp][1]) + oct;
 
-__device__ void attention_phase(const MegaParams &p, MkCtx &c, MkShared &sh, const AttnItem &it, KvRow &kr, KvRow &vr) {
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    if (!it.has_item) { mk_trace(p, c); mk_trace(p, c); mk_trace(p, c); return; }
-    const int G = p.n_heads / p.n_kv_heads, nsub = kMkConsumerWarps / G;
-    const int head = it.kvh * G + it.g;
-    const int r = warp_row_of_lane<32>(lane);   // the output dims (r, 32 + r) this lane holds after the merge
-    float M = -INFINITY, l_tot = 0.f, o_lo = 0.f, o_hi = 0.f;
-    if (it.active) {
-        // the warp's query, pre-scaled by 1/sqrt(64) = 0.125 (exact), broadcast-read from shared memory below
-        if (lane < 16) {
-            float4 qv = ld_act4(p.qkv + (size_t)head * kHeadDim + lane * 4);
-            qv.x *= 0.125f; qv.y *= 0.125f; qv.z *= 0.125f; qv.w *= 0.125f;
-            reinterpret_cast<float4 *>(sh.q[warp])[lane] = qv;
+    uint4 kk[8], vv[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {   // first batch, cached positions only
+        const int t = w0 + 4 * i + grp;
+        kk[i] = vv[i] = make_uint4(0, 0, 0, 0);
+        if (active && t < w1 && t < c.pos) { kk[i] = __ldcg(kg + (size_t)t * 8); vv[i] = __ldcg(vg + (size_t)t * 8); }
+    }
+    float q[8], M = -INFINITY, l = 0.f, o[8];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) { q[j] = 0.f; o[j] = 0.f; }
+    if (active) {
+        // the lane's octet of the query, pre-scaled by 1/sqrt(64) = 0.125 (exact); with has_new also this step's k and v of
+        // the KV head (2 words of each per lane).  One poll loop: every load of a round in flight.
+        const llw_t *qsrc = p.ll_qkv + (size_t)head * kHeadDim + oct * 8;
+        const llw_t *ksrc = p.ll_qkv + (size_t)(p.n_heads + kvh) * kHeadDim + lane * 2;
+        const llw_t *vsrc = ksrc + (size_t)p.n_kv_heads * kHeadDim;
+        llw_t wq[8], wk[2], wv[2];
+        unsigned spins = 0;
+        for (;;) {
+#pragma unroll
+            for (int j = 0; j < 8; j += 2) ll_load2(qsrc + j, wq[j], wq[j + 1]);
+            bool ok = true;
+            if (has_new) {
+                ll_load2(ksrc, wk[0], wk[1]);
+                ll_load2(vsrc, wv[0], wv[1]);
+                ok = ll_ok(wk[0], c.tag) && ll_ok(wk[1], c.tag) && ll_ok(wv[0], c.tag) && ll_ok(wv[1], c.tag);
+            }
+#pragma unroll
+            for (int j = 0; j < 8; ++j) ok = ok && ll_ok(wq[j], c.tag);
+            if (__all_sync(0xffffffffu, ok)) break;
+            if (++spins == kMaxPollSpins) mk_fail(p.err, 6);
+            __nanosleep(64);
+        }
+#pragma unroll
+        for (int j = 0; j < 8; ++j) q[j] = 0.125f * ll_val(wq[j]);
+        if (has_new) {
+            reinterpret_cast<__half2 *>(sh.kvnew[warp][0])[lane] = __floats2half2_rn(ll_val(wk[0]), ll_val(wk[1]));
+            reinterpret_cast<__half2 *>(sh.kvnew[warp][1])[lane] = __floats2half2_rn(ll_val(wv[0]), ll_val(wv[1]));
         }
         __syncwarp();
     }
-    mk_trace(p, c);
-    if (it.active) {
-        const kv_t *kg = p.kc + (size_t)c.layer * p.layer_kv + (size_t)it.kvh * p.max_seq * kHeadDim;
-        const kv_t *vg = p.vc + (size_t)c.layer * p.layer_kv + (size_t)it.kvh * p.max_seq * kHeadDim;
-        const float4 *q4 = reinterpret_cast<const float4 *>(sh.q[warp]);
-        float m = -INFINITY, l = 0.f, o[kHeadDim];
+    mk_trace<TRACE>(p, c);
+    if (active) {
+        float m = -INFINITY;
+#pragma unroll 1
+        for (int b0 = w0; b0 < w1; b0 += 32) {
 #pragma unroll
-        for (int d = 0; d < kHeadDim; ++d) o[d] = 0.f;
-        bool loaded = it.pre;
-        for (int t = it.t0; t < it.w1; t += 32) {
-            if (!loaded) {
-                ld_kv_row(kr, kg + (size_t)t * kHeadDim);
-                ld_kv_row(vr, vg + (size_t)t * kHeadDim);
+            for (int i = 0; i < 8; ++i) {
+                const int t = b0 + 4 * i + grp;
+                if (t < w1 && t == c.pos) { kk[i] = *kn; vv[i] = *vn; }
+                else if (b0 != w0 && t < w1) { kk[i] = __ldcg(kg + (size_t)t * 8); vv[i] = __ldcg(vg + (size_t)t * 8); }
             }
-            loaded = false;
-            float s = 0.f, s2 = 0.f;
 #pragma unroll
-            for (int j = 0; j < 8; ++j) {
-                const float4 qa = q4[2 * j], qb = q4[2 * j + 1];
-                const float2 k0 = h2f(kr.v[j].x), k1 = h2f(kr.v[j].y), k2 = h2f(kr.v[j].z), k3 = h2f(kr.v[j].w);
-                s = fmaf(qa.x, k0.x, s); s2 = fmaf(qa.y, k0.y, s2);
-                s = fmaf(qa.z, k1.x, s); s2 = fmaf(qa.w, k1.y, s2);
-                s = fmaf(qb.x, k2.x, s); s2 = fmaf(qb.y, k2.y, s2);
-                s = fmaf(qb.z, k3.x, s); s2 = fmaf(qb.w, k3.y, s2);
+            for (int i = 0; i < 8; ++i) {
+                const int t = b0 + 4 * i + grp;
+                const float2 k0 = h2f(kk[i].x), k1 = h2f(kk[i].y), k2 = h2f(kk[i].z), k3 = h2f(kk[i].w);
+                float s = q[0] * k0.x;
+                s = fmaf(q[1], k0.y, s); s = fmaf(q[2], k1.x, s); s = fmaf(q[3], k1.y, s);
+                s = fmaf(q[4], k2.x, s); s = fmaf(q[5], k2.y, s); s = fmaf(q[6], k3.x, s); s = fmaf(q[7], k3.y, s);
+                s += __shfl_xor_sync(0xffffffffu, s, 1);
+                s += __shfl_xor_sync(0xffffffffu, s, 2);
+                s += __shfl_xor_sync(0xffffffffu, s, 4);
+                if (t < w1) {
+                    const float m_new = fmaxf(m, s);
+                    const float corr = __expf(m - m_new);   // m = -inf the first time -> 0
+                    const float pr = __expf(s - m_new);
+                    const float2 v0 = h2f(vv[i].x), v1 = h2f(vv[i].y), v2 = h2f(vv[i].z), v3 = h2f(vv[i].w);
+                    l = l * corr + pr;
+                    o[0] = fmaf(pr, v0.x, o[0] * corr); o[1] = fmaf(pr, v0.y, o[1] * corr);
+                    o[2] = fmaf(pr, v1.x, o[2] * corr); o[3] = fmaf(pr, v1.y, o[3] * corr);
+                    o[4] = fmaf(pr, v2.x, o[4] * corr); o[5] = fmaf(pr, v2.y, o[5] * corr);
+                    o[6] = fmaf(pr, v3.x, o[6] * corr); o[7] = fmaf(pr, v3.y, o[7] * corr);
+                    m = m_new;
+                }
             }
-            s += s2;
-            const float m_new = fmaxf(m, s);
-            const float corr = __expf(m - m_new);   // m = -inf the first time -> 0
-            const float pr = __expf(s - m_new);
-            l = l * corr + pr;
-#pragma unroll
-            for (int j = 0; j < 8; ++j) {
-                const float2 v0 = h2f(vr.v[j].x), v1 = h2f(vr.v[j].y), v2 = h2f(vr.v[j].z), v3 = h2f(vr.v[j].w);
-                o[8 * j + 0] = fmaf(pr, v0.x, o[8 * j + 0] * corr);
-                o[8 * j + 1] = fmaf(pr, v0.y, o[8 * j + 1] * corr);
-                o[8 * j + 2] = fmaf(pr, v1.x, o[8 * j + 2] * corr);
-                o[8 * j + 3] = fmaf(pr, v1.y, o[8 * j + 3] * corr);
-                o[8 * j + 4] = fmaf(pr, v2.x, o[8 * j + 4] * corr);
-                o[8 * j + 5] = fmaf(pr, v2.y, o[8 * j + 5] * corr);
-                o[8 * j + 6] = fmaf(pr, v3.x, o[8 * j + 6] * corr);
-                o[8 * j + 7] = fmaf(pr, v3.y, o[8 * j + 7] * corr);
-            }
-            m = m_new;
         }
-        // merge the 32 lane states: common max, rescale, transposed butterfly over the 64 dims
-        M = warp_max(m);
+        // merge the 4 position streams of the warp
+        M = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 8));
+        M = fmaxf(M, __shfl_xor_sync(0xffffffffu, M, 16));
         const float sc = (m == -INFINITY) ? 0.f : __expf(m - M);
-        l_tot = warp_sum(l * sc);
+        l *= sc;
+        l += __shfl_xor_sync(0xffffffffu, l, 8);
+        l += __shfl_xor_sync(0xffffffffu, l, 16);
 #pragma unroll
-        for (int d = 0; d < kHeadDim; ++d) o[d] *= sc;
-        float(&h0)[32] = *reinterpret_cast<float(*)[32]>(&o[0]);
-        float(&h1)[32] = *reinterpret_cast<float(*)[32]>(&o[32]);
-        warp_reduce_rows<32>(h0, lane);
-        warp_reduce_rows<32>(h1, lane);
-        o_lo = h0[0];
-        o_hi = h1[0];
-        if (it.sub > 0) {   // park the state for the sub-split 0 warp of this head
-            sh.mrg[warp][r] = o_lo;
-            sh.mrg[warp][32 + r] = o_hi;
-            if (lane == 0) { sh.mrg[warp][kHeadDim] = M; sh.mrg[warp][kHeadDim + 1] = l_tot; }
+        for (int j = 0; j < 8; ++j) {
+            o[j] *= sc;
+            o[j] += __shfl_xor_sync(0xffffffffu, o[j], 8);
+            o[j] += __shfl_xor_sync(0xffffffffu, o[j], 16);
+        }
+        if (sub > 0 && lane < 8) {   // park the state for the sub-split 0 warp of this head
+#pragma unroll
+            for (int j = 0; j < 8; ++j) sh.mrg[warp][oct * 8 + j] = o[j];
+            if (lane == 0) { sh.mrg[warp][kHeadDim] = M; sh.mrg[warp][kHeadDim + 1] = l; }
         }
     }
+    mk_trace<TRACE>(p, c);
     if (nsub > 1) consumer_sync();
-    if (it.active && it.sub == 0) {
+    if (active && sub == 0 && lane < 8) {
+#pragma unroll 1
         for (int k = 1; k < nsub; ++k) {
-            const float *o2 = sh.mrg[k * G + it.g];
+            const float *o2 = sh.mrg[k * G + g];
             const float M2 = o2[kHeadDim], l2 = o2[kHeadDim + 1];
             const float Mn = fmaxf(M, M2);
             const float wa = (M == -INFINITY) ? 0.f : __expf(M - Mn), wb = (M2 == -INFINITY) ? 0.f : __expf(M2 - Mn);
-            l_tot = l_tot * wa + l2 * wb;
-            o_lo = o_lo * wa + o2[r] * wb;
-            o_hi = o_hi * wa + o2[32 + r] * wb;
+            l = l * wa + l2 * wb;
+#pragma unroll
+            for (int j = 0; j < 8; ++j) o[j] = o[j] * wa + o2[oct * 8 + j] * wb;
             M = Mn;
         }
-        // unnormalised split state; the O phase of every CTA merges the splits while it stages its input (stage_input)
-        const size_t pidx = (size_t)head * kMkMaxSplits + it.split;
-        p.part_o[pidx * kHeadDim + r] = o_lo;
-        p.part_o[pidx * kHeadDim + 32 + r] = o_hi;
-        if (lane == 0) p.part_ml[pidx] = make_float2(M, l_tot);
+        // unnormalised split state as tagged words; the O phase of every CTA merges the splits (stage_input)
+        const size_t pidx = (size_t)head * kMkMaxSplits + split;
+#pragma unroll
+        for (int j = 0; j < 8; ++j) ll_store(p.ll_part_o + pidx * kHeadDim + oct * 8 + j, o[j], c.tag);
+        if (lane == 0) {
+            ll_store(p.ll_part_ml + pidx * 2, M, c.tag);
+            ll_store(p.ll_part_ml + pidx * 2 + 1, l, c.tag);
+        }
     }
-    mk_trace(p, c);
-    mk_trace(p, c);
-    // sh.q / sh.mrg are next written after two more grid barriers
+    mk_trace<TRACE>(p, c);
+    // sh.kvnew / sh.mrg are next written in the next layer's attention, CTA syncs (stage_input) in between
 }
 
 // ---- the kernel -----------------------------------------------------------------------------------------------
+template <bool TRACE>
 __global__ void __launch_bounds__(kMkThreads, 1) mega_decode_kernel(const __grid_constant__ MegaParams p) {
     extern __shared__ __align__(128) uint8_t mk_smem[];
     uint8_t *ring = mk_smem;
@@ -704,6 +762,7 @@ __global__ void __launch_bounds__(kMkThreads, 1) mega_decode_kernel(const __grid
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
+    if (tid < 5) sh.geo[tid] = phase_geom(p, tid);
     __syncthreads();
 
     if (warp == kMkConsumerWarps) {
@@ -713,94 +772,119 @@ __global__ void __launch_bounds__(kMkThreads, 1) mega_decode_kernel(const __grid
 
     MkCtx c;
     c.g = 0;
-    c.bar_target = 0;
     c.best = 0ull;
     c.ti = 0;
+    c.rold = 0.f;
     c.pos = ld_act(p.pos);
     c.tok = ld_act(p.tok_src);
-    mk_trace(p, c);
+    // Steps run by earlier launches.  Written only by CTA 0 at its exit, which needs a result of this step from every
+    // CTA, i.e. after every CTA has read it here.
+    const uint32_t epoch0 = *reinterpret_cast<volatile unsigned int *>(p.epoch);
+    mk_trace<TRACE>(p, c);
     for (int step = 0; step < p.n_steps; ++step) {
         if (tid < 32) sh.rope[tid] = p.rope[(size_t)c.pos * 32 + tid];
         consumer_sync();
-        for (c.layer = 0; c.layer < p.n_layers; ++c.layer) {
-            run_phase(p, c, PH_QKV, ring, sh);
-            AttnItem it;
-            KvRow kr, vr;
-            attn_prefetch(p, c, it, kr, vr);
-            grid_barrier(p, c);
-            attention_phase(p, c, sh, it, kr, vr);
-            grid_barrier(p, c);
-            run_phase(p, c, PH_O, ring, sh);
-            grid_barrier(p, c);
-            run_phase(p, c, PH_GATEUP, ring, sh);
-            grid_barrier(p, c);
-            run_phase(p, c, PH_DOWN, ring, sh);
-            grid_barrier(p, c);
-            if (p.hidden_out && blockIdx.x == 0)
-                for (int i = tid; i < p.hidden; i += kMkConsumers)
-                    p.hidden_out[(size_t)c.layer * p.hidden_stride + i] = ld_act(p.x + i);
+        const uint32_t tag0 = (epoch0 + (uint32_t)step) * (uint32_t)(p.n_layers + 1) + 1u;   // >= 1: zeroed buffers never match
+        const int n_ph = p.n_layers * 4 + (p.with_head ? 1 : 0);
+#pragma unroll 1
+        for (int pi = 0; pi < n_ph; ++pi) {   // a loop, not straight-line code: one copy of every phase body (see consume_phase)
+            c.layer = pi >> 2;
+            const int ph = c.layer < p.n_layers ? (pi & 3) : PH_HEAD;
+            c.tag = tag0 + (uint32_t)c.layer;
+            c.tag_prev = c.tag - 1u;
+            if (ph == PH_HEAD) c.best = 0ull;
+            run_phase<TRACE>(p, c, ph, ring, sh);
+            if (ph == PH_QKV) attention_phase<TRACE>(p, c, sh);
         }
+        c.tag_prev = tag0 + (uint32_t)(p.n_layers - 1);
+        c.tag = tag0 + (uint32_t)p.n_layers;
         if (p.with_head) {
-            // A9: every CTA folds its best (logit, index) into the step's slot with one packed 64-bit atomicMax
-            // before the barrier; after it every CTA reads the winner = the next token.  Two slots alternate so
-            // the one not in use can be cleared without a further barrier.
-            c.best = 0ull;
-            run_phase(p, c, PH_HEAD, ring, sh);
-            unsigned long long *slot = p.best2 + (step & 1);
+            // A9: every CTA publishes its best (ordered logit key, index) as two tagged words; every CTA then polls all of
+            // them and takes the maximum = the next token (lowest index wins ties: the packing orders ~index).
             if ((tid & 31) == 0) sh.wbest[warp] = c.best;   // lane 0 ran every epilogue of its warp
             consumer_sync();
             if (tid == 0) {
                 unsigned long long b = sh.wbest[0];
                 for (int k = 1; k < kMkConsumerWarps; ++k) b = b > sh.wbest[k] ? b : sh.wbest[k];
-                if (b) atomicMax(slot, b);
+                ll_store_u32(p.ll_best + 2 * blockIdx.x, (uint32_t)(b >> 32), c.tag);
+                ll_store_u32(p.ll_best + 2 * blockIdx.x + 1, (uint32_t)b, c.tag);
             }
-            grid_barrier(p, c);
-            const unsigned long long win = __ldcg(slot);
+            unsigned long long mine = 0ull;
+#pragma unroll 1
+            for (int i = tid; i < (int)gridDim.x; i += kMkConsumers) {
+                llw_t a, b;
+                unsigned spins = 0;
+                for (;;) {
+                    ll_load2(p.ll_best + 2 * i, a, b);
+                    if (ll_ok(a, c.tag) && ll_ok(b, c.tag)) break;
+                    if (++spins == kMaxPollSpins) mk_fail(p.err, 7);
+                __nanosleep(64);
+                }
+                const unsigned long long v = ((a & 0xFFFFFFFFull) << 32) | (b & 0xFFFFFFFFull);
+                mine = mine > v ? mine : v;
+            }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                const unsigned long long other = __shfl_xor_sync(0xffffffffu, mine, o);
+                mine = mine > other ? mine : other;
+            }
+            consumer_sync();   // everyone has read sh.wbest above
+            if ((tid & 31) == 0) sh.wbest[warp] = mine;
+            consumer_sync();
+            unsigned long long win = sh.wbest[0];
+#pragma unroll
+            for (int k = 1; k < kMkConsumerWarps; ++k) win = win > sh.wbest[k] ? win : sh.wbest[k];
             c.tok = unpack_argmax_idx(win);
+            mk_trace<TRACE>(p, c);
             if (blockIdx.x == 0 && tid == 0) {
                 *p.cur_tok = c.tok;
                 p.tok_hist[c.pos + 1] = c.tok;
                 *p.pos = c.pos + 1;
-                p.best2[(step + 1) & 1] = 0ull;   // last read two barriers ago, next written after >= 1 more
             }
         } else {
-            if (blockIdx.x == 0 && tid == 0) *p.pos = c.pos + 1;
-            c.tok = 0;   // without the head the kernel runs one step (hq_prefill token walk)
+            // without the head the kernel runs one step (hq_prefill token walk)
+            if (blockIdx.x == 0) {
+                if (p.hidden_out && tid * 8 < p.hidden) {   // parity capture of the last layer
+                    float v[8];
+                    ll_poll<8>(p.ll_x + (size_t)p.hidden + (size_t)tid * 8, c.tag_prev, v, p.err);
+                    float4 *dst = reinterpret_cast<float4 *>(p.hidden_out + (size_t)(p.n_layers - 1) * p.hidden_stride + tid * 8);
+                    dst[0] = make_float4(v[0], v[1], v[2], v[3]);
+                    dst[1] = make_float4(v[4], v[5], v[6], v[7]);
+                }
+                if (tid == 0) *p.pos = c.pos + 1;
+            }
+            c.tok = 0;
         }
         c.pos += 1;
     }
-    // leave the barrier counter and the argmax slots at zero for the next launch: the last CTA out resets them
-    consumer_sync();
-    if (tid == 0) {
-        __threadfence();
-        const unsigned t = atomicAdd(p.exit_ticket, 1u);
-        if (t == gridDim.x - 1) {
-            *p.bar = 0u;
-            *p.exit_ticket = 0u;
-            p.best2[0] = 0ull;
-            p.best2[1] = 0ull;
-        }
-    }
+    if (blockIdx.x == 0 && tid == 0) *p.epoch = epoch0 + (uint32_t)p.n_steps;
 }
 
 // ---- host side ---------------------------------------------------------------------------------------------------
 size_t mega_smem_bytes() { return (size_t)kMkStages * kMkStageBytes + sizeof(MkShared) + 128; }
 
+size_t mega_ll_words(const hq_config &c) {
+    const size_t H = c.n_heads, Hkv = c.n_kv_heads;
+    return 2 * (size_t)c.hidden + (H + 2 * Hkv) * kHeadDim + (size_t)c.ffn + H * kMkMaxSplits * kHeadDim + H * kMkMaxSplits * 2 +
+           2 * (size_t)kMkMaxGrid;
+}
+
 bool mega_shape_supported(const hq_config &c, int n_sms) {
-    // RMSNorm phases keep the whole vector in one warp (hidden <= 2048); residual phases cut K into <= 8 slices;
+    // staged phases keep the whole vector in one warp (hidden, q <= 2048); the down projection cuts K into <= 8 slices;
     // the residual rows of one CTA must fit the partial buffer; the group must fit the consumer warps
     const int q = c.n_heads * c.head_dim;
     const int units_cta = (c.hidden / 2 + n_sms - 1) / n_sms;
-    return c.hidden <= kMkStagedK && q <= kMkStagedK && c.ffn <= 64 * kMkSliceChunks &&
+    return c.hidden <= kMkStagedK && q <= kMkStagedK && c.ffn <= 32 * kMkSliceChunks &&
            2 * units_cta <= kMkPartRows && c.n_heads / c.n_kv_heads <= kMkConsumerWarps && c.hidden % 8 == 0 &&
-           c.ffn % 8 == 0 && c.vocab % 2 == 0 && n_sms >= c.n_kv_heads;
+           c.ffn % 8 == 0 && c.vocab % 2 == 0 && n_sms >= c.n_kv_heads && n_sms <= kMkMaxGrid;
 }
 
 cudaError_t launch_mega(const LaunchCtx &c, const MegaParams &p, bool cooperative) {
     static bool attr_done = false;
     const size_t smem = mega_smem_bytes();
     if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(mega_decode_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaError_t e = cudaFuncSetAttribute(mega_decode_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(mega_decode_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         attr_done = true;
     }
@@ -809,13 +893,14 @@ cudaError_t launch_mega(const LaunchCtx &c, const MegaParams &p, bool cooperativ
     cfg.blockDim = dim3(kMkThreads);
     cfg.dynamicSmemBytes = smem;
     cfg.stream = c.stream;
-    // cooperative: the driver guarantees (and checks) that all CTAs are co-resident — the grid barrier needs it
+    // cooperative: the driver guarantees (and checks) that all CTAs are co-resident — the CTAs wait on one another
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeCooperative;
     attr[0].val.cooperative = 1;
     cfg.attrs = attr;
     cfg.numAttrs = cooperative ? 1 : 0;
-    return cudaLaunchKernelEx(&cfg, mega_decode_kernel, p);
+    // the timeline stamps live in their own instantiation: the production kernel's code has to stay small
+    return p.trace ? cudaLaunchKernelEx(&cfg, mega_decode_kernel<true>, p) : cudaLaunchKernelEx(&cfg, mega_decode_kernel<false>, p);
 }
 
 }  // namespace hq

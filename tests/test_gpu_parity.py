@@ -19,12 +19,11 @@ def rel_l2(got, want):
 
 
 def gpu_model(weights, max_seq, flags=None, max_batch=1, no_mega=False):
-    """no_mega=True: batch-1 decode as one kernel per step of the path (hq_decode.cu) instead of the
-    persistent kernel (hq_mega.cu); both must meet the same tolerances."""
+    """no_mega=True: batch-1 decode as one kernel per step of the path (hq_decode.cu, the default); False: the
+    persistent kernel (hq_mega.cu, HQ_FLAG_MEGA); both must meet the same tolerances."""
     import paper_2606_12154_b200 as hq
     f = hq.FLAG_CAPTURE_HIDDEN if flags is None else flags
-    if no_mega:
-        f |= hq.FLAG_NO_MEGA
+    f |= hq.FLAG_NO_MEGA if no_mega else hq.FLAG_MEGA
     return hq.Model.from_bf16_bits(weights.shape, weights.embedding, weights.final_norm, weights.layers,
                                    max_seq=max_seq, max_batch=max_batch, flags=f)
 
@@ -95,7 +94,7 @@ def test_tiny_free_running_matches_teacher_forced(tiny_weights, tiny_tokens):
     import paper_2606_12154_b200 as hq
     om = oracle.Model.from_datagen(tiny_weights, max_seq=64)
     ref = om.greedy(tiny_tokens, 16)
-    for family in (0, hq.FLAG_NO_MEGA):
+    for family in (hq.FLAG_MEGA, hq.FLAG_NO_MEGA):
         outs = []
         for flags in (0, hq.FLAG_NO_GRAPH, hq.FLAG_NO_PDL, hq.FLAG_NO_GRAPH | hq.FLAG_NO_PDL):
             gm = gpu_model(tiny_weights, max_seq=64, flags=flags | family)
