@@ -106,6 +106,7 @@ static size_t carve(const hq_config *c, char *base, Buffers *b) {
     o.pf_tok = (int *)take(R * sizeof(int));
     o.last_idx = (int *)take(B * sizeof(int));
     o.xs = (float *)take(R * d * sizeof(float));
+    o.delta = (float *)take(R * d * sizeof(float));
     o.hn = (act_t *)take(2 * R * d * sizeof(act_t));
     o.qkv = (float *)take(R * qkvd * sizeof(float));
     o.q16 = (__half *)take(R * qdim * sizeof(__half));
@@ -243,13 +244,32 @@ static cudaError_t capture_step_graph(hq_model *m) {
 // ---- row-batched (tensor-core) path: envelope prefill passes and batched decode steps ---------------
 static int tile_index(int rows) { return rows <= 32 ? 0 : rows <= 64 ? 1 : rows <= 128 ? 2 : 3; }
 
-// split-K so that about one CTA per SM streams weights; at least 4 K blocks per split
-static int pick_splits(const hq_model *m, int n_rows, int rows, int NT, int K) {
-    const int tiles = ((n_rows + 127) / 128) * ((rows + NT - 1) / NT);
-    int s = m->n_sms / (tiles > 0 ? tiles : 1);
-    const int kb = (K + 63) / 64;
-    if (s > kb / 4) s = kb / 4;
-    return s < 1 ? 1 : s;
+// Tile plan of one GEMM of a pass: token tile (index into kTokenTiles) and split-K factor.
+// Fill the SMs with (weight tile x token tile) CTAs first: a token tile of 64 still feeds the tensor core at full
+// rate (the 128-row weight tile is re-read from shared memory every 32 cycles), the weight tile's second reader hits
+// L2, and no atomics are needed.  Split K (fp32 atomics into the output) only when the grid is still under half the
+// SMs — 9-way split-K cost more in atomics than it gained (profiles/r01_launches_v2.md).  Prefill passes stay bit-
+// reproducible: at most 2 splits into a zeroed buffer (0 + a + b is order-independent), none into the residual
+// (x + a + b is not).  Batched decode steps (few rows, weight-stream bound) split as far as the SMs go.
+struct TilePlan { int ti, NT, splits; };
+static TilePlan plan_gemm(const hq_model *m, int n_rows, int rows, int K, int max_splits) {
+    const int n_tiles = (n_rows + 127) / 128;
+    const int ti_max = tile_index(rows);
+    int ti = ti_max;
+    while (ti > 1 && n_tiles * ((rows + kTokenTiles[ti] - 1) / kTokenTiles[ti]) < (m->n_sms * 3) / 4) --ti;
+    TilePlan p{ti, kTokenTiles[ti], 1};
+    if (max_splits > 1) {
+        const int tiles = n_tiles * ((rows + p.NT - 1) / p.NT);
+        const int kb = (K + 63) / 64;
+        int s = m->n_sms / (tiles > 0 ? tiles : 1);
+        // few token rows (batched decode): the weight stream is the bound, the atomics are few -> as many CTAs as SMs;
+        // many rows (prefill): at least 16 K blocks per split and at most 4 splits
+        const int min_kb = rows <= 32 ? 4 : 16;
+        if (s > kb / min_kb) s = kb / min_kb;
+        if (s > max_splits) s = max_splits;
+        p.splits = s < 1 ? 1 : s;
+    }
+    return p;
 }
 
 // All layers for `rows` = batch * Tc token rows already embedded in b.xs; positions start at *b.pos.
@@ -258,7 +278,7 @@ static cudaError_t enqueue_rows_layers(hq_model *m, int batch, int Tc, bool deco
     const hq_config &c = m->cfg;
     const LaunchCtx lc{m->stream, m->use_pdl, m->n_sms};
     const Buffers &b = m->b;
-    const int rows = batch * Tc, ti = tile_index(rows), NT = kTokenTiles[ti];
+    const int rows = batch * Tc;
     const int d = c.hidden, qdim = c.n_heads * kHeadDim, kvdim = c.n_kv_heads * kHeadDim, qkvd = qdim + 2 * kvdim;
     const size_t layer_kv = (size_t)c.max_batch * c.n_kv_heads * c.max_seq * kHeadDim;
     const int R = m->pf_rows;                                  // lo plane sits R rows below the hi plane
@@ -266,20 +286,33 @@ static cudaError_t enqueue_rows_layers(hq_model *m, int batch, int Tc, bool deco
     cudaError_t e;
     int n = 0;
 #define STEP(call) do { e = (call); if (e != cudaSuccess) return e; ++n; } while (0)
+    // Prefill passes defer the residual adds of the O and down projections (bit-reproducible split-K, see
+    // rmsnorm_rows_kernel); decode steps add atomically into the residual.
+    const bool defer = !decode;
+    if (defer) {
+        e = cudaMemsetAsync(b.delta, 0, (size_t)rows * d * sizeof(float), m->stream);
+        if (e != cudaSuccess) return e;
+    }
     for (int l = 0; l < c.n_layers; ++l) {
         const LayerW &w = m->layers[l];
         const LayerMaps &mp = m->maps[l];
         kv_t *kc = b.kcache + l * layer_kv, *vc = b.vcache + l * layer_kv;
-        STEP(launch_rmsnorm_rows(lc, b.xs, w.attn_norm, b.hn, lo_d, d, c.rms_eps, rows, nullptr, d));
-        // P1: QKV GEMMs (three weight pointers, no repack) into one fp32 [rows][qkvd] buffer
-        const int sq = pick_splits(m, qkvd, rows, NT, d);
-        if (sq > 1) {
+        STEP(launch_rmsnorm_rows(lc, b.xs, defer ? b.delta : nullptr, w.attn_norm, b.hn, lo_d, d, c.rms_eps, rows, nullptr, d));
+        // P1: Q, K, V projections (three weight pointers, no repack) into one fp32 [rows][qkvd] buffer
+        const bool stacked = qdim % 128 == 0 && kvdim % 128 == 0;
+        const int split_store = decode ? 16 : 2, split_resid = decode ? 16 : 2;
+        const TilePlan pq = plan_gemm(m, stacked ? qkvd : qdim, rows, d, split_store);
+        if (pq.splits > 1) {
             e = cudaMemsetAsync(b.qkv, 0, (size_t)rows * qkvd * sizeof(float), m->stream);
             if (e != cudaSuccess) return e;
         }
-        STEP(launch_gemm(lc, EPI_STORE, mp.wq, nullptr, m->map_hn[ti], R, qdim, d, rows, NT, sq, b.qkv, nullptr, 0, qkvd));
-        STEP(launch_gemm(lc, EPI_STORE, mp.wk, nullptr, m->map_hn[ti], R, kvdim, d, rows, NT, sq, b.qkv + qdim, nullptr, 0, qkvd));
-        STEP(launch_gemm(lc, EPI_STORE, mp.wv, nullptr, m->map_hn[ti], R, kvdim, d, rows, NT, sq, b.qkv + qdim + kvdim, nullptr, 0, qkvd));
+        if (stacked) {
+            STEP(launch_gemm_qkv(lc, mp.wq, mp.wk, mp.wv, m->map_hn[pq.ti], R, qdim, kvdim, kvdim, d, rows, pq.NT, pq.splits, b.qkv, qkvd));
+        } else {
+            STEP(launch_gemm(lc, EPI_STORE, mp.wq, nullptr, m->map_hn[pq.ti], R, qdim, d, rows, pq.NT, pq.splits, b.qkv, nullptr, 0, qkvd));
+            STEP(launch_gemm(lc, EPI_STORE, mp.wk, nullptr, m->map_hn[pq.ti], R, kvdim, d, rows, pq.NT, pq.splits, b.qkv + qdim, nullptr, 0, qkvd));
+            STEP(launch_gemm(lc, EPI_STORE, mp.wv, nullptr, m->map_hn[pq.ti], R, kvdim, d, rows, pq.NT, pq.splits, b.qkv + qdim + kvdim, nullptr, 0, qkvd));
+        }
         // P4: RoPE + KV append
         STEP(launch_rope_append(lc, b.qkv, b.q16, decode ? b.q : nullptr, kc, vc, b.rope, b.pos, rows, Tc, c.n_heads,
                                 c.n_kv_heads, c.max_seq));
@@ -292,13 +325,17 @@ static cudaError_t enqueue_rows_layers(hq_model *m, int batch, int Tc, bool deco
             // P2: causal flash attention
             STEP(launch_flash_prefill(lc, b.q16, kc, vc, b.ao, lo_q, b.pos, batch, Tc, c.n_heads, c.n_kv_heads, c.max_seq));
         }
-        STEP(launch_gemm(lc, EPI_RESID, mp.wo, nullptr, m->map_ao[ti], R, d, qdim, rows, NT,
-                         pick_splits(m, d, rows, NT, qdim), b.xs, nullptr, 0, d));
-        STEP(launch_rmsnorm_rows(lc, b.xs, w.ffn_norm, b.hn, lo_d, d, c.rms_eps, rows, nullptr, d));
-        STEP(launch_gemm(lc, EPI_SWIGLU, mp.w_gate, &mp.w_up, m->map_hn[ti], R, c.ffn, d, rows, NT, 1, nullptr, b.actb,
+        const TilePlan po = plan_gemm(m, d, rows, qdim, split_resid);
+        STEP(launch_gemm(lc, defer ? EPI_STORE : EPI_RESID, mp.wo, nullptr, m->map_ao[po.ti], R, d, qdim, rows, po.NT, po.splits,
+                         defer ? b.delta : b.xs, nullptr, 0, d));
+        STEP(launch_rmsnorm_rows(lc, b.xs, defer ? b.delta : nullptr, w.ffn_norm, b.hn, lo_d, d, c.rms_eps, rows, nullptr, d));
+        const TilePlan pg = plan_gemm(m, c.ffn, rows, d, 1);
+        STEP(launch_gemm(lc, EPI_SWIGLU, mp.w_gate, &mp.w_up, m->map_hn[pg.ti], R, c.ffn, d, rows, pg.NT, 1, nullptr, b.actb,
                          lo_f, c.ffn));
-        STEP(launch_gemm(lc, EPI_RESID, mp.w_down, nullptr, m->map_actb[ti], R, d, c.ffn, rows, NT,
-                         pick_splits(m, d, rows, NT, c.ffn), b.xs, nullptr, 0, d));
+        const TilePlan pd = plan_gemm(m, d, rows, c.ffn, split_resid);
+        STEP(launch_gemm(lc, defer ? EPI_STORE : EPI_RESID, mp.w_down, nullptr, m->map_actb[pd.ti], R, d, c.ffn, rows, pd.NT, pd.splits,
+                         defer ? b.delta : b.xs, nullptr, 0, d));
+        if (defer && capture_hidden) STEP(launch_add_delta_rows(lc, b.xs, b.delta, (size_t)rows * d));
         if (capture_hidden) {
             // residual of the last position of every sequence -> hidden[l][b]
             e = cudaMemcpy2DAsync(b.hidden + (size_t)l * c.max_batch * d, d * sizeof(float),
@@ -314,7 +351,7 @@ static cudaError_t enqueue_rows_layers(hq_model *m, int batch, int Tc, bool deco
 
 // LM head for the last row of every sequence: final norm -> GEMM (weights read once for all
 // sequences) -> fp32 logits [batch][vocab] -> argmax + step bookkeeping (pos += pos_inc).
-static cudaError_t enqueue_rows_head(hq_model *m, int batch, int Tc, int pos_inc, int *n_launched) {
+static cudaError_t enqueue_rows_head(hq_model *m, int batch, int Tc, int pos_inc, bool deferred, int *n_launched) {
     const hq_config &c = m->cfg;
     const LaunchCtx lc{m->stream, m->use_pdl, m->n_sms};
     const Buffers &b = m->b;
@@ -322,7 +359,7 @@ static cudaError_t enqueue_rows_head(hq_model *m, int batch, int Tc, int pos_inc
     int n = 0;
 #define STEP(call) do { e = (call); if (e != cudaSuccess) return e; ++n; } while (0)
     // rows (Tc-1), (2Tc-1), ... : stride Tc rows starting at row Tc-1
-    STEP(launch_rmsnorm_rows(lc, b.xs + (size_t)(Tc - 1) * c.hidden, m->final_norm, b.hn_last, (size_t)32 * c.hidden,
+    STEP(launch_rmsnorm_rows(lc, b.xs + (size_t)(Tc - 1) * c.hidden, deferred ? b.delta + (size_t)(Tc - 1) * c.hidden : nullptr, m->final_norm, b.hn_last, (size_t)32 * c.hidden,
                              c.hidden, c.rms_eps, batch, nullptr, Tc * c.hidden));
     STEP(launch_gemm(lc, EPI_STORE, m->map_lm_head, nullptr, m->map_hn_last, 32, c.vocab, c.hidden, batch, 32, 1, b.logits,
                      nullptr, 0, c.vocab));
@@ -341,7 +378,7 @@ static cudaError_t enqueue_batch_step(hq_model *m, int batch, int *n_launched) {
     ++n;
     e = enqueue_rows_layers(m, batch, 1, true, (m->cfg.flags & HQ_FLAG_CAPTURE_HIDDEN) != 0, &n);
     if (e != cudaSuccess) return e;
-    e = enqueue_rows_head(m, batch, 1, 1, &n);
+    e = enqueue_rows_head(m, batch, 1, 1, false, &n);
     if (e != cudaSuccess) return e;
     if (n_launched) *n_launched = n;
     return cudaSuccess;
@@ -579,7 +616,7 @@ extern "C" int32_t hq_prefill(hq_model *m, const int32_t *tokens_host, int32_t b
             HQ_CUDA(enqueue_rows_layers(m, batch, Tc, false, capture && last, &n));
             HQ_CUDA(launch_advance(lc, m->b.pos, Tc));
             ++n;
-            if (last) HQ_CUDA(enqueue_rows_head(m, batch, Tc, 0, &n));
+            if (last) HQ_CUDA(enqueue_rows_head(m, batch, Tc, 0, true, &n));
             m->kernel_count += n;
         }
     }

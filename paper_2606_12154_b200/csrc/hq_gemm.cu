@@ -93,7 +93,7 @@ __host__ __device__ inline uint32_t make_idesc(int n) {
 template <int MODE>
 __global__ void __launch_bounds__(kGemmThreads, 1)
 gemm_tc_kernel(const __grid_constant__ CUtensorMap map_w, const __grid_constant__ CUtensorMap map_w2,
-               const __grid_constant__ CUtensorMap map_x, const GemmParams p) {
+               const __grid_constant__ CUtensorMap map_w3, const __grid_constant__ CUtensorMap map_x, const GemmParams p) {
     extern __shared__ __align__(1024) uint8_t smem_raw[];
     constexpr int NACC = (MODE == EPI_SWIGLU) ? 2 : 1;
     const int NT = p.NT;
@@ -138,20 +138,39 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap map_w, const __grid_constant_
     const uint32_t tmem_base = *tmem_slot;
 
     pdl_launch_dependents();
-    pdl_wait();   // activations (and, for atomics/residual, the output buffer) come from earlier kernels
 
     if (warp == 0) {
         // ===== TMA producer =====
         if (lane == 0) {
+            // EPI_STORE with p.tiles_w1 > 0: three weight matrices stacked along n in one launch (Q | K | V)
+            const CUtensorMap *mw = &map_w;
+            int nw = n0;
+            if (MODE == EPI_STORE && p.tiles_w1 > 0 && (int)blockIdx.x >= p.tiles_w1) {
+                if ((int)blockIdx.x < p.tiles_w1 + p.tiles_w2) { mw = &map_w2; nw = n0 - p.tiles_w1 * kBlockM; }
+                else { mw = &map_w3; nw = n0 - (p.tiles_w1 + p.tiles_w2) * kBlockM; }
+            }
+            // Weights do not depend on the previous kernel: the first ring of weight tiles is requested BEFORE the
+            // programmatic-dependency wait, so the launch and the first HBM round trip overlap the previous kernel's tail.
+            const int pre = nkb < stages ? nkb : stages;
+            for (int i = 0; i < pre; ++i) {
+                uint8_t *st = smem + (size_t)i * stage_bytes;
+                mbarrier_expect_tx(&full_bar[i], stage_bytes);
+                const int kc = (kb0 + i) * kBlockK;
+                tma_load_2d(mw, &full_bar[i], st, kc, nw);
+                if (NACC == 2) tma_load_2d(&map_w2, &full_bar[i], st + a_bytes, kc, n0);
+            }
+            pdl_wait();   // activations come from earlier kernels
             for (int i = 0; i < nkb; ++i) {
                 const int s = i % stages;
                 const uint32_t ph = (i / stages) & 1;
-                mbarrier_wait(&empty_bar[s], ph ^ 1);
                 uint8_t *st = smem + (size_t)s * stage_bytes;
-                mbarrier_expect_tx(&full_bar[s], stage_bytes);
                 const int kc = (kb0 + i) * kBlockK;
-                tma_load_2d(&map_w, &full_bar[s], st, kc, n0);
-                if (NACC == 2) tma_load_2d(&map_w2, &full_bar[s], st + a_bytes, kc, n0);
+                if (i >= pre) {
+                    mbarrier_wait(&empty_bar[s], ph ^ 1);
+                    mbarrier_expect_tx(&full_bar[s], stage_bytes);
+                    tma_load_2d(mw, &full_bar[s], st, kc, nw);
+                    if (NACC == 2) tma_load_2d(&map_w2, &full_bar[s], st + a_bytes, kc, n0);
+                }
                 tma_load_2d(&map_x, &full_bar[s], st + NACC * a_bytes, kc, t0);
                 tma_load_2d(&map_x, &full_bar[s], st + NACC * a_bytes + b_bytes, kc, p.x_lo_row + t0);
             }
@@ -188,6 +207,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap map_w, const __grid_constant_
         // ===== epilogue: warp w owns TMEM lanes 32*(w%4) .. +31 =====
         const int q = warp & 3;
         const int n = n0 + 32 * q + lane;
+        pdl_wait();   // the output buffer (residual, zeroed split-K target) belongs to earlier kernels until now
         mbarrier_wait(acc_bar, 0);
         tcgen05_fence_after();
         const uint32_t lane_addr = tmem_base + ((uint32_t)(32 * q) << 16);
@@ -269,8 +289,8 @@ bool make_tensor_map_16b(TensorMap *out, const void *base, uint64_t rows, uint64
 static const int kSmemBudget = 200 * 1024;
 
 template <int MODE>
-static cudaError_t launch_mode(const LaunchCtx &c, const TensorMap &w, const TensorMap &w2, const TensorMap &x,
-                               GemmParams p, int n_tiles, int t_tiles, int splits) {
+static cudaError_t launch_mode(const LaunchCtx &c, const TensorMap &w, const TensorMap &w2, const TensorMap &w3,
+                               const TensorMap &x, GemmParams p, int n_tiles, int t_tiles, int splits) {
     const int nacc = (MODE == EPI_SWIGLU) ? 2 : 1;
     const int stage_bytes = nacc * kBlockM * kBlockK * 2 + 2 * p.NT * kBlockK * 2;
     int stages = kSmemBudget / stage_bytes;
@@ -295,7 +315,8 @@ static cudaError_t launch_mode(const LaunchCtx &c, const TensorMap &w, const Ten
     cfg.attrs = attr;
     cfg.numAttrs = c.pdl ? 1 : 0;
     return cudaLaunchKernelEx(&cfg, gemm_tc_kernel<MODE>, *reinterpret_cast<const CUtensorMap *>(&w),
-                              *reinterpret_cast<const CUtensorMap *>(&w2), *reinterpret_cast<const CUtensorMap *>(&x), p);
+                              *reinterpret_cast<const CUtensorMap *>(&w2), *reinterpret_cast<const CUtensorMap *>(&w3),
+                              *reinterpret_cast<const CUtensorMap *>(&x), p);
 }
 
 // n_rows: weight rows (output features; for EPI_SWIGLU the ffn size), K: reduction size (multiple of 64),
@@ -316,13 +337,31 @@ cudaError_t launch_gemm(const LaunchCtx &c, GemmEpilogue mode, const TensorMap &
     p.out_f32 = out_f32; p.out_act = out_act; p.out_lo_offset = out_lo_offset; p.x_lo_row = x_lo_row; p.ld_out = ld_out; p.atomic = splits > 1 ? 1 : 0;
     const int n_tiles = (n_rows + kBlockM - 1) / kBlockM, t_tiles = (T + NT - 1) / NT;
     switch (mode) {
-        case EPI_STORE: return launch_mode<EPI_STORE>(c, w, w, x, p, n_tiles, t_tiles, splits);
-        case EPI_RESID: return launch_mode<EPI_RESID>(c, w, w, x, p, n_tiles, t_tiles, splits);
+        case EPI_STORE: return launch_mode<EPI_STORE>(c, w, w, w, x, p, n_tiles, t_tiles, splits);
+        case EPI_RESID: return launch_mode<EPI_RESID>(c, w, w, w, x, p, n_tiles, t_tiles, splits);
         case EPI_SWIGLU:
             if (splits != 1 || !w2) return cudaErrorInvalidValue;
-            return launch_mode<EPI_SWIGLU>(c, w, *w2, x, p, n_tiles, t_tiles, 1);
+            return launch_mode<EPI_SWIGLU>(c, w, *w2, w, x, p, n_tiles, t_tiles, 1);
     }
     return cudaErrorInvalidValue;
+}
+
+// Q, K and V projections in ONE launch: three weight matrices with n1, n2, n3 rows (multiples of 128) stacked along
+// the output dimension of out_f32 [T][n1 + n2 + n3].
+cudaError_t launch_gemm_qkv(const LaunchCtx &c, const TensorMap &wq, const TensorMap &wk, const TensorMap &wv, const TensorMap &x,
+                            int x_lo_row, int n1, int n2, int n3, int K, int T, int NT, int splits, float *out_f32, int ld_out) {
+    if (K % 8 != 0 || NT % 32 != 0 || NT < 32 || NT > 256 || T <= 0 || n1 % kBlockM || n2 % kBlockM || n3 % kBlockM)
+        return cudaErrorInvalidValue;
+    const int kblocks = (K + kBlockK - 1) / kBlockK;
+    if (splits < 1) splits = 1;
+    if (splits > kblocks) splits = kblocks;
+    GemmParams p = {};
+    p.K = K; p.n_rows = n1 + n2 + n3; p.T = T; p.NT = NT; p.k_blocks = kblocks;
+    p.k_blocks_per_split = (kblocks + splits - 1) / splits;
+    splits = (kblocks + p.k_blocks_per_split - 1) / p.k_blocks_per_split;
+    p.out_f32 = out_f32; p.x_lo_row = x_lo_row; p.ld_out = ld_out; p.atomic = splits > 1 ? 1 : 0;
+    p.tiles_w1 = n1 / kBlockM; p.tiles_w2 = n2 / kBlockM;
+    return launch_mode<EPI_STORE>(c, wq, wk, wv, x, p, p.n_rows / kBlockM, (T + NT - 1) / NT, splits);
 }
 
 }  // namespace hq

@@ -65,6 +65,7 @@ struct Buffers {
     int *pf_tok = nullptr;                      // [pf_rows]
     int *last_idx = nullptr;                    // [B] row of the last position of every sequence
     float *xs = nullptr;                        // [pf_rows][d] residual stream
+    float *delta = nullptr;                     // [pf_rows][d] deferred output of the O / down projection (prefill passes)
     act_t *hn = nullptr;                        // [2][pf_rows][d] normalised hidden (GEMM operand, hi/lo)
     float *qkv = nullptr;                       // [pf_rows][(H+2Hkv)*64]
     __half *q16 = nullptr;                      // [pf_rows][H*64] rotated queries
@@ -205,16 +206,21 @@ struct GemmParams {
     int ld_out;
     int atomic;
     int x_lo_row;       // row offset of the lo plane inside the activation tensor map
+    int tiles_w1, tiles_w2;   // EPI_STORE over three stacked weight matrices: 128-row tiles of the first and second (0 = one matrix)
 };
 bool make_tensor_map_16b(TensorMap *out, const void *base, uint64_t rows, uint64_t cols, uint32_t box_rows);
 cudaError_t launch_gemm(const LaunchCtx &c, GemmEpilogue mode, const TensorMap &w, const TensorMap *w2,
                         const TensorMap &x, int x_lo_row, int n_rows, int K, int T, int NT, int splits, float *out_f32,
                         act_t *out_act, size_t out_lo_offset, int ld_out);
 
+cudaError_t launch_gemm_qkv(const LaunchCtx &c, const TensorMap &wq, const TensorMap &wk, const TensorMap &wv, const TensorMap &x,
+                            int x_lo_row, int n1, int n2, int n3, int K, int T, int NT, int splits, float *out_f32, int ld_out);
+
 // ---- row-batched kernels (hq_prefill.cu) -------------------------------------------------------------
 cudaError_t launch_embed_rows(const LaunchCtx &c, const bf16 *emb, const int *tok, float *x, int hidden, int rows);
-cudaError_t launch_rmsnorm_rows(const LaunchCtx &c, const float *x, const bf16 *gain, act_t *out, size_t lo_offset,
+cudaError_t launch_rmsnorm_rows(const LaunchCtx &c, float *x, float *delta, const bf16 *gain, act_t *out, size_t lo_offset,
                                 int hidden, float eps, int rows, const int *row_index, int x_stride_rows);
+cudaError_t launch_add_delta_rows(const LaunchCtx &c, float *x, float *delta, size_t n);
 cudaError_t launch_rope_append(const LaunchCtx &c, const float *qkv, __half *q16, float *q32, kv_t *kc, kv_t *vc,
                                const float2 *rope, const int *pos, int rows, int Tc, int n_heads, int n_kv_heads,
                                int max_seq);

@@ -27,7 +27,10 @@ __global__ void __launch_bounds__(256) embed_rows_kernel(const bf16 *__restrict_
 }
 
 // one CTA per row; x row stays in L1/L2 between the two passes
-__global__ void __launch_bounds__(256) rmsnorm_rows_kernel(const float *x, const bf16 *__restrict__ gain,
+// delta (optional): the deferred output of the previous residual projection, x += delta first (written back, delta
+// zeroed for its next use).  Keeps split-K of those projections bit-reproducible: two splits add into a zeroed buffer
+// (0 + a + b in either order) instead of into the residual (x + a + b is order-dependent).
+__global__ void __launch_bounds__(256) rmsnorm_rows_kernel(float *x, float *delta, const bf16 *__restrict__ gain,
                                                            act_t *__restrict__ out, size_t lo_offset, int hidden,
                                                            float eps, const int *row_index, int x_stride_rows) {
     pdl_launch_dependents();
@@ -36,10 +39,17 @@ __global__ void __launch_bounds__(256) rmsnorm_rows_kernel(const float *x, const
     const int m = blockIdx.x;
     // row_index (optional) gathers rows (e.g. last position of every sequence)
     const size_t src = row_index ? (size_t)row_index[m] : (size_t)m;
-    const float *xr = x + src * x_stride_rows;
+    float *xr = x + src * x_stride_rows;
+    float *dr = delta ? delta + src * x_stride_rows : nullptr;
     float ss = 0.f;
     for (int c = threadIdx.x; c < (hidden >> 2); c += blockDim.x) {
-        const float4 v = ld_act4(xr + c * 4);
+        float4 v = ld_act4(xr + c * 4);
+        if (dr) {
+            const float4 dv = ld_act4(dr + c * 4);
+            v.x += dv.x; v.y += dv.y; v.z += dv.z; v.w += dv.w;
+            *reinterpret_cast<float4 *>(xr + c * 4) = v;
+            *reinterpret_cast<float4 *>(dr + c * 4) = make_float4(0.f, 0.f, 0.f, 0.f);
+        }
         ss += v.x * v.x + v.y * v.y + v.z * v.z + v.w * v.w;
     }
     ss = warp_sum(ss);
@@ -50,7 +60,7 @@ __global__ void __launch_bounds__(256) rmsnorm_rows_kernel(const float *x, const
     for (int w = 0; w < 8; ++w) tot += red[w];
     const float inv = 1.0f / sqrtf(tot / (float)hidden + eps);
     for (int c = threadIdx.x; c < (hidden >> 2); c += blockDim.x) {
-        const float4 v = ld_act4(xr + c * 4);
+        const float4 v = dr ? *reinterpret_cast<const float4 *>(xr + c * 4) : ld_act4(xr + c * 4);   // own store above
         const uint2 g = *reinterpret_cast<const uint2 *>(gain + c * 4);
         uint2 oh, ol;
         split_bf16x2(v.x * inv * bf16lo(g.x), v.y * inv * bf16hi(g.x), oh.x, ol.x);
@@ -393,10 +403,25 @@ static cudaError_t launch_k(const LaunchCtx &c, void (*kernel)(KArgs...), dim3 g
 cudaError_t launch_embed_rows(const LaunchCtx &c, const bf16 *emb, const int *tok, float *x, int hidden, int rows) {
     return launch_k(c, embed_rows_kernel, dim3(rows), dim3(256), emb, tok, x, hidden);
 }
-cudaError_t launch_rmsnorm_rows(const LaunchCtx &c, const float *x, const bf16 *gain, act_t *out, size_t lo_offset,
+cudaError_t launch_rmsnorm_rows(const LaunchCtx &c, float *x, float *delta, const bf16 *gain, act_t *out, size_t lo_offset,
                                 int hidden, float eps, int rows, const int *row_index, int x_stride_rows) {
-    return launch_k(c, rmsnorm_rows_kernel, dim3(rows), dim3(256), x, gain, out, lo_offset, hidden, eps, row_index,
+    return launch_k(c, rmsnorm_rows_kernel, dim3(rows), dim3(256), x, delta, gain, out, lo_offset, hidden, eps, row_index,
                     x_stride_rows);
+}
+// x += delta, delta = 0 (parity capture needs the residual itself after every layer)
+__global__ void __launch_bounds__(256) add_delta_rows_kernel(float *x, float *delta, size_t n4) {
+    pdl_launch_dependents();
+    pdl_wait();
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += (size_t)gridDim.x * blockDim.x) {
+        float4 v = ld_act4(x + i * 4);
+        const float4 dv = ld_act4(delta + i * 4);
+        v.x += dv.x; v.y += dv.y; v.z += dv.z; v.w += dv.w;
+        *reinterpret_cast<float4 *>(x + i * 4) = v;
+        *reinterpret_cast<float4 *>(delta + i * 4) = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+}
+cudaError_t launch_add_delta_rows(const LaunchCtx &c, float *x, float *delta, size_t n) {
+    return launch_k(c, add_delta_rows_kernel, dim3(296), dim3(256), x, delta, n / 4);
 }
 cudaError_t launch_rope_append(const LaunchCtx &c, const float *qkv, __half *q16, float *q32, kv_t *kc, kv_t *vc,
                                const float2 *rope, const int *pos, int rows, int Tc, int n_heads, int n_kv_heads,
