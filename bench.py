@@ -296,7 +296,7 @@ def main():
     torch.cuda.synchronize(dev)
     gu_ms = a.elapsed_time(b) / reps
     kernels = {}
-    for which, name in ((1, "lm_head"), (2, "qkv"), (3, "o_proj"), (4, "down"), (5, "attn_decode")):
+    for which, name in ((1, "lm_head"), (2, "qkv"), (3, "o_proj"), (4, "down"), (5, "attn_decode"), (6, "attn_block")):
         r = 16 if which == 1 else reps
         gm.bench_kernel(which, 8)
         a, b = ev(), ev()

@@ -158,6 +158,8 @@ static MegaParams mega_params(const hq_model *m, const int *tok_src, int n_steps
     p.hidden_out = (c.flags & HQ_FLAG_CAPTURE_HIDDEN) ? b.hidden : nullptr;
     p.hidden_stride = (size_t)c.max_batch * c.hidden;
     p.n_steps = n_steps; p.with_head = with_head ? 1 : 0;
+    p.att_splits = mega_att_splits(c, m->n_sms, c.max_seq);
+    p.att_ctas = getenv("HQ_MEGA_DEDICATED") ? p.att_splits * c.n_kv_heads : 0;
     p.inflight_stages = m->mega_inflight;
     return p;
 }
@@ -181,6 +183,13 @@ static cudaError_t enqueue_step(hq_model *m, const int *tok_src, bool with_head,
     for (int l = 0; l < c.n_layers; ++l) {
         const LayerW &w = m->layers[l];
         GemvParams p = {};
+        if (m->use_attn_block) {
+            // A2-A6 of the layer in ONE launch (hq_mega.cu, phases QKV | attention | O): its 142 KB of weights per SM fit the
+            // shared-memory ring, so the launch is a pure latency chain and two kernel boundaries per layer disappear
+            MegaParams ab = mega_params(m, tok_src, 1, false);
+            ab.x_plain = b.x; ab.pi_begin = 4 * l; ab.pi_end = 4 * l + 2;
+            STEP(launch_mega(lc, ab, false));
+        } else {
         // A2+A3+A4: RMSNorm -> QKV GEMV -> RoPE + KV append
         p.w0 = w.wq; p.w1 = w.wk; p.w2 = w.wv; p.gain = w.attn_norm; p.xin = b.x; p.K = c.hidden;
         p.n_units = (c.n_heads + 2 * c.n_kv_heads) * 32; p.eps = c.rms_eps; p.out = b.q;
@@ -195,6 +204,7 @@ static cudaError_t enqueue_step(hq_model *m, const int *tok_src, bool with_head,
         po.w0 = w.wo; po.xin = b.part_o; po.part_ml = b.part_ml; po.K = qdim; po.n_units = c.hidden / 2;
         po.out = b.x; po.pos = b.pos;
         STEP(launch_gemv(lc, GEMV_RESID, XIN_ATTN, po));
+        }
         // A2+A7: RMSNorm -> gate/up GEMV -> SwiGLU
         GemvParams pg = {};
         pg.w0 = w.w_gate; pg.w1 = w.w_up; pg.gain = w.ffn_norm; pg.xin = b.x; pg.K = c.hidden;
@@ -480,6 +490,8 @@ extern "C" int32_t hq_model_create(const hq_config *cfg, const hq_weights *w, vo
     }
     m->use_pdl = !(cfg->flags & HQ_FLAG_NO_PDL) && !getenv("HQ_NO_PDL");
     if (const char *fl = getenv("HQ_MEGA_INFLIGHT")) m->mega_inflight = atoi(fl) < 1 ? 1 : (atoi(fl) > kMkStages ? kMkStages : atoi(fl));
+    m->use_attn_block = !(cfg->flags & HQ_FLAG_NO_MEGA) && !getenv("HQ_NO_MEGA") && !getenv("HQ_NO_ATTN_BLOCK") &&
+                        mega_shape_supported(*cfg, m->n_sms);
     m->use_mega = ((cfg->flags & HQ_FLAG_MEGA) || getenv("HQ_MEGA")) && !(cfg->flags & HQ_FLAG_NO_MEGA) && !getenv("HQ_NO_MEGA") &&
                   mega_shape_supported(*cfg, m->n_sms);
     {
@@ -791,6 +803,16 @@ extern "C" int32_t hq_bench_kernel(hq_model *m, int32_t which, int32_t reps, int
                                       b.pos, c.n_heads, c.n_kv_heads, c.max_seq};
                 HQ_CUDA(launch_attn_decode(lc, a, 1));
                 bytes = 2ll * 2 * c.n_kv_heads * kHeadDim * (m->seq_len + 1);
+                break;
+            }
+            case 6: {
+                // attention block: QKV + attention + O of layer l in one launch (rewrites the K/V row at the current position)
+                if (!mega_shape_supported(c, m->n_sms)) return fail(HQ_ERR_UNSUPPORTED, "hq_bench_kernel: shape not supported by the attention block");
+                MegaParams ab = mega_params(m, b.cur_tok, 1, false);
+                ab.x_plain = b.x; ab.pi_begin = 4 * l; ab.pi_end = 4 * l + 2;
+                HQ_CUDA(launch_mega(lc, ab, false));
+                bytes = 2ll * ((c.n_heads + 2 * c.n_kv_heads) * kHeadDim + c.hidden) * c.hidden +
+                        2ll * 2 * c.n_kv_heads * kHeadDim * (m->seq_len + 1);
                 break;
             }
             default:

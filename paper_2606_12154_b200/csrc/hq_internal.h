@@ -103,6 +103,7 @@ struct hq_model_impl {
     TensorMap map_hn[4], map_ao[4], map_actb[4], map_hn_last;   // activation maps per token tile
     cudaGraphExec_t batch_graph = nullptr;      // batched decode step (captured for batch_graph_b)
     int batch_graph_b = 0, batch_graph_kernels = 0, batch_eager_b = 0;
+    bool use_attn_block = false;                // per-step path: QKV + attention + O of a layer in one launch (hq_mega.cu)
     bool use_mega = false;                      // batch-1 decode runs in the persistent kernel
     bool mega_coop = true;                      // launched with the cooperative attribute
     int mega_inflight = 2;                      // bulk-copy stages in flight per SM during the layers (HQ_MEGA_INFLIGHT overrides)
@@ -189,11 +190,17 @@ struct MegaParams {
     float *hidden_out;           // NULL or [n_layers][hidden_stride] residual after every layer
     size_t hidden_stride;
     int n_steps, with_head;
+    int att_splits, att_ctas;    // context splits per KV head, and the n_kv_heads * att_splits CTAs (the last ones) that only do attention
+    // attention-block launch (per-step path): x_plain != NULL runs only the phases [pi_begin, pi_end) of one step (QKV,
+    // attention, O of one layer), residual stream in and out as the plain fp32 vector x_plain
+    float *x_plain;
+    int pi_begin, pi_end;
     int inflight_stages;         // producer: at most this many ring stages issued and not yet landed (1..kMkStages)
 };
 size_t mega_smem_bytes();
 size_t mega_ll_words(const hq_config &c);   // 64-bit words of exchange buffers
 bool mega_shape_supported(const hq_config &c, int n_sms);
+int mega_att_splits(const hq_config &c, int n_sms, int max_ctx);
 cudaError_t launch_mega(const LaunchCtx &c, const MegaParams &p, bool cooperative);
 
 // ---- tensor-core GEMM (hq_gemm.cu) -------------------------------------------------------------------

@@ -191,9 +191,12 @@ __device__ __forceinline__ PhaseGeom phase_geom(const MegaParams &p, int ph) {
     while ((chunks + g.S - 1) / g.S > lim) { g.S <<= 1; ++g.log2S; }
     g.cps = (chunks + g.S - 1) / g.S;
     g.ups = kMkConsumerWarps >> g.log2S;
-    const int n = phase_units(p, ph), per = n / gridDim.x, rem = n % gridDim.x, b = blockIdx.x;
-    g.u0 = b * per + min(b, rem);
-    g.u1 = g.u0 + per + (b < rem ? 1 : 0);
+    // optional (p.att_ctas > 0): the last p.att_ctas CTAs do nothing but attention and the weight rows are dealt to the
+    // others.  Measured slower (1,399 -> 1,334 tok/s): the weight stream loses more than the attention gains.
+    const int W = (int)gridDim.x - p.att_ctas;
+    const int n = phase_units(p, ph), per = n / W, rem = n % W, b = blockIdx.x;
+    g.u0 = b < W ? b * per + min(b, rem) : 0;
+    g.u1 = b < W ? g.u0 + per + (b < rem ? 1 : 0) : 0;
     g.n_stages = (g.u1 - g.u0 + g.ups - 1) / g.ups;
     return g;
 }
@@ -240,8 +243,9 @@ __device__ void mk_producer(const MegaParams &p, uint8_t *ring, MkShared &sh) {
     const uint64_t pol = mk_policy_evict_first();
     const int n_ph = p.n_layers * 4 + (p.with_head ? 1 : 0);
     unsigned g = 0;   // stages produced so far
+    const int pi0 = p.x_plain ? p.pi_begin : 0, pi1 = p.x_plain ? p.pi_end : n_ph;
     for (int step = 0; step < p.n_steps; ++step)
-        for (int pi = 0; pi < n_ph; ++pi) {
+        for (int pi = pi0; pi < pi1; ++pi) {
             const int layer = pi >> 2;
             const int ph = layer < p.n_layers ? (pi & 3) : PH_HEAD;
             const LayerW &w = p.layers[layer < p.n_layers ? layer : 0];
@@ -291,15 +295,12 @@ __device__ __forceinline__ void mk_trace(const MegaParams &p, MkCtx &c) {
     }
 }
 
-// attention split policy (device only; a function of the context length and the grid): one 32-position
-// iterations per warp before another split is added (every CTA re-reads all split states: few splits = one poll round).  n_kv_heads * splits <= gridDim.x, so
-// every CTA owns at most one (KV head, split) item.
-__device__ __forceinline__ int mk_num_splits(const MegaParams &p, int n_ctx, int nsub) {
-    int ns_max = (int)gridDim.x / p.n_kv_heads;
-    ns_max = ns_max < 1 ? 1 : (ns_max > kMkMaxSplits ? kMkMaxSplits : ns_max);
-    const int per = 64 * nsub;
+// context splits per KV head at this position: two 32-position batches per warp before another split is added, at most
+// p.att_splits (the attention CTAs the launch set aside).  A function of the device-resident position: graph safe.
+__device__ __forceinline__ int mk_num_splits(const MegaParams &p, int n_ctx) {
+    const int G = p.n_heads / p.n_kv_heads, per = 64 * (kMkConsumerWarps / G);
     const int want = (n_ctx + per - 1) / per;
-    return want < ns_max ? want : ns_max;
+    return want < p.att_splits ? want : p.att_splits;
 }
 
 // Phase input, K <= kMkStagedK: the CTA polls the tagged vector from L2 ONCE (thread t owns elements [8t, 8t+8)),
@@ -314,9 +315,33 @@ __device__ __forceinline__ void stage_input(const MegaParams &p, MkCtx &c, int p
 #pragma unroll
     for (int i = 0; i < 8; ++i) v[i] = 0.f;
     if (ph == PH_O) {
-        if (has) {
+        {
+            // Gate: ONE warp watches one word per attention CTA (the (m, l) word its first head writes last) with back-off;
+            // the other 7 warps sleep in the CTA barrier.  Without it 148 x 256 threads polled the ~100 lines of the split
+            // states for the whole attention phase and the writers' stores queued behind those reads: 5 us from the last
+            // store to the first successful poll on an otherwise idle chip (profiles/r01_mega_sync_microbench.md).
             const int G = p.n_heads / p.n_kv_heads;
-            const int ns = mk_num_splits(p, c.pos + 1, kMkConsumerWarps / G);
+            const int ns = mk_num_splits(p, c.pos + 1);
+            if (tid < 32) {
+                const int items = p.n_kv_heads * ns;
+                unsigned spins = 0;
+                for (;;) {
+                    bool ok = true;
+                    for (int it = lane; it < items; it += 32) {
+                        llw_t w0;
+                        asm volatile("ld.volatile.global.u64 %0, [%1];" : "=l"(w0)
+                                     : "l"(p.ll_part_ml + ((size_t)((it / ns) * G) * kMkMaxSplits + (it % ns)) * 2) : "memory");
+                        ok = ok && ll_ok(w0, c.tag);
+                    }
+                    if (__all_sync(0xffffffffu, ok)) break;
+                    if (++spins == kMaxPollSpins) mk_fail(p.err, 8);
+                    __nanosleep(200);
+                }
+            }
+            consumer_sync();
+        }
+        if (has) {
+            const int ns = mk_num_splits(p, c.pos + 1);
             const int h = tid >> 3, d0 = (tid & 7) * 8;
             const llw_t *ml = p.ll_part_ml + (size_t)h * kMkMaxSplits * 2;
             const llw_t *po = p.ll_part_o + (size_t)h * kMkMaxSplits * kHeadDim + d0;
@@ -342,7 +367,7 @@ __device__ __forceinline__ void stage_input(const MegaParams &p, MkCtx &c, int p
                     }
                     if (ok) break;
                     if (++spins == kMaxPollSpins) mk_fail(p.err, 4);
-                __nanosleep(64);
+                    __nanosleep(64);
                 }
 #pragma unroll
                 for (int k = 0; k < 4; ++k) {
@@ -367,7 +392,10 @@ __device__ __forceinline__ void stage_input(const MegaParams &p, MkCtx &c, int p
         uint4 gq = make_uint4(0, 0, 0, 0);
         if (has) gq = __ldg(reinterpret_cast<const uint4 *>(gain) + tid);
         if (has) {
-            if (ph == PH_QKV && c.layer == 0) {   // A1: the residual stream starts as the embedding row
+            if (p.x_plain) {   // attention-block launch: the residual stream is a plain vector written by the previous kernel
+                const float4 a = ld_act4(p.x_plain + (size_t)tid * 8), b = ld_act4(p.x_plain + (size_t)tid * 8 + 4);
+                v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w; v[4] = b.x; v[5] = b.y; v[6] = b.z; v[7] = b.w;
+            } else if (ph == PH_QKV && c.layer == 0) {   // A1: the residual stream starts as the embedding row
                 const uint4 e = __ldg(reinterpret_cast<const uint4 *>(p.emb + (size_t)c.tok * p.hidden) + tid);
                 v[0] = bf16lo(e.x); v[1] = bf16hi(e.x); v[2] = bf16lo(e.y); v[3] = bf16hi(e.y);
                 v[4] = bf16lo(e.z); v[5] = bf16hi(e.z); v[6] = bf16lo(e.w); v[7] = bf16hi(e.w);
@@ -574,7 +602,8 @@ __device__ __forceinline__ void consume_phase(const MegaParams &p, MkCtx &c, int
 #pragma unroll 1
             for (int k = 0; k < geo.S; ++k) t += sh.part[tid][k];
             c.rold = t;
-            ll_store(p.ll_x + (ph == PH_DOWN ? (size_t)p.hidden : 0) + 2 * geo.u0 + tid, t, c.tag);
+            if (p.x_plain) p.x_plain[2 * geo.u0 + tid] = t;   // read by the next kernel
+            else ll_store(p.ll_x + (ph == PH_DOWN ? (size_t)p.hidden : 0) + 2 * geo.u0 + tid, t, c.tag);
         }
         // sh.part is next written after the next phase's stage_input (CTA syncs in between)
     }
@@ -588,8 +617,10 @@ __device__ __forceinline__ void run_phase(const MegaParams &p, MkCtx &c, int ph,
         return;
     }   // no unit of this phase here
     // A6 of layer 0: the residual stream starts as the embedding row; afterwards the owner of a row keeps it in c.rold
-    if (ph == PH_O && c.layer == 0 && (int)threadIdx.x < 2 * (geo.u1 - geo.u0))
-        c.rold = __bfloat162float(p.emb[(size_t)c.tok * p.hidden + 2 * geo.u0 + threadIdx.x]);
+    if (ph == PH_O && (int)threadIdx.x < 2 * (geo.u1 - geo.u0)) {
+        if (p.x_plain) c.rold = ld_act(p.x_plain + 2 * geo.u0 + threadIdx.x);
+        else if (c.layer == 0) c.rold = __bfloat162float(p.emb[(size_t)c.tok * p.hidden + 2 * geo.u0 + threadIdx.x]);
+    }
     if (geo.K <= kMkStagedK) stage_input(p, c, ph, geo.K, sh);
     consume_phase<kMkSliceChunks / 32, TRACE>(p, c, ph, geo, ring, sh);
     mk_trace<TRACE>(p, c);
@@ -609,10 +640,12 @@ __device__ __forceinline__ void attention_phase(const MegaParams &p, MkCtx &c, M
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int G = p.n_heads / p.n_kv_heads, nsub = kMkConsumerWarps / G;
     const int n_ctx = c.pos + 1;
-    const int ns = mk_num_splits(p, n_ctx, nsub);
-    if ((int)blockIdx.x >= p.n_kv_heads * ns) { mk_trace<TRACE>(p, c); mk_trace<TRACE>(p, c); mk_trace<TRACE>(p, c); return; }
+    const int ns = mk_num_splits(p, n_ctx);
+    // att_ctas > 0: the last att_ctas CTAs are set aside for attention; 0: the first CTAs do it besides their weight rows
+    const int item = p.att_ctas > 0 ? (int)blockIdx.x - ((int)gridDim.x - p.att_ctas) : (int)blockIdx.x;
+    if (item < 0 || item >= p.n_kv_heads * ns) { mk_trace<TRACE>(p, c); mk_trace<TRACE>(p, c); mk_trace<TRACE>(p, c); return; }
     const int len = (n_ctx + ns - 1) / ns;
-    const int kvh = (int)blockIdx.x / ns, split = (int)blockIdx.x % ns;
+    const int kvh = item / ns, split = item % ns;
     const int g = warp % G, sub = warp / G;
     const bool active = warp < G * nsub;
     const int head = kvh * G + g;
@@ -770,6 +803,10 @@ __global__ void __launch_bounds__(kMkThreads, 1) mega_decode_kernel(const __grid
         return;
     }
 
+    // Attention-block launches sit between per-step kernels with programmatic edges: the producer warp (above) is already
+    // streaming this launch's weights (immutable), everything else waits for the previous kernel here.
+    pdl_launch_dependents();
+    pdl_wait();
     MkCtx c;
     c.g = 0;
     c.best = 0ull;
@@ -786,8 +823,9 @@ __global__ void __launch_bounds__(kMkThreads, 1) mega_decode_kernel(const __grid
         consumer_sync();
         const uint32_t tag0 = (epoch0 + (uint32_t)step) * (uint32_t)(p.n_layers + 1) + 1u;   // >= 1: zeroed buffers never match
         const int n_ph = p.n_layers * 4 + (p.with_head ? 1 : 0);
+        const int pi0 = p.x_plain ? p.pi_begin : 0, pi1 = p.x_plain ? p.pi_end : n_ph;
 #pragma unroll 1
-        for (int pi = 0; pi < n_ph; ++pi) {   // a loop, not straight-line code: one copy of every phase body (see consume_phase)
+        for (int pi = pi0; pi < pi1; ++pi) {   // a loop, not straight-line code: one copy of every phase body (see consume_phase)
             c.layer = pi >> 2;
             const int ph = c.layer < p.n_layers ? (pi & 3) : PH_HEAD;
             c.tag = tag0 + (uint32_t)c.layer;
@@ -796,6 +834,7 @@ __global__ void __launch_bounds__(kMkThreads, 1) mega_decode_kernel(const __grid
             run_phase<TRACE>(p, c, ph, ring, sh);
             if (ph == PH_QKV) attention_phase<TRACE>(p, c, sh);
         }
+        if (p.x_plain) break;   // attention-block launch: one step, no head, position advanced by the LM-head kernel
         c.tag_prev = tag0 + (uint32_t)(p.n_layers - 1);
         c.tag = tag0 + (uint32_t)p.n_layers;
         if (p.with_head) {
@@ -869,14 +908,28 @@ size_t mega_ll_words(const hq_config &c) {
            2 * (size_t)kMkMaxGrid;
 }
 
+// Most context splits per KV head a model will use = attention CTAs set aside per KV head: enough for max_ctx at two
+// 32-position batches per warp, at most kMkMaxSplits (every CTA re-reads all split states) and a quarter of the SMs.
+int mega_att_splits(const hq_config &c, int n_sms, int max_ctx) {
+    const int G = c.n_heads / c.n_kv_heads, nsub = kMkConsumerWarps / (G > 0 ? G : 1);
+    const int per = 64 * (nsub > 0 ? nsub : 1);
+    int ns = (max_ctx + per - 1) / per;
+    int cap = (n_sms / 4) / c.n_kv_heads;
+    if (cap < 1) cap = 1;
+    if (cap > kMkMaxSplits) cap = kMkMaxSplits;
+    if (ns > cap) ns = cap;
+    return ns < 1 ? 1 : ns;
+}
+
 bool mega_shape_supported(const hq_config &c, int n_sms) {
     // staged phases keep the whole vector in one warp (hidden, q <= 2048); the down projection cuts K into <= 8 slices;
     // the residual rows of one CTA must fit the partial buffer; the group must fit the consumer warps
     const int q = c.n_heads * c.head_dim;
-    const int units_cta = (c.hidden / 2 + n_sms - 1) / n_sms;
+    const int w_ctas = n_sms - mega_att_splits(c, n_sms, 1 << 30) * c.n_kv_heads;
+    const int units_cta = (c.hidden / 2 + w_ctas - 1) / w_ctas;   // fewest weight CTAs a launch can have
     return c.hidden <= kMkStagedK && q <= kMkStagedK && c.ffn <= 32 * kMkSliceChunks &&
            2 * units_cta <= kMkPartRows && c.n_heads / c.n_kv_heads <= kMkConsumerWarps && c.hidden % 8 == 0 &&
-           c.ffn % 8 == 0 && c.vocab % 2 == 0 && n_sms >= c.n_kv_heads && n_sms <= kMkMaxGrid;
+           c.ffn % 8 == 0 && c.vocab % 2 == 0 && n_sms >= 2 * c.n_kv_heads && n_sms <= kMkMaxGrid && w_ctas >= 1;
 }
 
 cudaError_t launch_mega(const LaunchCtx &c, const MegaParams &p, bool cooperative) {
@@ -895,10 +948,18 @@ cudaError_t launch_mega(const LaunchCtx &c, const MegaParams &p, bool cooperativ
     cfg.stream = c.stream;
     // cooperative: the driver guarantees (and checks) that all CTAs are co-resident — the CTAs wait on one another
     cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeCooperative;
-    attr[0].val.cooperative = 1;
     cfg.attrs = attr;
-    cfg.numAttrs = cooperative ? 1 : 0;
+    if (p.x_plain) {
+        // one CTA per SM (shared memory) and no dependence of the neighbouring kernels on this one's CTAs: all CTAs become
+        // resident as the previous kernel drains; a programmatic edge lets the weight stream start under its tail
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.numAttrs = c.pdl ? 1 : 0;
+    } else {
+        attr[0].id = cudaLaunchAttributeCooperative;
+        attr[0].val.cooperative = 1;
+        cfg.numAttrs = cooperative ? 1 : 0;
+    }
     // the timeline stamps live in their own instantiation: the production kernel's code has to stay small
     return p.trace ? cudaLaunchKernelEx(&cfg, mega_decode_kernel<true>, p) : cudaLaunchKernelEx(&cfg, mega_decode_kernel<false>, p);
 }

@@ -18,12 +18,14 @@ def rel_l2(got, want):
     return float(np.linalg.norm(got - want) / np.linalg.norm(want))
 
 
-def gpu_model(weights, max_seq, flags=None, max_batch=1, no_mega=False):
-    """no_mega=True: batch-1 decode as one kernel per step of the path (hq_decode.cu, the default); False: the
-    persistent kernel (hq_mega.cu, HQ_FLAG_MEGA); both must meet the same tolerances."""
+def gpu_model(weights, max_seq, flags=None, max_batch=1, no_mega=None):
+    """Batch-1 decode paths, all held to the same tolerances.  no_mega=None: the default (per-step kernels with QKV +
+    attention + O of a layer in one launch); True: one kernel per step of the path (hq_decode.cu only, HQ_FLAG_NO_MEGA);
+    False: the persistent kernel (hq_mega.cu, HQ_FLAG_MEGA)."""
     import paper_2606_12154_b200 as hq
     f = hq.FLAG_CAPTURE_HIDDEN if flags is None else flags
-    f |= hq.FLAG_NO_MEGA if no_mega else hq.FLAG_MEGA
+    if no_mega is not None:
+        f |= hq.FLAG_NO_MEGA if no_mega else hq.FLAG_MEGA
     return hq.Model.from_bf16_bits(weights.shape, weights.embedding, weights.final_norm, weights.layers,
                                    max_seq=max_seq, max_batch=max_batch, flags=f)
 
@@ -64,7 +66,7 @@ def run_teacher_forced(gm, om, prompt, n_steps, check_every=1):
 # ---------------------------------------------------------------------------------------------------
 # configs[0]: tiny model, 32-token prompt, 16 greedy steps
 # ---------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("no_mega", [False, True])
+@pytest.mark.parametrize("no_mega", [None, False, True])
 def test_tiny_prefill_and_decode(tiny_weights, tiny_tokens, no_mega):
     gm = gpu_model(tiny_weights, max_seq=64, no_mega=no_mega)
     om = oracle.Model.from_datagen(tiny_weights, max_seq=64)
@@ -73,7 +75,7 @@ def test_tiny_prefill_and_decode(tiny_weights, tiny_tokens, no_mega):
     print("tiny parity:", stats)
 
 
-@pytest.mark.parametrize("no_mega", [False, True])
+@pytest.mark.parametrize("no_mega", [None, False, True])
 def test_tiny_every_prompt_position(tiny_weights, tiny_tokens, no_mega):
     """configs[0] additionally compares all prompt positions (chunked prefill, one token at a time)."""
     gm = gpu_model(tiny_weights, max_seq=64, no_mega=no_mega)
@@ -94,7 +96,7 @@ def test_tiny_free_running_matches_teacher_forced(tiny_weights, tiny_tokens):
     import paper_2606_12154_b200 as hq
     om = oracle.Model.from_datagen(tiny_weights, max_seq=64)
     ref = om.greedy(tiny_tokens, 16)
-    for family in (hq.FLAG_MEGA, hq.FLAG_NO_MEGA):
+    for family in (0, hq.FLAG_MEGA, hq.FLAG_NO_MEGA):
         outs = []
         for flags in (0, hq.FLAG_NO_GRAPH, hq.FLAG_NO_PDL, hq.FLAG_NO_GRAPH | hq.FLAG_NO_PDL):
             gm = gpu_model(tiny_weights, max_seq=64, flags=flags | family)
@@ -127,7 +129,7 @@ def test_tiny_kv_reset_and_reuse(tiny_weights, tiny_tokens):
     assert np.array_equal(a, b) and np.array_equal(la, lb)
 
 
-@pytest.mark.parametrize("no_mega", [False, True])
+@pytest.mark.parametrize("no_mega", [None, False, True])
 def test_tiny_ragged_lengths(tiny_weights, no_mega):
     """Context lengths around the 16/32/64/128 tile and split boundaries of the attention kernels: the
     prompt goes through prefill, then ONE decode step attends over n+1 positions (decode attention)."""
@@ -182,7 +184,7 @@ def one_b_weights():
     return datagen.make_weights(datagen.ONE_B)
 
 
-@pytest.mark.parametrize("no_mega", [False, True])
+@pytest.mark.parametrize("no_mega", [None, False, True])
 def test_1b_config1_teacher_forced(one_b_weights, no_mega):
     s = datagen.ONE_B
     prompt = datagen.tokens(1001, s.vocab, 256)
