@@ -152,6 +152,7 @@ static MegaParams mega_params(const hq_model *m, const int *tok_src, int n_steps
         p.ll_act = w; w += c.ffn;
         p.ll_part_o = w; w += H * kMkMaxSplits * kHeadDim;
         p.ll_part_ml = w; w += H * kMkMaxSplits * 2;
+        p.ll_attn = w; w += H * kHeadDim;
         p.ll_best = w;
     }
     p.logits = b.logits;

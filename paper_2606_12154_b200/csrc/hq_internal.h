@@ -185,6 +185,7 @@ struct MegaParams {
     unsigned long long *ll_act;      // [ffn] SwiGLU output
     unsigned long long *ll_part_o;   // [H][kMkMaxSplits][64] split-KV partial outputs (unnormalised)
     unsigned long long *ll_part_ml;  // [H][kMkMaxSplits][2] (m, l)
+    unsigned long long *ll_attn;     // [H*64] merged, normalised attention output
     unsigned long long *ll_best;     // [grid][2] per-CTA argmax (ordered logit key, index)
     float *logits;
     float *hidden_out;           // NULL or [n_layers][hidden_stride] residual after every layer

@@ -281,6 +281,7 @@ struct MkCtx {
     int layer;
     uint32_t tag;        // epoch tag of (step, layer): every word exchanged in this layer carries it
     uint32_t tag_prev;   // tag of the previous layer of this step (input of the QKV phase / the LM head)
+    uint4 gain_pre;      // attention-block launch: the layer's attn_norm gains, loaded before the dependency wait
     float rold;          // residual phases: thread tid < rows of this CTA keeps x[row] in a register
     int ti;              // trace cursor (thread 0)
     unsigned long long best;
@@ -295,10 +296,10 @@ __device__ __forceinline__ void mk_trace(const MegaParams &p, MkCtx &c) {
     }
 }
 
-// context splits per KV head at this position: two 32-position batches per warp before another split is added, at most
+// context splits per KV head at this position: one 32-position batch per warp before another split is added, at most
 // p.att_splits (the attention CTAs the launch set aside).  A function of the device-resident position: graph safe.
 __device__ __forceinline__ int mk_num_splits(const MegaParams &p, int n_ctx) {
-    const int G = p.n_heads / p.n_kv_heads, per = 64 * (kMkConsumerWarps / G);
+    const int G = p.n_heads / p.n_kv_heads, per = 32 * (kMkConsumerWarps / G);
     const int want = (n_ctx + per - 1) / per;
     return want < p.att_splits ? want : p.att_splits;
 }
@@ -308,6 +309,7 @@ __device__ __forceinline__ int mk_num_splits(const MegaParams &p, int n_ctx) {
 //   QKV, gate/up, LM head: A2 RMSNorm (sum of squares reduced across the CTA, deterministic), gain multiply
 //   O:                     A5 merge of the split-KV states (m, l, o) written by the attention phase
 //   down (small models):   plain copy
+template <bool BLOCK>
 __device__ __forceinline__ void stage_input(const MegaParams &p, MkCtx &c, int ph, int K, MkShared &sh) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const bool has = tid * 8 < K;
@@ -315,84 +317,34 @@ __device__ __forceinline__ void stage_input(const MegaParams &p, MkCtx &c, int p
 #pragma unroll
     for (int i = 0; i < 8; ++i) v[i] = 0.f;
     if (ph == PH_O) {
-        {
-            // Gate: ONE warp watches one word per attention CTA (the (m, l) word its first head writes last) with back-off;
-            // the other 7 warps sleep in the CTA barrier.  Without it 148 x 256 threads polled the ~100 lines of the split
-            // states for the whole attention phase and the writers' stores queued behind those reads: 5 us from the last
-            // store to the first successful poll on an otherwise idle chip (profiles/r01_mega_sync_microbench.md).
-            const int G = p.n_heads / p.n_kv_heads;
-            const int ns = mk_num_splits(p, c.pos + 1);
-            if (tid < 32) {
-                const int items = p.n_kv_heads * ns;
-                unsigned spins = 0;
-                for (;;) {
-                    bool ok = true;
-                    for (int it = lane; it < items; it += 32) {
-                        llw_t w0;
-                        asm volatile("ld.volatile.global.u64 %0, [%1];" : "=l"(w0)
-                                     : "l"(p.ll_part_ml + ((size_t)((it / ns) * G) * kMkMaxSplits + (it % ns)) * 2) : "memory");
-                        ok = ok && ll_ok(w0, c.tag);
-                    }
-                    if (__all_sync(0xffffffffu, ok)) break;
-                    if (++spins == kMaxPollSpins) mk_fail(p.err, 8);
-                    __nanosleep(200);
+        // A5 output: the normalised attention vector published by the split-0 CTA of every KV head.  Gate: ONE warp
+        // watches one word per head with back-off while the other 7 sleep in the CTA barrier, so that the chip does not
+        // poll the same 128 lines for the whole attention phase.
+        if (tid < 32) {
+            unsigned spins = 0;
+            for (;;) {
+                bool ok = true;
+                for (int h = lane; h < p.n_heads; h += 32) {
+                    llw_t w0;
+                    asm volatile("ld.volatile.global.u64 %0, [%1];" : "=l"(w0) : "l"(p.ll_attn + (size_t)h * kHeadDim + kHeadDim - 1) : "memory");
+                    ok = ok && ll_ok(w0, c.tag);
                 }
+                if (__all_sync(0xffffffffu, ok)) break;
+                if (++spins == kMaxPollSpins) mk_fail(p.err, 8);
+                __nanosleep(100);
             }
-            consumer_sync();
         }
-        if (has) {
-            const int ns = mk_num_splits(p, c.pos + 1);
-            const int h = tid >> 3, d0 = (tid & 7) * 8;
-            const llw_t *ml = p.ll_part_ml + (size_t)h * kMkMaxSplits * 2;
-            const llw_t *po = p.ll_part_o + (size_t)h * kMkMaxSplits * kHeadDim + d0;
-            // online merge in split order (deterministic); the 20 loads of up to 4 splits are in flight together
-            float Mx = -INFINITY, den = 0.f;
-#pragma unroll 1
-            for (int s0 = 0; s0 < ns; s0 += 4) {
-                llw_t w[4][10];
-                unsigned spins = 0;
-                for (;;) {
-#pragma unroll
-                    for (int k = 0; k < 4; ++k) {
-                        const int sk = min(s0 + k, ns - 1);   // past the end: re-read the last split (registers stay registers)
-                        ll_load2(ml + (size_t)sk * 2, w[k][0], w[k][1]);
-#pragma unroll
-                        for (int i = 0; i < 8; i += 2) ll_load2(po + (size_t)sk * kHeadDim + i, w[k][2 + i], w[k][3 + i]);
-                    }
-                    bool ok = true;
-#pragma unroll
-                    for (int k = 0; k < 4; ++k) {
-#pragma unroll
-                        for (int i = 0; i < 10; ++i) ok = ok && ll_ok(w[k][i], c.tag);
-                    }
-                    if (ok) break;
-                    if (++spins == kMaxPollSpins) mk_fail(p.err, 4);
-                    __nanosleep(64);
-                }
-#pragma unroll
-                for (int k = 0; k < 4; ++k) {
-                    const float m = s0 + k < ns ? ll_val(w[k][0]) : -INFINITY, l = ll_val(w[k][1]);
-                    const float Mn = fmaxf(Mx, m);
-                    const float corr = (Mx == -INFINITY) ? 0.f : __expf(Mx - Mn);
-                    const float wgt = (m == -INFINITY) ? 0.f : __expf(m - Mn);
-                    den = den * corr + wgt * l;
-#pragma unroll
-                    for (int i = 0; i < 8; ++i) v[i] = v[i] * corr + wgt * ll_val(w[k][2 + i]);
-                    Mx = Mn;
-                }
-            }
-            const float inv = 1.0f / den;
-#pragma unroll
-            for (int i = 0; i < 8; ++i) v[i] *= inv;
-        }
-    } else if (ph == PH_DOWN) {
+        consumer_sync();
+        if (has) ll_poll<8>(p.ll_attn + (size_t)tid * 8, c.tag, v, p.err);
+    } else if (!BLOCK && ph == PH_DOWN) {
         if (has) ll_poll<8>(p.ll_act + (size_t)tid * 8, c.tag, v, p.err);
     } else {
         const bf16 *gain = ph == PH_QKV ? p.layers[c.layer].attn_norm : (ph == PH_GATEUP ? p.layers[c.layer].ffn_norm : p.final_norm);
         uint4 gq = make_uint4(0, 0, 0, 0);
-        if (has) gq = __ldg(reinterpret_cast<const uint4 *>(gain) + tid);
+        if (BLOCK) gq = c.gain_pre;
+        else if (has) gq = __ldg(reinterpret_cast<const uint4 *>(gain) + tid);
         if (has) {
-            if (p.x_plain) {   // attention-block launch: the residual stream is a plain vector written by the previous kernel
+            if (BLOCK) {   // attention-block launch: the residual stream is a plain vector written by the previous kernel
                 const float4 a = ld_act4(p.x_plain + (size_t)tid * 8), b = ld_act4(p.x_plain + (size_t)tid * 8 + 4);
                 v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w; v[4] = b.x; v[5] = b.y; v[6] = b.z; v[7] = b.w;
             } else if (ph == PH_QKV && c.layer == 0) {   // A1: the residual stream starts as the embedding row
@@ -497,8 +449,9 @@ __device__ __forceinline__ void load_x_direct(const MegaParams &p, const MkCtx &
 }
 
 // fused epilogue of one finished unit (two row totals a, b) of a phase whose rows are whole in one warp
+template <bool BLOCK>
 __device__ __forceinline__ void finish_unit(const MegaParams &p, MkCtx &c, int ph, int u, float a, float b, const MkShared &sh) {
-    if (ph == PH_QKV) {
+    if (BLOCK || ph == PH_QKV) {
         // A4: RoPE on q and k heads (pair (i, i+32)); q, k, v of the token -> tagged words; k, v also -> cache (fp16)
         const int hh = u >> 5, i = u & 31;
         float o0 = a, o1 = b;
@@ -532,7 +485,7 @@ __device__ __forceinline__ void finish_unit(const MegaParams &p, MkCtx &c, int p
 // (the kernel loops over the phases): inlined into five call sites with four instantiations each the kernel was 352 KB of
 // SASS, every phase ran code that was not in the 32 KB instruction cache, and every fetch waited in the same saturated
 // memory system as the weights (0.5-1 us per straight-line section, profiles/r01_mega_timeline.md).
-template <int NCH, bool TRACE>
+template <int NCH, bool TRACE, bool BLOCK>
 __device__ __forceinline__ void consume_phase(const MegaParams &p, MkCtx &c, int ph, const PhaseGeom &geo, const uint8_t *ring,
                                            MkShared &sh) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -543,7 +496,7 @@ __device__ __forceinline__ void consume_phase(const MegaParams &p, MkCtx &c, int
     const int n_rows_cta = 2 * (geo.u1 - geo.u0);
 
     float xr[NCH][8];
-    if (geo.K <= kMkStagedK) {   // S == 1: the warp holds the whole vector, staged by run_phase
+    if (BLOCK || geo.K <= kMkStagedK) {   // S == 1: the warp holds the whole vector, staged by run_phase
         load_x_staged<NCH>(sh, my_chunks, xr);
     } else {
         load_x_direct<NCH>(p, c, c0, my_chunks, xr);   // only the down projection has K > kMkStagedK
@@ -588,7 +541,7 @@ __device__ __forceinline__ void consume_phase(const MegaParams &p, MkCtx &c, int
                     sh.part[rl][slice] = v;
                     sh.part[rl + 1][slice] = w;
                 } else {
-                    finish_unit(p, lc, ph, ub + pair, v, w, sh);
+                    finish_unit<BLOCK>(p, lc, ph, ub + pair, v, w, sh);
                 }
             }
         }
@@ -602,14 +555,14 @@ __device__ __forceinline__ void consume_phase(const MegaParams &p, MkCtx &c, int
 #pragma unroll 1
             for (int k = 0; k < geo.S; ++k) t += sh.part[tid][k];
             c.rold = t;
-            if (p.x_plain) p.x_plain[2 * geo.u0 + tid] = t;   // read by the next kernel
+            if (BLOCK) p.x_plain[2 * geo.u0 + tid] = t;   // read by the next kernel
             else ll_store(p.ll_x + (ph == PH_DOWN ? (size_t)p.hidden : 0) + 2 * geo.u0 + tid, t, c.tag);
         }
         // sh.part is next written after the next phase's stage_input (CTA syncs in between)
     }
 }
 
-template <bool TRACE>
+template <bool TRACE, bool BLOCK>
 __device__ __forceinline__ void run_phase(const MegaParams &p, MkCtx &c, int ph, const uint8_t *ring, MkShared &sh) {
     const PhaseGeom &geo = sh.geo[ph];
     if (geo.n_stages == 0) {
@@ -618,11 +571,11 @@ __device__ __forceinline__ void run_phase(const MegaParams &p, MkCtx &c, int ph,
     }   // no unit of this phase here
     // A6 of layer 0: the residual stream starts as the embedding row; afterwards the owner of a row keeps it in c.rold
     if (ph == PH_O && (int)threadIdx.x < 2 * (geo.u1 - geo.u0)) {
-        if (p.x_plain) c.rold = ld_act(p.x_plain + 2 * geo.u0 + threadIdx.x);
+        if (BLOCK) c.rold = ld_act(p.x_plain + 2 * geo.u0 + threadIdx.x);
         else if (c.layer == 0) c.rold = __bfloat162float(p.emb[(size_t)c.tok * p.hidden + 2 * geo.u0 + threadIdx.x]);
     }
-    if (geo.K <= kMkStagedK) stage_input(p, c, ph, geo.K, sh);
-    consume_phase<kMkSliceChunks / 32, TRACE>(p, c, ph, geo, ring, sh);
+    if (BLOCK || geo.K <= kMkStagedK) stage_input<BLOCK>(p, c, ph, geo.K, sh);
+    consume_phase<kMkSliceChunks / 32, TRACE, BLOCK>(p, c, ph, geo, ring, sh);
     mk_trace<TRACE>(p, c);
 }
 
@@ -755,7 +708,8 @@ __device__ __forceinline__ void attention_phase(const MegaParams &p, MkCtx &c, M
     }
     mk_trace<TRACE>(p, c);
     if (nsub > 1) consumer_sync();
-    if (active && sub == 0 && lane < 8) {
+    if (active && sub == 0) {
+        // every lane: the CTA's state of (head, octet) = its own plus the parked sub-splits
 #pragma unroll 1
         for (int k = 1; k < nsub; ++k) {
             const float *o2 = sh.mrg[k * G + g];
@@ -767,13 +721,77 @@ __device__ __forceinline__ void attention_phase(const MegaParams &p, MkCtx &c, M
             for (int j = 0; j < 8; ++j) o[j] = o[j] * wa + o2[oct * 8 + j] * wb;
             M = Mn;
         }
-        // unnormalised split state as tagged words; the O phase of every CTA merges the splits (stage_input)
         const size_t pidx = (size_t)head * kMkMaxSplits + split;
+        if (ns > 1 && split > 0) {
+            // split state (unnormalised) as tagged words for the CTA of split 0 of this KV head
+            if (lane < 8) {
 #pragma unroll
-        for (int j = 0; j < 8; ++j) ll_store(p.ll_part_o + pidx * kHeadDim + oct * 8 + j, o[j], c.tag);
-        if (lane == 0) {
-            ll_store(p.ll_part_ml + pidx * 2, M, c.tag);
-            ll_store(p.ll_part_ml + pidx * 2 + 1, l, c.tag);
+                for (int j = 0; j < 8; ++j) ll_store(p.ll_part_o + pidx * kHeadDim + oct * 8 + j, o[j], c.tag);
+                if (lane == 0) {
+                    ll_store(p.ll_part_ml + pidx * 2, M, c.tag);
+                    ll_store(p.ll_part_ml + pidx * 2 + 1, l, c.tag);
+                }
+            }
+        } else {
+            // Split 0 merges the other splits of its heads (second level: the ~3 KB it reads are nothing next to every
+            // CTA of the chip reading every split state, 12 MB of L2 reads per layer = 3.5 us in one poll round) and
+            // publishes the final, normalised attention output: the O phase of every CTA polls 8 words per thread.
+            // Lane group j (8 lanes) takes splits j, j + 4 (group 0: its own state and split 4).
+            if (grp > 0) {
+                M = -INFINITY; l = 0.f;
+#pragma unroll
+                for (int j = 0; j < 8; ++j) o[j] = 0.f;
+            }
+#pragma unroll 1
+            for (int r4 = 0; r4 < kMkMaxSplits; r4 += 4) {   // warp-uniform trip count: the poll below votes across the warp
+                const int s = r4 + grp;
+                const bool mine = s >= 1 && s < ns;
+                if (!__any_sync(0xffffffffu, mine)) break;
+                const size_t q2 = (size_t)head * kMkMaxSplits + (mine ? s : 0);
+                llw_t wm[2], wo[8];
+                unsigned spins = 0;
+                for (;;) {
+                    bool ok = true;
+                    if (mine) {
+                        ll_load2(p.ll_part_ml + q2 * 2, wm[0], wm[1]);
+#pragma unroll
+                        for (int j = 0; j < 8; j += 2) ll_load2(p.ll_part_o + q2 * kHeadDim + oct * 8 + j, wo[j], wo[j + 1]);
+                        ok = ll_ok(wm[0], c.tag) && ll_ok(wm[1], c.tag);
+#pragma unroll
+                        for (int j = 0; j < 8; ++j) ok = ok && ll_ok(wo[j], c.tag);
+                    }
+                    if (__all_sync(0xffffffffu, ok)) break;
+                    if (++spins == kMaxPollSpins) mk_fail(p.err, 9);
+                    __nanosleep(64);
+                }
+                if (mine) {
+                    const float M2 = ll_val(wm[0]), l2 = ll_val(wm[1]);
+                    const float Mn = fmaxf(M, M2);
+                    const float wa = (M == -INFINITY) ? 0.f : __expf(M - Mn), wb = (M2 == -INFINITY) ? 0.f : __expf(M2 - Mn);
+                    l = l * wa + l2 * wb;
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) o[j] = o[j] * wa + ll_val(wo[j]) * wb;
+                    M = Mn;
+                }
+            }
+            // merge the 4 lane groups
+            float Mg = fmaxf(M, __shfl_xor_sync(0xffffffffu, M, 8));
+            Mg = fmaxf(Mg, __shfl_xor_sync(0xffffffffu, Mg, 16));
+            const float sg = (M == -INFINITY) ? 0.f : __expf(M - Mg);
+            l *= sg;
+            l += __shfl_xor_sync(0xffffffffu, l, 8);
+            l += __shfl_xor_sync(0xffffffffu, l, 16);
+            const float inv = 1.0f / l;
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                o[j] *= sg;
+                o[j] += __shfl_xor_sync(0xffffffffu, o[j], 8);
+                o[j] += __shfl_xor_sync(0xffffffffu, o[j], 16);
+            }
+            if (lane < 8) {
+#pragma unroll
+                for (int j = 0; j < 8; ++j) ll_store(p.ll_attn + (size_t)head * kHeadDim + oct * 8 + j, o[j] * inv, c.tag);
+            }
         }
     }
     mk_trace<TRACE>(p, c);
@@ -781,7 +799,7 @@ __device__ __forceinline__ void attention_phase(const MegaParams &p, MkCtx &c, M
 }
 
 // ---- the kernel -----------------------------------------------------------------------------------------------
-template <bool TRACE>
+template <bool TRACE, bool BLOCK>
 __global__ void __launch_bounds__(kMkThreads, 1) mega_decode_kernel(const __grid_constant__ MegaParams p) {
     extern __shared__ __align__(128) uint8_t mk_smem[];
     uint8_t *ring = mk_smem;
@@ -805,9 +823,12 @@ __global__ void __launch_bounds__(kMkThreads, 1) mega_decode_kernel(const __grid
 
     // Attention-block launches sit between per-step kernels with programmatic edges: the producer warp (above) is already
     // streaming this launch's weights (immutable), everything else waits for the previous kernel here.
+    MkCtx c;
+    c.gain_pre = make_uint4(0, 0, 0, 0);
+    if (BLOCK && tid * 8 < p.hidden)   // immutable like the weights: its HBM latency overlaps the previous kernel's tail
+        c.gain_pre = __ldg(reinterpret_cast<const uint4 *>(p.layers[p.pi_begin >> 2].attn_norm) + tid);
     pdl_launch_dependents();
     pdl_wait();
-    MkCtx c;
     c.g = 0;
     c.best = 0ull;
     c.ti = 0;
@@ -823,18 +844,18 @@ __global__ void __launch_bounds__(kMkThreads, 1) mega_decode_kernel(const __grid
         consumer_sync();
         const uint32_t tag0 = (epoch0 + (uint32_t)step) * (uint32_t)(p.n_layers + 1) + 1u;   // >= 1: zeroed buffers never match
         const int n_ph = p.n_layers * 4 + (p.with_head ? 1 : 0);
-        const int pi0 = p.x_plain ? p.pi_begin : 0, pi1 = p.x_plain ? p.pi_end : n_ph;
+        const int pi0 = BLOCK ? p.pi_begin : 0, pi1 = BLOCK ? p.pi_end : n_ph;
 #pragma unroll 1
         for (int pi = pi0; pi < pi1; ++pi) {   // a loop, not straight-line code: one copy of every phase body (see consume_phase)
             c.layer = pi >> 2;
-            const int ph = c.layer < p.n_layers ? (pi & 3) : PH_HEAD;
+            const int ph = BLOCK ? (pi & 1 ? PH_O : PH_QKV) : (c.layer < p.n_layers ? (pi & 3) : PH_HEAD);
             c.tag = tag0 + (uint32_t)c.layer;
             c.tag_prev = c.tag - 1u;
             if (ph == PH_HEAD) c.best = 0ull;
-            run_phase<TRACE>(p, c, ph, ring, sh);
+            run_phase<TRACE, BLOCK>(p, c, ph, ring, sh);
             if (ph == PH_QKV) attention_phase<TRACE>(p, c, sh);
         }
-        if (p.x_plain) break;   // attention-block launch: one step, no head, position advanced by the LM-head kernel
+        if (BLOCK) break;   // attention-block launch: one step, no head, position advanced by the LM-head kernel
         c.tag_prev = tag0 + (uint32_t)(p.n_layers - 1);
         c.tag = tag0 + (uint32_t)p.n_layers;
         if (p.with_head) {
@@ -904,17 +925,17 @@ size_t mega_smem_bytes() { return (size_t)kMkStages * kMkStageBytes + sizeof(MkS
 
 size_t mega_ll_words(const hq_config &c) {
     const size_t H = c.n_heads, Hkv = c.n_kv_heads;
-    return 2 * (size_t)c.hidden + (H + 2 * Hkv) * kHeadDim + (size_t)c.ffn + H * kMkMaxSplits * kHeadDim + H * kMkMaxSplits * 2 +
+    return 2 * (size_t)c.hidden + (H + 2 * Hkv) * kHeadDim + (size_t)c.ffn + H * kMkMaxSplits * kHeadDim + H * kMkMaxSplits * 2 + H * kHeadDim +
            2 * (size_t)kMkMaxGrid;
 }
 
 // Most context splits per KV head a model will use = attention CTAs set aside per KV head: enough for max_ctx at two
-// 32-position batches per warp, at most kMkMaxSplits (every CTA re-reads all split states) and a quarter of the SMs.
+// 32-position batch per warp, at most kMkMaxSplits and half of the SMs.
 int mega_att_splits(const hq_config &c, int n_sms, int max_ctx) {
     const int G = c.n_heads / c.n_kv_heads, nsub = kMkConsumerWarps / (G > 0 ? G : 1);
-    const int per = 64 * (nsub > 0 ? nsub : 1);
+    const int per = 32 * (nsub > 0 ? nsub : 1);
     int ns = (max_ctx + per - 1) / per;
-    int cap = (n_sms / 4) / c.n_kv_heads;
+    int cap = (n_sms / 2) / c.n_kv_heads;
     if (cap < 1) cap = 1;
     if (cap > kMkMaxSplits) cap = kMkMaxSplits;
     if (ns > cap) ns = cap;
@@ -936,8 +957,10 @@ cudaError_t launch_mega(const LaunchCtx &c, const MegaParams &p, bool cooperativ
     static bool attr_done = false;
     const size_t smem = mega_smem_bytes();
     if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(mega_decode_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(mega_decode_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaError_t e = cudaFuncSetAttribute(mega_decode_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(mega_decode_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(mega_decode_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(mega_decode_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         attr_done = true;
     }
@@ -961,7 +984,10 @@ cudaError_t launch_mega(const LaunchCtx &c, const MegaParams &p, bool cooperativ
         cfg.numAttrs = cooperative ? 1 : 0;
     }
     // the timeline stamps live in their own instantiation: the production kernel's code has to stay small
-    return p.trace ? cudaLaunchKernelEx(&cfg, mega_decode_kernel<true>, p) : cudaLaunchKernelEx(&cfg, mega_decode_kernel<false>, p);
+    // ... and so does the attention block (its per-launch path has to stay resident in the instruction cache between
+    // launches: everything it does not need is compiled out)
+    if (p.x_plain) return p.trace ? cudaLaunchKernelEx(&cfg, mega_decode_kernel<true, true>, p) : cudaLaunchKernelEx(&cfg, mega_decode_kernel<false, true>, p);
+    return p.trace ? cudaLaunchKernelEx(&cfg, mega_decode_kernel<true, false>, p) : cudaLaunchKernelEx(&cfg, mega_decode_kernel<false, false>, p);
 }
 
 }  // namespace hq
