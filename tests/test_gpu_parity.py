@@ -196,6 +196,19 @@ def test_1b_config1_teacher_forced(one_b_weights, no_mega):
     assert stats["argmax_checked"] >= 16
 
 
+def test_1b_config2_long_context_sampled(one_b_weights):
+    """configs[2] at full size: 2,048-token prompt (one tensor-core pass, causal flash attention over 32 query tiles),
+    then teacher-forced decode steps at context 2,048+ (8 context splits per KV head in the attention block).  The
+    oracle is run on the first steps only (sampled outputs; 256 steps would cost minutes of CPU)."""
+    s = datagen.ONE_B
+    prompt = datagen.tokens(1002, s.vocab, 2048)
+    gm = gpu_model(one_b_weights, max_seq=2304)
+    om = oracle.Model.from_datagen(one_b_weights, max_seq=2304)
+    ref, stats = run_teacher_forced(gm, om, prompt, 6, check_every=1)
+    print("1b config[2] parity:", stats)
+    assert stats["argmax_checked"] >= 2
+
+
 # ---------------------------------------------------------------------------------------------------
 # batched serving (configs[3] shape on the tiny model): tensor-core prefill + batched decode
 # ---------------------------------------------------------------------------------------------------
@@ -242,6 +255,18 @@ def test_tiny_batched_prefill_and_decode(tiny_weights):
     refs, stats = run_batched(gm, tiny_weights, prompts, steps, 64)
     print("tiny batched parity:", stats)
     assert stats["argmax_checked"] >= B * 4
+
+
+def test_1b_config3_batch8_sampled(one_b_weights):
+    """configs[3] at full size: 8 sequences x 192-token prompts in one tensor-core pass (1,536 rows), then batched
+    decode steps (tcgen05 GEMMs with a 32-token tile, split-K across the SMs).  Sampled: the first steps only."""
+    s = datagen.ONE_B
+    B, T, steps = 8, 192, 3
+    prompts = datagen.tokens(1003, s.vocab, B * T).reshape(B, T)
+    gm = gpu_model(one_b_weights, max_seq=T + 192, max_batch=B)
+    refs, stats = run_batched(gm, one_b_weights, prompts, steps, T + 192)
+    print("1b config[3] parity:", stats)
+    assert stats["argmax_checked"] >= B
 
 
 def test_tiny_batch_invariance(tiny_weights):
