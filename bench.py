@@ -186,6 +186,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="hq", choices=["hq", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg")
+    ap.add_argument("--sweep", action="store_true",
+                    help="configs[4]: batch {1,4,16,32} x context {512,4096}, 128 decode steps each; one JSON line per point")
     ap.add_argument("--profile", type=int, default=0, metavar="N",
                     help="ncu helper: one prefill + N decode steps of the bench workload, no timing")
     args = ap.parse_args()
@@ -234,6 +236,42 @@ def main():
         gm.decode_run(DECODE_STEPS, want_tokens=False)
         if events:
             events[2].record(stream)
+
+    if args.sweep:
+        # BASELINE.json configs[4] (and the shapes of configs[2], [3]): tokens/s, per-token latency and algorithmic HBM GB/s
+        peak, _ = measured_peak()
+        lay = gm.weight_tensors()
+        for B in (1, 4, 16, 32):
+            for ctx in (512, 4096):
+                steps = 128
+                m = hq.Model(hq.binding.make_config(n_layers=s.n_layers, hidden=s.hidden, n_heads=s.n_heads, n_kv_heads=s.n_kv_heads,
+                                            head_dim=s.head_dim, ffn=s.ffn, vocab=s.vocab, rms_eps=s.rms_eps,
+                                            rope_theta=s.rope_theta, max_batch=B, max_seq=ctx + steps + 8, flags=0), *lay)
+                pr = datagen.tokens(1004, s.vocab, B * ctx).reshape(B, ctx)
+                ms, pf = [], []
+                for it in range(3):
+                    m.kv_reset()
+                    a, b, c2 = ev(), ev(), ev()
+                    a.record(m.stream)
+                    m.prefill(pr, want_token=False)
+                    b.record(m.stream)
+                    m.decode_run(steps, want_tokens=False, batch=B)
+                    c2.record(m.stream)
+                    torch.cuda.synchronize(dev)
+                    if it:
+                        pf.append(a.elapsed_time(b))
+                        ms.append(b.elapsed_time(c2))
+                step_ms = float(np.mean(ms)) / steps
+                bpt = bytes_per_token(s, ctx + steps // 2, B)
+                print(json.dumps({"sweep": True, "batch": B, "context": ctx, "decode_steps": steps,
+                                  "tokens_per_s": B / (step_ms * 1e-3), "ms_per_step": step_ms,
+                                  "prefill_ms": float(np.mean(pf)), "prefill_tokens_per_s": B * ctx / (float(np.mean(pf)) * 1e-3),
+                                  "bytes_per_step": bpt, "GBps": bpt / (step_ms * 1e-3) / 1e9,
+                                  "frac_of_measured_peak": bpt / (step_ms * 1e-3) / 1e9 / peak}), flush=True)
+                m.close()
+                del m
+                torch.cuda.empty_cache()
+        return
 
     if args.profile:
         gm.kv_reset()
