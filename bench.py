@@ -403,6 +403,11 @@ def main():
             "step_roofline": {"bytes_per_token": bpt, "achieved_GBps": step_gbs, "frac_of_measured": step_gbs / peak,
                               "frac_of_8TBps_spec": step_gbs / 8000.0},
             "kernels_alone": kernels,
+            # the kernel with the largest share of the step TIME (41 %, 8.5 % of the bytes): a latency chain, not a stream
+            "roofline_largest_time_share": {"bound": "hbm", "kernel": "mega_decode_kernel<attention block> (A2-A6 of a layer)",
+                                            "achieved": kernels["attn_block"]["GBps"], "peak": peak, "unit": "GB/s",
+                                            "frac": kernels["attn_block"]["GBps"] / peak,
+                                            "us_per_launch": kernels["attn_block"]["us"]},
             "persistent_kernel": {"value": mega_tok_s, "unit": UNIT,
                                   "note": "HQ_FLAG_MEGA: the same 128 decode steps in ONE launch (hq_mega.cu), this rank"},
         }
