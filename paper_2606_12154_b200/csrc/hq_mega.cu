@@ -130,7 +130,7 @@ __device__ __forceinline__ void ll_poll(const llw_t *src, uint32_t tag, float (&
         for (int i = 0; i < N; ++i) ok = ok && ll_ok(w[i], tag);
         if (ok) break;
         if (++spins == kMaxPollSpins) mk_fail(err, 3);
-        __nanosleep(64);
+        __nanosleep(20);
     }
 #pragma unroll
     for (int i = 0; i < N; ++i) v[i] = ll_val(w[i]);
@@ -331,7 +331,7 @@ __device__ __forceinline__ void stage_input(const MegaParams &p, MkCtx &c, int p
                 }
                 if (__all_sync(0xffffffffu, ok)) break;
                 if (++spins == kMaxPollSpins) mk_fail(p.err, 8);
-                __nanosleep(100);
+                __nanosleep(20);
             }
         }
         consumer_sync();
@@ -437,7 +437,7 @@ __device__ __forceinline__ void load_x_direct(const MegaParams &p, const MkCtx &
                 for (int i = 0; i < 8; ++i) ok = ok && ll_ok(w[k][i], c.tag);
             if (ok) break;
             if (++spins == kMaxPollSpins) mk_fail(p.err, 5);
-                __nanosleep(64);
+                __nanosleep(20);
         }
 #pragma unroll
         for (int k = 0; k < NB; ++k) {
@@ -642,7 +642,7 @@ __device__ __forceinline__ void attention_phase(const MegaParams &p, MkCtx &c, M
             for (int j = 0; j < 8; ++j) ok = ok && ll_ok(wq[j], c.tag);
             if (__all_sync(0xffffffffu, ok)) break;
             if (++spins == kMaxPollSpins) mk_fail(p.err, 6);
-            __nanosleep(64);
+            __nanosleep(20);
         }
 #pragma unroll
         for (int j = 0; j < 8; ++j) q[j] = 0.125f * ll_val(wq[j]);
@@ -762,7 +762,7 @@ __device__ __forceinline__ void attention_phase(const MegaParams &p, MkCtx &c, M
                     }
                     if (__all_sync(0xffffffffu, ok)) break;
                     if (++spins == kMaxPollSpins) mk_fail(p.err, 9);
-                    __nanosleep(64);
+                    __nanosleep(20);
                 }
                 if (mine) {
                     const float M2 = ll_val(wm[0]), l2 = ll_val(wm[1]);
@@ -878,7 +878,7 @@ __global__ void __launch_bounds__(kMkThreads, 1) mega_decode_kernel(const __grid
                     ll_load2(p.ll_best + 2 * i, a, b);
                     if (ll_ok(a, c.tag) && ll_ok(b, c.tag)) break;
                     if (++spins == kMaxPollSpins) mk_fail(p.err, 7);
-                __nanosleep(64);
+                __nanosleep(20);
                 }
                 const unsigned long long v = ((a & 0xFFFFFFFFull) << 32) | (b & 0xFFFFFFFFull);
                 mine = mine > v ? mine : v;
