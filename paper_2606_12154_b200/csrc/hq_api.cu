@@ -374,7 +374,7 @@ static cudaError_t enqueue_rows_head(hq_model *m, int batch, int Tc, int pos_inc
                              c.hidden, c.rms_eps, batch, nullptr, Tc * c.hidden));
     STEP(launch_gemm(lc, EPI_STORE, m->map_lm_head, nullptr, m->map_hn_last, 32, c.vocab, c.hidden, batch, 32, 1, b.logits,
                      nullptr, 0, c.vocab));
-    STEP(launch_argmax_rows(lc, b.logits, c.vocab, batch, b.cur_tok, b.tok_hist, b.pos, pos_inc, b.counter));
+    STEP(launch_argmax_rows(lc, b.logits, c.vocab, batch, b.cur_tok, b.tok_hist, b.pos, pos_inc, b.counter, b.best));
 #undef STEP
     if (n_launched) *n_launched += n;
     return cudaSuccess;

@@ -237,7 +237,7 @@ cudaError_t launch_flash_prefill(const LaunchCtx &c, const __half *q16, const kv
 cudaError_t launch_attn_combine(const LaunchCtx &c, const float *part_o, const float2 *part_ml, act_t *out,
                                 size_t lo_offset, const int *pos, int batch, int n_heads);
 cudaError_t launch_argmax_rows(const LaunchCtx &c, const float *logits, int vocab, int batch, int *cur_tok,
-                               int *tok_hist, int *pos, int pos_inc, unsigned int *counter);
+                               int *tok_hist, int *pos, int pos_inc, unsigned int *counter, unsigned long long *best_rows);
 
 // ---- launchers (hq_decode.cu) ------------------------------------------------------------------------
 cudaError_t launch_embed(const LaunchCtx &c, const bf16 *emb, const int *tok, float *x, int hidden, int batch);

@@ -342,19 +342,36 @@ __global__ void __launch_bounds__(256) attn_combine_kernel(const float *part_o, 
 
 // =====================================================================================================
 // greedy argmax per sequence over fp32 logits [B][V] (lowest index on ties) + step bookkeeping.
-// grid (B), block 1024.  The last block to finish advances the shared position.
+// grid (slices, B), block 256: per-slice winner -> packed 64-bit atomicMax per row; the last CTA of the launch writes
+// the tokens, clears the winners and advances the shared position.
 // =====================================================================================================
-__global__ void __launch_bounds__(1024) argmax_rows_kernel(const float *logits, int vocab, int batch, int *cur_tok,
-                                                           int *tok_hist, int *pos, int pos_inc, unsigned int *counter) {
+__global__ void __launch_bounds__(256) argmax_rows_kernel(const float *logits, int vocab, int batch, int *cur_tok,
+                                                          int *tok_hist, int *pos, int pos_inc, unsigned int *counter,
+                                                          unsigned long long *best_rows) {
     pdl_launch_dependents();
     pdl_wait();
-    __shared__ unsigned long long red[32];
-    const int b = blockIdx.x;
+    __shared__ unsigned long long red[8];
+    __shared__ int last;
+    const int b = blockIdx.y;
     const float *row = logits + (size_t)b * vocab;
+    // slice of the row: float4 loads where the row start is 16-byte aligned, scalar otherwise
+    const int per = ((vocab + (int)gridDim.x - 1) / (int)gridDim.x + 3) & ~3;
+    const int i0 = blockIdx.x * per, i1 = min(vocab, i0 + per);
     unsigned long long best = 0ull;
-    for (int i = threadIdx.x; i < vocab; i += blockDim.x) {
-        const unsigned long long k = pack_argmax(ld_act(row + i), i);
-        best = best > k ? best : k;
+    if ((vocab & 3) == 0) {
+        for (int i = i0 + 4 * threadIdx.x; i + 3 < i1; i += 4 * blockDim.x) {
+            const float4 v = ld_act4(row + i);
+            unsigned long long k0 = pack_argmax(v.x, i), k1 = pack_argmax(v.y, i + 1), k2 = pack_argmax(v.z, i + 2), k3 = pack_argmax(v.w, i + 3);
+            k0 = k0 > k1 ? k0 : k1;
+            k2 = k2 > k3 ? k2 : k3;
+            k0 = k0 > k2 ? k0 : k2;
+            best = best > k0 ? best : k0;
+        }
+    } else {
+        for (int i = i0 + threadIdx.x; i < i1; i += blockDim.x) {
+            const unsigned long long k = pack_argmax(ld_act(row + i), i);
+            best = best > k ? best : k;
+        }
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
@@ -363,24 +380,27 @@ __global__ void __launch_bounds__(1024) argmax_rows_kernel(const float *logits, 
     }
     if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = best;
     __syncthreads();
-    if (threadIdx.x < 32) {
-        best = red[threadIdx.x];
+    if (threadIdx.x == 0) {
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            const unsigned long long other = __shfl_xor_sync(0xffffffffu, best, o);
-            best = best > other ? best : other;
+        for (int w = 1; w < 8; ++w) best = best > red[w] ? best : red[w];
+        if (best) atomicMax(best_rows + b, best);   // packed (ordered logit, ~index): lowest index wins ties
+        __threadfence();
+        const unsigned int ticket = atomicAdd(counter, 1u);
+        last = ticket == gridDim.x * gridDim.y - 1u;
+    }
+    __syncthreads();
+    if (last) {   // the last CTA of the launch: every row's winner is final
+        __threadfence();
+        const int p = ld_act(pos);
+        for (int r = threadIdx.x; r < batch; r += blockDim.x) {
+            const int tok = unpack_argmax_idx(__ldcg(best_rows + r));
+            cur_tok[r] = tok;
+            tok_hist[(size_t)(p + pos_inc) * batch + r] = tok;
+            best_rows[r] = 0ull;
         }
         if (threadIdx.x == 0) {
-            const int p = ld_act(pos);
-            const int tok = unpack_argmax_idx(best);
-            cur_tok[b] = tok;
-            tok_hist[(size_t)(p + pos_inc) * batch + b] = tok;
-            __threadfence();
-            const unsigned int ticket = atomicAdd(counter, 1u);
-            if (ticket == (unsigned int)batch - 1) {
-                *pos = p + pos_inc;
-                *counter = 0u;
-            }
+            *pos = p + pos_inc;
+            *counter = 0u;
         }
     }
 }
@@ -440,9 +460,10 @@ cudaError_t launch_attn_combine(const LaunchCtx &c, const float *part_o, const f
     return launch_k(c, attn_combine_kernel, dim3(batch), dim3(256), part_o, part_ml, out, lo_offset, pos, n_heads);
 }
 cudaError_t launch_argmax_rows(const LaunchCtx &c, const float *logits, int vocab, int batch, int *cur_tok,
-                               int *tok_hist, int *pos, int pos_inc, unsigned int *counter) {
-    return launch_k(c, argmax_rows_kernel, dim3(batch), dim3(1024), logits, vocab, batch, cur_tok, tok_hist, pos,
-                    pos_inc, counter);
+                               int *tok_hist, int *pos, int pos_inc, unsigned int *counter, unsigned long long *best_rows) {
+    const int slices = vocab >= 32768 ? 32 : (vocab >= 4096 ? 4 : 1);
+    return launch_k(c, argmax_rows_kernel, dim3(slices, batch), dim3(256), logits, vocab, batch, cur_tok, tok_hist, pos,
+                    pos_inc, counter, best_rows);
 }
 
 }  // namespace hq
