@@ -92,9 +92,12 @@ size_t hq_workspace_bytes(const hq_config *cfg);
  * >= hq_workspace_bytes).  cuda_stream is a cudaStream_t (NULL = legacy default stream).
  * Supported shapes: head_dim == 64, n_heads % n_kv_heads == 0 with group size <= 8, hidden and
  * ffn multiples of 8 and <= 8192, max_batch <= 32; anything else returns HQ_ERR_UNSUPPORTED.
- * batch 1 decodes with one fused GEMV kernel per step of the path inside a CUDA graph (default, the faster of the two
- * on B200 today), or with HQ_FLAG_MEGA in one persistent kernel per call (TMA-fed weight ring, tagged-word exchange
- * between the SMs, no grid barrier); batch > 1 and prompts of >= 8 tokens run on the tcgen05 GEMM path.
+ * batch 1 decodes, by default, with one CUDA graph per token: per layer one "attention block" launch (RMSNorm, QKV,
+ * RoPE + KV append, split-KV attention, O projection, residual; shapes with hidden and n_heads*head_dim <= 2048) and two
+ * fused GEMV kernels (gate/up + SwiGLU, down + residual), then the LM-head GEMV with fused argmax.  HQ_FLAG_MEGA runs the
+ * whole of hq_decode_run in ONE persistent kernel (TMA-fed weight ring, tagged-word exchange between the SMs, no grid
+ * barrier); HQ_FLAG_NO_MEGA uses one kernel per step of the path.  batch > 1 and prompts of >= 8 tokens run on the tcgen05
+ * GEMM path.
  * Requires compute capability 10.x. */
 int32_t hq_model_create(const hq_config *cfg, const hq_weights *weights, void *workspace_dev,
                         size_t workspace_bytes, void *cuda_stream, hq_model **out);
@@ -161,11 +164,12 @@ int32_t hq_debug_gemm(void *cuda_stream, int32_t mode, const void *w_dev, const 
 
 /* Diagnostics: timeline of the persistent batch-1 decode kernel.  trace_dev: DEVICE uint64 [n_ctas][cap] (n_ctas =
  * number of SMs), or NULL to switch tracing off.  While set, thread 0 of every CTA stores the GPU global timer (ns)
- * at the start of the launch, after every weight phase, after the attention phase and after every grid barrier, in
- * program order (per layer: QKV, barrier, attention, barrier, O, barrier, gate/up, barrier, down, barrier; then LM
- * head, barrier), for every step of every later launch, restarting at index 0 each launch; stamps beyond cap are
- * dropped.  The buffer is BORROWED until tracing is switched off.  Takes effect for direct launches (hq_decode_run);
- * a captured single-step graph keeps the setting it was captured with. */
+ * at the start of the launch and then, in program order, three times per phase — weight phases (QKV, O, gate/up, down,
+ * LM head): input staged / first ring stage landed / phase consumed; attention (after QKV): query polled / computed /
+ * published — plus once when the next token is known, for every step of every later launch, restarting at index 0 each
+ * launch; stamps beyond cap are dropped.  The buffer is BORROWED until tracing is switched off.  Takes effect for direct
+ * launches (hq_decode_run with HQ_FLAG_MEGA, the attention block of hq_bench_kernel); a captured graph keeps the setting it
+ * was captured with. */
 int32_t hq_debug_trace(hq_model *m, uint64_t *trace_dev, int32_t cap);
 
 /* Thread-local message of the last failing call on this thread; static storage, never NULL. */
