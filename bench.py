@@ -113,6 +113,25 @@ class ClockSampler(threading.Thread):
                 "reasons": sorted(self.reasons), "samples": len(self.samples)}
 
 
+def aggregate_over_ranks(dist, dev, dec_total_ms, total_ms, ttft_ms, launches):
+    """N independent replicas: the job's time is the slowest rank's, its launch
+    count the sum.  dist = torch.distributed or None (single process); tensors live on dev (cuda for nccl, cpu for gloo)."""
+    if dist is None:
+        return dec_total_ms, total_ms, ttft_ms, launches
+    import torch
+    t = torch.tensor([dec_total_ms, total_ms, ttft_ms], device=dev, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ln = torch.tensor([launches], device=dev, dtype=torch.int64)
+    dist.all_reduce(ln)
+    a, b, c = [float(v) for v in t.tolist()]
+    return a, b, c, int(ln.item())
+
+
+def job_tokens_per_s(world, steps, dec_total_ms):
+    """Whole-job decode throughput: tokens of all replicas / the slowest replica's decode time."""
+    return world * steps * DECODE_STEPS / (dec_total_ms * 1e-3)
+
+
 def oracle_sample(weights, s, prompt_len=16, steps=24):
     """cpu_baseline: the oracle as it stands on the host cores, on a bounded sample of the workload."""
     import datagen
@@ -363,21 +382,12 @@ def main():
     mega_tok_s = DECODE_STEPS / (float(np.mean(mega_ms)) * 1e-3)
 
     # ---- aggregate over ranks (max time) -----------------------------------------------------------------
-    dec_total_ms = float(sum(decode_ms))
-    if dist is not None:
-        t = torch.tensor([dec_total_ms, total_ms, float(np.mean(prefill_ms))], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dec_total_ms, total_ms, ttft = [float(v) for v in t.tolist()]
-        ln = torch.tensor([launches], device=dev, dtype=torch.int64)
-        dist.all_reduce(ln)
-        launches = int(ln.item())
-    else:
-        ttft = float(np.mean(prefill_ms))
+    dec_total_ms, total_ms, ttft, launches = aggregate_over_ranks(dist, dev, float(sum(decode_ms)), total_ms,
+                                                                  float(np.mean(prefill_ms)), launches)
 
     if rank == 0:
         peak, peak_src = measured_peak()
-        tokens_total = world * args.steps * DECODE_STEPS
-        value = tokens_total / (dec_total_ms * 1e-3)
+        value = job_tokens_per_s(world, args.steps, dec_total_ms)
         ms_per_token = dec_total_ms / (args.steps * DECODE_STEPS)
         ctx_mid = PROMPT_LEN + DECODE_STEPS // 2
         bpt = bytes_per_token(s, ctx_mid)
