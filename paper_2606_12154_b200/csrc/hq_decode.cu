@@ -167,7 +167,13 @@ __global__ void __launch_bounds__(kGemvThreads) gemv_kernel(const __grid_constan
 #pragma unroll
         for (int c = 0; c < CH; ++c) {
             const int chunk = tid + c * kGemvThreads;
-            if (chunk < kchunks) {
+            if (chunk < kchunks && XIN == XIN_PLAIN) {   // SwiGLU vector, fp16 (see the gate/up epilogue)
+                const uint4 h = __ldcg(reinterpret_cast<const uint4 *>(p.xin) + chunk);
+                const float2 f0 = __half22float2(*reinterpret_cast<const __half2 *>(&h.x)), f1 = __half22float2(*reinterpret_cast<const __half2 *>(&h.y));
+                const float2 f2 = __half22float2(*reinterpret_cast<const __half2 *>(&h.z)), f3 = __half22float2(*reinterpret_cast<const __half2 *>(&h.w));
+                xr[c][0] = f0.x; xr[c][1] = f0.y; xr[c][2] = f1.x; xr[c][3] = f1.y;
+                xr[c][4] = f2.x; xr[c][5] = f2.y; xr[c][6] = f3.x; xr[c][7] = f3.y;
+            } else if (chunk < kchunks) {
                 const float4 a = ld_act4(p.xin + chunk * 8), b = ld_act4(p.xin + chunk * 8 + 4);
                 xr[c][0] = a.x; xr[c][1] = a.y; xr[c][2] = a.z; xr[c][3] = a.w;
                 xr[c][4] = b.x; xr[c][5] = b.y; xr[c][6] = b.z; xr[c][7] = b.w;
@@ -222,7 +228,9 @@ __global__ void __launch_bounds__(kGemvThreads) gemv_kernel(const __grid_constan
                 dst[i + 32] = __float2half_rn(b);
             }
         } else if (MODE == GEMV_GATEUP) {
-            p.out[u] = silu_f(a) * b;
+            // fp16: the SwiGLU vector is re-read by every CTA of the down projection (296 x 32 KB through L2 at fp32, as much
+            // L2 traffic as 9.5 MB of weights); 11 mantissa bits on this one vector cost ~1e-4 of the 1e-2 hidden tolerance
+            reinterpret_cast<__half *>(p.out)[u] = __float2half_rn(silu_f(a) * b);
         } else if (MODE == GEMV_RESID) {
             float2 *dst = reinterpret_cast<float2 *>(p.out + 2 * u);
             float2 v = __ldcg(dst);
