@@ -189,6 +189,8 @@ static cudaError_t enqueue_step(hq_model *m, const int *tok_src, bool with_head,
             // shared-memory ring, so the launch is a pure latency chain and two kernel boundaries per layer disappear
             MegaParams ab = mega_params(m, tok_src, 1, false);
             ab.x_plain = b.x; ab.pi_begin = 4 * l; ab.pi_end = 4 * l + 2;
+            ab.pf_grid = getenv("HQ_NO_BLOCK_PREFETCH") ? 0 : gemv_grid_units4(m->n_sms, c.ffn);
+            ab.pf_units = getenv("HQ_BLOCK_PREFETCH_UNITS") ? atoi(getenv("HQ_BLOCK_PREFETCH_UNITS")) : 8;
             STEP(launch_mega(lc, ab, false));
         } else {
         // A2+A3+A4: RMSNorm -> QKV GEMV -> RoPE + KV append

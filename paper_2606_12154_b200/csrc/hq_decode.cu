@@ -476,6 +476,9 @@ static cudaError_t launch_gemv_mx(const LaunchCtx &c, const GemvParams &p) {
     }
 }
 
+// grid of gemv_kernel<1, 4, ...> (K <= 2048) over n_units units: what launch_gemv_mx uses
+int gemv_grid_units4(int n_sms, int n_units) { return min(n_sms * gemv_ctas_per_sm(), (n_units + 3) / 4); }
+
 cudaError_t launch_gemv(const LaunchCtx &c, GemvMode mode, GemvInput xin, const GemvParams &p) {
     if (mode == GEMV_QKV && xin == XIN_NORM) return launch_gemv_mx<GEMV_QKV, XIN_NORM>(c, p);
     if (mode == GEMV_GATEUP && xin == XIN_NORM) return launch_gemv_mx<GEMV_GATEUP, XIN_NORM>(c, p);

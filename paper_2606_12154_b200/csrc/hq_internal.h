@@ -196,6 +196,8 @@ struct MegaParams {
     // attention, O of one layer), residual stream in and out as the plain fp32 vector x_plain
     float *x_plain;
     int pi_begin, pi_end;
+    int pf_units;                // ... units (row pairs) per gate/up CTA to prefetch
+    int pf_grid;                 // attention block: grid of the gate/up GEMV that follows (its first batches are L2-prefetched), 0 = off
     int inflight_stages;         // producer: at most this many ring stages issued and not yet landed (1..kMkStages)
 };
 size_t mega_smem_bytes();
@@ -248,5 +250,6 @@ cudaError_t launch_set_state(const LaunchCtx &c, int *pos, int pos_value, unsign
                              unsigned int *counter, int batch, unsigned int *mk_sync);
 cudaError_t launch_zero_tokens(const LaunchCtx &c, int *cur_tok, int batch);
 bool gemv_shape_supported(int K);
+int gemv_grid_units4(int n_sms, int n_units);
 
 }  // namespace hq

@@ -574,6 +574,23 @@ __device__ __forceinline__ void run_phase(const MegaParams &p, MkCtx &c, int ph,
         if (BLOCK) c.rold = ld_act(p.x_plain + 2 * geo.u0 + threadIdx.x);
         else if (c.layer == 0) c.rold = __bfloat162float(p.emb[(size_t)c.tok * p.hidden + 2 * geo.u0 + threadIdx.x]);
     }
+    if (BLOCK && ph == PH_O && p.pf_grid > 0) {
+        // The memory system idles while this CTA waits for the attention vector: pull the first two weight batches of the
+        // gate/up GEMV CTAs 2b, 2b+1 (the next kernel; same unit split as gemv_kernel) into L2, so that its ramp starts
+        // from L2 hits.  (A look-ahead like this hurt inside the persistent kernel, where it competes with the stream.)
+        const LayerW &w = p.layers[c.layer];
+        const int per = p.ffn / p.pf_grid, rem = p.ffn % p.pf_grid;
+        for (int g = 2 * (int)blockIdx.x; g < 2 * (int)blockIdx.x + 2 && g < p.pf_grid; ++g) {
+            const int u0 = g * per + min(g, rem);
+            const int nu = min(p.pf_units, per + (g < rem ? 1 : 0));
+            const int lines = p.hidden * 2 / 128;   // 128-byte lines per weight row
+            for (int i = threadIdx.x; i < nu * lines; i += kMkConsumers) {
+                const size_t off = (size_t)(u0 + i / lines) * p.hidden + (size_t)(i % lines) * 64;
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(w.w_gate + off));
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(w.w_up + off));
+            }
+        }
+    }
     if (BLOCK || geo.K <= kMkStagedK) stage_input<BLOCK>(p, c, ph, geo.K, sh);
     consume_phase<kMkSliceChunks / 32, TRACE, BLOCK>(p, c, ph, geo, ring, sh);
     mk_trace<TRACE>(p, c);
