@@ -150,6 +150,10 @@ int32_t hq_kv_reset(hq_model *m);
  * residual stream is garbage afterwards: call hq_kv_reset + prefill again before decoding).
  * bytes_per_launch (HOST, may be NULL) receives the algorithmic HBM bytes of one launch. */
 int64_t hq_kernel_count(const hq_model *m);
+/* Which batch-1 decode path this model runs (decided at create from the shape, the flags and the device): static
+ * string, "attention-block-cluster" (default), "kernel-per-row" (HQ_FLAG_NO_MEGA or unsupported shape / clusters not
+ * co-resident) or "persistent" (HQ_FLAG_MEGA). */
+const char *hq_decode_path(const hq_model *m);
 int32_t hq_bench_kernel(hq_model *m, int32_t which, int32_t reps, int64_t *bytes_per_launch);
 
 /* Diagnostics: the tcgen05 GEMM of the prefill / batched-decode path on its own (unit tests).

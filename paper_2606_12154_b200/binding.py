@@ -27,7 +27,7 @@ _CODE_NAMES = {-1: "HQ_ERR_INVALID_ARG", -2: "HQ_ERR_CAPACITY", -3: "HQ_ERR_STAT
 DECLARED_SYMBOLS = (
     "hq_workspace_bytes", "hq_model_create", "hq_model_destroy", "hq_prefill", "hq_decode_step",
     "hq_decode_run", "hq_decode_logits", "hq_get_hidden", "hq_sync", "hq_seq_len", "hq_kv_reset",
-    "hq_kernel_count", "hq_bench_kernel", "hq_debug_gemm", "hq_debug_trace", "hq_last_error", "hq_version",
+    "hq_kernel_count", "hq_decode_path", "hq_bench_kernel", "hq_debug_gemm", "hq_debug_trace", "hq_last_error", "hq_version",
 )
 
 
@@ -93,6 +93,8 @@ def load_library(path: Optional[str] = None):
     l.hq_kv_reset.argtypes = [vp]
     l.hq_kernel_count.restype = i64
     l.hq_kernel_count.argtypes = [vp]
+    l.hq_decode_path.restype = ctypes.c_char_p
+    l.hq_decode_path.argtypes = [vp]
     l.hq_bench_kernel.restype = i32
     l.hq_bench_kernel.argtypes = [vp, i32, i32, ctypes.POINTER(i64)]
     l.hq_debug_gemm.restype = i32
@@ -260,6 +262,9 @@ class Model:
 
     def kernel_count(self) -> int:
         return int(self._lib.hq_kernel_count(self._h))
+
+    def decode_path(self) -> str:
+        return self._lib.hq_decode_path(self._h).decode()
 
     def debug_trace(self, cap: int = 0):
         """Switch the persistent kernel's timeline on (cap > 0: returns the uint64 [n_sms][cap] device tensor the

@@ -117,6 +117,8 @@ static size_t carve(const hq_config *c, char *base, Buffers *b) {
     o.mk_ll = (unsigned long long *)take(mega_ll_words(*c) * sizeof(unsigned long long));
     o.mk_epoch = (unsigned int *)take(sizeof(unsigned int));
     o.mk_sync = (unsigned int *)take(64 * sizeof(unsigned int));
+    o.ab_ll = (unsigned long long *)take((size_t)H * kHeadDim * sizeof(unsigned long long));
+    o.ab_epoch = (unsigned int *)take(sizeof(unsigned int));
     return off;
 }
 
@@ -165,6 +167,24 @@ static MegaParams mega_params(const hq_model *m, const int *tok_src, int n_steps
     return p;
 }
 
+static AttnBlockParams attn_block_params(const hq_model *m, int l) {
+    const hq_config &c = m->cfg;
+    const Buffers &b = m->b;
+    const LayerW &w = m->layers[l];
+    const size_t layer_kv = (size_t)c.max_batch * c.n_kv_heads * c.max_seq * kHeadDim;
+    AttnBlockParams a = {};
+    a.wq = w.wq; a.wk = w.wk; a.wv = w.wv; a.wo = w.wo; a.gain = w.attn_norm;
+    a.x = b.x; a.kc = b.kcache + l * layer_kv; a.vc = b.vcache + l * layer_kv; a.rope = b.rope; a.pos = b.pos;
+    a.ll_attn = b.ab_ll; a.epoch = b.ab_epoch; a.err = (int *)(b.mk_sync + 3);
+    a.hidden = c.hidden; a.n_heads = c.n_heads; a.n_kv_heads = c.n_kv_heads; a.max_seq = c.max_seq; a.eps = c.rms_eps;
+    a.trace = m->trace; a.trace_cap = m->trace_cap;
+    if (m->l2_prefetch & 1) {
+        a.pf_ptr[0] = w.w_gate; a.pf_ptr[1] = w.w_up;
+        a.pf_bytes[0] = a.pf_bytes[1] = (size_t)c.ffn * c.hidden * sizeof(bf16) * m->pf_frac / 100;
+    }
+    return a;
+}
+
 static cudaError_t enqueue_step(hq_model *m, const int *tok_src, bool with_head, int *n_launched) {
     const hq_config &c = m->cfg;
     const LaunchCtx lc{m->stream, m->use_pdl, m->n_sms};
@@ -184,7 +204,10 @@ static cudaError_t enqueue_step(hq_model *m, const int *tok_src, bool with_head,
     for (int l = 0; l < c.n_layers; ++l) {
         const LayerW &w = m->layers[l];
         GemvParams p = {};
-        if (m->use_attn_block) {
+        if (m->use_attn_block && !m->use_old_block) {
+            // A2-A6 of the layer in ONE cluster launch (hq_attn.cu)
+            STEP(launch_attn_block(lc, attn_block_params(m, l)));
+        } else if (m->use_attn_block) {
             // A2-A6 of the layer in ONE launch (hq_mega.cu, phases QKV | attention | O): its 142 KB of weights per SM fit the
             // shared-memory ring, so the launch is a pure latency chain and two kernel boundaries per layer disappear
             MegaParams ab = mega_params(m, tok_src, 1, false);
@@ -212,10 +235,18 @@ static cudaError_t enqueue_step(hq_model *m, const int *tok_src, bool with_head,
         GemvParams pg = {};
         pg.w0 = w.w_gate; pg.w1 = w.w_up; pg.gain = w.ffn_norm; pg.xin = b.x; pg.K = c.hidden;
         pg.n_units = c.ffn; pg.eps = c.rms_eps; pg.out = b.act;
+        const bool pf = m->use_attn_block && !m->use_old_block;
+        if (pf && (m->l2_prefetch & 2)) { pg.pf_ptr[0] = w.w_down; pg.pf_bytes[0] = (size_t)c.hidden * c.ffn * sizeof(bf16); }
         STEP(launch_gemv(lc, GEMV_GATEUP, XIN_NORM, pg));
         // A8: down GEMV -> residual
         GemvParams pd = {};
         pd.w0 = w.w_down; pd.xin = b.act; pd.K = c.ffn; pd.n_units = c.hidden / 2; pd.out = b.x;
+        if (pf && (m->l2_prefetch & 4) && l + 1 < c.n_layers) {
+            const LayerW &nw = m->layers[l + 1];
+            const size_t qb = (size_t)qdim * c.hidden * sizeof(bf16), kb = (size_t)c.n_kv_heads * kHeadDim * c.hidden * sizeof(bf16);
+            pd.pf_ptr[0] = nw.wq; pd.pf_bytes[0] = qb; pd.pf_ptr[1] = nw.wk; pd.pf_bytes[1] = kb;
+            pd.pf_ptr[2] = nw.wv; pd.pf_bytes[2] = kb; pd.pf_ptr[3] = nw.wo; pd.pf_bytes[3] = qb;
+        }
         STEP(launch_gemv(lc, GEMV_RESID, XIN_PLAIN, pd));
         if (c.flags & HQ_FLAG_CAPTURE_HIDDEN) {
             e = cudaMemcpyAsync(b.hidden + (size_t)l * c.max_batch * c.hidden, b.x, c.hidden * sizeof(float),
@@ -506,8 +537,21 @@ extern "C" int32_t hq_model_create(const hq_config *cfg, const hq_weights *w, vo
     }
     m->use_pdl = !(cfg->flags & HQ_FLAG_NO_PDL) && !getenv("HQ_NO_PDL");
     if (const char *fl = getenv("HQ_MEGA_INFLIGHT")) m->mega_inflight = atoi(fl) < 1 ? 1 : (atoi(fl) > kMkStages ? kMkStages : atoi(fl));
-    m->use_attn_block = !(cfg->flags & HQ_FLAG_NO_MEGA) && !getenv("HQ_NO_MEGA") && !getenv("HQ_NO_ATTN_BLOCK") &&
-                        mega_shape_supported(*cfg, m->n_sms);
+    m->use_old_block = getenv("HQ_OLD_BLOCK") != nullptr;
+    m->l2_prefetch = getenv("HQ_L2_PREFETCH") ? atoi(getenv("HQ_L2_PREFETCH")) : 0;
+    m->pf_frac = getenv("HQ_PF_FRAC") ? atoi(getenv("HQ_PF_FRAC")) : 100;
+    if (m->use_old_block) {
+        m->use_attn_block = !(cfg->flags & HQ_FLAG_NO_MEGA) && !getenv("HQ_NO_MEGA") && mega_shape_supported(*cfg, m->n_sms);
+    } else {
+        m->use_attn_block = !(cfg->flags & HQ_FLAG_NO_MEGA) && !getenv("HQ_NO_MEGA") && attn_block_shape_supported(*cfg);
+        if (m->use_attn_block) {
+            // the clusters of one launch wait for one another's attention vector: all of them must be resident at once
+            bool co_resident = false;
+            cudaError_t e = attn_block_prepare(cfg->n_kv_heads, &co_resident);
+            if (e != cudaSuccess) { cudaGetLastError(); co_resident = false; }
+            m->use_attn_block = co_resident;
+        }
+    }
     m->use_mega = ((cfg->flags & HQ_FLAG_MEGA) || getenv("HQ_MEGA")) && !(cfg->flags & HQ_FLAG_NO_MEGA) && !getenv("HQ_NO_MEGA") &&
                   mega_shape_supported(*cfg, m->n_sms);
     {
@@ -516,6 +560,9 @@ extern "C" int32_t hq_model_create(const hq_config *cfg, const hq_weights *w, vo
         // tagged exchange words start with tag 0 (never a valid epoch); the epoch counter only ever grows
         if (e == cudaSuccess) e = cudaMemsetAsync(m->b.mk_ll, 0, mega_ll_words(*cfg) * sizeof(unsigned long long), m->stream);
         if (e == cudaSuccess) e = cudaMemsetAsync(m->b.mk_epoch, 0, sizeof(unsigned int), m->stream);
+        const unsigned int one = 1u;
+        if (e == cudaSuccess) e = cudaMemsetAsync(m->b.ab_ll, 0, (size_t)cfg->n_heads * kHeadDim * sizeof(unsigned long long), m->stream);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(m->b.ab_epoch, &one, sizeof(one), cudaMemcpyHostToDevice, m->stream);
         if (e == cudaSuccess) e = cudaStreamSynchronize(m->stream);
         if (e != cudaSuccess) {
             delete m;
@@ -604,6 +651,13 @@ extern "C" int32_t hq_kv_reset(hq_model *m) {
 }
 
 extern "C" int64_t hq_kernel_count(const hq_model *m) { return m ? m->kernel_count : 0; }
+
+extern "C" const char *hq_decode_path(const hq_model *m) {
+    if (!m) return "";
+    if (m->use_mega) return "persistent";
+    if (m->use_attn_block) return m->use_old_block ? "attention-block-l2" : "attention-block-cluster";
+    return "kernel-per-row";
+}
 
 // ---- prefill -----------------------------------------------------------------------------------------
 extern "C" int32_t hq_prefill(hq_model *m, const int32_t *tokens_host, int32_t batch, int32_t n_tokens,
@@ -823,6 +877,12 @@ extern "C" int32_t hq_bench_kernel(hq_model *m, int32_t which, int32_t reps, int
             }
             case 6: {
                 // attention block: QKV + attention + O of layer l in one launch (rewrites the K/V row at the current position)
+                if (m->use_attn_block && !m->use_old_block) {
+                    HQ_CUDA(launch_attn_block(lc, attn_block_params(m, l)));
+                    bytes = 2ll * ((c.n_heads + 2 * c.n_kv_heads) * kHeadDim + c.hidden) * c.hidden +
+                            2ll * 2 * c.n_kv_heads * kHeadDim * (m->seq_len + 1);
+                    break;
+                }
                 if (!mega_shape_supported(c, m->n_sms)) return fail(HQ_ERR_UNSUPPORTED, "hq_bench_kernel: shape not supported by the attention block");
                 MegaParams ab = mega_params(m, b.cur_tok, 1, false);
                 ab.x_plain = b.x; ab.pi_begin = 4 * l; ab.pi_end = 4 * l + 2;

@@ -14,6 +14,111 @@ __device__ __forceinline__ void pdl_launch_dependents() {
 }
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 
+// ---- mbarrier / bulk async copy (TMA) / thread-block cluster wrappers -------------------------------------
+__device__ __forceinline__ uint32_t smem_addr_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_addr_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_fence_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_addr_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_addr_u32(bar)) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(uint64_t *bar, uint32_t parity) {
+    uint32_t ok;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"(smem_addr_u32(bar)), "r"(parity)
+        : "memory");
+    return ok != 0;
+}
+// acquire at cluster scope: pairs with remote arrives (mbar_arrive_remote) of other CTAs of the cluster
+__device__ __forceinline__ bool mbar_try_wait_cluster(uint64_t *bar, uint32_t parity) {
+    uint32_t ok;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"(smem_addr_u32(bar)), "r"(parity)
+        : "memory");
+    return ok != 0;
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
+    while (!mbar_try_wait(bar, parity)) {}
+}
+__device__ __forceinline__ void bulk_g2s(void *smem_dst, const void *gmem_src, uint32_t bytes, uint64_t *bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     smem_addr_u32(smem_dst)),
+                 "l"(gmem_src), "r"(bytes), "r"(smem_addr_u32(bar))
+                 : "memory");
+}
+// weights are read once per token: evict-first keeps the KV cache and the activations resident in the 126 MB L2
+__device__ __forceinline__ uint64_t l2_policy_evict_first() {
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+__device__ __forceinline__ void bulk_g2s_hint(void *smem_dst, const void *gmem_src, uint32_t bytes, uint64_t *bar, uint64_t pol) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(
+                     smem_addr_u32(smem_dst)),
+                 "l"(gmem_src), "r"(bytes), "r"(smem_addr_u32(bar)), "l"(pol)
+                 : "memory");
+}
+__device__ __forceinline__ uint32_t cluster_ctarank() { uint32_t r; asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r)); return r; }
+__device__ __forceinline__ uint32_t cluster_id_x() { uint32_t r; asm volatile("mov.u32 %0, %%clusterid.x;" : "=r"(r)); return r; }
+__device__ __forceinline__ void cluster_sync_all() {
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+// address of the same shared-memory location in CTA `rank` of the cluster (distributed shared memory)
+__device__ __forceinline__ uint32_t cluster_map(uint32_t smem_addr, uint32_t rank) {
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(smem_addr), "r"(rank));
+    return r;
+}
+__device__ __forceinline__ void st_cluster_f32x2(uint32_t addr, float a, float b) {
+    asm volatile("st.shared::cluster.v2.f32 [%0], {%1, %2};" ::"r"(addr), "f"(a), "f"(b) : "memory");
+}
+__device__ __forceinline__ float ld_cluster_f32(uint32_t addr) {
+    float v;
+    asm volatile("ld.shared::cluster.f32 %0, [%1];" : "=f"(v) : "r"(addr) : "memory");
+    return v;
+}
+// Asynchronous store of two floats into the shared memory of a CTA of the cluster; the bytes are credited (complete_tx)
+// to an mbarrier of the SAME destination CTA, whose waiters then see the data: a push with no fence and no release (a
+// release at cluster scope also waits for the SM's bulk copies in flight: measured ~1.5 us under a weight prefetch).
+__device__ __forceinline__ void st_async_f32x2(uint32_t cluster_addr, float a, float b, uint32_t cluster_mbar) {
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.f32 [%0], {%1, %2}, [%3];" ::"r"(cluster_addr),
+                 "f"(a), "f"(b), "r"(cluster_mbar)
+                 : "memory");
+}
+// L2 prefetch of a contiguous global range (bytes a multiple of 16)
+__device__ __forceinline__ void bulk_prefetch_l2(const void *gmem_src, uint32_t bytes) {
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(gmem_src), "r"(bytes) : "memory");
+}
+
+// Slice `part` of `n_parts` of a contiguous (immutable) global range -> L2, in pieces of <= 64 KB.  One thread.  Used to
+// pull the NEXT kernel's weights into the 126 MB L2 while this kernel is latency-bound: HBM keeps streaming, and the next
+// kernel reads L2 hits (measured: L2 -> SM ~13 TB/s chip-wide, HBM ~6.5 TB/s).
+__device__ __forceinline__ void prefetch_slice_l2(const void *base, size_t bytes, int part, int n_parts) {
+    if (!base) return;
+    size_t per = (bytes + (size_t)n_parts - 1) / (size_t)n_parts;
+    per = (per + 127) & ~(size_t)127;
+    const size_t b0 = (size_t)part * per;
+    if (b0 >= bytes) return;
+    const size_t b1 = b0 + per < bytes ? b0 + per : bytes;
+    const char *p = static_cast<const char *>(base);
+    for (size_t o = b0; o < b1; o += 65536) {
+        const size_t n = b1 - o < 65536 ? b1 - o : 65536;
+        bulk_prefetch_l2(p + o, (uint32_t)(n & ~(size_t)15));
+    }
+}
+
 // ---- loads ------------------------------------------------------------------------------------------
 // Weights: immutable, streamed once per token -> non-coherent path, do not allocate in L1.
 __device__ __forceinline__ uint4 ld_weight16(const void *p) {
@@ -44,6 +149,31 @@ __device__ __forceinline__ float dot8(const uint4 &w, const float (&x)[8], float
     acc = fmaf(bf16lo(w.w), x[6], acc);
     acc = fmaf(bf16hi(w.w), x[7], acc);
     return acc;
+}
+
+// ---- packed fp32 pairs: Blackwell issues two fp32 FMAs per instruction (fma.rn.f32x2 -> FFMA2) ----------------------
+typedef unsigned long long f32x2_t;
+__device__ __forceinline__ f32x2_t pack_f32x2(float lo, float hi) {
+    f32x2_t r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ float sum_f32x2(f32x2_t v) {
+    float lo, hi;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+    return lo + hi;
+}
+__device__ __forceinline__ void ffma2(f32x2_t &acc, f32x2_t a, f32x2_t b) {
+    asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(acc) : "l"(a), "l"(b));
+}
+// two bf16 packed in a u32 (element 0 in the low half) -> fp32 pair, exact
+__device__ __forceinline__ f32x2_t bf16x2_to_f32x2(uint32_t u) { return pack_f32x2(__uint_as_float(u << 16), __uint_as_float(u & 0xFFFF0000u)); }
+// 8 bf16 (one 16-byte chunk) times 8 fp32 held as 4 pairs, accumulated pairwise into acc[0..3]: 4 FFMA2 + 8 ALU ops
+__device__ __forceinline__ void dot8_x2(const uint4 &w, const f32x2_t (&x)[4], f32x2_t (&acc)[4]) {
+    ffma2(acc[0], bf16x2_to_f32x2(w.x), x[0]);
+    ffma2(acc[1], bf16x2_to_f32x2(w.y), x[1]);
+    ffma2(acc[2], bf16x2_to_f32x2(w.z), x[2]);
+    ffma2(acc[3], bf16x2_to_f32x2(w.w), x[3]);
 }
 
 __device__ __forceinline__ float warp_sum(float v) {

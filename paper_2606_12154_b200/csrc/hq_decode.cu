@@ -130,6 +130,10 @@ __global__ void __launch_bounds__(kGemvThreads) gemv_kernel(const __grid_constan
     }
     pdl_launch_dependents();
     pdl_wait();
+    if (tid == 0) {
+#pragma unroll
+        for (int i = 0; i < 4; ++i) prefetch_slice_l2(p.pf_ptr[i], p.pf_bytes[i], blockIdx.x, gridDim.x);
+    }
 
     // ---- input vector into registers -------------------------------------------------------------
     float xr[CH][8];
@@ -310,29 +314,6 @@ __global__ void __launch_bounds__(kGemvThreads) gemv_kernel(const __grid_constan
 // =====================================================================================================
 constexpr int kAttnTile = 128;  // positions per staged tile (16 KB of K + 16 KB of V)
 
-__device__ __forceinline__ void mbar_init(uint64_t *bar, int count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((uint32_t)__cvta_generic_to_shared(bar)), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"((uint32_t)__cvta_generic_to_shared(bar)),
-                 "r"(bytes)
-                 : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
-    asm volatile(
-        "{\n\t.reg .pred P1;\n\tWAIT_LOOP:\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n\t"
-        "@P1 bra DONE;\n\tbra WAIT_LOOP;\n\tDONE:\n\t}" ::"r"((uint32_t)__cvta_generic_to_shared(bar)),
-        "r"(parity)
-        : "memory");
-}
-__device__ __forceinline__ void bulk_g2s(void *smem_dst, const void *gmem_src, uint32_t bytes, uint64_t *bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
-                     (uint32_t)__cvta_generic_to_shared(smem_dst)),
-                 "l"(gmem_src), "r"(bytes), "r"((uint32_t)__cvta_generic_to_shared(bar))
-                 : "memory");
-}
-
 __global__ void __launch_bounds__(256) attn_decode_kernel(const __grid_constant__ AttnDecodeParams p) {
     __shared__ __align__(128) kv_t Ks[kAttnTile * kHeadDim];
     __shared__ __align__(128) kv_t Vs[kAttnTile * kHeadDim];
@@ -345,7 +326,7 @@ __global__ void __launch_bounds__(256) attn_decode_kernel(const __grid_constant_
 
     if (threadIdx.x == 0) {
         mbar_init(&bar, 1);
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        mbar_fence_init();
     }
     __syncthreads();
     pdl_launch_dependents();

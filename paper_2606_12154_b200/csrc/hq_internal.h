@@ -77,6 +77,8 @@ struct Buffers {
     unsigned long long *mk_ll = nullptr;        // tagged-word exchange buffers (mega_ll_words() words, zeroed at create)
     unsigned int *mk_epoch = nullptr;           // steps run so far by the persistent kernel (never reset: tags only grow)
     unsigned int *mk_sync = nullptr;            // [3] error flag of the persistent kernel
+    unsigned long long *ab_ll = nullptr;        // attention block: tagged words of the attention vector [H * 64] (zeroed at create)
+    unsigned int *ab_epoch = nullptr;           // attention block: tag of the next launch (starts at 1, never reset)
 };
 
 constexpr int kTokenTiles[4] = {32, 64, 128, 256};
@@ -103,7 +105,10 @@ struct hq_model_impl {
     TensorMap map_hn[4], map_ao[4], map_actb[4], map_hn_last;   // activation maps per token tile
     cudaGraphExec_t batch_graph = nullptr;      // batched decode step (captured for batch_graph_b)
     int batch_graph_b = 0, batch_graph_kernels = 0, batch_eager_b = 0;
-    bool use_attn_block = false;                // per-step path: QKV + attention + O of a layer in one launch (hq_mega.cu)
+    bool use_attn_block = false;                // per-step path: QKV + attention + O of a layer in one cluster launch (hq_attn.cu)
+    bool use_old_block = false;                 // round-1 attention block (hq_mega.cu), A/B only
+    int l2_prefetch = 0;                        // bit 0: attention block -> gate/up weights, 1: gate/up -> down, 2: down -> next layer's attention weights
+    int pf_frac = 100;
     bool use_mega = false;                      // batch-1 decode runs in the persistent kernel
     bool mega_coop = true;                      // launched with the cooperative attribute
     int mega_inflight = 2;                      // bulk-copy stages in flight per SM during the layers (HQ_MEGA_INFLIGHT overrides)
@@ -136,6 +141,9 @@ struct GemvParams {
     int *cur_tok, *tok_hist;
     int *pos_rw;
     int pos_inc;
+    // weights of the kernel(s) that follow, pulled into L2 by this launch after its dependency wait (NULL / 0 = none)
+    const void *pf_ptr[4];
+    size_t pf_bytes[4];
 };
 
 struct AttnDecodeParams {
@@ -205,6 +213,29 @@ size_t mega_ll_words(const hq_config &c);   // 64-bit words of exchange buffers
 bool mega_shape_supported(const hq_config &c, int n_sms);
 int mega_att_splits(const hq_config &c, int n_sms, int max_ctx);
 cudaError_t launch_mega(const LaunchCtx &c, const MegaParams &p, bool cooperative);
+
+// ---- attention block: A2-A6 of a layer in one cluster launch (hq_attn.cu) -----------------------------------
+constexpr int kAbCluster = 8;        // CTAs per cluster = per KV head (portable cluster size)
+struct AttnBlockParams {
+    const bf16 *wq, *wk, *wv, *wo, *gain;   // this layer's projections and attn_norm gains
+    float *x;                        // [hidden] residual stream, in and out
+    kv_t *kc, *vc;                   // this layer's cache of sequence 0: [n_kv_heads][max_seq][64]
+    const float2 *rope;              // [max_seq][32]
+    const int *pos;                  // device-resident position
+    unsigned long long *ll_attn;     // [n_heads * 64] tagged words (fp32 value | epoch tag): the attention vector
+    unsigned int *epoch;             // launches so far + 1: the tag of this launch (advanced by the kernel, never reset)
+    int *err;                        // device error flag (a lost arrival traps instead of hanging)
+    int hidden, n_heads, n_kv_heads, max_seq;
+    float eps;
+    unsigned long long *trace;       // NULL or [grid][trace_cap] global-timer stamps (hq_debug_trace)
+    int trace_cap;
+    const void *pf_ptr[2];           // weights of the gate/up GEMV that follows, pulled into L2 meanwhile (NULL = none)
+    size_t pf_bytes[2];
+};
+size_t attn_block_smem_bytes();
+bool attn_block_shape_supported(const hq_config &c);
+cudaError_t attn_block_prepare(int n_kv_heads, bool *co_resident);
+cudaError_t launch_attn_block(const LaunchCtx &c, const AttnBlockParams &p);
 
 // ---- tensor-core GEMM (hq_gemm.cu) -------------------------------------------------------------------
 enum GemmEpilogue { EPI_STORE = 0, EPI_RESID = 1, EPI_SWIGLU = 2 };
