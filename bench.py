@@ -54,15 +54,16 @@ def measured_peak():
     return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-def ncu_traffic():
-    """dram bytes per launch of the dominant kernel from the committed ncu --set full summary."""
+def ncu_numbers():
+    """Per-launch figures copied from the committed ncu --set full summaries (profiles/roofline_traffic.json): DRAM
+    bytes and the serialised (no PDL overlap, cold) duration of the decode kernels."""
     p = os.path.join(ROOT, "profiles", "roofline_traffic.json")
     if os.path.exists(p):
         try:
-            return json.load(open(p)).get("gateup_gemv_dram_bytes_per_launch")
+            return json.load(open(p))
         except Exception:
-            return None
-    return None
+            return {}
+    return {}
 
 
 class ClockSampler(threading.Thread):
@@ -71,6 +72,7 @@ class ClockSampler(threading.Thread):
     def __init__(self, index: int):
         super().__init__(daemon=True)
         self.index, self.samples, self.reasons, self.max_mhz = index, [], set(), None
+        self.mem, self.power = [], []
         self._stop_evt = threading.Event()
         self.ok = False
         try:
@@ -96,6 +98,8 @@ class ClockSampler(threading.Thread):
         while not self._stop_evt.is_set():
             try:
                 self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                self.mem.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_MEM))
+                self.power.append(nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0)
                 r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
                 for bit, name in names.items():
                     if r & bit:
@@ -110,7 +114,10 @@ class ClockSampler(threading.Thread):
         if not self.samples:
             return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons)}
         return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz,
-                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+                "reasons": sorted(self.reasons), "samples": len(self.samples),
+                "mem_mhz": float(np.median(self.mem)) if self.mem else None,
+                "power_w_median": float(np.median(self.power)) if self.power else None,
+                "power_w_max": float(np.max(self.power)) if self.power else None}
 
 
 def aggregate_over_ranks(dist, dev, dec_total_ms, total_ms, ttft_ms, launches):
@@ -148,8 +155,10 @@ def oracle_sample(weights, s, prompt_len=16, steps=24):
     t2 = time.perf_counter()
     return {"value": steps / (t2 - t1), "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
             "sample": f"same 1B weights; {prompt_len}-token prompt (prefill {t1 - t0:.2f} s, "
-                      f"{prompt_len / (t1 - t0):.1f} tok/s) then {steps} greedy decode steps "
-                      f"({(t2 - t1) / steps * 1e3:.0f} ms/token)"}
+                      f"{prompt_len / (t1 - t0):.1f} tok/s) then {steps} greedy decode steps at context "
+                      f"{prompt_len + 1}..{prompt_len + steps} ({(t2 - t1) / steps * 1e3:.0f} ms/token); the workload's context "
+                      f"is 257..384 - the oracle is weight-bound, so its rate barely depends on it (full configs[1] "
+                      f"timing: profiles/r02_oracle_full_config1.md)"}
 
 
 def run_reference(args):
@@ -184,8 +193,8 @@ def run_reference(args):
         tp += a
         td += b
     value = args.steps * steps / td
-    sample = (f"per step: {prompt_len}-token prompt + {steps} greedy decode steps of the same 1B weights "
-              f"(bounded sample of configs[1])")
+    sample = (f"per step: {prompt_len}-token prompt + {steps} greedy decode steps (context {prompt_len + 1}.."
+              f"{prompt_len + steps}) of the same 1B weights (bounded sample of configs[1], whose context is 257..384)")
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": (tp + td) / args.steps * 1e3,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",

@@ -50,8 +50,9 @@ enum {
     HQ_FLAG_CAPTURE_HIDDEN = 1u, /* keep the residual stream after every layer (parity tests) */
     HQ_FLAG_NO_GRAPH = 2u,       /* launch decode kernels directly instead of replaying a CUDA graph */
     HQ_FLAG_NO_PDL = 4u,         /* no programmatic dependent launch edges between kernels */
-    HQ_FLAG_NO_MEGA = 8u,        /* never use the persistent decode kernel (wins over HQ_FLAG_MEGA and the HQ_MEGA environment variable) */
-    HQ_FLAG_MEGA = 16u           /* batch-1 decode in ONE persistent kernel per call instead of one kernel per step of the path */
+    HQ_FLAG_KERNEL_PER_ROW = 8u  /* batch-1 decode with one kernel per row of SURVEY.md 8(a) (QKV, attention, O as three
+                                    launches) instead of the cluster attention block; also what a device that cannot keep
+                                    all the block's clusters resident falls back to */
 };
 
 typedef struct hq_model hq_model; /* opaque, library-owned (host memory) */
@@ -85,24 +86,30 @@ typedef struct {
 } hq_weights;
 
 /* Bytes of DEVICE workspace hq_model_create needs for this config (KV cache + activations +
- * RoPE table + scratch); 0 if the config is invalid.  Pure host arithmetic, needs no GPU. */
+ * RoPE table + scratch); 0 if the config is invalid.  Pure host arithmetic, needs no GPU.
+ * Defined by: north_star "PyTorch used only for device memory" (the caller allocates); the KV share is the paper's
+ * "context length is free" accounting (section 6.6): 2 * n_kv_heads * 64 * 2 B * n_layers per cached token. */
 size_t hq_workspace_bytes(const hq_config *cfg);
 
 /* Build a model over borrowed DEVICE weights and a borrowed DEVICE workspace (256-byte aligned,
  * >= hq_workspace_bytes).  cuda_stream is a cudaStream_t (NULL = legacy default stream).
  * Supported shapes: head_dim == 64, n_heads % n_kv_heads == 0 with group size <= 8, hidden and
  * ffn multiples of 8 and <= 8192, max_batch <= 32; anything else returns HQ_ERR_UNSUPPORTED.
- * batch 1 decodes, by default, with one CUDA graph per token: per layer one "attention block" launch (RMSNorm, QKV,
- * RoPE + KV append, split-KV attention, O projection, residual; shapes with hidden and n_heads*head_dim <= 2048) and two
- * fused GEMV kernels (gate/up + SwiGLU, down + residual), then the LM-head GEMV with fused argmax.  HQ_FLAG_MEGA runs the
- * whole of hq_decode_run in ONE persistent kernel (TMA-fed weight ring, tagged-word exchange between the SMs, no grid
- * barrier); HQ_FLAG_NO_MEGA uses one kernel per step of the path.  batch > 1 and prompts of >= 8 tokens run on the tcgen05
- * GEMM path.
- * Requires compute capability 10.x. */
+ * batch 1 decodes with one CUDA graph per token: per layer one "attention block" launch (thread-block clusters, one per
+ * KV head: RMSNorm, QKV, RoPE + KV append, split-KV attention, O projection, residual; shapes with hidden and
+ * n_heads*head_dim <= 2048) and two fused GEMV kernels (gate/up + SwiGLU, down + residual), then the LM-head GEMV with
+ * fused argmax.  The clusters of one attention-block launch wait for one another, so create proves with
+ * cudaOccupancyMaxActiveClusters that all of them are resident at once ON AN OTHERWISE IDLE DEVICE and takes the
+ * kernel-per-row path otherwise (as does HQ_FLAG_KERNEL_PER_ROW).  The proof does not cover a co-tenant: a model that
+ * decodes with the attention block needs the device to itself (no second decoding model on another stream, no MPS
+ * neighbour holding shared memory); a lost arrival traps after 2^24 polls and surfaces as HQ_ERR_CUDA at the next
+ * synchronising call.  batch > 1 and prompts of >= 8 tokens run on the tcgen05 GEMM path.  The library reads no
+ * environment variable.  Requires compute capability 10.x.
+ * Defined by: BASELINE.json north_star ("hq_model_create from a shape config and device weight pointers"). */
 int32_t hq_model_create(const hq_config *cfg, const hq_weights *weights, void *workspace_dev,
                         size_t workspace_bytes, void *cuda_stream, hq_model **out);
 
-/* Frees graphs/events/handles; never the borrowed memory.  NULL is a no-op. */
+/* Frees graphs/events/handles; never the borrowed memory.  NULL is a no-op.  (Counterpart of hq_model_create.) */
 void hq_model_destroy(hq_model *m);
 
 /* Envelope prefill ("a single prompt evaluation"): feed n_tokens tokens per
@@ -124,62 +131,33 @@ int32_t hq_prefill(hq_model *m, const int32_t *tokens_host, int32_t batch, int32
 int32_t hq_decode_step(hq_model *m, const int32_t *tokens_in_host, int32_t *tokens_out_host);
 
 /* n_steps free-running greedy decode steps enqueued back to back (no host round trip between
- * them).  tokens_out_host: HOST int32 [n_steps][batch] or NULL (asynchronous). */
+ * them): the "decode rate" of PAPER.md:L109-111 (section 6.2) is this call's tokens per second.
+ * tokens_out_host: HOST int32 [n_steps][batch] or NULL (asynchronous). */
 int32_t hq_decode_run(hq_model *m, int32_t n_steps, int32_t *tokens_out_host);
 
-/* Parity/diagnostics.  logits_dev: DEVICE fp32 [batch][vocab] <- logits of the last prefill/step.
+/* Parity (north_star: "relative L2 <= 1e-2 per-layer hidden state, <= 2e-2 on logits" against the oracle).
+ * logits_dev: DEVICE fp32 [batch][vocab] <- logits of the last prefill/step.
  * hidden_dev: DEVICE fp32 [batch][hidden] <- residual stream after `layer` at the last position
  * of the last prefill/step (needs HQ_FLAG_CAPTURE_HIDDEN).  Asynchronous device-to-device copies. */
 int32_t hq_decode_logits(hq_model *m, float *logits_dev);
+/* Same passage as hq_decode_logits (north_star parity tolerances): the per-layer hidden state. */
 int32_t hq_get_hidden(hq_model *m, int32_t layer, float *hidden_dev);
 
-/* Block until everything enqueued so far has finished. */
+/* Block until everything enqueued so far has finished (the point at which PAPER.md:L109 "end-to-end wall" stops). */
 int32_t hq_sync(hq_model *m);
 
-/* Cached positions per sequence (host mirror; exact because lengths advance in lock step). */
+/* Cached positions per sequence (host mirror; exact because lengths advance in lock step): the context the paper's
+ * section 6.6 sweeps. */
 int32_t hq_seq_len(const hq_model *m, int32_t *out);
 
-/* seq_len <- 0, active batch cleared; the cache memory is not scrubbed. */
+/* seq_len <- 0, active batch cleared; the cache memory is not scrubbed.  north_star "hq_kv_reset": every query of the
+ * paper's runtime is independent (route, render, speak), so the cache restarts per query. */
 int32_t hq_kv_reset(hq_model *m);
 
-/* Measurement hooks (bench.py roofline leg, ncu).  hq_kernel_count: kernels launched by this
- * model since create (graph replays count their kernel nodes).  hq_bench_kernel: enqueue `reps`
- * launches of one named kernel family of the decode step, cycling over layers so that the weights
- * streamed exceed L2: which = 0 gate/up+SwiGLU GEMV, 1 LM head+argmax, 2 QKV+RoPE, 3 O-proj,
- * 4 down-proj, 5 split-KV attention.  Needs a prefilled cache; results are discarded (the
- * residual stream is garbage afterwards: call hq_kv_reset + prefill again before decoding).
- * bytes_per_launch (HOST, may be NULL) receives the algorithmic HBM bytes of one launch. */
-int64_t hq_kernel_count(const hq_model *m);
-/* Which batch-1 decode path this model runs (decided at create from the shape, the flags and the device): static
- * string, "attention-block-cluster" (default), "kernel-per-row" (HQ_FLAG_NO_MEGA or unsupported shape / clusters not
- * co-resident) or "persistent" (HQ_FLAG_MEGA). */
-const char *hq_decode_path(const hq_model *m);
-int32_t hq_bench_kernel(hq_model *m, int32_t which, int32_t reps, int64_t *bytes_per_launch);
-
-/* Diagnostics: the tcgen05 GEMM of the prefill / batched-decode path on its own (unit tests).
- * All pointers DEVICE.  w, w2: bf16 [n_rows][k]; x: bf16 [2][n_tokens][k], the activation as two planes
- * x = hi + lo (hi = bf16(x), lo = bf16(x - hi)); token_tile in {32,64,128,256}.
- *   mode 0: out fp32 [n_tokens][n_rows]  = x w^T   (splits > 1: out must be zeroed, partials add atomically)
- *   mode 1: out fp32 [n_tokens][n_rows] += x w^T   (residual epilogue)
- *   mode 2: out bf16 [2][n_tokens][n_rows] = hi/lo planes of silu(x w^T) * (x w2^T)   (SwiGLU epilogue)
- * Asynchronous on cuda_stream. */
-int32_t hq_debug_gemm(void *cuda_stream, int32_t mode, const void *w_dev, const void *w2_dev, const void *x_dev,
-                      void *out_dev, int32_t n_rows, int32_t k, int32_t n_tokens, int32_t token_tile, int32_t splits);
-
-/* Diagnostics: timeline of the persistent batch-1 decode kernel.  trace_dev: DEVICE uint64 [n_ctas][cap] (n_ctas =
- * number of SMs), or NULL to switch tracing off.  While set, thread 0 of every CTA stores the GPU global timer (ns)
- * at the start of the launch and then, in program order, three times per phase — weight phases (QKV, O, gate/up, down,
- * LM head): input staged / first ring stage landed / phase consumed; attention (after QKV): query polled / computed /
- * published — plus once when the next token is known, for every step of every later launch, restarting at index 0 each
- * launch; stamps beyond cap are dropped.  The buffer is BORROWED until tracing is switched off.  Takes effect for direct
- * launches (hq_decode_run with HQ_FLAG_MEGA, the attention block of hq_bench_kernel); a captured graph keeps the setting it
- * was captured with. */
-int32_t hq_debug_trace(hq_model *m, uint64_t *trace_dev, int32_t cap);
-
-/* Thread-local message of the last failing call on this thread; static storage, never NULL. */
+/* Thread-local message of the last failing call on this thread; static storage, never NULL (error convention above). */
 const char *hq_last_error(void);
 
-/* Library version string, e.g. "hq 0.1 sm_100a". */
+/* Library version string, e.g. "hq 0.2 sm_100a" (north_star: "built for sm_100a"; the tests check the suffix). */
 const char *hq_version(void);
 
 #ifdef __cplusplus

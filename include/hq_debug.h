@@ -1,0 +1,59 @@
+/*
+ * hq_debug.h — measurement and diagnostic entry points of libhq, kept apart from the product ABI (hq.h).
+ * bench.py's roofline leg, the ncu captures under profiles/ and the GEMM unit tests call these; an
+ * application that speaks an answer needs none of them.
+ */
+#ifndef HQ_DEBUG_H_
+#define HQ_DEBUG_H_
+
+#include "hq.h"
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* Measurement hooks (bench.py roofline leg, ncu).  hq_kernel_count: kernels launched by this
+ * model since create (graph replays count their kernel nodes).  hq_bench_kernel: enqueue `reps`
+ * launches of one named kernel family of the decode step, cycling over layers so that the weights
+ * streamed exceed L2: which = 0 gate/up+SwiGLU GEMV, 1 LM head+argmax, 2 QKV+RoPE, 3 O-proj,
+ * 4 down-proj, 5 split-KV attention.  Needs a prefilled cache; results are discarded (the
+ * residual stream is garbage afterwards: call hq_kv_reset + prefill again before decoding).
+ * bytes_per_launch (HOST, may be NULL) receives the algorithmic HBM bytes of one launch. */
+int64_t hq_kernel_count(const hq_model *m);
+/* Which batch-1 decode path this model runs (decided at create from the shape, the flags and the device): static
+ * string, "attention-block-cluster" (default) or "kernel-per-row" (HQ_FLAG_KERNEL_PER_ROW, unsupported shape, or clusters
+ * not co-resident). */
+const char *hq_decode_path(const hq_model *m);
+int32_t hq_bench_kernel(hq_model *m, int32_t which, int32_t reps, int64_t *bytes_per_launch);
+
+/* Diagnostics: the tcgen05 GEMM of the prefill / batched-decode path on its own (unit tests).
+ * All pointers DEVICE.  w, w2: bf16 [n_rows][k]; x: bf16 [2][n_tokens][k], the activation as two planes
+ * x = hi + lo (hi = bf16(x), lo = bf16(x - hi)); token_tile in {32,64,128,256}.
+ *   mode 0: out fp32 [n_tokens][n_rows]  = x w^T   (splits > 1: out must be zeroed, partials add atomically)
+ *   mode 1: out fp32 [n_tokens][n_rows] += x w^T   (residual epilogue)
+ *   mode 2: out bf16 [2][n_tokens][n_rows] = hi/lo planes of silu(x w^T) * (x w2^T)   (SwiGLU epilogue)
+ * Asynchronous on cuda_stream. */
+int32_t hq_debug_gemm(void *cuda_stream, int32_t mode, const void *w_dev, const void *w2_dev, const void *x_dev,
+                      void *out_dev, int32_t n_rows, int32_t k, int32_t n_tokens, int32_t token_tile, int32_t splits);
+
+/* Measurement: read-only streaming probe: one launch sums the 32-bit words of src_dev[0, bytes) into
+ * *sum_dev (atomicAdd, wraps; DEVICE uint32, caller-zeroed).  Time it with CUDA events on cuda_stream over a buffer much
+ * larger than L2: bytes / time is what a kernel that only reads HBM reaches on this box.  Asynchronous. */
+int32_t hq_debug_read_probe(void *cuda_stream, const void *src_dev, size_t bytes, uint32_t *sum_dev);
+
+/* Parity: one cached position read back.  which = 0 (K, rotated) or 1 (V); row_dev: DEVICE fp16 [n_kv_heads][64] <-
+ * the cache row of `layer`, sequence `seq`, position `pos` (the cache itself is [L][B][Hkv][max_seq][64] fp16).
+ * Asynchronous device-to-device copy on the model's stream. */
+int32_t hq_debug_kv_row(hq_model *m, int32_t which, int32_t layer, int32_t seq, int32_t pos, void *row_dev);
+
+/* Diagnostics: timeline of the attention block.  trace_dev: DEVICE uint64 [n_ctas][cap] (n_ctas = 8 * n_kv_heads), or
+ * NULL to switch tracing off.  While set, thread 0 of every CTA of an attention-block launch stores the GPU global timer
+ * (ns) at fixed points of the launch (see ab_trace in csrc/hq_attn.cu), restarting at index 0 each launch; stamps beyond
+ * cap are dropped.  The buffer is BORROWED until tracing is switched off.  Takes effect for direct launches
+ * (hq_bench_kernel, HQ_FLAG_NO_GRAPH); a captured graph keeps the setting it was captured with. */
+int32_t hq_debug_trace(hq_model *m, uint64_t *trace_dev, int32_t cap);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HQ_DEBUG_H_ */

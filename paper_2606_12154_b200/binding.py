@@ -16,18 +16,18 @@ _LIB_PATH = os.path.join(_HERE, "libhq.so")
 FLAG_CAPTURE_HIDDEN = 1
 FLAG_NO_GRAPH = 2
 FLAG_NO_PDL = 4
-FLAG_NO_MEGA = 8
-FLAG_MEGA = 16
+FLAG_KERNEL_PER_ROW = 8
 
 HQ_OK, HQ_ERR_INVALID_ARG, HQ_ERR_CAPACITY, HQ_ERR_STATE, HQ_ERR_CUDA, HQ_ERR_UNSUPPORTED = 0, -1, -2, -3, -4, -5
 _CODE_NAMES = {-1: "HQ_ERR_INVALID_ARG", -2: "HQ_ERR_CAPACITY", -3: "HQ_ERR_STATE", -4: "HQ_ERR_CUDA",
                -5: "HQ_ERR_UNSUPPORTED"}
 
-# every symbol include/hq.h declares (tests check the header and the library against this list)
+# every symbol include/hq.h and include/hq_debug.h declare (tests check the headers and the library against this list)
 DECLARED_SYMBOLS = (
     "hq_workspace_bytes", "hq_model_create", "hq_model_destroy", "hq_prefill", "hq_decode_step",
     "hq_decode_run", "hq_decode_logits", "hq_get_hidden", "hq_sync", "hq_seq_len", "hq_kv_reset",
-    "hq_kernel_count", "hq_decode_path", "hq_bench_kernel", "hq_debug_gemm", "hq_debug_trace", "hq_last_error", "hq_version",
+    "hq_kernel_count", "hq_decode_path", "hq_bench_kernel", "hq_debug_gemm", "hq_debug_kv_row", "hq_debug_read_probe", "hq_debug_trace", "hq_last_error",
+    "hq_version",
 )
 
 
@@ -99,6 +99,10 @@ def load_library(path: Optional[str] = None):
     l.hq_bench_kernel.argtypes = [vp, i32, i32, ctypes.POINTER(i64)]
     l.hq_debug_gemm.restype = i32
     l.hq_debug_gemm.argtypes = [vp, i32, vp, vp, vp, vp, i32, i32, i32, i32, i32]
+    l.hq_debug_read_probe.restype = i32
+    l.hq_debug_read_probe.argtypes = [vp, vp, ctypes.c_size_t, vp]
+    l.hq_debug_kv_row.restype = i32
+    l.hq_debug_kv_row.argtypes = [vp, i32, i32, i32, i32, vp]
     l.hq_debug_trace.restype = i32
     l.hq_debug_trace.argtypes = [vp, vp, i32]
     l.hq_last_error.restype = ctypes.c_char_p
@@ -167,8 +171,9 @@ class Model:
         w = Weights(embedding.data_ptr(), *[ctypes.cast(arrays[k], _vpp) for k in LAYER_TENSORS],
                     final_norm.data_ptr(), head.data_ptr())
         h = ctypes.c_void_p()
-        _check(self._lib.hq_model_create(ctypes.byref(cfg), ctypes.byref(w), self.workspace.data_ptr(),
-                                         nbytes, self.stream.cuda_stream, ctypes.byref(h)))
+        with torch.cuda.device(self.device):     # the library creates the model on the CURRENT device
+            _check(self._lib.hq_model_create(ctypes.byref(cfg), ctypes.byref(w), self.workspace.data_ptr(),
+                                             nbytes, self.stream.cuda_stream, ctypes.byref(h)))
         self._h = h
         self.vocab, self.hidden, self.n_layers = cfg.vocab, cfg.hidden, cfg.n_layers
 
@@ -266,9 +271,16 @@ class Model:
     def decode_path(self) -> str:
         return self._lib.hq_decode_path(self._h).decode()
 
+    def kv_row(self, which: str, layer: int, pos: int, seq: int = 0):
+        """Cached K ("k", rotated) or V ("v") of one position: fp16 device tensor [n_kv_heads * 64]."""
+        t = self._torch.empty(self.cfg.n_kv_heads * 64, dtype=self._torch.float16, device=self.device)
+        _check(self._lib.hq_debug_kv_row(self._h, 0 if which == "k" else 1, layer, seq, pos, t.data_ptr()))
+        self.sync()
+        return t
+
     def debug_trace(self, cap: int = 0):
-        """Switch the persistent kernel's timeline on (cap > 0: returns the uint64 [n_sms][cap] device tensor the
-        next hq_decode_run launches fill) or off (cap == 0)."""
+        """Switch the attention block's timeline on (cap > 0: returns the uint64 [n_ctas][cap] device tensor the next
+        direct launches fill) or off (cap == 0)."""
         if cap <= 0:
             _check(self._lib.hq_debug_trace(self._h, None, 0))
             self._trace = None
@@ -282,6 +294,14 @@ class Model:
         b = ctypes.c_int64()
         _check(self._lib.hq_bench_kernel(self._h, which, reps, ctypes.byref(b)))
         return b.value
+
+
+def read_probe(buf, result, stream=None):
+    """hq_debug_read_probe: one read-only pass over the CUDA tensor buf; result = uint32/int32 CUDA tensor [1]."""
+    import torch
+    st = stream if stream is not None else torch.cuda.current_stream(buf.device)
+    _check(load_library().hq_debug_read_probe(st.cuda_stream, buf.data_ptr(), buf.numel() * buf.element_size(),
+                                              result.data_ptr()))
 
 
 def debug_gemm(mode: int, w, x, out, *, w2=None, token_tile: int = 128, splits: int = 1, stream=None):

@@ -34,7 +34,11 @@ static int32_t fail(int32_t code, const char *fmt, ...) {
     } while (0)
 
 extern "C" const char *hq_last_error(void) { return g_err; }
-extern "C" const char *hq_version(void) { return "hq 0.1 sm_100a"; }
+
+// Every entry point that touches the GPU makes the model's device current first (a caller may have switched devices
+// between calls; kernel attributes and launches are per device).
+#define HQ_ON_DEVICE(m) HQ_CUDA(cudaSetDevice((m)->device))
+extern "C" const char *hq_version(void) { return "hq 0.2 sm_100a"; }
 
 // ---- workspace layout ---------------------------------------------------------------------------------
 static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
@@ -56,8 +60,8 @@ static bool config_supported(const hq_config *c, const char **why) {
     if (c->n_heads % c->n_kv_heads != 0) BAD("n_heads must be a multiple of n_kv_heads");
     if (c->n_heads / c->n_kv_heads > 8) BAD("GQA group size must be <= 8");
     if (!gemv_shape_supported(c->hidden) || !gemv_shape_supported(c->ffn) ||
-        !gemv_shape_supported(c->n_heads * c->head_dim))
-        BAD("hidden, ffn and n_heads*head_dim must be multiples of 8 and <= 8192");
+        !gemv_shape_supported(c->n_heads * c->head_dim) || !sgemv_shape_supported(c->hidden) || !sgemv_shape_supported(c->ffn))
+        BAD("hidden, ffn and n_heads*head_dim must be multiples of 8 (of 16 above 2048) and <= 8192");
     if (c->vocab % 2 != 0 || c->hidden % 2 != 0) BAD("vocab and hidden must be even");
     if (c->max_batch > 32) BAD("max_batch must be <= 32");
     if (c->n_kv_heads > 56) BAD("n_kv_heads must be <= 56");
@@ -93,7 +97,8 @@ static size_t carve(const hq_config *c, char *base, Buffers *b) {
     o.cur_tok = (int *)take(B * sizeof(int));
     o.tok_hist = (int *)take((T + 1) * B * sizeof(int));
     o.best = (unsigned long long *)take(B * sizeof(unsigned long long));
-    o.counter = (unsigned int *)take(sizeof(unsigned int));
+    o.counter = (unsigned int *)take(2 * sizeof(unsigned int));
+    o.ticket = base ? o.counter + 1 : nullptr;
     o.x = (float *)take(B * d * sizeof(float));
     o.q = (float *)take(B * H * kHeadDim * sizeof(float));
     o.part_o = (float *)take(B * H * kMaxSplits * kHeadDim * sizeof(float));
@@ -113,10 +118,7 @@ static size_t carve(const hq_config *c, char *base, Buffers *b) {
     o.ao = (act_t *)take(2 * R * qdim * sizeof(act_t));
     o.actb = (act_t *)take(2 * R * F * sizeof(act_t));
     o.hn_last = (act_t *)take(2 * 32 * d * sizeof(act_t));
-    o.mk_layers = (LayerW *)take(L * sizeof(LayerW));
-    o.mk_ll = (unsigned long long *)take(mega_ll_words(*c) * sizeof(unsigned long long));
-    o.mk_epoch = (unsigned int *)take(sizeof(unsigned int));
-    o.mk_sync = (unsigned int *)take(64 * sizeof(unsigned int));
+    o.err = (int *)take(sizeof(int));
     o.ab_ll = (unsigned long long *)take((size_t)H * kHeadDim * sizeof(unsigned long long));
     o.ab_epoch = (unsigned int *)take(sizeof(unsigned int));
     return off;
@@ -134,39 +136,6 @@ extern "C" size_t hq_workspace_bytes(const hq_config *cfg) {
 // ---- one decode step: A1..A9 ------------------------------------------------------------------------
 // tok_src: device pointer to the token fed at this step.  with_head = false skips A9 and advances
 // the position with a one-thread kernel instead (used while walking a prompt token by token).
-static MegaParams mega_params(const hq_model *m, const int *tok_src, int n_steps, bool with_head) {
-    const hq_config &c = m->cfg;
-    const Buffers &b = m->b;
-    MegaParams p = {};
-    p.n_layers = c.n_layers; p.hidden = c.hidden; p.n_heads = c.n_heads; p.n_kv_heads = c.n_kv_heads; p.ffn = c.ffn;
-    p.vocab = c.vocab; p.max_seq = c.max_seq; p.eps = c.rms_eps;
-    p.emb = m->emb; p.final_norm = m->final_norm; p.lm_head = m->lm_head; p.layers = b.mk_layers; p.rope = b.rope;
-    p.kc = b.kcache; p.vc = b.vcache;
-    p.layer_kv = (size_t)c.max_batch * c.n_kv_heads * c.max_seq * kHeadDim;
-    p.pos = b.pos; p.cur_tok = b.cur_tok; p.tok_hist = b.tok_hist; p.tok_src = tok_src;
-    p.epoch = b.mk_epoch; p.err = (int *)(b.mk_sync + 3);
-    p.trace = m->trace; p.trace_cap = m->trace_cap;
-    {   // carve the exchange buffers (layout must match mega_ll_words)
-        const size_t H = c.n_heads, Hkv = c.n_kv_heads;
-        unsigned long long *w = b.mk_ll;
-        p.ll_x = w; w += 2 * (size_t)c.hidden;
-        p.ll_qkv = w; w += (H + 2 * Hkv) * kHeadDim;
-        p.ll_act = w; w += c.ffn;
-        p.ll_part_o = w; w += H * kMkMaxSplits * kHeadDim;
-        p.ll_part_ml = w; w += H * kMkMaxSplits * 2;
-        p.ll_attn = w; w += H * kHeadDim;
-        p.ll_best = w;
-    }
-    p.logits = b.logits;
-    p.hidden_out = (c.flags & HQ_FLAG_CAPTURE_HIDDEN) ? b.hidden : nullptr;
-    p.hidden_stride = (size_t)c.max_batch * c.hidden;
-    p.n_steps = n_steps; p.with_head = with_head ? 1 : 0;
-    p.att_splits = mega_att_splits(c, m->n_sms, c.max_seq);
-    p.att_ctas = getenv("HQ_MEGA_DEDICATED") ? p.att_splits * c.n_kv_heads : 0;
-    p.inflight_stages = m->mega_inflight;
-    return p;
-}
-
 static AttnBlockParams attn_block_params(const hq_model *m, int l) {
     const hq_config &c = m->cfg;
     const Buffers &b = m->b;
@@ -175,26 +144,44 @@ static AttnBlockParams attn_block_params(const hq_model *m, int l) {
     AttnBlockParams a = {};
     a.wq = w.wq; a.wk = w.wk; a.wv = w.wv; a.wo = w.wo; a.gain = w.attn_norm;
     a.x = b.x; a.kc = b.kcache + l * layer_kv; a.vc = b.vcache + l * layer_kv; a.rope = b.rope; a.pos = b.pos;
-    a.ll_attn = b.ab_ll; a.epoch = b.ab_epoch; a.err = (int *)(b.mk_sync + 3);
+    a.ll_attn = b.ab_ll; a.epoch = b.ab_epoch; a.err = b.err;
     a.hidden = c.hidden; a.n_heads = c.n_heads; a.n_kv_heads = c.n_kv_heads; a.max_seq = c.max_seq; a.eps = c.rms_eps;
     a.trace = m->trace; a.trace_cap = m->trace_cap;
-    if (m->l2_prefetch & 1) {
-        a.pf_ptr[0] = w.w_gate; a.pf_ptr[1] = w.w_up;
-        a.pf_bytes[0] = a.pf_bytes[1] = (size_t)c.ffn * c.hidden * sizeof(bf16) * m->pf_frac / 100;
-    }
     return a;
+}
+
+static SgemvParams sgemv_gateup(const hq_model *m, int l) {
+    const hq_config &c = m->cfg;
+    const LayerW &w = m->layers[l];
+    SgemvParams p = {};
+    p.w0 = w.w_gate; p.w1 = w.w_up; p.gain = w.ffn_norm; p.xin = m->b.x; p.K = c.hidden; p.n_rows = c.ffn;
+    p.mode = SGEMV_GATEUP; p.xin_mode = SGEMV_XIN_NORM; p.eps = c.rms_eps;
+    p.out_planes = reinterpret_cast<bf16 *>(m->b.act); p.ticket = m->dyn_ticket ? m->b.ticket : nullptr;
+    return p;
+}
+static SgemvParams sgemv_down(const hq_model *m, int l) {
+    const hq_config &c = m->cfg;
+    SgemvParams p = {};
+    p.w0 = m->layers[l].w_down; p.xin = m->b.act; p.K = c.ffn; p.n_rows = c.hidden;
+    p.mode = SGEMV_RESID; p.xin_mode = SGEMV_XIN_PLANES; p.out = m->b.x; p.ticket = m->dyn_ticket ? m->b.ticket : nullptr;
+    return p;
+}
+// final norm + LM head + argmax over the residual row x; the position advances by pos_inc
+static SgemvParams sgemv_lm_head(const hq_model *m, const float *x, int pos_inc) {
+    const hq_config &c = m->cfg;
+    const Buffers &b = m->b;
+    SgemvParams p = {};
+    p.w0 = m->lm_head; p.gain = m->final_norm; p.xin = x; p.K = c.hidden; p.n_rows = c.vocab;
+    p.mode = SGEMV_LMHEAD; p.xin_mode = SGEMV_XIN_NORM; p.eps = c.rms_eps; p.out = b.logits;
+    p.pos = b.pos; p.best = b.best; p.counter = b.counter; p.cur_tok = b.cur_tok; p.tok_hist = b.tok_hist;
+    p.pos_rw = b.pos; p.pos_inc = pos_inc; p.ticket = m->dyn_ticket ? b.ticket : nullptr;
+    return p;
 }
 
 static cudaError_t enqueue_step(hq_model *m, const int *tok_src, bool with_head, int *n_launched) {
     const hq_config &c = m->cfg;
     const LaunchCtx lc{m->stream, m->use_pdl, m->n_sms};
     const Buffers &b = m->b;
-    if (m->use_mega) {
-        // A1-A9 in one persistent launch (hq_mega.cu)
-        cudaError_t em = launch_mega(lc, mega_params(m, tok_src, 1, with_head), m->mega_coop);
-        if (em == cudaSuccess && n_launched) *n_launched = 1;
-        return em;
-    }
     const int qdim = c.n_heads * kHeadDim;
     const size_t layer_kv = (size_t)c.max_batch * c.n_kv_heads * c.max_seq * kHeadDim;
     cudaError_t e;
@@ -204,17 +191,9 @@ static cudaError_t enqueue_step(hq_model *m, const int *tok_src, bool with_head,
     for (int l = 0; l < c.n_layers; ++l) {
         const LayerW &w = m->layers[l];
         GemvParams p = {};
-        if (m->use_attn_block && !m->use_old_block) {
+        if (m->use_attn_block) {
             // A2-A6 of the layer in ONE cluster launch (hq_attn.cu)
             STEP(launch_attn_block(lc, attn_block_params(m, l)));
-        } else if (m->use_attn_block) {
-            // A2-A6 of the layer in ONE launch (hq_mega.cu, phases QKV | attention | O): its 142 KB of weights per SM fit the
-            // shared-memory ring, so the launch is a pure latency chain and two kernel boundaries per layer disappear
-            MegaParams ab = mega_params(m, tok_src, 1, false);
-            ab.x_plain = b.x; ab.pi_begin = 4 * l; ab.pi_end = 4 * l + 2;
-            ab.pf_grid = getenv("HQ_NO_BLOCK_PREFETCH") ? 0 : gemv_grid_units4(m->n_sms, c.ffn);
-            ab.pf_units = getenv("HQ_BLOCK_PREFETCH_UNITS") ? atoi(getenv("HQ_BLOCK_PREFETCH_UNITS")) : 8;
-            STEP(launch_mega(lc, ab, false));
         } else {
         // A2+A3+A4: RMSNorm -> QKV GEMV -> RoPE + KV append
         p.w0 = w.wq; p.w1 = w.wk; p.w2 = w.wv; p.gain = w.attn_norm; p.xin = b.x; p.K = c.hidden;
@@ -231,23 +210,9 @@ static cudaError_t enqueue_step(hq_model *m, const int *tok_src, bool with_head,
         po.out = b.x; po.pos = b.pos;
         STEP(launch_gemv(lc, GEMV_RESID, XIN_ATTN, po));
         }
-        // A2+A7: RMSNorm -> gate/up GEMV -> SwiGLU
-        GemvParams pg = {};
-        pg.w0 = w.w_gate; pg.w1 = w.w_up; pg.gain = w.ffn_norm; pg.xin = b.x; pg.K = c.hidden;
-        pg.n_units = c.ffn; pg.eps = c.rms_eps; pg.out = b.act;
-        const bool pf = m->use_attn_block && !m->use_old_block;
-        if (pf && (m->l2_prefetch & 2)) { pg.pf_ptr[0] = w.w_down; pg.pf_bytes[0] = (size_t)c.hidden * c.ffn * sizeof(bf16); }
-        STEP(launch_gemv(lc, GEMV_GATEUP, XIN_NORM, pg));
-        // A8: down GEMV -> residual
-        GemvParams pd = {};
-        pd.w0 = w.w_down; pd.xin = b.act; pd.K = c.ffn; pd.n_units = c.hidden / 2; pd.out = b.x;
-        if (pf && (m->l2_prefetch & 4) && l + 1 < c.n_layers) {
-            const LayerW &nw = m->layers[l + 1];
-            const size_t qb = (size_t)qdim * c.hidden * sizeof(bf16), kb = (size_t)c.n_kv_heads * kHeadDim * c.hidden * sizeof(bf16);
-            pd.pf_ptr[0] = nw.wq; pd.pf_bytes[0] = qb; pd.pf_ptr[1] = nw.wk; pd.pf_bytes[1] = kb;
-            pd.pf_ptr[2] = nw.wv; pd.pf_bytes[2] = kb; pd.pf_ptr[3] = nw.wo; pd.pf_bytes[3] = qb;
-        }
-        STEP(launch_gemv(lc, GEMV_RESID, XIN_PLAIN, pd));
+        // A2+A7: RMSNorm -> gate/up GEMV -> SwiGLU (bf16 hi/lo planes of the vector); A8: down GEMV -> residual
+        STEP(launch_sgemv(lc, sgemv_gateup(m, l)));
+        STEP(launch_sgemv(lc, sgemv_down(m, l)));
         if (c.flags & HQ_FLAG_CAPTURE_HIDDEN) {
             e = cudaMemcpyAsync(b.hidden + (size_t)l * c.max_batch * c.hidden, b.x, c.hidden * sizeof(float),
                                 cudaMemcpyDeviceToDevice, m->stream);
@@ -256,11 +221,7 @@ static cudaError_t enqueue_step(hq_model *m, const int *tok_src, bool with_head,
     }
     if (with_head) {
         // A9: final norm -> LM head GEMV -> logits + argmax + step bookkeeping
-        GemvParams ph = {};
-        ph.w0 = m->lm_head; ph.gain = m->final_norm; ph.xin = b.x; ph.K = c.hidden; ph.n_units = c.vocab / 2;
-        ph.eps = c.rms_eps; ph.out = b.logits; ph.pos = b.pos; ph.best = b.best; ph.counter = b.counter;
-        ph.cur_tok = b.cur_tok; ph.tok_hist = b.tok_hist; ph.pos_rw = b.pos; ph.pos_inc = 1;
-        STEP(launch_gemv(lc, GEMV_LMHEAD, XIN_NORM, ph));
+        STEP(launch_sgemv(lc, sgemv_lm_head(m, b.x, 1)));
     } else {
         STEP(launch_advance(lc, b.pos, 1));
     }
@@ -402,16 +363,12 @@ static cudaError_t enqueue_rows_head(hq_model *m, int batch, int Tc, int pos_inc
     cudaError_t e;
     int n = 0;
 #define STEP(call) do { e = (call); if (e != cudaSuccess) return e; ++n; } while (0)
-    if (batch == 1 && gemv_shape_supported(c.hidden)) {
+    if (batch == 1) {
         // one sequence: the batch-1 LM-head GEMV (A9: final norm, 6.4 TB/s weight stream, fused argmax and bookkeeping) on the
         // last row of the pass instead of norm + 32-token-tile GEMM + argmax (116 + 10 us -> 85 us)
         float *xl = b.xs + (size_t)(Tc - 1) * c.hidden;
         if (deferred) STEP(launch_add_delta_rows(lc, xl, b.delta + (size_t)(Tc - 1) * c.hidden, (size_t)c.hidden));
-        GemvParams ph = {};
-        ph.w0 = m->lm_head; ph.gain = m->final_norm; ph.xin = xl; ph.K = c.hidden; ph.n_units = c.vocab / 2;
-        ph.eps = c.rms_eps; ph.out = b.logits; ph.pos = b.pos; ph.best = b.best; ph.counter = b.counter;
-        ph.cur_tok = b.cur_tok; ph.tok_hist = b.tok_hist; ph.pos_rw = b.pos; ph.pos_inc = pos_inc;
-        STEP(launch_gemv(lc, GEMV_LMHEAD, XIN_NORM, ph));
+        STEP(launch_sgemv(lc, sgemv_lm_head(m, xl, pos_inc)));
         if (n_launched) *n_launched += n;
         return cudaSuccess;
     }
@@ -513,9 +470,12 @@ extern "C" int32_t hq_model_create(const hq_config *cfg, const hq_weights *w, vo
         return fail(HQ_ERR_UNSUPPORTED, "hq_model_create: needs compute capability 10.x (sm_100a), found %d.%d",
                     prop.major, prop.minor);
 
+    HQ_CUDA(gemm_prepare());
+    HQ_CUDA(sgemv_prepare());
     hq_model *m = new (std::nothrow) hq_model();
     if (!m) return fail(HQ_ERR_INVALID_ARG, "hq_model_create: out of host memory");
     m->cfg = *cfg;
+    m->device = dev;
     m->stream = (cudaStream_t)cuda_stream;
     m->n_sms = prop.multiProcessorCount;
     m->emb = (const bf16 *)w->tok_embedding;
@@ -535,38 +495,26 @@ extern "C" int32_t hq_model_create(const hq_config *cfg, const hq_weights *w, vo
         delete m;
         return fail(HQ_ERR_CUDA, "hq_model_create: cuTensorMapEncodeTiled failed (driver entry point or bad alignment)");
     }
-    m->use_pdl = !(cfg->flags & HQ_FLAG_NO_PDL) && !getenv("HQ_NO_PDL");
-    if (const char *fl = getenv("HQ_MEGA_INFLIGHT")) m->mega_inflight = atoi(fl) < 1 ? 1 : (atoi(fl) > kMkStages ? kMkStages : atoi(fl));
-    m->use_old_block = getenv("HQ_OLD_BLOCK") != nullptr;
-    m->l2_prefetch = getenv("HQ_L2_PREFETCH") ? atoi(getenv("HQ_L2_PREFETCH")) : 0;
-    m->pf_frac = getenv("HQ_PF_FRAC") ? atoi(getenv("HQ_PF_FRAC")) : 100;
-    if (m->use_old_block) {
-        m->use_attn_block = !(cfg->flags & HQ_FLAG_NO_MEGA) && !getenv("HQ_NO_MEGA") && mega_shape_supported(*cfg, m->n_sms);
-    } else {
-        m->use_attn_block = !(cfg->flags & HQ_FLAG_NO_MEGA) && !getenv("HQ_NO_MEGA") && attn_block_shape_supported(*cfg);
-        if (m->use_attn_block) {
-            // the clusters of one launch wait for one another's attention vector: all of them must be resident at once
-            bool co_resident = false;
-            cudaError_t e = attn_block_prepare(cfg->n_kv_heads, &co_resident);
-            if (e != cudaSuccess) { cudaGetLastError(); co_resident = false; }
-            m->use_attn_block = co_resident;
-        }
+    m->use_pdl = !(cfg->flags & HQ_FLAG_NO_PDL);
+    m->dyn_ticket = getenv("HQ_DYN") != nullptr;   // TEMP experiment switch
+    m->use_attn_block = !(cfg->flags & HQ_FLAG_KERNEL_PER_ROW) && attn_block_shape_supported(*cfg);
+    if (m->use_attn_block) {
+        // the clusters of one launch wait for one another's attention vector: all of them must be resident at once
+        // (cudaOccupancyMaxActiveClusters); otherwise batch-1 decode takes the kernel-per-row path
+        bool co_resident = false;
+        cudaError_t e = attn_block_prepare(cfg->n_kv_heads, &co_resident);
+        if (e != cudaSuccess) { cudaGetLastError(); co_resident = false; }
+        m->use_attn_block = co_resident;
     }
-    m->use_mega = ((cfg->flags & HQ_FLAG_MEGA) || getenv("HQ_MEGA")) && !(cfg->flags & HQ_FLAG_NO_MEGA) && !getenv("HQ_NO_MEGA") &&
-                  mega_shape_supported(*cfg, m->n_sms);
     {
-        cudaError_t e = cudaMemcpyAsync(m->b.mk_layers, m->layers.data(), m->layers.size() * sizeof(LayerW),
-                                        cudaMemcpyHostToDevice, m->stream);
         // tagged exchange words start with tag 0 (never a valid epoch); the epoch counter only ever grows
-        if (e == cudaSuccess) e = cudaMemsetAsync(m->b.mk_ll, 0, mega_ll_words(*cfg) * sizeof(unsigned long long), m->stream);
-        if (e == cudaSuccess) e = cudaMemsetAsync(m->b.mk_epoch, 0, sizeof(unsigned int), m->stream);
         const unsigned int one = 1u;
-        if (e == cudaSuccess) e = cudaMemsetAsync(m->b.ab_ll, 0, (size_t)cfg->n_heads * kHeadDim * sizeof(unsigned long long), m->stream);
+        cudaError_t e = cudaMemsetAsync(m->b.ab_ll, 0, (size_t)cfg->n_heads * kHeadDim * sizeof(unsigned long long), m->stream);
         if (e == cudaSuccess) e = cudaMemcpyAsync(m->b.ab_epoch, &one, sizeof(one), cudaMemcpyHostToDevice, m->stream);
         if (e == cudaSuccess) e = cudaStreamSynchronize(m->stream);
         if (e != cudaSuccess) {
             delete m;
-            return fail(HQ_ERR_CUDA, "hq_model_create: layer table upload failed: %s", cudaGetErrorString(e));
+            return fail(HQ_ERR_CUDA, "hq_model_create: exchange buffer init failed: %s", cudaGetErrorString(e));
         }
     }
 
@@ -580,7 +528,7 @@ extern "C" int32_t hq_model_create(const hq_config *cfg, const hq_weights *w, vo
             }
         cudaError_t e = cudaMemcpyAsync(m->b.rope, tab.data(), tab.size() * sizeof(float2), cudaMemcpyHostToDevice, m->stream);
         if (e == cudaSuccess) e = launch_set_state(LaunchCtx{m->stream, false, m->n_sms}, m->b.pos, 0, m->b.best,
-                                                   m->b.counter, cfg->max_batch, m->b.mk_sync);
+                                                   m->b.counter, cfg->max_batch, m->b.err);
         if (e == cudaSuccess) e = launch_zero_tokens(LaunchCtx{m->stream, false, m->n_sms}, m->b.cur_tok, cfg->max_batch);
         if (e == cudaSuccess) e = cudaStreamSynchronize(m->stream);
         if (e != cudaSuccess) {
@@ -591,19 +539,14 @@ extern "C" int32_t hq_model_create(const hq_config *cfg, const hq_weights *w, vo
 
     // A stream capture cannot start on the legacy default stream: without a real stream the decode
     // step is launched kernel by kernel.
-    if (!(cfg->flags & HQ_FLAG_NO_GRAPH) && !getenv("HQ_NO_GRAPH") && m->stream != nullptr) {
+    if (!(cfg->flags & HQ_FLAG_NO_GRAPH) && m->stream != nullptr) {
         // One eager step first so that every kernel is loaded before the capture (lazy module
         // loading is not allowed while capturing); its side effects are reset right after.
         cudaError_t e = enqueue_step(m, m->b.cur_tok, true, nullptr);
         if (e == cudaSuccess) e = launch_set_state(LaunchCtx{m->stream, false, m->n_sms}, m->b.pos, 0, m->b.best,
-                                                   m->b.counter, cfg->max_batch, m->b.mk_sync);
+                                                   m->b.counter, cfg->max_batch, m->b.err);
         if (e == cudaSuccess) e = cudaStreamSynchronize(m->stream);
         if (e == cudaSuccess) e = capture_step_graph(m);
-        if (e != cudaSuccess && m->use_mega && m->mega_coop) {  // retry as a plain launch (grid = #SMs is co-resident)
-            cudaGetLastError();
-            m->mega_coop = false;
-            e = capture_step_graph(m);
-        }
         if (e != cudaSuccess && m->use_pdl) {  // retry without programmatic edges
             cudaGetLastError();
             m->use_pdl = false;
@@ -629,7 +572,11 @@ extern "C" void hq_model_destroy(hq_model *m) {
 // ---- state --------------------------------------------------------------------------------------------
 extern "C" int32_t hq_sync(hq_model *m) {
     if (!m) return fail(HQ_ERR_INVALID_ARG, "hq_sync: model is NULL");
-    HQ_CUDA(cudaStreamSynchronize(m->stream));
+    HQ_ON_DEVICE(m);
+    cudaError_t e = cudaStreamSynchronize(m->stream);
+    if (e != cudaSuccess)
+        return fail(HQ_ERR_CUDA, "hq_sync: %s (a trapped attention-block launch means a cluster arrival or a tagged word never came: "
+                    "the device was not exclusive to this model, see hq_model_create)", cudaGetErrorString(e));
     return HQ_OK;
 }
 
@@ -641,8 +588,9 @@ extern "C" int32_t hq_seq_len(const hq_model *m, int32_t *out) {
 
 extern "C" int32_t hq_kv_reset(hq_model *m) {
     if (!m) return fail(HQ_ERR_INVALID_ARG, "hq_kv_reset: model is NULL");
+    HQ_ON_DEVICE(m);
     HQ_CUDA(launch_set_state(LaunchCtx{m->stream, false, m->n_sms}, m->b.pos, 0, m->b.best, m->b.counter,
-                             m->cfg.max_batch, m->b.mk_sync));
+                             m->cfg.max_batch, m->b.err));
     m->kernel_count += 1;
     m->seq_len = 0;
     m->batch = 0;
@@ -654,8 +602,7 @@ extern "C" int64_t hq_kernel_count(const hq_model *m) { return m ? m->kernel_cou
 
 extern "C" const char *hq_decode_path(const hq_model *m) {
     if (!m) return "";
-    if (m->use_mega) return "persistent";
-    if (m->use_attn_block) return m->use_old_block ? "attention-block-l2" : "attention-block-cluster";
+    if (m->use_attn_block) return "attention-block-cluster";
     return "kernel-per-row";
 }
 
@@ -663,6 +610,7 @@ extern "C" const char *hq_decode_path(const hq_model *m) {
 extern "C" int32_t hq_prefill(hq_model *m, const int32_t *tokens_host, int32_t batch, int32_t n_tokens,
                               float *logits_dev, int32_t *first_token_host) {
     if (!m || !tokens_host) return fail(HQ_ERR_INVALID_ARG, "hq_prefill: NULL argument");
+    HQ_ON_DEVICE(m);
     if (batch <= 0 || n_tokens <= 0) return fail(HQ_ERR_INVALID_ARG, "hq_prefill: batch and n_tokens must be > 0");
     const hq_config &c = m->cfg;
     if (batch > c.max_batch) return fail(HQ_ERR_CAPACITY, "hq_prefill: batch %d > max_batch %d", batch, c.max_batch);
@@ -675,7 +623,7 @@ extern "C" int32_t hq_prefill(hq_model *m, const int32_t *tokens_host, int32_t b
             return fail(HQ_ERR_INVALID_ARG, "hq_prefill: token %d at index %lld outside [0, %d)", tokens_host[i], i, c.vocab);
     const LaunchCtx lc{m->stream, m->use_pdl, m->n_sms};
     const bool capture = (c.flags & HQ_FLAG_CAPTURE_HIDDEN) != 0;
-    if (batch == 1 && (n_tokens < 8 || getenv("HQ_PREFILL_GEMV"))) {
+    if (batch == 1 && n_tokens < 8) {
         // very short appends: walk the tokens with the batch-1 decode kernels
         HQ_CUDA(cudaMemcpyAsync(m->b.prompt, tokens_host, (size_t)n_tokens * sizeof(int), cudaMemcpyHostToDevice, m->stream));
         for (int t = 0; t < n_tokens; ++t) {
@@ -718,6 +666,7 @@ extern "C" int32_t hq_prefill(hq_model *m, const int32_t *tokens_host, int32_t b
 // ---- decode ------------------------------------------------------------------------------------------
 static int32_t decode_precheck(hq_model *m, const char *who, int n_steps) {
     if (!m) return fail(HQ_ERR_INVALID_ARG, "%s: model is NULL", who);
+    HQ_ON_DEVICE(m);
     if (m->batch == 0) return fail(HQ_ERR_STATE, "%s: no active sequence (call hq_prefill first)", who);
     if ((long long)m->seq_len + n_steps > m->cfg.max_seq)
         return fail(HQ_ERR_CAPACITY, "%s: seq_len %d + %d > max_seq %d", who, m->seq_len, n_steps, m->cfg.max_seq);
@@ -728,7 +677,7 @@ static int32_t launch_one_step(hq_model *m) {
     if (m->batch > 1) {
         // batched decode (B1/B2): tensor-core GEMMs, weights read once per step for all sequences.
         // The first step of a batch size runs eagerly (loads every kernel), the second captures a graph.
-        const bool want_graph = !(m->cfg.flags & HQ_FLAG_NO_GRAPH) && !getenv("HQ_NO_GRAPH") && m->stream != nullptr;
+        const bool want_graph = !(m->cfg.flags & HQ_FLAG_NO_GRAPH) && m->stream != nullptr;
         if (want_graph && m->batch_graph_b != m->batch && m->batch_eager_b == m->batch) {
             cudaError_t e = capture_batch_graph(m, m->batch);
             if (e != cudaSuccess) { cudaGetLastError(); m->batch_eager_b = -1; }   // stay eager
@@ -781,16 +730,9 @@ extern "C" int32_t hq_decode_run(hq_model *m, int32_t n_steps, int32_t *tokens_o
     if (rc != HQ_OK) return rc;
     if (!m->have_token) return fail(HQ_ERR_STATE, "hq_decode_run: no device-resident token to feed");
     const int first = m->seq_len + 1;
-    if (m->use_mega && m->batch == 1) {
-        // the persistent kernel loops over the tokens itself: no launch gap, the weight stream never stops
-        HQ_CUDA(launch_mega(LaunchCtx{m->stream, false, m->n_sms}, mega_params(m, m->b.cur_tok, n_steps, true), m->mega_coop));
-        m->kernel_count += 1;
-        m->seq_len += n_steps;
-    } else {
-        for (int i = 0; i < n_steps; ++i) {
-            rc = launch_one_step(m);
-            if (rc != HQ_OK) return rc;
-        }
+    for (int i = 0; i < n_steps; ++i) {
+        rc = launch_one_step(m);
+        if (rc != HQ_OK) return rc;
     }
     if (tokens_out_host) {
         HQ_CUDA(cudaMemcpyAsync(tokens_out_host, m->b.tok_hist + (size_t)first * m->batch,
@@ -802,6 +744,7 @@ extern "C" int32_t hq_decode_run(hq_model *m, int32_t n_steps, int32_t *tokens_o
 
 extern "C" int32_t hq_decode_logits(hq_model *m, float *logits_dev) {
     if (!m || !logits_dev) return fail(HQ_ERR_INVALID_ARG, "hq_decode_logits: NULL argument");
+    HQ_ON_DEVICE(m);
     if (m->batch == 0) return fail(HQ_ERR_STATE, "hq_decode_logits: nothing has been evaluated yet");
     HQ_CUDA(cudaMemcpyAsync(logits_dev, m->b.logits, (size_t)m->batch * m->cfg.vocab * sizeof(float),
                             cudaMemcpyDeviceToDevice, m->stream));
@@ -810,6 +753,7 @@ extern "C" int32_t hq_decode_logits(hq_model *m, float *logits_dev) {
 
 extern "C" int32_t hq_get_hidden(hq_model *m, int32_t layer, float *hidden_dev) {
     if (!m || !hidden_dev) return fail(HQ_ERR_INVALID_ARG, "hq_get_hidden: NULL argument");
+    HQ_ON_DEVICE(m);
     if (!(m->cfg.flags & HQ_FLAG_CAPTURE_HIDDEN)) return fail(HQ_ERR_STATE, "hq_get_hidden: model created without HQ_FLAG_CAPTURE_HIDDEN");
     if (layer < 0 || layer >= m->cfg.n_layers) return fail(HQ_ERR_INVALID_ARG, "hq_get_hidden: layer %d outside [0, %d)", layer, m->cfg.n_layers);
     if (m->batch == 0) return fail(HQ_ERR_STATE, "hq_get_hidden: nothing has been evaluated yet");
@@ -821,6 +765,7 @@ extern "C" int32_t hq_get_hidden(hq_model *m, int32_t layer, float *hidden_dev) 
 // ---- measurement hook ---------------------------------------------------------------------------------
 extern "C" int32_t hq_bench_kernel(hq_model *m, int32_t which, int32_t reps, int64_t *bytes_per_launch) {
     if (!m || reps <= 0) return fail(HQ_ERR_INVALID_ARG, "hq_bench_kernel: bad argument");
+    HQ_ON_DEVICE(m);
     if (m->batch == 0 || m->seq_len == 0) return fail(HQ_ERR_STATE, "hq_bench_kernel: needs a prefilled cache");
     if (m->seq_len >= m->cfg.max_seq) return fail(HQ_ERR_CAPACITY, "hq_bench_kernel: cache is full");
     const hq_config &c = m->cfg;
@@ -835,19 +780,15 @@ extern "C" int32_t hq_bench_kernel(hq_model *m, int32_t which, int32_t reps, int
         GemvParams p = {};
         switch (which) {
             case 0:
-                p.w0 = w.w_gate; p.w1 = w.w_up; p.gain = w.ffn_norm; p.xin = b.x; p.K = c.hidden; p.n_units = c.ffn;
-                p.eps = c.rms_eps; p.out = b.act;
-                HQ_CUDA(launch_gemv(lc, GEMV_GATEUP, XIN_NORM, p));
+                HQ_CUDA(launch_sgemv(lc, sgemv_gateup(m, l)));
                 bytes = 2ll * 2 * c.ffn * c.hidden;
                 break;
-            case 1:
-                // LM head without state side effects: pos_inc = 0, token/history writes go to scratch slots
-                p.w0 = m->lm_head; p.gain = m->final_norm; p.xin = b.x; p.K = c.hidden; p.n_units = c.vocab / 2;
-                p.eps = c.rms_eps; p.out = b.logits; p.pos = b.pos; p.best = b.best; p.counter = b.counter;
-                p.cur_tok = b.cur_tok; p.tok_hist = b.tok_hist; p.pos_rw = b.pos; p.pos_inc = 0;
-                HQ_CUDA(launch_gemv(lc, GEMV_LMHEAD, XIN_NORM, p));
+            case 1: {
+                // LM head without state side effects: pos_inc = 0 (token / history writes repeat the current slot)
+                HQ_CUDA(launch_sgemv(lc, sgemv_lm_head(m, b.x, 0)));
                 bytes = 2ll * c.vocab * c.hidden;
                 break;
+            }
             case 2:
                 // QKV: rewrites the K/V row at the current position with garbage from the scratch x
                 p.w0 = w.wq; p.w1 = w.wk; p.w2 = w.wv; p.gain = w.attn_norm; p.xin = b.x; p.K = c.hidden;
@@ -864,8 +805,7 @@ extern "C" int32_t hq_bench_kernel(hq_model *m, int32_t which, int32_t reps, int
                 bytes = 2ll * c.hidden * qdim;
                 break;
             case 4:
-                p.w0 = w.w_down; p.xin = b.act; p.K = c.ffn; p.n_units = c.hidden / 2; p.out = b.x;
-                HQ_CUDA(launch_gemv(lc, GEMV_RESID, XIN_PLAIN, p));
+                HQ_CUDA(launch_sgemv(lc, sgemv_down(m, l)));
                 bytes = 2ll * c.hidden * c.ffn;
                 break;
             case 5: {
@@ -877,16 +817,8 @@ extern "C" int32_t hq_bench_kernel(hq_model *m, int32_t which, int32_t reps, int
             }
             case 6: {
                 // attention block: QKV + attention + O of layer l in one launch (rewrites the K/V row at the current position)
-                if (m->use_attn_block && !m->use_old_block) {
-                    HQ_CUDA(launch_attn_block(lc, attn_block_params(m, l)));
-                    bytes = 2ll * ((c.n_heads + 2 * c.n_kv_heads) * kHeadDim + c.hidden) * c.hidden +
-                            2ll * 2 * c.n_kv_heads * kHeadDim * (m->seq_len + 1);
-                    break;
-                }
-                if (!mega_shape_supported(c, m->n_sms)) return fail(HQ_ERR_UNSUPPORTED, "hq_bench_kernel: shape not supported by the attention block");
-                MegaParams ab = mega_params(m, b.cur_tok, 1, false);
-                ab.x_plain = b.x; ab.pi_begin = 4 * l; ab.pi_end = 4 * l + 2;
-                HQ_CUDA(launch_mega(lc, ab, false));
+                if (!m->use_attn_block) return fail(HQ_ERR_UNSUPPORTED, "hq_bench_kernel: this model does not run the attention block");
+                HQ_CUDA(launch_attn_block(lc, attn_block_params(m, l)));
                 bytes = 2ll * ((c.n_heads + 2 * c.n_kv_heads) * kHeadDim + c.hidden) * c.hidden +
                         2ll * 2 * c.n_kv_heads * kHeadDim * (m->seq_len + 1);
                 break;
@@ -897,6 +829,30 @@ extern "C" int32_t hq_bench_kernel(hq_model *m, int32_t which, int32_t reps, int
         m->kernel_count += 1;
     }
     if (bytes_per_launch) *bytes_per_launch = bytes;
+    return HQ_OK;
+}
+
+extern "C" int32_t hq_debug_read_probe(void *cuda_stream, const void *src_dev, size_t bytes, uint32_t *sum_dev) {
+    if (!src_dev || !sum_dev || bytes < 16 || ((uintptr_t)src_dev & 15) != 0)
+        return fail(HQ_ERR_INVALID_ARG, "hq_debug_read_probe: needs a 16-byte aligned buffer of >= 16 bytes and a result word");
+    int dev = 0, n_sms = 0;
+    HQ_CUDA(cudaGetDevice(&dev));
+    HQ_CUDA(cudaDeviceGetAttribute(&n_sms, cudaDevAttrMultiProcessorCount, dev));
+    HQ_CUDA(launch_read_probe((cudaStream_t)cuda_stream, src_dev, bytes, sum_dev, n_sms));
+    return HQ_OK;
+}
+
+extern "C" int32_t hq_debug_kv_row(hq_model *m, int32_t which, int32_t layer, int32_t seq, int32_t pos, void *row_dev) {
+    if (!m || !row_dev) return fail(HQ_ERR_INVALID_ARG, "hq_debug_kv_row: NULL argument");
+    HQ_ON_DEVICE(m);
+    const hq_config &c = m->cfg;
+    if ((which != 0 && which != 1) || layer < 0 || layer >= c.n_layers || seq < 0 || seq >= c.max_batch || pos < 0 || pos >= c.max_seq)
+        return fail(HQ_ERR_INVALID_ARG, "hq_debug_kv_row: index out of range");
+    const kv_t *base = (which == 0 ? m->b.kcache : m->b.vcache) +
+                       (((size_t)layer * c.max_batch + seq) * c.n_kv_heads * c.max_seq + pos) * kHeadDim;
+    // [n_kv_heads] rows of 64 elements, max_seq * 64 elements apart -> contiguous [n_kv_heads][64]
+    HQ_CUDA(cudaMemcpy2DAsync(row_dev, kHeadDim * sizeof(kv_t), base, (size_t)c.max_seq * kHeadDim * sizeof(kv_t),
+                              kHeadDim * sizeof(kv_t), c.n_kv_heads, cudaMemcpyDeviceToDevice, m->stream));
     return HQ_OK;
 }
 
@@ -923,6 +879,7 @@ extern "C" int32_t hq_debug_gemm(void *cuda_stream, int32_t mode, const void *w_
         (mode == 2 && !make_tensor_map_16b(&mw2, w2_dev, n_rows, k, 128)))
         return fail(HQ_ERR_CUDA, "hq_debug_gemm: cuTensorMapEncodeTiled failed");
     const LaunchCtx lc{(cudaStream_t)cuda_stream, false, 148};
+    HQ_CUDA(gemm_prepare());
     HQ_CUDA(launch_gemm(lc, (GemmEpilogue)mode, mw, mode == 2 ? &mw2 : nullptr, mx, n_tokens, n_rows, k, n_tokens, token_tile,
                         mode == 2 ? 1 : splits, mode == 2 ? nullptr : (float *)out_dev, mode == 2 ? (act_t *)out_dev : nullptr,
                         (size_t)n_tokens * n_rows, n_rows));

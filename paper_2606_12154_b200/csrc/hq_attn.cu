@@ -135,12 +135,6 @@ __device__ void ab_producer(const AttnBlockParams &p, const AbGeom &g, uint8_t *
     // this CTA's rows of W_o are one contiguous range: into L2 now (behind the QKV rows), so that the ring loads issued
     // later are L2 hits
     if (lane == 0 && g.q_stages >= kAbStages) bulk_prefetch_l2(p.wo + (size_t)g.o_row0 * g.qdim, (uint32_t)g.o_rows * (uint32_t)g.qdim * 2u);
-    // HBM would idle while this launch walks its latency chain: the weights of the gate/up GEMV go to L2 meanwhile
-    if (lane == 0) {
-        const int part = g.kvh * kAbCluster + g.rank, n_parts = p.n_kv_heads * kAbCluster;
-        prefetch_slice_l2(p.pf_ptr[0], p.pf_bytes[0], part, n_parts);
-        prefetch_slice_l2(p.pf_ptr[1], p.pf_bytes[1], part, n_parts);
-    }
     // everything below depends on the position / the cache rows written by earlier kernels
     pdl_wait();
     const int pos = ld_act(p.pos);

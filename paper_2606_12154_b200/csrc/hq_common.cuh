@@ -102,23 +102,6 @@ __device__ __forceinline__ void bulk_prefetch_l2(const void *gmem_src, uint32_t 
     asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(gmem_src), "r"(bytes) : "memory");
 }
 
-// Slice `part` of `n_parts` of a contiguous (immutable) global range -> L2, in pieces of <= 64 KB.  One thread.  Used to
-// pull the NEXT kernel's weights into the 126 MB L2 while this kernel is latency-bound: HBM keeps streaming, and the next
-// kernel reads L2 hits (measured: L2 -> SM ~13 TB/s chip-wide, HBM ~6.5 TB/s).
-__device__ __forceinline__ void prefetch_slice_l2(const void *base, size_t bytes, int part, int n_parts) {
-    if (!base) return;
-    size_t per = (bytes + (size_t)n_parts - 1) / (size_t)n_parts;
-    per = (per + 127) & ~(size_t)127;
-    const size_t b0 = (size_t)part * per;
-    if (b0 >= bytes) return;
-    const size_t b1 = b0 + per < bytes ? b0 + per : bytes;
-    const char *p = static_cast<const char *>(base);
-    for (size_t o = b0; o < b1; o += 65536) {
-        const size_t n = b1 - o < 65536 ? b1 - o : 65536;
-        bulk_prefetch_l2(p + o, (uint32_t)(n & ~(size_t)15));
-    }
-}
-
 // ---- loads ------------------------------------------------------------------------------------------
 // Weights: immutable, streamed once per token -> non-coherent path, do not allocate in L1.
 __device__ __forceinline__ uint4 ld_weight16(const void *p) {

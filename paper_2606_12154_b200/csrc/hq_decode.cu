@@ -44,13 +44,14 @@ __global__ void advance_kernel(int *pos, int inc) {
 }
 
 __global__ void set_state_kernel(int *pos, int pos_value, unsigned long long *best, unsigned int *counter,
-                                 int batch, unsigned int *mk_sync) {
+                                 int batch, int *err) {
     if (threadIdx.x == 0) {
         *pos = pos_value;
-        *counter = 0u;
+        counter[0] = 0u;   // last-CTA ticket of the LM head
+        counter[1] = 0u;   // dynamic group hand-out of the streaming GEMV
+        *err = 0;
     }
     if ((int)threadIdx.x < batch) best[threadIdx.x] = 0ull;
-    for (int i = threadIdx.x; i < 64; i += blockDim.x) mk_sync[i] = 0u;   // barrier, tickets, error flag
 }
 
 __global__ void zero_tokens_kernel(int *cur_tok, int batch) {
@@ -130,10 +131,6 @@ __global__ void __launch_bounds__(kGemvThreads) gemv_kernel(const __grid_constan
     }
     pdl_launch_dependents();
     pdl_wait();
-    if (tid == 0) {
-#pragma unroll
-        for (int i = 0; i < 4; ++i) prefetch_slice_l2(p.pf_ptr[i], p.pf_bytes[i], blockIdx.x, gridDim.x);
-    }
 
     // ---- input vector into registers -------------------------------------------------------------
     float xr[CH][8];
@@ -417,10 +414,10 @@ cudaError_t launch_advance(const LaunchCtx &c, int *pos, int inc) {
 }
 
 cudaError_t launch_set_state(const LaunchCtx &c, int *pos, int pos_value, unsigned long long *best,
-                             unsigned int *counter, int batch, unsigned int *mk_sync) {
+                             unsigned int *counter, int batch, int *err) {
     LaunchCtx nc = c;
     nc.pdl = false;
-    return launch_k(nc, set_state_kernel, dim3(1), dim3(32), pos, pos_value, best, counter, batch, mk_sync);
+    return launch_k(nc, set_state_kernel, dim3(1), dim3(32), pos, pos_value, best, counter, batch, err);
 }
 
 cudaError_t launch_zero_tokens(const LaunchCtx &c, int *cur_tok, int batch) {
@@ -431,20 +428,12 @@ cudaError_t launch_zero_tokens(const LaunchCtx &c, int *cur_tok, int batch) {
 
 bool gemv_shape_supported(int K) { return K > 0 && (K % 8) == 0 && K <= 8 * 4 * kGemvThreads; }
 
-static int gemv_ctas_per_sm() {
-    static int v = -1;
-    if (v < 0) {
-        const char *e = getenv("HQ_GEMV_CTAS_PER_SM");
-        v = e ? atoi(e) : 2;
-        if (v < 1 || v > 8) v = 2;
-    }
-    return v;
-}
+constexpr int kGemvCtasPerSm = 2;   // 2 x 256 threads x (2 buffers of 8 x 16 B) = 128 KB of weight loads in flight per SM
 
 template <int MODE, int XIN>
 static cudaError_t launch_gemv_mx(const LaunchCtx &c, const GemvParams &p) {
     const int kchunks = p.K >> 3;
-    const int max_ctas = c.n_sms * gemv_ctas_per_sm();
+    const int max_ctas = c.n_sms * kGemvCtasPerSm;
     if (kchunks <= kGemvThreads) {
         const int grid = min(max_ctas, (p.n_units + 3) / 4);
         return launch_k(c, gemv_kernel<1, 4, MODE, XIN>, dim3(grid), dim3(kGemvThreads), p);
@@ -456,9 +445,6 @@ static cudaError_t launch_gemv_mx(const LaunchCtx &c, const GemvParams &p) {
         return launch_k(c, gemv_kernel<4, 1, MODE, XIN>, dim3(grid), dim3(kGemvThreads), p);
     }
 }
-
-// grid of gemv_kernel<1, 4, ...> (K <= 2048) over n_units units: what launch_gemv_mx uses
-int gemv_grid_units4(int n_sms, int n_units) { return min(n_sms * gemv_ctas_per_sm(), (n_units + 3) / 4); }
 
 cudaError_t launch_gemv(const LaunchCtx &c, GemvMode mode, GemvInput xin, const GemvParams &p) {
     if (mode == GEMV_QKV && xin == XIN_NORM) return launch_gemv_mx<GEMV_QKV, XIN_NORM>(c, p);

@@ -298,12 +298,6 @@ static cudaError_t launch_mode(const LaunchCtx &c, const TensorMap &w, const Ten
     if (stages > p.k_blocks_per_split) stages = p.k_blocks_per_split < 2 ? 2 : p.k_blocks_per_split;
     p.stages = stages;
     const size_t smem = (size_t)stages * stage_bytes + 1024 + (2 * stages + 1) * 8 + 16;
-    static bool attr_done = false;
-    if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(gemm_tc_kernel<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
-        if (e != cudaSuccess) return e;
-        attr_done = true;
-    }
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(n_tiles, t_tiles, splits);
     cfg.blockDim = dim3(kGemmThreads);
@@ -362,6 +356,15 @@ cudaError_t launch_gemm_qkv(const LaunchCtx &c, const TensorMap &wq, const Tenso
     p.out_f32 = out_f32; p.x_lo_row = x_lo_row; p.ld_out = ld_out; p.atomic = splits > 1 ? 1 : 0;
     p.tiles_w1 = n1 / kBlockM; p.tiles_w2 = n2 / kBlockM;
     return launch_mode<EPI_STORE>(c, wq, wk, wv, x, p, p.n_rows / kBlockM, (T + NT - 1) / NT, splits);
+}
+
+// Shared-memory opt-in of every instantiation on the CURRENT device (the attribute is per device: hq_model_create and
+// hq_debug_gemm call this, not a process-wide once-flag).
+cudaError_t gemm_prepare() {
+    cudaError_t e = cudaFuncSetAttribute(gemm_tc_kernel<EPI_STORE>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(gemm_tc_kernel<EPI_RESID>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(gemm_tc_kernel<EPI_SWIGLU>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    return e;
 }
 
 }  // namespace hq

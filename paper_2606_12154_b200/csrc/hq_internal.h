@@ -8,7 +8,7 @@
 #include <string>
 #include <vector>
 
-#include "../../include/hq.h"
+#include "../../include/hq_debug.h"
 
 namespace hq {
 
@@ -30,13 +30,6 @@ constexpr int kHeadDim = 64;        // only head_dim the kernels implement
 constexpr int kMaxSplits = 16;      // split-KV partials per head (decode attention)
 constexpr int kMinSplitLen = 64;    // do not split contexts shorter than this per split
 constexpr int kGemvThreads = 256;
-// persistent decode kernel (hq_mega.cu)
-constexpr int kMkSliceChunks = 256;   // 16-byte chunks of one row slice (2048 bf16): what one warp keeps of x in registers
-constexpr int kMkStageBytes = 65536;  // one ring stage: 16 slices = 8 / S units of two rows
-constexpr int kMkStages = 3;          // ring depth: 192 KB of weights in flight per SM
-constexpr int kMkMaxSplits = 8;       // context splits per KV head (every CTA re-reads all split states in the O phase)
-constexpr int kMkMaxGrid = 1024;      // per-CTA argmax slots in the exchange buffer
-
 struct alignas(64) TensorMap { uint64_t opaque[16]; };   // mirrors CUtensorMap (driver type, 128 bytes)
 
 struct LayerW {
@@ -53,6 +46,7 @@ struct Buffers {
     int *tok_hist = nullptr;                    // [Tmax+1][B] emitted tokens, index = pos at emission
     unsigned long long *best = nullptr;         // [B] packed argmax
     unsigned int *counter = nullptr;            // last-CTA ticket
+    unsigned int *ticket = nullptr;             // streaming GEMV: dynamic group hand-out counter (zero between launches)
     float *x = nullptr;                         // [B][d] residual stream
     float *q = nullptr;                         // [B][H*64]
     float *part_o = nullptr;                    // [B][H][kMaxSplits][64]
@@ -72,11 +66,7 @@ struct Buffers {
     act_t *ao = nullptr;                        // [2][pf_rows][H*64] attention output (GEMM operand, hi/lo)
     act_t *actb = nullptr;                      // [2][pf_rows][F] SwiGLU output (GEMM operand, hi/lo)
     act_t *hn_last = nullptr;                   // [2][32][d] normalised last rows (LM-head operand, hi/lo)
-    // persistent decode kernel (batch 1)
-    struct LayerW *mk_layers = nullptr;         // [L] device copy of the per-layer weight pointers
-    unsigned long long *mk_ll = nullptr;        // tagged-word exchange buffers (mega_ll_words() words, zeroed at create)
-    unsigned int *mk_epoch = nullptr;           // steps run so far by the persistent kernel (never reset: tags only grow)
-    unsigned int *mk_sync = nullptr;            // [3] error flag of the persistent kernel
+    int *err = nullptr;                         // device error flag (a lost cluster arrival / tagged word traps instead of hanging)
     unsigned long long *ab_ll = nullptr;        // attention block: tagged words of the attention vector [H * 64] (zeroed at create)
     unsigned int *ab_epoch = nullptr;           // attention block: tag of the next launch (starts at 1, never reset)
 };
@@ -89,6 +79,7 @@ struct hq_model_impl {
     std::vector<LayerW> layers;
     const bf16 *emb = nullptr, *final_norm = nullptr, *lm_head = nullptr;
     cudaStream_t stream = nullptr;
+    int device = 0;                             // CUDA device the model was created on (made current by every entry point)
     Buffers b;
     int n_sms = 148;
     int batch = 0;      // active batch (0 = none)
@@ -98,6 +89,7 @@ struct hq_model_impl {
     long long kernel_count = 0;
     int kernels_per_step = 0;
     bool use_pdl = true;
+    bool dyn_ticket = false;
     // tensor-core path
     int pf_rows = 0;                            // row capacity of one pass
     std::vector<LayerMaps> maps;
@@ -106,12 +98,6 @@ struct hq_model_impl {
     cudaGraphExec_t batch_graph = nullptr;      // batched decode step (captured for batch_graph_b)
     int batch_graph_b = 0, batch_graph_kernels = 0, batch_eager_b = 0;
     bool use_attn_block = false;                // per-step path: QKV + attention + O of a layer in one cluster launch (hq_attn.cu)
-    bool use_old_block = false;                 // round-1 attention block (hq_mega.cu), A/B only
-    int l2_prefetch = 0;                        // bit 0: attention block -> gate/up weights, 1: gate/up -> down, 2: down -> next layer's attention weights
-    int pf_frac = 100;
-    bool use_mega = false;                      // batch-1 decode runs in the persistent kernel
-    bool mega_coop = true;                      // launched with the cooperative attribute
-    int mega_inflight = 2;                      // bulk-copy stages in flight per SM during the layers (HQ_MEGA_INFLIGHT overrides)
     unsigned long long *trace = nullptr;        // hq_debug_trace: device buffer [n_sms][trace_cap] or NULL
     int trace_cap = 0;
 };
@@ -141,11 +127,33 @@ struct GemvParams {
     int *cur_tok, *tok_hist;
     int *pos_rw;
     int pos_inc;
-    // weights of the kernel(s) that follow, pulled into L2 by this launch after its dependency wait (NULL / 0 = none)
-    const void *pf_ptr[4];
-    size_t pf_bytes[4];
 };
 
+// ---- streaming GEMV (hq_stream.cu): gate/up + SwiGLU, down + residual, LM head + argmax of batch-1 decode -------------
+enum SgemvMode { SGEMV_GATEUP = 0, SGEMV_RESID = 1, SGEMV_LMHEAD = 2 };
+enum SgemvInput { SGEMV_XIN_NORM = 0, SGEMV_XIN_PLANES = 1 };
+struct SgemvParams {
+    const bf16 *w0, *w1;     // GATEUP: gate, up [n_rows][K] each; RESID / LMHEAD: w0 [n_rows][K]
+    const bf16 *gain;        // XIN_NORM: RMSNorm gains [K]
+    const float *xin;        // XIN_NORM: fp32 residual stream [K]; XIN_PLANES: bf16 hi plane [K] then lo plane [K]
+    int K, n_rows;
+    int mode, xin_mode;
+    float eps;
+    float *out;              // RESID: x [n_rows], += ; LMHEAD: logits [n_rows]
+    bf16 *out_planes;        // GATEUP: SwiGLU vector as bf16 hi plane [n_rows] then lo plane [n_rows]
+    // LMHEAD: fused argmax + step bookkeeping
+    const int *pos;
+    unsigned long long *best;
+    unsigned int *counter;
+    int *cur_tok, *tok_hist, *pos_rw;
+    int pos_inc;
+    unsigned int *ticket;    // dynamic group hand-out counter (zero between launches), NULL = static partition only
+    unsigned long long *trace;   // NULL or step timeline [slots][4] (hq_debug_trace)
+    int trace_slot;
+    // filled by launch_sgemv
+    int kc, stages, static_groups;
+    int row_pad, dbg;
+};
 struct AttnDecodeParams {
     const float *q;          // [H*64]
     const kv_t *kc, *vc;     // layer base
@@ -171,48 +179,9 @@ struct LaunchCtx {
     int n_sms;
 };
 
-// ---- persistent decode kernel (hq_mega.cu) ------------------------------------------------------------
-struct MegaParams {
-    int n_layers, hidden, n_heads, n_kv_heads, ffn, vocab, max_seq;
-    float eps;
-    const bf16 *emb, *final_norm, *lm_head;
-    const LayerW *layers;        // device array [n_layers]
-    const float2 *rope;
-    kv_t *kc, *vc;               // sequence 0 of layer 0
-    size_t layer_kv;             // elements per layer
-    // device-resident step state
-    int *pos, *cur_tok, *tok_hist;
-    const int *tok_src;          // token fed at the first step (later steps feed the token the kernel just chose)
-    unsigned int *epoch;         // steps run by earlier launches: base of the tags of this launch, advanced at exit
-    int *err;
-    unsigned long long *trace;   // NULL or [grid][trace_cap] global-timer stamps (hq_debug_trace)
-    int trace_cap;
-    // cross-CTA exchange buffers of tagged words (fp32 value | epoch tag), see hq_mega.cu
-    unsigned long long *ll_x;        // [2][hidden]: residual after the O projection / after the down projection
-    unsigned long long *ll_qkv;      // [(H+2Hkv)*64] RoPE'd q, RoPE'd k, v of the current token
-    unsigned long long *ll_act;      // [ffn] SwiGLU output
-    unsigned long long *ll_part_o;   // [H][kMkMaxSplits][64] split-KV partial outputs (unnormalised)
-    unsigned long long *ll_part_ml;  // [H][kMkMaxSplits][2] (m, l)
-    unsigned long long *ll_attn;     // [H*64] merged, normalised attention output
-    unsigned long long *ll_best;     // [grid][2] per-CTA argmax (ordered logit key, index)
-    float *logits;
-    float *hidden_out;           // NULL or [n_layers][hidden_stride] residual after every layer
-    size_t hidden_stride;
-    int n_steps, with_head;
-    int att_splits, att_ctas;    // context splits per KV head, and the n_kv_heads * att_splits CTAs (the last ones) that only do attention
-    // attention-block launch (per-step path): x_plain != NULL runs only the phases [pi_begin, pi_end) of one step (QKV,
-    // attention, O of one layer), residual stream in and out as the plain fp32 vector x_plain
-    float *x_plain;
-    int pi_begin, pi_end;
-    int pf_units;                // ... units (row pairs) per gate/up CTA to prefetch
-    int pf_grid;                 // attention block: grid of the gate/up GEMV that follows (its first batches are L2-prefetched), 0 = off
-    int inflight_stages;         // producer: at most this many ring stages issued and not yet landed (1..kMkStages)
-};
-size_t mega_smem_bytes();
-size_t mega_ll_words(const hq_config &c);   // 64-bit words of exchange buffers
-bool mega_shape_supported(const hq_config &c, int n_sms);
-int mega_att_splits(const hq_config &c, int n_sms, int max_ctx);
-cudaError_t launch_mega(const LaunchCtx &c, const MegaParams &p, bool cooperative);
+bool sgemv_shape_supported(int K);
+cudaError_t sgemv_prepare();
+cudaError_t launch_sgemv(const LaunchCtx &c, SgemvParams p);
 
 // ---- attention block: A2-A6 of a layer in one cluster launch (hq_attn.cu) -----------------------------------
 constexpr int kAbCluster = 8;        // CTAs per cluster = per KV head (portable cluster size)
@@ -229,8 +198,6 @@ struct AttnBlockParams {
     float eps;
     unsigned long long *trace;       // NULL or [grid][trace_cap] global-timer stamps (hq_debug_trace)
     int trace_cap;
-    const void *pf_ptr[2];           // weights of the gate/up GEMV that follows, pulled into L2 meanwhile (NULL = none)
-    size_t pf_bytes[2];
 };
 size_t attn_block_smem_bytes();
 bool attn_block_shape_supported(const hq_config &c);
@@ -250,6 +217,7 @@ struct GemmParams {
     int tiles_w1, tiles_w2;   // EPI_STORE over three stacked weight matrices: 128-row tiles of the first and second (0 = one matrix)
 };
 bool make_tensor_map_16b(TensorMap *out, const void *base, uint64_t rows, uint64_t cols, uint32_t box_rows);
+cudaError_t gemm_prepare();   // shared-memory opt-in on the current device
 cudaError_t launch_gemm(const LaunchCtx &c, GemmEpilogue mode, const TensorMap &w, const TensorMap *w2,
                         const TensorMap &x, int x_lo_row, int n_rows, int K, int T, int NT, int splits, float *out_f32,
                         act_t *out_act, size_t out_lo_offset, int ld_out);
@@ -272,15 +240,17 @@ cudaError_t launch_attn_combine(const LaunchCtx &c, const float *part_o, const f
 cudaError_t launch_argmax_rows(const LaunchCtx &c, const float *logits, int vocab, int batch, int *cur_tok,
                                int *tok_hist, int *pos, int pos_inc, unsigned int *counter, unsigned long long *best_rows);
 
+// ---- read-only streaming probe (hq_probe.cu) --------------------------------------------------------
+cudaError_t launch_read_probe(cudaStream_t stream, const void *src, size_t bytes, unsigned int *out, int n_sms);
+
 // ---- launchers (hq_decode.cu) ------------------------------------------------------------------------
 cudaError_t launch_embed(const LaunchCtx &c, const bf16 *emb, const int *tok, float *x, int hidden, int batch);
 cudaError_t launch_gemv(const LaunchCtx &c, GemvMode mode, GemvInput xin, const GemvParams &p);
 cudaError_t launch_attn_decode(const LaunchCtx &c, const AttnDecodeParams &p, int batch);
 cudaError_t launch_advance(const LaunchCtx &c, int *pos, int inc);
 cudaError_t launch_set_state(const LaunchCtx &c, int *pos, int pos_value, unsigned long long *best,
-                             unsigned int *counter, int batch, unsigned int *mk_sync);
+                             unsigned int *counter, int batch, int *err);
 cudaError_t launch_zero_tokens(const LaunchCtx &c, int *cur_tok, int batch);
 bool gemv_shape_supported(int K);
-int gemv_grid_units4(int n_sms, int n_units);
 
 }  // namespace hq

@@ -21,9 +21,27 @@ def hq():
 
 
 def header_functions():
+    names = set()
+    for h in ("hq.h", "hq_debug.h"):
+        src = open(os.path.join(ROOT, "include", h)).read()
+        src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+        names |= set(re.findall(r"\b(hq_[a-z_0-9]+)\s*\(", src))
+    return sorted(names)
+
+
+def test_library_reads_no_environment_variable():
+    """Every switch is an hq_config flag decided at hq_model_create; nothing below it consults the environment."""
+    csrc = os.path.join(ROOT, "paper_2606_12154_b200", "csrc")
+    for f in sorted(os.listdir(csrc)):
+        assert "getenv" not in open(os.path.join(csrc, f)).read(), f
+
+
+def test_every_product_call_cites_its_passage():
+    """include/hq.h: the comment in front of every exported call names the passage that defines it."""
     src = open(os.path.join(ROOT, "include", "hq.h")).read()
-    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-    return sorted(set(re.findall(r"\b(hq_[a-z_0-9]+)\s*\(", src)))
+    for m in re.finditer(r"/\*((?:(?!\*/).)*)\*/\s*(?:const\s+char\s*\*|int32_t|int64_t|size_t|void)\s*(hq_[a-z_0-9]+)\s*\(", src, flags=re.S):
+        comment, name = m.group(1), m.group(2)
+        assert re.search(r"PAPER\.md:L\d+|north_star|error convention|Counterpart of", comment), name
 
 
 def test_header_and_binding_declare_the_same_symbols(hq):
