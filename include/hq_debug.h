@@ -46,6 +46,14 @@ int32_t hq_debug_read_probe(void *cuda_stream, const void *src_dev, size_t bytes
  * Asynchronous device-to-device copy on the model's stream. */
 int32_t hq_debug_kv_row(hq_model *m, int32_t which, int32_t layer, int32_t seq, int32_t pos, void *row_dev);
 
+/* Diagnostics: timeline of one batch-1 decode step.  trace_dev: DEVICE uint64 [n_slots][4] with n_slots >= 2 + 3 *
+ * n_layers, or NULL to switch off.  While set, every directly launched decode kernel (HQ_FLAG_NO_GRAPH; a captured graph
+ * keeps the setting it was captured with) updates its slot — 1 + 3 l attention block, 2 + 3 l gate/up, 3 + 3 l down of
+ * layer l, 1 + 3 n_layers the LM head — with global-timer stamps (ns): [0] min over CTAs of the CTA start, [1] min of the
+ * end of the dependency wait, [2] max of the CTA end, [3] max of the CTA start.  The caller initialises [0], [1] to
+ * UINT64_MAX and [2], [3] to 0 before the step.  The buffer is BORROWED until tracing is switched off. */
+int32_t hq_debug_step_trace(hq_model *m, uint64_t *trace_dev, int32_t n_slots);
+
 /* Diagnostics: timeline of the attention block.  trace_dev: DEVICE uint64 [n_ctas][cap] (n_ctas = 8 * n_kv_heads), or
  * NULL to switch tracing off.  While set, thread 0 of every CTA of an attention-block launch stores the GPU global timer
  * (ns) at fixed points of the launch (see ab_trace in csrc/hq_attn.cu), restarting at index 0 each launch; stamps beyond

@@ -26,7 +26,7 @@ _CODE_NAMES = {-1: "HQ_ERR_INVALID_ARG", -2: "HQ_ERR_CAPACITY", -3: "HQ_ERR_STAT
 DECLARED_SYMBOLS = (
     "hq_workspace_bytes", "hq_model_create", "hq_model_destroy", "hq_prefill", "hq_decode_step",
     "hq_decode_run", "hq_decode_logits", "hq_get_hidden", "hq_sync", "hq_seq_len", "hq_kv_reset",
-    "hq_kernel_count", "hq_decode_path", "hq_bench_kernel", "hq_debug_gemm", "hq_debug_kv_row", "hq_debug_read_probe", "hq_debug_trace", "hq_last_error",
+    "hq_kernel_count", "hq_decode_path", "hq_bench_kernel", "hq_debug_gemm", "hq_debug_kv_row", "hq_debug_read_probe", "hq_debug_step_trace", "hq_debug_trace", "hq_last_error",
     "hq_version",
 )
 
@@ -103,6 +103,8 @@ def load_library(path: Optional[str] = None):
     l.hq_debug_read_probe.argtypes = [vp, vp, ctypes.c_size_t, vp]
     l.hq_debug_kv_row.restype = i32
     l.hq_debug_kv_row.argtypes = [vp, i32, i32, i32, i32, vp]
+    l.hq_debug_step_trace.restype = i32
+    l.hq_debug_step_trace.argtypes = [vp, vp, i32]
     l.hq_debug_trace.restype = i32
     l.hq_debug_trace.argtypes = [vp, vp, i32]
     l.hq_last_error.restype = ctypes.c_char_p
@@ -276,6 +278,19 @@ class Model:
         t = self._torch.empty(self.cfg.n_kv_heads * 64, dtype=self._torch.float16, device=self.device)
         _check(self._lib.hq_debug_kv_row(self._h, 0 if which == "k" else 1, layer, seq, pos, t.data_ptr()))
         self.sync()
+        return t
+
+    def step_trace(self, on: bool = True):
+        """Step timeline (hq_debug_step_trace): returns the int64 [slots][4] device tensor, initialised, or None (off)."""
+        if not on:
+            _check(self._lib.hq_debug_step_trace(self._h, None, 0))
+            self._step_trace = None
+            return None
+        slots = 2 + 3 * self.n_layers
+        t = self._torch.zeros((slots, 4), dtype=self._torch.int64, device=self.device)
+        t[:, :2] = (1 << 63) - 1      # atomicMin targets (unsigned compare: below every real stamp's complement)
+        self._step_trace = t
+        _check(self._lib.hq_debug_step_trace(self._h, t.data_ptr(), slots))
         return t
 
     def debug_trace(self, cap: int = 0):

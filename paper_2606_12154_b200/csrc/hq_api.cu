@@ -97,8 +97,7 @@ static size_t carve(const hq_config *c, char *base, Buffers *b) {
     o.cur_tok = (int *)take(B * sizeof(int));
     o.tok_hist = (int *)take((T + 1) * B * sizeof(int));
     o.best = (unsigned long long *)take(B * sizeof(unsigned long long));
-    o.counter = (unsigned int *)take(2 * sizeof(unsigned int));
-    o.ticket = base ? o.counter + 1 : nullptr;
+    o.counter = (unsigned int *)take(sizeof(unsigned int));
     o.x = (float *)take(B * d * sizeof(float));
     o.q = (float *)take(B * H * kHeadDim * sizeof(float));
     o.part_o = (float *)take(B * H * kMaxSplits * kHeadDim * sizeof(float));
@@ -147,6 +146,7 @@ static AttnBlockParams attn_block_params(const hq_model *m, int l) {
     a.ll_attn = b.ab_ll; a.epoch = b.ab_epoch; a.err = b.err;
     a.hidden = c.hidden; a.n_heads = c.n_heads; a.n_kv_heads = c.n_kv_heads; a.max_seq = c.max_seq; a.eps = c.rms_eps;
     a.trace = m->trace; a.trace_cap = m->trace_cap;
+    a.step_trace = m->step_trace; a.step_slot = 1 + 3 * l;
     return a;
 }
 
@@ -156,14 +156,16 @@ static SgemvParams sgemv_gateup(const hq_model *m, int l) {
     SgemvParams p = {};
     p.w0 = w.w_gate; p.w1 = w.w_up; p.gain = w.ffn_norm; p.xin = m->b.x; p.K = c.hidden; p.n_rows = c.ffn;
     p.mode = SGEMV_GATEUP; p.xin_mode = SGEMV_XIN_NORM; p.eps = c.rms_eps;
-    p.out_planes = reinterpret_cast<bf16 *>(m->b.act); p.ticket = m->dyn_ticket ? m->b.ticket : nullptr;
+    p.trace = m->step_trace; p.trace_slot = 2 + 3 * l;
+    p.out_planes = reinterpret_cast<bf16 *>(m->b.act);
     return p;
 }
 static SgemvParams sgemv_down(const hq_model *m, int l) {
     const hq_config &c = m->cfg;
     SgemvParams p = {};
     p.w0 = m->layers[l].w_down; p.xin = m->b.act; p.K = c.ffn; p.n_rows = c.hidden;
-    p.mode = SGEMV_RESID; p.xin_mode = SGEMV_XIN_PLANES; p.out = m->b.x; p.ticket = m->dyn_ticket ? m->b.ticket : nullptr;
+    p.trace = m->step_trace; p.trace_slot = 3 + 3 * l;
+    p.mode = SGEMV_RESID; p.xin_mode = SGEMV_XIN_PLANES; p.out = m->b.x;
     return p;
 }
 // final norm + LM head + argmax over the residual row x; the position advances by pos_inc
@@ -174,7 +176,8 @@ static SgemvParams sgemv_lm_head(const hq_model *m, const float *x, int pos_inc)
     p.w0 = m->lm_head; p.gain = m->final_norm; p.xin = x; p.K = c.hidden; p.n_rows = c.vocab;
     p.mode = SGEMV_LMHEAD; p.xin_mode = SGEMV_XIN_NORM; p.eps = c.rms_eps; p.out = b.logits;
     p.pos = b.pos; p.best = b.best; p.counter = b.counter; p.cur_tok = b.cur_tok; p.tok_hist = b.tok_hist;
-    p.pos_rw = b.pos; p.pos_inc = pos_inc; p.ticket = m->dyn_ticket ? b.ticket : nullptr;
+    p.trace = m->step_trace; p.trace_slot = 1 + 3 * c.n_layers;
+    p.pos_rw = b.pos; p.pos_inc = pos_inc;
     return p;
 }
 
@@ -496,7 +499,6 @@ extern "C" int32_t hq_model_create(const hq_config *cfg, const hq_weights *w, vo
         return fail(HQ_ERR_CUDA, "hq_model_create: cuTensorMapEncodeTiled failed (driver entry point or bad alignment)");
     }
     m->use_pdl = !(cfg->flags & HQ_FLAG_NO_PDL);
-    m->dyn_ticket = getenv("HQ_DYN") != nullptr;   // TEMP experiment switch
     m->use_attn_block = !(cfg->flags & HQ_FLAG_KERNEL_PER_ROW) && attn_block_shape_supported(*cfg);
     if (m->use_attn_block) {
         // the clusters of one launch wait for one another's attention vector: all of them must be resident at once
@@ -853,6 +855,15 @@ extern "C" int32_t hq_debug_kv_row(hq_model *m, int32_t which, int32_t layer, in
     // [n_kv_heads] rows of 64 elements, max_seq * 64 elements apart -> contiguous [n_kv_heads][64]
     HQ_CUDA(cudaMemcpy2DAsync(row_dev, kHeadDim * sizeof(kv_t), base, (size_t)c.max_seq * kHeadDim * sizeof(kv_t),
                               kHeadDim * sizeof(kv_t), c.n_kv_heads, cudaMemcpyDeviceToDevice, m->stream));
+    return HQ_OK;
+}
+
+extern "C" int32_t hq_debug_step_trace(hq_model *m, uint64_t *trace_dev, int32_t n_slots) {
+    if (!m) return fail(HQ_ERR_INVALID_ARG, "hq_debug_step_trace: model is NULL");
+    if (trace_dev && n_slots < 2 + 3 * m->cfg.n_layers)
+        return fail(HQ_ERR_INVALID_ARG, "hq_debug_step_trace: needs %d slots", 2 + 3 * m->cfg.n_layers);
+    m->step_trace = (unsigned long long *)trace_dev;
+    m->step_trace_slots = trace_dev ? n_slots : 0;
     return HQ_OK;
 }
 

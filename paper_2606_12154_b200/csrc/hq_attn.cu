@@ -481,6 +481,7 @@ __global__ void __launch_bounds__(kAbThreads, 1) attn_block_kernel(const __grid_
     extern __shared__ __align__(128) uint8_t ab_smem[];
     int ti = 0;
     ab_trace<TRACE>(p, ti);   // CTA started
+    if (threadIdx.x == 0) { step_stamp(p.step_trace, p.step_slot, 0); step_stamp(p.step_trace, p.step_slot, 3); }
     uint8_t *ring = ab_smem;
     AbShared &sh = *reinterpret_cast<AbShared *>(ab_smem + (size_t)kAbStages * kAbStageBytes);
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -516,6 +517,7 @@ __global__ void __launch_bounds__(kAbThreads, 1) attn_block_kernel(const __grid_
     pdl_launch_dependents();
     pdl_wait();
     ab_trace<TRACE>(p, ti);   // dependency wait over
+    if (tid == 0) step_stamp(p.step_trace, p.step_slot, 1);
     const int pos = ld_act(p.pos);
     const uint32_t tag = *reinterpret_cast<volatile unsigned int *>(p.epoch);
     float v[8];
@@ -629,6 +631,7 @@ __global__ void __launch_bounds__(kAbThreads, 1) attn_block_kernel(const __grid_
     // Every word polled above was published after its writer had received everything other CTAs push into its shared
     // memory, and every CTA read the epoch before it published: no CTA needs this one's shared memory or the old epoch.
     if (g.kvh == 0 && g.rank == 0 && tid == 0) *p.epoch = tag + 1u == 0u ? 1u : tag + 1u;
+    if (tid == 0) step_stamp(p.step_trace, p.step_slot, 2);
 }
 
 // ---- host side ---------------------------------------------------------------------------------------------------

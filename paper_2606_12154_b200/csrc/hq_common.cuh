@@ -102,6 +102,17 @@ __device__ __forceinline__ void bulk_prefetch_l2(const void *gmem_src, uint32_t 
     asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(gmem_src), "r"(bytes) : "memory");
 }
 
+// ---- step timeline (hq_debug_step_trace): per launch [0] earliest CTA start, [1] earliest end of the dependency wait,
+// [2] latest CTA end, [3] latest CTA start (global timer, ns).  One thread per CTA stamps; NULL = off.
+__device__ __forceinline__ void step_stamp(unsigned long long *trace, int slot, int which) {
+    if (trace) {
+        unsigned long long t;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+        if (which < 2) atomicMin(trace + 4 * slot + which, t);
+        else atomicMax(trace + 4 * slot + which, t);
+    }
+}
+
 // ---- loads ------------------------------------------------------------------------------------------
 // Weights: immutable, streamed once per token -> non-coherent path, do not allocate in L1.
 __device__ __forceinline__ uint4 ld_weight16(const void *p) {

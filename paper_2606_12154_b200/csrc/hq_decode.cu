@@ -47,8 +47,7 @@ __global__ void set_state_kernel(int *pos, int pos_value, unsigned long long *be
                                  int batch, int *err) {
     if (threadIdx.x == 0) {
         *pos = pos_value;
-        counter[0] = 0u;   // last-CTA ticket of the LM head
-        counter[1] = 0u;   // dynamic group hand-out of the streaming GEMV
+        *counter = 0u;     // last-CTA ticket of the LM head
         *err = 0;
     }
     if ((int)threadIdx.x < batch) best[threadIdx.x] = 0ull;

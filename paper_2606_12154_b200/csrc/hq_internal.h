@@ -46,7 +46,6 @@ struct Buffers {
     int *tok_hist = nullptr;                    // [Tmax+1][B] emitted tokens, index = pos at emission
     unsigned long long *best = nullptr;         // [B] packed argmax
     unsigned int *counter = nullptr;            // last-CTA ticket
-    unsigned int *ticket = nullptr;             // streaming GEMV: dynamic group hand-out counter (zero between launches)
     float *x = nullptr;                         // [B][d] residual stream
     float *q = nullptr;                         // [B][H*64]
     float *part_o = nullptr;                    // [B][H][kMaxSplits][64]
@@ -89,7 +88,6 @@ struct hq_model_impl {
     long long kernel_count = 0;
     int kernels_per_step = 0;
     bool use_pdl = true;
-    bool dyn_ticket = false;
     // tensor-core path
     int pf_rows = 0;                            // row capacity of one pass
     std::vector<LayerMaps> maps;
@@ -99,6 +97,8 @@ struct hq_model_impl {
     int batch_graph_b = 0, batch_graph_kernels = 0, batch_eager_b = 0;
     bool use_attn_block = false;                // per-step path: QKV + attention + O of a layer in one cluster launch (hq_attn.cu)
     unsigned long long *trace = nullptr;        // hq_debug_trace: device buffer [n_sms][trace_cap] or NULL
+    unsigned long long *step_trace = nullptr;   // hq_debug_step_trace: device buffer [slots][4] or NULL
+    int step_trace_slots = 0;
     int trace_cap = 0;
 };
 
@@ -147,12 +147,8 @@ struct SgemvParams {
     unsigned int *counter;
     int *cur_tok, *tok_hist, *pos_rw;
     int pos_inc;
-    unsigned int *ticket;    // dynamic group hand-out counter (zero between launches), NULL = static partition only
-    unsigned long long *trace;   // NULL or step timeline [slots][4] (hq_debug_trace)
+    unsigned long long *trace;   // NULL or step timeline [slots][4] (hq_debug_step_trace)
     int trace_slot;
-    // filled by launch_sgemv
-    int kc, stages, static_groups;
-    int row_pad, dbg;
 };
 struct AttnDecodeParams {
     const float *q;          // [H*64]
@@ -181,7 +177,7 @@ struct LaunchCtx {
 
 bool sgemv_shape_supported(int K);
 cudaError_t sgemv_prepare();
-cudaError_t launch_sgemv(const LaunchCtx &c, SgemvParams p);
+cudaError_t launch_sgemv(const LaunchCtx &c, const SgemvParams &p);
 
 // ---- attention block: A2-A6 of a layer in one cluster launch (hq_attn.cu) -----------------------------------
 constexpr int kAbCluster = 8;        // CTAs per cluster = per KV head (portable cluster size)
@@ -198,6 +194,8 @@ struct AttnBlockParams {
     float eps;
     unsigned long long *trace;       // NULL or [grid][trace_cap] global-timer stamps (hq_debug_trace)
     int trace_cap;
+    unsigned long long *step_trace;  // NULL or the step timeline [slots][4] (hq_debug_step_trace); this launch fills step_slot
+    int step_slot;
 };
 size_t attn_block_smem_bytes();
 bool attn_block_shape_supported(const hq_config &c);
