@@ -25,8 +25,8 @@ namespace hq {
 constexpr int kAbWarps = 8;                       // consumer warps
 constexpr int kAbConsumers = 32 * kAbWarps;
 constexpr int kAbThreads = kAbConsumers + 32;     // + producer warp
-constexpr int kAbRowPad = 16;                     // bytes between the rows of a stage: shifts every row by one 16-byte bank group (ldmatrix)
-constexpr int kAbStageBytes = 16 * (2 * 2048 + kAbRowPad);   // ring stage: 8 units of two rows of <= 4 KB (+ pad), or 256 cached positions (K | V)
+constexpr int kAbStageBytes = 16 * 2 * 2048;      // ring stage: 16 rows of <= 4 KB back to back (ONE or two bulk copies: an SM pulls 4 KB copies at
+                                                  // ~58 GB/s, 32-64 KB ones at 135-160 GB/s), or 256 cached positions (K | V)
 constexpr int kAbStages = 3;
 constexpr int kAbUnitsPerStage = 8;
 constexpr int kAbTile0 = 56;                      // cached positions of the first K/V tile (own buffer, requested right after the wait)
@@ -123,13 +123,19 @@ __device__ void ab_producer(const AttnBlockParams &p, const AbGeom &g, uint8_t *
         const int ub = s * kAbUnitsPerStage, nu = min(kAbUnitsPerStage, g.q_units - ub);
         uint64_t *bar = &sh.full[n % kAbStages];
         uint8_t *dst = ring + (size_t)(n % kAbStages) * kAbStageBytes;
-        if (lane == 0) mbar_expect_tx(bar, 2u * nu * qrb);
-        __syncwarp();
-        if (lane < 2 * nu) {
-            const int cu = g.q_u0 + ub + (lane >> 1), hh = cu >> 5, i = (cu & 31) + 32 * (lane & 1);
-            const bf16 *row = hh < g.G ? p.wq + (size_t)((g.kvh * g.G + hh) * kHeadDim + i) * g.K
-                                       : (hh == g.G ? p.wk : p.wv) + (size_t)(g.kvh * kHeadDim + i) * g.K;
-            bulk_g2s_hint(dst + (size_t)lane * (qrb + kAbRowPad), row, qrb, bar, pol);
+        if (lane == 0) {
+            // stage rows 0-7: row i of the units' RoPE pairs, rows 8-15: row i + 32.  Consecutive units are consecutive rows
+            // of one head, so each half is one copy (two where the 8 units straddle a head boundary).
+            mbar_expect_tx(bar, 2u * nu * qrb);
+            for (int j = 0; j < nu;) {
+                const int cu = g.q_u0 + ub + j, hh = cu >> 5, i = cu & 31;
+                const int run = min(nu - j, 32 - i);
+                const bf16 *row = hh < g.G ? p.wq + (size_t)((g.kvh * g.G + hh) * kHeadDim + i) * g.K
+                                           : (hh == g.G ? p.wk : p.wv) + (size_t)(g.kvh * kHeadDim + i) * g.K;
+                bulk_g2s_hint(dst + (size_t)j * qrb, row, (uint32_t)run * qrb, bar, pol);
+                bulk_g2s_hint(dst + (size_t)(8 + j) * qrb, row + (size_t)32 * g.K, (uint32_t)run * qrb, bar, pol);
+                j += run;
+            }
         }
     }
     // this CTA's rows of W_o are one contiguous range: into L2 now (behind the QKV rows), so that the ring loads issued
@@ -166,57 +172,72 @@ __device__ void ab_producer(const AttnBlockParams &p, const AbGeom &g, uint8_t *
     const uint32_t orb = (uint32_t)g.qdim * 2;
     for (int s = 0; s < g.o_stages; ++s, ++n) {
         slot_wait(n);
-        const int ub = s * kAbUnitsPerStage, nu = min(kAbUnitsPerStage, g.o_rows / 2 - ub);
-        uint64_t *bar = &sh.full[n % kAbStages];
-        uint8_t *dst = ring + (size_t)(n % kAbStages) * kAbStageBytes;
-        if (lane == 0) mbar_expect_tx(bar, 2u * nu * orb);
-        __syncwarp();
-        if (lane < 2 * nu) bulk_g2s_hint(dst + (size_t)lane * (orb + kAbRowPad), p.wo + (size_t)(g.o_row0 + 2 * ub + lane) * g.qdim, orb, bar, pol);
+        const int nr = min(16, g.o_rows - 16 * s);   // rows of W_o of this stage: one contiguous copy
+        if (lane == 0) {
+            uint64_t *bar = &sh.full[n % kAbStages];
+            mbar_expect_tx(bar, (uint32_t)nr * orb);
+            bulk_g2s_hint(ring + (size_t)(n % kAbStages) * kAbStageBytes, p.wo + (size_t)(g.o_row0 + 16 * s) * g.qdim, (uint32_t)nr * orb, bar, pol);
+        }
     }
 }
 
 // ---- consumers ---------------------------------------------------------------------------------------------------
 // The 16 rows of a stage against the input vector on the tensor cores (mma.sync m16n8k16 bf16, fp32 accumulate): the
-// launch is bound by instruction issue, not by bytes (2 warps per scheduler, every instruction executed once), and one
-// ldmatrix + one MMA replace ~50 load / convert / FMA instructions.  A = 16 rows x 16 K elements of the stage (rows
-// kAbRowPad apart so that the 8 rows of an 8x8 matrix hit 8 different bank groups); B = the input as two bf16 planes in
-// columns 0 (hi) and 1 (lo) of the 16 x 8 operand, the other columns zero: C[:, 0] + C[:, 1] is the product with 16
-// mantissa bits of the input.  Warp w owns K tiles [w * nkt, (w + 1) * nkt): the 8 partial sums of a row meet in shared memory.
-__device__ __forceinline__ void ab_ldmatrix_x4(uint32_t (&r)[4], uint32_t addr) {
-    asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];" : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(addr));
+// launch is bound by instruction issue, not by bytes, and two LDS.128 + two MMAs replace ~100 load / convert / FMA
+// instructions.  Fragment scheme of hq_stream.cu: the rows of a stage lie back to back (a multiple of 128 bytes apart), lane
+// (g, t) loads elements [8t, 8t + 8) of a 32-element K block of A rows g and g + 8 — words 0, 1 feed the first k-tile, words
+// 2, 3 the second (a permutation of K, applied to B alike) — and odd rows take the neighbouring 64-byte block, so a
+// quarter-warp covers all 32 banks.  B = the input as bf16 planes hi | lo in columns 0, 1 (block order of the even rows)
+// and 2, 3 (block order of the odd rows); row m reads D[m][2 (m & 1)] + D[m][2 (m & 1) + 1].  Warp w owns K blocks
+// [w * nb, (w + 1) * nb): the 8 partial sums of a row meet in shared memory.
+__device__ __forceinline__ void ab_mma_bf16(float (&d)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, uint32_t b0, uint32_t b1) {
+    asm("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+        : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
+        : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
 }
-__device__ __forceinline__ void ab_mma_bf16(float (&d)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1) {
-    asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
-                 : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
-                 : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
+__device__ __forceinline__ uint4 ab_lds128(uint32_t addr) {
+    uint4 v;
+    asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
+    return v;
 }
-constexpr int kAbMaxKt = kAbMaxK / 16 / kAbWarps;   // K tiles per warp at the longest row
-// B fragments of this warp's K tiles: lane = (n = lane >> 2, k pair = (lane & 3) * 2); n = 0 reads the hi plane, n = 1 the lo plane
-__device__ __forceinline__ void ab_load_b(const AbShared &sh, int K, int nkt, int warp, int lane, uint32_t (&bf)[kAbMaxKt][2]) {
-    const int n = lane >> 2, kk = (lane & 3) * 2;
-    const bf16 *src = n == 0 ? sh.xh : sh.xl;
+constexpr int kAbMaxBlocks = kAbMaxK / 32 / kAbWarps;   // 32-element K blocks per warp at the longest row
+// K blocks per row (even: odd rows read block b ^ 1) and per warp
+__device__ __forceinline__ int ab_nblk(int K) { return 2 * ((K + 63) / 64); }
+// B fragments of this warp's K blocks: lane = (column n = lane >> 2, t = lane & 3); n: plane n & 1, block order n >> 1
+__device__ __forceinline__ void ab_load_b(const AbShared &sh, int K, int nb, int warp, int lane, uint4 (&bq)[kAbMaxBlocks]) {
+    const int n = lane >> 2, t = lane & 3, nblk = ab_nblk(K);
+    const bf16 *src = (n & 1) ? sh.xl : sh.xh;
 #pragma unroll
-    for (int i = 0; i < kAbMaxKt; ++i) {
-        const int k0 = (warp * nkt + i) * 16 + kk;
-        const bool ok = n < 2 && i < nkt && k0 < K;
-        bf[i][0] = ok ? *reinterpret_cast<const uint32_t *>(src + k0) : 0u;
-        bf[i][1] = ok ? *reinterpret_cast<const uint32_t *>(src + k0 + 8) : 0u;
+    for (int i = 0; i < kAbMaxBlocks; ++i) {
+        const int blk = warp * nb + i, ks = (blk ^ (n >> 1)) * 32 + t * 8;
+        const bool ok = n < 4 && i < nb && blk < nblk && ks < K;
+        bq[i] = ok ? *reinterpret_cast<const uint4 *>(src + ks) : make_uint4(0, 0, 0, 0);
     }
 }
-__device__ __forceinline__ void ab_dot16(uint32_t stage_addr, uint32_t row_stride, int K, int nkt, int warp, int lane,
-                                         const uint32_t (&bf)[kAbMaxKt][2], float (&c)[4]) {
+__device__ __forceinline__ void ab_dot16(uint32_t stage_addr, uint32_t row_bytes, int K, int nb, int warp, int lane,
+                                         const uint4 (&bq)[kAbMaxBlocks], float (&c)[4]) {
     float cc[4][4];   // four chains: an MMA waits ~30 cycles for its accumulator
 #pragma unroll
     for (int i = 0; i < 4; ++i) cc[i][0] = cc[i][1] = cc[i][2] = cc[i][3] = 0.f;
-    // ldmatrix.x4: lanes 0-7 rows 0-7 / k 0-7, lanes 8-15 rows 8-15 / k 0-7, lanes 16-23 rows 0-7 / k 8-15, lanes 24-31 rows 8-15 / k 8-15
-    const uint32_t a_base = stage_addr + (uint32_t)((lane & 7) + ((lane >> 3) & 1) * 8) * row_stride + (uint32_t)(lane >> 4) * 16u +
-                            (uint32_t)(warp * nkt) * 32u;
+    const int g = lane >> 2, t = lane & 3, nblk = ab_nblk(K);
+    const uint32_t a_base = stage_addr + (uint32_t)g * row_bytes + (uint32_t)t * 16u;
+    uint4 a0[kAbMaxBlocks], a1[kAbMaxBlocks];
 #pragma unroll
-    for (int i = 0; i < kAbMaxKt; ++i) {
-        if (i < nkt && (warp * nkt + i) * 16 < K) {   // warp-uniform
-            uint32_t a[4];
-            ab_ldmatrix_x4(a, a_base + (uint32_t)i * 32u);
-            ab_mma_bf16(cc[i & 3], a, bf[i][0], bf[i][1]);
+    for (int i = 0; i < kAbMaxBlocks; ++i) {
+        const int blk = warp * nb + i;
+        if (i < nb && blk < nblk) {   // warp-uniform
+            const uint32_t off = (uint32_t)(blk ^ (g & 1)) * 64u;
+            a0[i] = ab_lds128(a_base + off);
+            a1[i] = ab_lds128(a_base + 8u * row_bytes + off);
+        } else {
+            a0[i] = a1[i] = make_uint4(0, 0, 0, 0);
+        }
+    }
+#pragma unroll
+    for (int i = 0; i < kAbMaxBlocks; ++i) {
+        if (i < nb) {
+            ab_mma_bf16(cc[(2 * i) & 3], a0[i].x, a1[i].x, a0[i].y, a1[i].y, bq[i].x, bq[i].y);
+            ab_mma_bf16(cc[(2 * i + 1) & 3], a0[i].z, a1[i].z, a0[i].w, a1[i].w, bq[i].z, bq[i].w);
         }
     }
 #pragma unroll
@@ -562,9 +583,9 @@ __global__ void __launch_bounds__(kAbThreads, 1) attn_block_kernel(const __grid_
     for (int ph = 0; ph < 2; ++ph) {
         if (ph == 1) ab_attention<TRACE>(p, g, ring, sh, pos, tag, n, ti);
         const int K = ph ? g.qdim : g.K, units = ph ? g.o_rows / 2 : g.q_units;
-        const int nkt = (K / 16 + kAbWarps - 1) / kAbWarps;
-        uint32_t bf[kAbMaxKt][2];
-        ab_load_b(sh, K, nkt, warp, lane, bf);
+        const int nb = (ab_nblk(K) + kAbWarps - 1) / kAbWarps;
+        uint4 bq[kAbMaxBlocks];
+        ab_load_b(sh, K, nb, warp, lane, bq);
         // RoPE factors of the units this thread finishes (phase 0): loaded now, needed after the barrier below
         float2 cs[kAbMaxPhaseStages];
 #pragma unroll
@@ -580,12 +601,13 @@ __global__ void __launch_bounds__(kAbThreads, 1) attn_block_kernel(const __grid_
             if (s * kAbUnitsPerStage < units) {   // uniform
                 const int slot = n % kAbStages;
                 ab_wait(&sh.full[slot], (n / kAbStages) & 1, p.err);
-                ab_dot16(smem_addr_u32(ring + (size_t)slot * kAbStageBytes), (uint32_t)(K * 2 + kAbRowPad), K, nkt, warp, lane, bf, c[s]);
+                ab_dot16(smem_addr_u32(ring + (size_t)slot * kAbStageBytes), (uint32_t)(K * 2), K, nb, warp, lane, bq, c[s]);
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&sh.empty[slot]);
                 ++n;
-                // C fragment: lane holds (row lane >> 2, cols 2 (lane & 3), +1) in c0, c1 and row + 8 in c2, c3; columns 0 and 1 are the two planes
-                if ((lane & 3) == 0) {
+                // C fragment: lane holds (row lane >> 2, cols 2 (lane & 3), +1) in c0, c1 and row + 8 in c2, c3; a row reads the
+                // (hi, lo) column pair of its block order
+                if ((lane & 3) == ((lane >> 2) & 1)) {
                     sh.dpart[s][warp][lane >> 2] = c[s][0] + c[s][1];
                     sh.dpart[s][warp][(lane >> 2) + 8] = c[s][2] + c[s][3];
                 }
@@ -593,17 +615,18 @@ __global__ void __launch_bounds__(kAbThreads, 1) attn_block_kernel(const __grid_
         }
         ab_trace<TRACE>(p, ti);   // this warp's dots done
         ab_consumer_sync();
-        // epilogue: thread t = (unit u = t >> 3 of a stage, destination rank t & 7) sums the 8 K slices of the unit's two rows
+        // epilogue: thread t = (u = t >> 3, destination rank t & 7) sums the 8 K slices of stage rows u and u + 8: the RoPE
+        // pair of unit u (phase 0), rows 16 s + u and 16 s + u + 8 of this CTA's slice of W_o (phase 1)
         if (tid < 64) {
             const int u = tid >> 3, dst = tid & 7;
 #pragma unroll
             for (int s = 0; s < kAbMaxPhaseStages; ++s) {
-                if (s * kAbUnitsPerStage + u < units) {
+                if (s * kAbUnitsPerStage + u < units || (ph == 1 && s * kAbUnitsPerStage < units)) {
                     float a = 0.f, b = 0.f;
 #pragma unroll
                     for (int w = 0; w < kAbWarps; ++w) {
-                        a += sh.dpart[s][w][2 * u];
-                        b += sh.dpart[s][w][2 * u + 1];
+                        a += sh.dpart[s][w][u];
+                        b += sh.dpart[s][w][u + 8];
                     }
                     if (ph == 0) {
                         const int cu = g.q_u0 + s * kAbUnitsPerStage + u, hh = cu >> 5, i = cu & 31;
@@ -620,8 +643,9 @@ __global__ void __launch_bounds__(kAbThreads, 1) attn_block_kernel(const __grid_
                             row[i + 32] = __float2half_rn(o1);
                         }
                     } else if (dst == 0) {
-                        const int r = 2 * (s * kAbUnitsPerStage + u);
-                        *reinterpret_cast<float2 *>(p.x + g.o_row0 + r) = make_float2(sh.xo[r] + a, sh.xo[r + 1] + b);
+                        const int r = 16 * s + u;
+                        if (r < g.o_rows) p.x[g.o_row0 + r] = sh.xo[r] + a;
+                        if (r + 8 < g.o_rows) p.x[g.o_row0 + r + 8] = sh.xo[r + 8] + b;
                     }
                 }
             }
@@ -641,7 +665,7 @@ bool attn_block_shape_supported(const hq_config &c) {
     const int G = c.n_kv_heads > 0 ? c.n_heads / c.n_kv_heads : 0, qdim = c.n_heads * c.head_dim;
     const int o_den = c.n_kv_heads * kAbCluster;
     return c.head_dim == kHeadDim && G >= 1 && G <= 8 && c.hidden % 8 == 0 && c.hidden <= kAbMaxK && qdim <= kAbMaxK &&
-           c.hidden % 16 == 0 && c.hidden % (2 * o_den) == 0 && c.hidden / o_den <= kAbMaxORows;
+           c.hidden % 64 == 0 && c.hidden % (2 * o_den) == 0 && c.hidden / o_den <= kAbMaxORows;   // % 64: whole K block pairs (ab_dot16)
 }
 
 static void attn_block_config(cudaLaunchConfig_t &cfg, cudaLaunchAttribute *attr, const LaunchCtx &c, int n_kv_heads) {
