@@ -269,14 +269,17 @@ def main():
         # BASELINE.json configs[4] (and the shapes of configs[2], [3]): tokens/s, per-token latency and algorithmic HBM GB/s
         peak, _ = measured_peak()
         lay = gm.weight_tensors()
-        for B in (1, 4, 16, 32):
-            for ctx in (512, 4096):
-                steps = 128
+        points = [(B, ctx, 128, "configs[4]") for B in (1, 4, 16, 32) for ctx in (512, 4096)]
+        points += [(1, 2048, 256, "configs[2]"), (8, 192, 192, "configs[3]")]
+        for B, ctx, steps, cfg_name in points:
+            if True:   # (indentation kept: one model per point)
                 m = hq.Model(hq.binding.make_config(n_layers=s.n_layers, hidden=s.hidden, n_heads=s.n_heads, n_kv_heads=s.n_kv_heads,
                                             head_dim=s.head_dim, ffn=s.ffn, vocab=s.vocab, rms_eps=s.rms_eps,
                                             rope_theta=s.rope_theta, max_batch=B, max_seq=ctx + steps + 8, flags=0), *lay)
                 pr = datagen.tokens(1004, s.vocab, B * ctx).reshape(B, ctx)
                 ms, pf = [], []
+                sampler = ClockSampler(local_rank)
+                sampler.start()
                 for it in range(3):
                     m.kv_reset()
                     a, b, c2 = ev(), ev(), ev()
@@ -289,9 +292,11 @@ def main():
                     if it:
                         pf.append(a.elapsed_time(b))
                         ms.append(b.elapsed_time(c2))
+                clk = sampler.stop()
                 step_ms = float(np.mean(ms)) / steps
                 bpt = bytes_per_token(s, ctx + steps // 2, B)
-                print(json.dumps({"sweep": True, "batch": B, "context": ctx, "decode_steps": steps,
+                print(json.dumps({"sweep": True, "config": cfg_name, "batch": B, "context": ctx, "decode_steps": steps,
+                                  "clocks": clk,
                                   "tokens_per_s": B / (step_ms * 1e-3), "ms_per_step": step_ms,
                                   "prefill_ms": float(np.mean(pf)), "prefill_tokens_per_s": B * ctx / (float(np.mean(pf)) * 1e-3),
                                   "bytes_per_step": bpt, "GBps": bpt / (step_ms * 1e-3) / 1e9,
@@ -305,11 +310,11 @@ def main():
         gm.kv_reset()
         gm.prefill(prompt, want_token=False)
         gm.sync()
-        before = gm.kernel_count() + 86      # + launches made by hq_model_create
+        before = gm.kernel_count()
         gm.decode_run(args.profile, want_tokens=False)
         gm.sync()
-        print(json.dumps({"profile": True, "launches_before_decode": before,
-                          "decode_launches": gm.kernel_count() + 86 - before}), flush=True)
+        print(json.dumps({"profile": True, "decode_launches": gm.kernel_count() - before,
+                          "decode_path": gm.decode_path()}), flush=True)
         return
 
     for _ in range(max(args.warmup, 3)):
@@ -335,34 +340,31 @@ def main():
     decode_ms = [e[1].elapsed_time(e[2]) for e in evs]
 
     # ---- e2e: same metric through the C ABI with HOST buffers, streaming one token per call ------------
-    first = np.empty(1, dtype=np.int32)
+    # (SURVEY.md 8(d) second pass: per-step sync + 4-byte D2H => true streaming per-token latency, p50 / p99)
     out = np.empty(1, dtype=np.int32)
-    e2e_decode_s, e2e_ttft_s = [], []
+    e2e_decode_s, e2e_ttft_s, tok_lat_us = [], [], []
     for _ in range(max(1, min(args.steps, 3))):
         gm.kv_reset()
         gm.sync()
         t0 = time.perf_counter()
         gm.prefill(prompt, want_token=True)                   # H2D prompt, D2H first token, sync
         t1 = time.perf_counter()
+        tp = t1
         for _ in range(DECODE_STEPS):
             gm.decode_step(want_token=True, out=out)          # D2H 4 bytes + sync every token
-        t2 = time.perf_counter()
+            tn = time.perf_counter()
+            tok_lat_us.append((tn - tp) * 1e6)
+            tp = tn
         e2e_ttft_s.append(t1 - t0)
-        e2e_decode_s.append(t2 - t1)
-    del first
+        e2e_decode_s.append(tp - t1)
 
-    # ---- dominant kernel, timed alone over layers cycling (weights streamed > L2) ----------------------
+    # ---- every decode kernel timed alone (CUDA events on the library's stream, launches back to back under PDL,
+    #      cycling the 16 layers so that the weights streamed exceed L2) ------------------------------------------
     reps = 16 * 8
-    gm.bench_kernel(0, 32)
-    torch.cuda.synchronize(dev)
-    a, b = ev(), ev()
-    a.record(stream)
-    gu_bytes = gm.bench_kernel(0, reps)
-    b.record(stream)
-    torch.cuda.synchronize(dev)
-    gu_ms = a.elapsed_time(b) / reps
+    per_step = {"attn_block": s.n_layers, "gate_up": s.n_layers, "down": s.n_layers, "lm_head": 1}
     kernels = {}
-    for which, name in ((1, "lm_head"), (2, "qkv"), (3, "o_proj"), (4, "down"), (5, "attn_decode"), (6, "attn_block")):
+    gm.kv_reset(); gm.prefill(prompt, want_token=False); gm.sync()
+    for which, name in ((0, "gate_up"), (1, "lm_head"), (4, "down"), (6, "attn_block")):
         r = 16 if which == 1 else reps
         gm.bench_kernel(which, 8)
         a, b = ev(), ev()
@@ -371,24 +373,30 @@ def main():
         b.record(stream)
         torch.cuda.synchronize(dev)
         ms = a.elapsed_time(b) / r
-        kernels[name] = {"us": ms * 1e3, "GBps": nbytes / ms / 1e6}
-    kernels["gate_up"] = {"us": gu_ms * 1e3, "GBps": gu_bytes / gu_ms / 1e6}
+        kernels[name] = {"us": ms * 1e3, "GBps": nbytes / ms / 1e6, "bytes_per_launch": nbytes,
+                         "launches_per_step": per_step[name]}
 
-    # ---- the persistent-kernel path, same workload, reported beside the default ------------------------------
-    gm_mega = hq.Model(gm.cfg_with_flags(hq.FLAG_MEGA), *gm.weight_tensors())   # same device weights
-    for _ in range(3):
-        gm_mega.kv_reset(); gm_mega.prefill(prompt, want_token=False); gm_mega.decode_run(DECODE_STEPS, want_tokens=False)
-    torch.cuda.synchronize(dev)
-    mega_ms = []
-    for _ in range(max(1, min(args.steps, 3))):
-        gm_mega.kv_reset(); gm_mega.prefill(prompt, want_token=False)
-        a, b = ev(), ev()
-        a.record(gm_mega.stream)
-        gm_mega.decode_run(DECODE_STEPS, want_tokens=False)
-        b.record(gm_mega.stream)
+    # ---- read-only streaming probe: a sum-reduction over 4 GiB, the practical ceiling of a kernel that
+    #      only reads HBM ------------------------------------------------------------------------------------------
+    probe_gbs = None
+    try:
+        buf = torch.empty(4 << 30, dtype=torch.uint8, device=dev)
+        buf.zero_()
+        acc = torch.zeros(1, dtype=torch.int32, device=dev)
+        with torch.cuda.stream(stream):
+            for _ in range(2):
+                hq.read_probe(buf, acc, stream=stream)
+            a, b = ev(), ev()
+            a.record(stream)
+            for _ in range(5):
+                hq.read_probe(buf, acc, stream=stream)
+            b.record(stream)
         torch.cuda.synchronize(dev)
-        mega_ms.append(a.elapsed_time(b))
-    mega_tok_s = DECODE_STEPS / (float(np.mean(mega_ms)) * 1e-3)
+        probe_gbs = 5 * buf.numel() / (a.elapsed_time(b) * 1e-3) / 1e9
+        del buf
+    except Exception as e:    # e.g. not enough free memory for the probe buffer
+        probe_gbs = None
+        print("read probe skipped:", e, file=sys.stderr)
 
     # ---- aggregate over ranks (max time) -----------------------------------------------------------------
     dec_total_ms, total_ms, ttft, launches = aggregate_over_ranks(dist, dev, float(sum(decode_ms)), total_ms,
@@ -396,39 +404,59 @@ def main():
 
     if rank == 0:
         peak, peak_src = measured_peak()
+        ncu = ncu_numbers()
         value = job_tokens_per_s(world, args.steps, dec_total_ms)
         ms_per_token = dec_total_ms / (args.steps * DECODE_STEPS)
         ctx_mid = PROMPT_LEN + DECODE_STEPS // 2
         bpt = bytes_per_token(s, ctx_mid)
         step_gbs = bpt / (ms_per_token * 1e-3) / 1e9
-        achieved = gu_bytes / (gu_ms * 1e-3) / 1e9
         e2e_value = world * DECODE_STEPS / float(np.mean(e2e_decode_s))
+        # the kernel with the largest share of the step TIME, chosen from what was just measured
+        dom = max(kernels, key=lambda k: kernels[k]["us"] * kernels[k]["launches_per_step"])
+        kd = kernels[dom]
+        label = {"attn_block": "attn_block_kernel (A2-A6 of a layer in one cluster launch: a latency chain, 8.5 % of the bytes)",
+                 "gate_up": "sgemv_kernel<gate/up + SwiGLU> (43 % of the bytes per token)",
+                 "down": "sgemv_kernel<down + residual> (22 % of the bytes)",
+                 "lm_head": "sgemv_kernel<LM head + argmax> (21 % of the bytes)"}
+        lat = np.array(tok_lat_us)
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "bf16 weights/KV, f32 accumulate", "data": "synthetic",
+            "scaling": "weak", "vs_baseline": None,
+            "dtype": "bf16 weights, f32 accumulate and residual stream; fp16 KV cache; activations into tensor-core MMAs "
+                     "(decode GEMVs via mma.sync, prefill GEMMs via tcgen05) as two bf16 planes hi + lo; prefill attention fp16 mma.sync",
+            "data": "synthetic",
             "config": {"workload": WORKLOAD, "l2": "inputs larger than L2 (2.47 GB of weights per token vs 126 MB)",
-                       "multi_gpu": "independent replicas, no collective"},
+                       "multi_gpu": "independent replicas, no collective", "decode_path": gm.decode_path()},
             "ttft_ms": ttft, "ms_per_token": ms_per_token, "clocks": clocks, "gpu_launches": launches,
+            "latency_us_per_token_streaming": {"p50": float(np.percentile(lat, 50)), "p99": float(np.percentile(lat, 99)),
+                                               "mean": float(lat.mean()), "n": int(lat.size),
+                                               "how": "hq_decode_step with a host token out: one sync + 4-byte D2H per token, host wall clock"},
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": PROMPT_LEN * 4,
                     "d2h_bytes_per_step": (DECODE_STEPS + 1) * 4,
                     "ttft_ms": float(np.mean(e2e_ttft_s)) * 1e3,
                     "how": "hq_prefill(host tokens -> host first token) then 128 x hq_decode_step(host token out), "
                            "host wall clock, one sync + 4-byte D2H per token"},
-            "roofline": {"bound": "hbm", "kernel": "gemv_kernel<gate/up + SwiGLU> (43% of bytes per token)",
-                         "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": ncu_traffic(), "peak_source": peak_src,
-                         "bytes_per_launch": gu_bytes, "us_per_launch": gu_ms * 1e3},
+            "roofline": {"bound": "hbm", "kernel": label[dom], "chosen": "largest us_per_launch x launches_per_step of kernels_alone",
+                         "achieved": kd["GBps"], "peak": peak, "unit": "GB/s", "frac": kd["GBps"] / peak,
+                         "traffic": ncu.get(dom + "_dram_bytes_per_launch"), "peak_source": peak_src,
+                         "bytes_per_launch": kd["bytes_per_launch"], "us_per_launch": kd["us"],
+                         "share_of_step_time": kd["us"] * kd["launches_per_step"] / (ms_per_token * 1e3)},
+            # the kernel with the largest share of the BYTES: both its PDL-chained figure (back-to-back launches overlap the
+            # predecessor's tail) and the serialised, cold-cache one from the committed ncu pass
+            "roofline_gate_up": {"bound": "hbm", "kernel": label["gate_up"], "achieved": kernels["gate_up"]["GBps"], "peak": peak,
+                                 "unit": "GB/s", "frac": kernels["gate_up"]["GBps"] / peak,
+                                 "us_per_launch": kernels["gate_up"]["us"],
+                                 "bytes_per_launch": kernels["gate_up"]["bytes_per_launch"],
+                                 "traffic": ncu.get("gate_up_dram_bytes_per_launch"),
+                                 "ncu_serialised_us": ncu.get("gate_up_ncu_us"),
+                                 "ncu_serialised_frac": (kernels["gate_up"]["bytes_per_launch"] / (ncu["gate_up_ncu_us"] * 1e-6) / 1e9 / peak)
+                                 if ncu.get("gate_up_ncu_us") else None},
             "step_roofline": {"bytes_per_token": bpt, "achieved_GBps": step_gbs, "frac_of_measured": step_gbs / peak,
-                              "frac_of_8TBps_spec": step_gbs / 8000.0},
+                              "frac_of_8TBps_spec": step_gbs / 8000.0,
+                              "read_probe_GBps": probe_gbs,
+                              "frac_of_read_probe": (step_gbs / probe_gbs) if probe_gbs else None},
             "kernels_alone": kernels,
-            # the kernel with the largest share of the step TIME (41 %, 8.5 % of the bytes): a latency chain, not a stream
-            "roofline_largest_time_share": {"bound": "hbm", "kernel": "mega_decode_kernel<attention block> (A2-A6 of a layer)",
-                                            "achieved": kernels["attn_block"]["GBps"], "peak": peak, "unit": "GB/s",
-                                            "frac": kernels["attn_block"]["GBps"] / peak,
-                                            "us_per_launch": kernels["attn_block"]["us"]},
-            "persistent_kernel": {"value": mega_tok_s, "unit": UNIT,
-                                  "note": "HQ_FLAG_MEGA: the same 128 decode steps in ONE launch (hq_mega.cu), this rank"},
         }
         if not args.no_cpu_baseline:
             line["cpu_baseline"] = oracle_sample(weights, s)

@@ -150,6 +150,10 @@ static AttnBlockParams attn_block_params(const hq_model *m, int l) {
     return a;
 }
 
+// Stages (64 KB) by which a gate/up CTA that was resident during the attention block is ahead of one that starts on an SM
+// the block has just left: two of its three ring stages (measured optimum 2-4, flat; 0 costs 1.5 % of the step).
+constexpr float kLateDeficit = 2.0f;
+
 static SgemvParams sgemv_gateup(const hq_model *m, int l) {
     const hq_config &c = m->cfg;
     const LayerW &w = m->layers[l];
@@ -157,6 +161,7 @@ static SgemvParams sgemv_gateup(const hq_model *m, int l) {
     p.w0 = w.w_gate; p.w1 = w.w_up; p.gain = w.ffn_norm; p.xin = m->b.x; p.K = c.hidden; p.n_rows = c.ffn;
     p.mode = SGEMV_GATEUP; p.xin_mode = SGEMV_XIN_NORM; p.eps = c.rms_eps;
     p.trace = m->step_trace; p.trace_slot = 2 + 3 * l;
+    if (m->use_attn_block) { p.n_early = m->n_sms - kAbCluster * c.n_kv_heads; p.late_deficit = kLateDeficit; }
     p.out_planes = reinterpret_cast<bf16 *>(m->b.act);
     return p;
 }
@@ -781,10 +786,13 @@ extern "C" int32_t hq_bench_kernel(hq_model *m, int32_t which, int32_t reps, int
         const LayerW &w = m->layers[l];
         GemvParams p = {};
         switch (which) {
-            case 0:
-                HQ_CUDA(launch_sgemv(lc, sgemv_gateup(m, l)));
+            case 0: {
+                SgemvParams pg = sgemv_gateup(m, l);
+                pg.n_early = 0;   // timed alone there is no attention block in front of it: even split
+                HQ_CUDA(launch_sgemv(lc, pg));
                 bytes = 2ll * 2 * c.ffn * c.hidden;
                 break;
+            }
             case 1: {
                 // LM head without state side effects: pos_inc = 0 (token / history writes repeat the current slot)
                 HQ_CUDA(launch_sgemv(lc, sgemv_lm_head(m, b.x, 0)));

@@ -2,12 +2,11 @@
 //
 // One token per step is a chain of HBM-bound matrix-vector products (2.47 GB of bf16 weights per
 // token), so every kernel here is built around one idea: keep 16-byte weight loads in flight.
-//   * gemv_kernel: a CTA of 256 threads owns a contiguous range of "units" (2 output rows each).
-//     Thread t owns the same 8-element k-slices of every row, so the (normalised) input vector
-//     lives in registers, a row is read by 512-byte coalesced warp loads, and 2U*CH independent
-//     16-byte loads per thread are double buffered.  Fused in: RMSNorm prologue (A2), split-KV
-//     merge prologue (A5 combine), RoPE + KV append (A4), SwiGLU (A7), residual add (A6, A8),
-//     logits + packed-atomicMax argmax + step bookkeeping (A9).
+//   * gemv_kernel (kernel-per-row path: QKV and O projections; the big streams are hq_stream.cu): a CTA of 256
+//     threads owns a contiguous range of "units" (2 output rows each).  Thread t owns the same 8-element k-slices of
+//     every row, so the (normalised) input vector lives in registers, a row is read by 512-byte coalesced warp
+//     loads, and 2U*CH independent 16-byte loads per thread are double buffered.  Fused in: RMSNorm prologue (A2),
+//     split-KV merge prologue (A5 combine), RoPE + KV append (A4), residual add (A6).
 //   * Weight loads for the first batch are issued BEFORE griddepcontrol.wait (weights are
 //     immutable), so under programmatic dependent launch they overlap the previous kernel's tail.
 //   * attn_decode_kernel: GQA split-KV flash-decode; K/V tiles staged in shared memory with one
@@ -72,9 +71,6 @@ __device__ __forceinline__ void unit_rows(const GemvParams &p, int u, const bf16
         else { base = p.w2; h = hh - p.n_heads - p.n_kv_heads; }
         ra = base + (size_t)(h * kHeadDim + i) * p.K;
         rb = ra + (size_t)32 * p.K;
-    } else if (MODE == GEMV_GATEUP) {
-        ra = p.w0 + (size_t)u * p.K;
-        rb = p.w1 + (size_t)u * p.K;
     } else {
         ra = p.w0 + (size_t)(2 * u) * p.K;
         rb = ra + p.K;
@@ -167,13 +163,7 @@ __global__ void __launch_bounds__(kGemvThreads) gemv_kernel(const __grid_constan
 #pragma unroll
         for (int c = 0; c < CH; ++c) {
             const int chunk = tid + c * kGemvThreads;
-            if (chunk < kchunks && XIN == XIN_PLAIN) {   // SwiGLU vector, fp16 (see the gate/up epilogue)
-                const uint4 h = __ldcg(reinterpret_cast<const uint4 *>(p.xin) + chunk);
-                const float2 f0 = __half22float2(*reinterpret_cast<const __half2 *>(&h.x)), f1 = __half22float2(*reinterpret_cast<const __half2 *>(&h.y));
-                const float2 f2 = __half22float2(*reinterpret_cast<const __half2 *>(&h.z)), f3 = __half22float2(*reinterpret_cast<const __half2 *>(&h.w));
-                xr[c][0] = f0.x; xr[c][1] = f0.y; xr[c][2] = f1.x; xr[c][3] = f1.y;
-                xr[c][4] = f2.x; xr[c][5] = f2.y; xr[c][6] = f3.x; xr[c][7] = f3.y;
-            } else if (chunk < kchunks) {
+            if (chunk < kchunks) {
                 const float4 a = ld_act4(p.xin + chunk * 8), b = ld_act4(p.xin + chunk * 8 + 4);
                 xr[c][0] = a.x; xr[c][1] = a.y; xr[c][2] = a.z; xr[c][3] = a.w;
                 xr[c][4] = b.x; xr[c][5] = b.y; xr[c][6] = b.z; xr[c][7] = b.w;
@@ -207,8 +197,7 @@ __global__ void __launch_bounds__(kGemvThreads) gemv_kernel(const __grid_constan
 
     // per-kernel constants for the epilogues
     int pos = 0;
-    if (MODE == GEMV_QKV || MODE == GEMV_LMHEAD) pos = ld_act(p.pos);
-    unsigned long long my_best = 0ull;
+    if (MODE == GEMV_QKV) pos = ld_act(p.pos);
 
     auto epilogue = [&](int u, float a, float b) {
         if (MODE == GEMV_QKV) {
@@ -227,21 +216,12 @@ __global__ void __launch_bounds__(kGemvThreads) gemv_kernel(const __grid_constan
                 dst[i] = __float2half_rn(a);
                 dst[i + 32] = __float2half_rn(b);
             }
-        } else if (MODE == GEMV_GATEUP) {
-            // fp16: the SwiGLU vector is re-read by every CTA of the down projection (296 x 32 KB through L2 at fp32, as much
-            // L2 traffic as 9.5 MB of weights); 11 mantissa bits on this one vector cost ~1e-4 of the 1e-2 hidden tolerance
-            reinterpret_cast<__half *>(p.out)[u] = __float2half_rn(silu_f(a) * b);
-        } else if (MODE == GEMV_RESID) {
+        } else {  // GEMV_RESID
             float2 *dst = reinterpret_cast<float2 *>(p.out + 2 * u);
             float2 v = __ldcg(dst);
             v.x += a;
             v.y += b;
             *dst = v;
-        } else {  // GEMV_LMHEAD
-            *reinterpret_cast<float2 *>(p.out + 2 * u) = make_float2(a, b);
-            unsigned long long ka = pack_argmax(a, 2 * u), kb = pack_argmax(b, 2 * u + 1);
-            ka = ka > kb ? ka : kb;
-            my_best = my_best > ka ? my_best : ka;
         }
     };
 
@@ -277,31 +257,6 @@ __global__ void __launch_bounds__(kGemvThreads) gemv_kernel(const __grid_constan
         compute(buf1, ub + U);
     }
 
-    if (MODE == GEMV_LMHEAD) {
-        // fused argmax (A9): per-CTA best -> one packed 64-bit atomicMax; the last CTA to finish
-        // publishes the token and advances the position (device-resident step state).
-        if (warp == 0) {
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) {
-                unsigned long long other = __shfl_xor_sync(0xffffffffu, my_best, o);
-                my_best = my_best > other ? my_best : other;
-            }
-            if (lane == 0) {
-                if (my_best) atomicMax(p.best, my_best);
-                __threadfence();
-                const unsigned int ticket = atomicAdd(p.counter, 1u);
-                if (ticket == gridDim.x - 1) {
-                    __threadfence();
-                    const unsigned long long win = atomicExch(p.best, 0ull);
-                    const int tok = unpack_argmax_idx(win);
-                    *p.cur_tok = tok;
-                    p.tok_hist[pos + p.pos_inc] = tok;
-                    *p.pos_rw = pos + p.pos_inc;
-                    *p.counter = 0u;
-                }
-            }
-        }
-    }
 }
 
 // =====================================================================================================
@@ -447,10 +402,7 @@ static cudaError_t launch_gemv_mx(const LaunchCtx &c, const GemvParams &p) {
 
 cudaError_t launch_gemv(const LaunchCtx &c, GemvMode mode, GemvInput xin, const GemvParams &p) {
     if (mode == GEMV_QKV && xin == XIN_NORM) return launch_gemv_mx<GEMV_QKV, XIN_NORM>(c, p);
-    if (mode == GEMV_GATEUP && xin == XIN_NORM) return launch_gemv_mx<GEMV_GATEUP, XIN_NORM>(c, p);
     if (mode == GEMV_RESID && xin == XIN_ATTN) return launch_gemv_mx<GEMV_RESID, XIN_ATTN>(c, p);
-    if (mode == GEMV_RESID && xin == XIN_PLAIN) return launch_gemv_mx<GEMV_RESID, XIN_PLAIN>(c, p);
-    if (mode == GEMV_LMHEAD && xin == XIN_NORM) return launch_gemv_mx<GEMV_LMHEAD, XIN_NORM>(c, p);
     return cudaErrorInvalidValue;
 }
 

@@ -103,30 +103,24 @@ struct hq_model_impl {
 };
 
 // ---- parameter blocks --------------------------------------------------------------------------------
-enum GemvMode { GEMV_QKV = 0, GEMV_GATEUP = 1, GEMV_RESID = 2, GEMV_LMHEAD = 3 };
-enum GemvInput { XIN_NORM = 0, XIN_PLAIN = 1, XIN_ATTN = 2 };
+enum GemvMode { GEMV_QKV = 0, GEMV_RESID = 2 };
+enum GemvInput { XIN_NORM = 0, XIN_ATTN = 2 };
 
 struct GemvParams {
-    // weights: QKV uses w0=wq, w1=wk, w2=wv; GATEUP w0=gate, w1=up; RESID/LMHEAD w0
+    // weights: QKV uses w0=wq, w1=wk, w2=wv; RESID w0
     const bf16 *w0, *w1, *w2;
     const bf16 *gain;        // XIN_NORM
-    const float *xin;        // XIN_NORM: residual x [K]; XIN_PLAIN: act [K]; XIN_ATTN: part_o
+    const float *xin;        // XIN_NORM: residual x [K]; XIN_ATTN: part_o
     const float2 *part_ml;   // XIN_ATTN
     int K;                   // input features
     int n_units;             // work units (2 output rows each)
     float eps;
     // outputs
-    float *out;              // QKV: q [H*64]; GATEUP: act [F]; RESID: x (read-modify-write); LMHEAD: logits
+    float *out;              // QKV: q [H*64]; RESID: x (read-modify-write)
     kv_t *kc, *vc;           // QKV: this layer's cache base for sequence 0
     const float2 *rope;
     const int *pos;          // device-resident position
     int n_heads, n_kv_heads, max_seq;
-    // LMHEAD
-    unsigned long long *best;
-    unsigned int *counter;
-    int *cur_tok, *tok_hist;
-    int *pos_rw;
-    int pos_inc;
 };
 
 // ---- streaming GEMV (hq_stream.cu): gate/up + SwiGLU, down + residual, LM head + argmax of batch-1 decode -------------
@@ -147,6 +141,8 @@ struct SgemvParams {
     unsigned int *counter;
     int *cur_tok, *tok_hist, *pos_rw;
     int pos_inc;
+    int n_early;             // CTAs expected to start (and pre-fill their rings) while the previous kernel holds the other SMs
+    float late_deficit;      // ... and how many stages more than the others each of them takes
     unsigned long long *trace;   // NULL or step timeline [slots][4] (hq_debug_step_trace)
     int trace_slot;
 };

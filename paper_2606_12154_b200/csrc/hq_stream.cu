@@ -86,12 +86,16 @@ __global__ void __launch_bounds__(kSgThreads, 1) sgemv_kernel(const __grid_const
     SgShared &sh = *reinterpret_cast<SgShared *>(sg_smem + (size_t)kSgStages * kSgStageBytes);
     bf16 *xh = reinterpret_cast<bf16 *>(sg_smem + (size_t)kSgStages * kSgStageBytes + ((sizeof(SgShared) + 15) & ~(size_t)15));
     bf16 *xl = xh + p.K;                         // XIN_NORM only: the normalised input as two bf16 planes
-    // contiguous share of the stages
+    // contiguous share of the stages.  The first n_early CTAs are expected to be resident (and to have pre-filled their rings)
+    // while the previous kernel still holds the other SMs: they take late_deficit stages more than the rest.
     int s0, s1;
     {
-        const int per = g.n_stages_total / (int)gridDim.x, rem = g.n_stages_total % (int)gridDim.x, b = (int)blockIdx.x;
-        s0 = b * per + min(b, rem);
-        s1 = s0 + per + (b < rem ? 1 : 0);
+        const int S = g.n_stages_total, G = (int)gridDim.x, b = (int)blockIdx.x;
+        const int ne = min(p.n_early, G);
+        const float l = fmaxf(0.f, (float)S - (float)ne * p.late_deficit) / (float)G, e = ((float)S - l * (float)(G - ne)) / (float)max(ne, 1);
+        auto cum = [&](int i) { return i >= G ? S : min(S, (int)((i <= ne ? (float)i * e : (float)ne * e + (float)(i - ne) * l) + 0.5f)); };
+        s0 = cum(b);
+        s1 = cum(b + 1);
     }
 
     if (tid == 0) {
