@@ -216,6 +216,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg")
     ap.add_argument("--sweep", action="store_true",
                     help="configs[4]: batch {1,4,16,32} x context {512,4096}, 128 decode steps each; one JSON line per point")
+    ap.add_argument("--probes", action="store_true",
+                    help="memory-system probes behind the kernel design: bulk-copy size vs per-SM rate, read-only stream; JSON lines")
     ap.add_argument("--profile", type=int, default=0, metavar="N",
                     help="ncu helper: one prefill + N decode steps of the bench workload, no timing")
     args = ap.parse_args()
@@ -304,6 +306,37 @@ def main():
                 m.close()
                 del m
                 torch.cuda.empty_cache()
+        return
+
+    if args.probes:
+        # what one SM / the chip pulls through cp.async.bulk as a function of the copy size (hq_debug_copy_probe), and the
+        # read-only LDG stream (hq_debug_read_probe); 2 GiB buffer, CUDA events on the launching stream
+        buf = torch.empty(2 << 30, dtype=torch.uint8, device=dev)
+        buf.zero_()
+        acc = torch.zeros(1, dtype=torch.int32, device=dev)
+        n_sms = torch.cuda.get_device_properties(dev).multi_processor_count
+        with torch.cuda.stream(stream):
+            for n_ctas in (8, 16, 64, n_sms):
+                for copy in (1024, 4096, 16384, 32768, 65536):
+                    sub = buf[: (256 << 20) if n_ctas <= 16 else (2 << 30)]
+                    hq.copy_probe(sub, copy, n_ctas, stream=stream)
+                    a, b = ev(), ev()
+                    a.record(stream)
+                    for _ in range(3):
+                        nb = hq.copy_probe(sub, copy, n_ctas, stream=stream)
+                    b.record(stream)
+                    torch.cuda.synchronize(dev)
+                    gbs = 3 * nb / (a.elapsed_time(b) * 1e-3) / 1e9
+                    print(json.dumps({"probe": "bulk_copy", "n_ctas": n_ctas, "copy_bytes": copy, "GBps": gbs,
+                                      "GBps_per_sm": gbs / n_ctas}), flush=True)
+            hq.read_probe(buf, acc, stream=stream)
+            a, b = ev(), ev()
+            a.record(stream)
+            for _ in range(5):
+                hq.read_probe(buf, acc, stream=stream)
+            b.record(stream)
+            torch.cuda.synchronize(dev)
+            print(json.dumps({"probe": "read_only_ldg", "GBps": 5 * buf.numel() / (a.elapsed_time(b) * 1e-3) / 1e9}), flush=True)
         return
 
     if args.profile:

@@ -41,6 +41,12 @@ int32_t hq_debug_gemm(void *cuda_stream, int32_t mode, const void *w_dev, const 
  * larger than L2: bytes / time is what a kernel that only reads HBM reaches on this box.  Asynchronous. */
 int32_t hq_debug_read_probe(void *cuda_stream, const void *src_dev, size_t bytes, uint32_t *sum_dev);
 
+/* Measurement: what an SM pulls from HBM through cp.async.bulk as a function of the size of the individual copy.  One
+ * launch: n_ctas CTAs (one per SM) each stream their share of src_dev[0, bytes) through a ring of 3 x 64 KB shared-memory
+ * stages, a stage being 64 KB / copy_bytes bulk copies; nothing is computed.  bytes_streamed = n_ctas * floor(bytes /
+ * 65536 / n_ctas) * 65536.  copy_bytes: power of two in [16, 65536].  Time it with CUDA events.  Asynchronous. */
+int32_t hq_debug_copy_probe(void *cuda_stream, const void *src_dev, size_t bytes, int32_t copy_bytes, int32_t n_ctas);
+
 /* Parity: one cached position read back.  which = 0 (K, rotated) or 1 (V); row_dev: DEVICE fp16 [n_kv_heads][64] <-
  * the cache row of `layer`, sequence `seq`, position `pos` (the cache itself is [L][B][Hkv][max_seq][64] fp16).
  * Asynchronous device-to-device copy on the model's stream. */

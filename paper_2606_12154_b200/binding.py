@@ -26,7 +26,7 @@ _CODE_NAMES = {-1: "HQ_ERR_INVALID_ARG", -2: "HQ_ERR_CAPACITY", -3: "HQ_ERR_STAT
 DECLARED_SYMBOLS = (
     "hq_workspace_bytes", "hq_model_create", "hq_model_destroy", "hq_prefill", "hq_decode_step",
     "hq_decode_run", "hq_decode_logits", "hq_get_hidden", "hq_sync", "hq_seq_len", "hq_kv_reset",
-    "hq_kernel_count", "hq_decode_path", "hq_bench_kernel", "hq_debug_gemm", "hq_debug_kv_row", "hq_debug_read_probe", "hq_debug_step_trace", "hq_debug_trace", "hq_last_error",
+    "hq_kernel_count", "hq_decode_path", "hq_bench_kernel", "hq_debug_copy_probe", "hq_debug_gemm", "hq_debug_kv_row", "hq_debug_read_probe", "hq_debug_step_trace", "hq_debug_trace", "hq_last_error",
     "hq_version",
 )
 
@@ -99,6 +99,8 @@ def load_library(path: Optional[str] = None):
     l.hq_bench_kernel.argtypes = [vp, i32, i32, ctypes.POINTER(i64)]
     l.hq_debug_gemm.restype = i32
     l.hq_debug_gemm.argtypes = [vp, i32, vp, vp, vp, vp, i32, i32, i32, i32, i32]
+    l.hq_debug_copy_probe.restype = i32
+    l.hq_debug_copy_probe.argtypes = [vp, vp, ctypes.c_size_t, i32, i32]
     l.hq_debug_read_probe.restype = i32
     l.hq_debug_read_probe.argtypes = [vp, vp, ctypes.c_size_t, vp]
     l.hq_debug_kv_row.restype = i32
@@ -317,6 +319,15 @@ def read_probe(buf, result, stream=None):
     st = stream if stream is not None else torch.cuda.current_stream(buf.device)
     _check(load_library().hq_debug_read_probe(st.cuda_stream, buf.data_ptr(), buf.numel() * buf.element_size(),
                                               result.data_ptr()))
+
+
+def copy_probe(buf, copy_bytes: int, n_ctas: int, stream=None) -> int:
+    """hq_debug_copy_probe on a CUDA tensor; returns the bytes one launch streams."""
+    import torch
+    st = stream if stream is not None else torch.cuda.current_stream(buf.device)
+    nbytes = buf.numel() * buf.element_size()
+    _check(load_library().hq_debug_copy_probe(st.cuda_stream, buf.data_ptr(), nbytes, copy_bytes, n_ctas))
+    return n_ctas * (nbytes // 65536 // n_ctas) * 65536
 
 
 def debug_gemm(mode: int, w, x, out, *, w2=None, token_tile: int = 128, splits: int = 1, stream=None):

@@ -852,6 +852,14 @@ extern "C" int32_t hq_debug_read_probe(void *cuda_stream, const void *src_dev, s
     return HQ_OK;
 }
 
+extern "C" int32_t hq_debug_copy_probe(void *cuda_stream, const void *src_dev, size_t bytes, int32_t copy_bytes, int32_t n_ctas) {
+    if (!src_dev || ((uintptr_t)src_dev & 127) != 0 || n_ctas <= 0 || copy_bytes < 16 || copy_bytes > 65536 || (copy_bytes & (copy_bytes - 1)) != 0 ||
+        bytes / 65536 / (size_t)n_ctas == 0)
+        return fail(HQ_ERR_INVALID_ARG, "hq_debug_copy_probe: needs a 128-byte aligned buffer of >= 64 KB per CTA and a power-of-two copy size in [16, 65536]");
+    HQ_CUDA(launch_copy_probe((cudaStream_t)cuda_stream, src_dev, bytes, copy_bytes, n_ctas));
+    return HQ_OK;
+}
+
 extern "C" int32_t hq_debug_kv_row(hq_model *m, int32_t which, int32_t layer, int32_t seq, int32_t pos, void *row_dev) {
     if (!m || !row_dev) return fail(HQ_ERR_INVALID_ARG, "hq_debug_kv_row: NULL argument");
     HQ_ON_DEVICE(m);

@@ -236,6 +236,7 @@ cudaError_t launch_argmax_rows(const LaunchCtx &c, const float *logits, int voca
 
 // ---- read-only streaming probe (hq_probe.cu) --------------------------------------------------------
 cudaError_t launch_read_probe(cudaStream_t stream, const void *src, size_t bytes, unsigned int *out, int n_sms);
+cudaError_t launch_copy_probe(cudaStream_t stream, const void *src, size_t bytes, int copy_bytes, int n_ctas);
 
 // ---- launchers (hq_decode.cu) ------------------------------------------------------------------------
 cudaError_t launch_embed(const LaunchCtx &c, const bf16 *emb, const int *tok, float *x, int hidden, int batch);

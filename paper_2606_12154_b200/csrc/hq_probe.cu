@@ -32,4 +32,49 @@ cudaError_t launch_read_probe(cudaStream_t stream, const void *src, size_t bytes
     return cudaGetLastError();
 }
 
+// ---- bulk-copy size probe ---------------------------------------------------------------------------------------------
+// What one SM pulls from HBM through cp.async.bulk as a function of the size of the individual copy: n_ctas CTAs (one per
+// SM) each stream their share of the buffer through a ring of 3 x 64 KB stages, a stage being 64 KB / copy_bytes copies
+// issued by 16 lanes; nothing is computed (a consumer thread releases every stage as soon as it has landed).  This is the
+// measurement behind "one copy per stage" in hq_stream.cu / hq_attn.cu (profiles/r02_copy_size.md).
+constexpr int kCpStages = 3, kCpStageBytes = 65536;
+__global__ void __launch_bounds__(64, 1) copy_probe_kernel(const uint8_t *__restrict__ src, size_t bytes, int copy_bytes) {
+    extern __shared__ __align__(128) uint8_t cp_smem[];
+    __shared__ uint64_t full[kCpStages], empty[kCpStages];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < kCpStages; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
+        mbar_fence_init();
+    }
+    __syncthreads();
+    const size_t n_stages = bytes / kCpStageBytes / gridDim.x;
+    const uint8_t *base = src + (size_t)blockIdx.x * n_stages * kCpStageBytes;
+    const int per_stage = kCpStageBytes / copy_bytes;
+    if (warp == 0) {
+        const uint64_t pol = l2_policy_evict_first();
+        for (size_t n = 0; n < n_stages; ++n) {
+            const int slot = (int)(n % kCpStages);
+            while (!mbar_try_wait(&empty[slot], (uint32_t)(((n / kCpStages) & 1) ^ 1))) {}
+            if (lane == 0) mbar_expect_tx(&full[slot], kCpStageBytes);
+            __syncwarp();
+            for (int c = lane; c < per_stage; c += 32)
+                bulk_g2s_hint(cp_smem + (size_t)slot * kCpStageBytes + (size_t)c * copy_bytes,
+                              base + n * kCpStageBytes + (size_t)c * copy_bytes, (uint32_t)copy_bytes, &full[slot], pol);
+        }
+    } else if (lane == 0) {
+        for (size_t n = 0; n < n_stages; ++n) {
+            const int slot = (int)(n % kCpStages);
+            while (!mbar_try_wait(&full[slot], (uint32_t)((n / kCpStages) & 1))) {}
+            mbar_arrive(&empty[slot]);
+        }
+    }
+}
+
+cudaError_t launch_copy_probe(cudaStream_t stream, const void *src, size_t bytes, int copy_bytes, int n_ctas) {
+    cudaError_t e = cudaFuncSetAttribute(copy_probe_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kCpStages * kCpStageBytes);
+    if (e != cudaSuccess) return e;
+    copy_probe_kernel<<<n_ctas, 64, kCpStages * kCpStageBytes, stream>>>(static_cast<const uint8_t *>(src), bytes, copy_bytes);
+    return cudaGetLastError();
+}
+
 }  // namespace hq
