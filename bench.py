@@ -216,6 +216,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg")
     ap.add_argument("--sweep", action="store_true",
                     help="configs[4]: batch {1,4,16,32} x context {512,4096}, 128 decode steps each; one JSON line per point")
+    ap.add_argument("--window-sweep", action="store_true",
+                    help="PAPER.md:L170 (section 6.6): context WINDOW 4,096 -> 131,072 with the configs[1] query; one JSON line per window")
     ap.add_argument("--probes", action="store_true",
                     help="memory-system probes behind the kernel design: bulk-copy size vs per-SM rate, read-only stream; JSON lines")
     ap.add_argument("--profile", type=int, default=0, metavar="N",
@@ -306,6 +308,43 @@ def main():
                 m.close()
                 del m
                 torch.cuda.empty_cache()
+        return
+
+    if args.window_sweep:
+        # "Context length is free": the window (KV capacity, max_seq) grows 32x, the USED context stays the
+        # configs[1] query (256-token envelope + 128 tokens); decode rate and TTFT must stay flat, memory grows by 32 KiB per
+        # window position (the paper's 4-bit laptop setup: ~22 MiB per 1k positions)
+        lay = gm.weight_tensors()
+        for window in (4096, 8192, 16384, 32768, 65536, 131072):
+            cfg = hq.binding.make_config(n_layers=s.n_layers, hidden=s.hidden, n_heads=s.n_heads, n_kv_heads=s.n_kv_heads,
+                                         head_dim=s.head_dim, ffn=s.ffn, vocab=s.vocab, rms_eps=s.rms_eps,
+                                         rope_theta=s.rope_theta, max_batch=1, max_seq=window, flags=0)
+            m = hq.Model(cfg, *lay)
+            dec, pf = [], []
+            sampler = ClockSampler(local_rank)
+            sampler.start()
+            for it in range(5):
+                m.kv_reset()
+                a, b, c2 = ev(), ev(), ev()
+                a.record(m.stream)
+                m.prefill(prompt, want_token=False)
+                b.record(m.stream)
+                m.decode_run(DECODE_STEPS, want_tokens=False)
+                c2.record(m.stream)
+                torch.cuda.synchronize(dev)
+                if it >= 2:
+                    pf.append(a.elapsed_time(b))
+                    dec.append(b.elapsed_time(c2))
+            clk = sampler.stop()
+            ws = hq.workspace_bytes(cfg)
+            kv_bytes = 2 * s.n_layers * s.n_kv_heads * s.head_dim * 2 * window
+            print(json.dumps({"window_sweep": True, "window": window, "tokens_per_s": DECODE_STEPS / (float(np.mean(dec)) * 1e-3),
+                              "ttft_ms": float(np.mean(pf)), "workspace_MiB": ws / 2 ** 20, "kv_cache_MiB": kv_bytes / 2 ** 20,
+                              "kv_MiB_per_1k_positions": kv_bytes / 2 ** 20 / (window / 1024), "decode_path": m.decode_path(),
+                              "clocks": clk}), flush=True)
+            m.close()
+            del m
+            torch.cuda.empty_cache()
         return
 
     if args.probes:

@@ -50,6 +50,7 @@ enum {
     HQ_FLAG_CAPTURE_HIDDEN = 1u, /* keep the residual stream after every layer (parity tests) */
     HQ_FLAG_NO_GRAPH = 2u,       /* launch decode kernels directly instead of replaying a CUDA graph */
     HQ_FLAG_NO_PDL = 4u,         /* no programmatic dependent launch edges between kernels */
+    HQ_FLAG_VERIFY = 16u,        /* reserve workspace for hq_verify_relay: fp32 logits of 256 positions (vocab * 1 KiB) */
     HQ_FLAG_KERNEL_PER_ROW = 8u  /* batch-1 decode with one kernel per row of SURVEY.md 8(a) (QKV, attention, O as three
                                     launches) instead of the cluster attention block; also what a device that cannot keep
                                     all the block's clusters resident falls back to */
@@ -134,6 +135,22 @@ int32_t hq_decode_step(hq_model *m, const int32_t *tokens_in_host, int32_t *toke
  * them): the "decode rate" of PAPER.md:L109-111 (section 6.2) is this call's tokens per second.
  * tokens_out_host: HOST int32 [n_steps][batch] or NULL (asynchronous). */
 int32_t hq_decode_run(hq_model *m, int32_t n_steps, int32_t *tokens_out_host);
+
+/* Verbatim-relay verification in one dense pass.  The paper's renderer LOCKS the answer line before
+ * the mouth speaks it ("the factual content is locked by the renderer, and the small model's job is
+ * delivery") and its section 6.4 measures whether the mouth then repeats the line verbatim.  Since
+ * the expected tokens are known in advance, one prefill-style pass over envelope + answer scores every answer position at
+ * once (tensor-core GEMMs, weights read once) instead of one decode step per token; speculative decoding is the related
+ * work the paper cites.  The call is not in the paper.
+ *   tokens_host      HOST int32 [n_envelope + n_answer]: the rendered envelope, then the answer line; ONE sequence,
+ *                    appended at seq_len; n_answer <= 255, n_envelope + n_answer <= 2,048
+ *   n_accepted_host  HOST int32: how many leading answer tokens the greedy argmax reproduces (0 .. n_answer); synchronises
+ * On return the cache holds envelope + accepted tokens (seq_len += n_envelope + n_accepted) and the device-resident
+ * "last emitted token" is the model's own greedy choice at the first mismatch (after the whole answer when everything
+ * matched), so hq_decode_step(m, NULL, ...) streams on from there and hq_decode_logits returns the logits that chose it.
+ * Needs HQ_FLAG_VERIFY (HQ_ERR_STATE otherwise). */
+int32_t hq_verify_relay(hq_model *m, const int32_t *tokens_host, int32_t n_envelope, int32_t n_answer,
+                        int32_t *n_accepted_host);
 
 /* Parity (north_star: "relative L2 <= 1e-2 per-layer hidden state, <= 2e-2 on logits" against the oracle).
  * logits_dev: DEVICE fp32 [batch][vocab] <- logits of the last prefill/step.

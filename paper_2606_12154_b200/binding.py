@@ -17,6 +17,7 @@ FLAG_CAPTURE_HIDDEN = 1
 FLAG_NO_GRAPH = 2
 FLAG_NO_PDL = 4
 FLAG_KERNEL_PER_ROW = 8
+FLAG_VERIFY = 16
 
 HQ_OK, HQ_ERR_INVALID_ARG, HQ_ERR_CAPACITY, HQ_ERR_STATE, HQ_ERR_CUDA, HQ_ERR_UNSUPPORTED = 0, -1, -2, -3, -4, -5
 _CODE_NAMES = {-1: "HQ_ERR_INVALID_ARG", -2: "HQ_ERR_CAPACITY", -3: "HQ_ERR_STATE", -4: "HQ_ERR_CUDA",
@@ -25,7 +26,7 @@ _CODE_NAMES = {-1: "HQ_ERR_INVALID_ARG", -2: "HQ_ERR_CAPACITY", -3: "HQ_ERR_STAT
 # every symbol include/hq.h and include/hq_debug.h declare (tests check the headers and the library against this list)
 DECLARED_SYMBOLS = (
     "hq_workspace_bytes", "hq_model_create", "hq_model_destroy", "hq_prefill", "hq_decode_step",
-    "hq_decode_run", "hq_decode_logits", "hq_get_hidden", "hq_sync", "hq_seq_len", "hq_kv_reset",
+    "hq_decode_run", "hq_verify_relay", "hq_decode_logits", "hq_get_hidden", "hq_sync", "hq_seq_len", "hq_kv_reset",
     "hq_kernel_count", "hq_decode_path", "hq_bench_kernel", "hq_debug_copy_probe", "hq_debug_gemm", "hq_debug_kv_row", "hq_debug_read_probe", "hq_debug_step_trace", "hq_debug_trace", "hq_last_error",
     "hq_version",
 )
@@ -81,6 +82,8 @@ def load_library(path: Optional[str] = None):
     l.hq_decode_step.argtypes = [vp, vp, vp]
     l.hq_decode_run.restype = i32
     l.hq_decode_run.argtypes = [vp, i32, vp]
+    l.hq_verify_relay.restype = i32
+    l.hq_verify_relay.argtypes = [vp, vp, i32, i32, vp]
     l.hq_decode_logits.restype = i32
     l.hq_decode_logits.argtypes = [vp, vp]
     l.hq_get_hidden.restype = i32
@@ -245,6 +248,15 @@ class Model:
         out = np.empty((n_steps, batch), dtype=np.int32) if want_tokens else None
         _check(self._lib.hq_decode_run(self._h, n_steps, out.ctypes.data if want_tokens else None))
         return out
+
+    def verify_relay(self, envelope, answer) -> int:
+        """hq_verify_relay: envelope and answer token arrays on the HOST; returns the number of accepted answer tokens."""
+        env = np.ascontiguousarray(envelope, dtype=np.int32).reshape(-1)
+        ans = np.ascontiguousarray(answer, dtype=np.int32).reshape(-1)
+        toks = np.concatenate([env, ans])
+        out = ctypes.c_int32()
+        _check(self._lib.hq_verify_relay(self._h, toks.ctypes.data, env.size, ans.size, ctypes.byref(out)))
+        return out.value
 
     def decode_logits(self, batch: int = 1):
         t = self._torch.empty((batch, self.vocab), dtype=self._torch.float32, device=self.device)

@@ -118,6 +118,10 @@ static size_t carve(const hq_config *c, char *base, Buffers *b) {
     o.actb = (act_t *)take(2 * R * F * sizeof(act_t));
     o.hn_last = (act_t *)take(2 * 32 * d * sizeof(act_t));
     o.err = (int *)take(sizeof(int));
+    const bool verify = (c->flags & HQ_FLAG_VERIFY) != 0;
+    o.verify_logits = (float *)take(verify ? (size_t)kVerifyRows * V * sizeof(float) : 0);
+    o.verify_best = (unsigned long long *)take(verify ? kVerifyRows * sizeof(unsigned long long) : 0);
+    o.verify_out = (int *)take(sizeof(int));
     o.ab_ll = (unsigned long long *)take((size_t)H * kHeadDim * sizeof(unsigned long long));
     o.ab_epoch = (unsigned int *)take(sizeof(unsigned int));
     return off;
@@ -518,6 +522,8 @@ extern "C" int32_t hq_model_create(const hq_config *cfg, const hq_weights *w, vo
         const unsigned int one = 1u;
         cudaError_t e = cudaMemsetAsync(m->b.ab_ll, 0, (size_t)cfg->n_heads * kHeadDim * sizeof(unsigned long long), m->stream);
         if (e == cudaSuccess) e = cudaMemcpyAsync(m->b.ab_epoch, &one, sizeof(one), cudaMemcpyHostToDevice, m->stream);
+        if (e == cudaSuccess && (cfg->flags & HQ_FLAG_VERIFY))
+            e = cudaMemsetAsync(m->b.verify_best, 0, kVerifyRows * sizeof(unsigned long long), m->stream);
         if (e == cudaSuccess) e = cudaStreamSynchronize(m->stream);
         if (e != cudaSuccess) {
             delete m;
@@ -667,6 +673,59 @@ extern "C" int32_t hq_prefill(hq_model *m, const int32_t *tokens_host, int32_t b
         HQ_CUDA(cudaMemcpyAsync(first_token_host, m->b.cur_tok, batch * sizeof(int), cudaMemcpyDeviceToHost, m->stream));
         HQ_CUDA(cudaStreamSynchronize(m->stream));
     }
+    return HQ_OK;
+}
+
+// ---- verbatim-relay verification in one dense pass -------------------------------------------
+extern "C" int32_t hq_verify_relay(hq_model *m, const int32_t *tokens_host, int32_t n_envelope, int32_t n_answer,
+                                   int32_t *n_accepted_host) {
+    if (!m || !tokens_host || !n_accepted_host) return fail(HQ_ERR_INVALID_ARG, "hq_verify_relay: NULL argument");
+    HQ_ON_DEVICE(m);
+    const hq_config &c = m->cfg;
+    if (!(c.flags & HQ_FLAG_VERIFY)) return fail(HQ_ERR_STATE, "hq_verify_relay: model created without HQ_FLAG_VERIFY");
+    if (n_envelope <= 0 || n_answer <= 0) return fail(HQ_ERR_INVALID_ARG, "hq_verify_relay: n_envelope and n_answer must be > 0");
+    if (m->batch > 1) return fail(HQ_ERR_STATE, "hq_verify_relay: one sequence only (active batch is %d)", m->batch);
+    const int T = n_envelope + n_answer, nv = n_answer + 1;
+    if (nv > kVerifyRows) return fail(HQ_ERR_CAPACITY, "hq_verify_relay: n_answer %d > %d", n_answer, kVerifyRows - 1);
+    if (T > m->pf_rows) return fail(HQ_ERR_CAPACITY, "hq_verify_relay: %d tokens > %d rows of one pass", T, m->pf_rows);
+    if ((long long)m->seq_len + T > c.max_seq)
+        return fail(HQ_ERR_CAPACITY, "hq_verify_relay: seq_len %d + %d tokens > max_seq %d", m->seq_len, T, c.max_seq);
+    for (int i = 0; i < T; ++i)
+        if (tokens_host[i] < 0 || tokens_host[i] >= c.vocab)
+            return fail(HQ_ERR_INVALID_ARG, "hq_verify_relay: token %d at index %d outside [0, %d)", tokens_host[i], i, c.vocab);
+    const LaunchCtx lc{m->stream, m->use_pdl, m->n_sms};
+    const Buffers &b = m->b;
+    const int d = c.hidden;
+    // one tensor-core pass over envelope + answer (the cache rows of the answer are written speculatively: rows beyond the
+    // accepted prefix are simply never read, the position decides what is cached)
+    HQ_CUDA(cudaMemcpyAsync(b.pf_tok, tokens_host, (size_t)T * sizeof(int), cudaMemcpyHostToDevice, m->stream));
+    int n = 0;
+    HQ_CUDA(launch_embed_rows(lc, m->emb, b.pf_tok, b.xs, d, T));
+    ++n;
+    HQ_CUDA(enqueue_rows_layers(m, 1, T, false, false, &n));
+    // LM head at the n_answer + 1 positions n_envelope - 1 .. T - 1: final norm (folds the deferred residual of the last
+    // layer in) -> one GEMM over the vocabulary (weights read once per 256-token tile) -> per-row argmax against the answer
+    const int r0 = n_envelope - 1;
+    HQ_CUDA(launch_rmsnorm_rows(lc, b.xs + (size_t)r0 * d, b.delta + (size_t)r0 * d, m->final_norm, b.hn, (size_t)m->pf_rows * d, d,
+                                c.rms_eps, nv, nullptr, d));
+    const TilePlan pv = plan_gemm(m, c.vocab, nv, d, 1);
+    HQ_CUDA(launch_gemm(lc, EPI_STORE, m->map_lm_head, nullptr, m->map_hn[pv.ti], m->pf_rows, c.vocab, d, nv, pv.NT, 1,
+                        b.verify_logits, nullptr, 0, c.vocab));
+    HQ_CUDA(launch_verify_rows(lc, b.verify_logits, c.vocab, nv, b.pf_tok + n_envelope, n_envelope, b.cur_tok, b.tok_hist, b.pos,
+                               b.counter, b.verify_best, b.verify_out));
+    m->kernel_count += n + 3;
+    int accepted = 0;
+    HQ_CUDA(cudaMemcpyAsync(&accepted, b.verify_out, sizeof(int), cudaMemcpyDeviceToHost, m->stream));
+    HQ_CUDA(cudaStreamSynchronize(m->stream));
+    // the rows of the pass that were not consumed by the final norm still carry a deferred residual: clear it for the next pass
+    HQ_CUDA(cudaMemsetAsync(b.delta, 0, (size_t)T * d * sizeof(float), m->stream));
+    // hq_decode_logits: the logits that chose the token now waiting to be fed
+    HQ_CUDA(cudaMemcpyAsync(b.logits, b.verify_logits + (size_t)accepted * c.vocab, (size_t)c.vocab * sizeof(float),
+                            cudaMemcpyDeviceToDevice, m->stream));
+    m->batch = 1;
+    m->seq_len += n_envelope + accepted;
+    m->have_token = true;
+    *n_accepted_host = accepted;
     return HQ_OK;
 }
 

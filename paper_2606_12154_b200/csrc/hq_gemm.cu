@@ -114,8 +114,13 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap map_w, const __grid_constant_
     const int kb0 = blockIdx.z * p.k_blocks_per_split;
     const int kb1 = min(kb0 + p.k_blocks_per_split, p.k_blocks);
     const int nkb = kb1 - kb0;
-    const uint32_t tmem_cols = (NACC * NT <= 32) ? 32 : (NACC * NT <= 64) ? 64 : (NACC * NT <= 128) ? 128
-                               : (NACC * NT <= 256) ? 256 : 512;
+    // NT <= 128: the hi and lo activation planes of a stage lie back to back and are ONE B operand of 2 NT rows: one MMA per
+    // K step fills D columns [0, NT) with W x_hi and [NT, 2 NT) with W x_lo (half the MMA instructions, a quarter less
+    // operand traffic from shared memory than two MMAs into the same columns); the epilogue adds the two halves
+    const bool stacked = NT <= 128;
+    const int acc_cols = stacked ? 2 * NT : NT;          // TMEM columns of one accumulator
+    const uint32_t need_cols = (uint32_t)(NACC * acc_cols);
+    const uint32_t tmem_cols = need_cols <= 32 ? 32 : need_cols <= 64 ? 64 : need_cols <= 128 ? 128 : need_cols <= 256 ? 256 : 512;
 
     if (warp == 0 && lane == 0) {
         asm volatile("prefetch.tensormap [%0];" ::"l"(&map_w) : "memory");
@@ -178,7 +183,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap map_w, const __grid_constant_
     } else if (warp == 1) {
         // ===== MMA issuer (one elected thread) =====
         if (lane == 0) {
-            const uint32_t idesc = make_idesc(NT);
+            const uint32_t idesc = make_idesc(stacked ? 2 * NT : NT);
             for (int i = 0; i < nkb; ++i) {
                 const int s = i % stages;
                 const uint32_t ph = (i / stages) & 1;
@@ -192,11 +197,16 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap map_w, const __grid_constant_
                 for (int k = 0; k < kBlockK / 16; ++k) {
                     const uint32_t acc = (i > 0 || k > 0) ? 1u : 0u;
                     // advance 16 elements = 32 bytes inside the 128-byte swizzle row: +2 in the >>4 address field
-                    umma_bf16(tmem_base, da + 2 * k, db + 2 * k, idesc, acc);       // W * x_hi
-                    umma_bf16(tmem_base, da + 2 * k, dbl + 2 * k, idesc, 1u);       // W * x_lo
-                    if (NACC == 2) {
-                        umma_bf16(tmem_base + NT, da2 + 2 * k, db + 2 * k, idesc, acc);
-                        umma_bf16(tmem_base + NT, da2 + 2 * k, dbl + 2 * k, idesc, 1u);
+                    if (stacked) {
+                        umma_bf16(tmem_base, da + 2 * k, db + 2 * k, idesc, acc);       // W * [x_hi ; x_lo]
+                        if (NACC == 2) umma_bf16(tmem_base + acc_cols, da2 + 2 * k, db + 2 * k, idesc, acc);
+                    } else {
+                        umma_bf16(tmem_base, da + 2 * k, db + 2 * k, idesc, acc);       // W * x_hi
+                        umma_bf16(tmem_base, da + 2 * k, dbl + 2 * k, idesc, 1u);       // W * x_lo
+                        if (NACC == 2) {
+                            umma_bf16(tmem_base + acc_cols, da2 + 2 * k, db + 2 * k, idesc, acc);
+                            umma_bf16(tmem_base + acc_cols, da2 + 2 * k, dbl + 2 * k, idesc, 1u);
+                        }
                     }
                 }
                 tcgen05_commit(&empty_bar[s]);   // frees the smem stage when these MMAs retire
@@ -215,9 +225,21 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap map_w, const __grid_constant_
         for (int c = 0; c < NT; c += 32) {
             uint32_t v[32];
             tmem_ld32(lane_addr + c, v);
+            if (stacked) {
+                uint32_t w[32];
+                tmem_ld32(lane_addr + NT + c, w);
+#pragma unroll
+                for (int j = 0; j < 32; ++j) v[j] = __float_as_uint(__uint_as_float(v[j]) + __uint_as_float(w[j]));
+            }
             if (MODE == EPI_SWIGLU) {
                 uint32_t u[32];
-                tmem_ld32(lane_addr + NT + c, u);
+                tmem_ld32(lane_addr + acc_cols + c, u);
+                if (stacked) {
+                    uint32_t w[32];
+                    tmem_ld32(lane_addr + acc_cols + NT + c, w);
+#pragma unroll
+                    for (int j = 0; j < 32; ++j) u[j] = __float_as_uint(__uint_as_float(u[j]) + __uint_as_float(w[j]));
+                }
                 if (row_ok) {
 #pragma unroll
                     for (int j = 0; j < 32; ++j) {

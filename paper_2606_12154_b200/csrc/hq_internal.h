@@ -30,6 +30,7 @@ constexpr int kHeadDim = 64;        // only head_dim the kernels implement
 constexpr int kMaxSplits = 16;      // split-KV partials per head (decode attention)
 constexpr int kMinSplitLen = 64;    // do not split contexts shorter than this per split
 constexpr int kGemvThreads = 256;
+constexpr int kVerifyRows = 256;    // answer tokens + 1 of one hq_verify_relay call (the paper's rule: answer lines of at most ~230 tokens)
 struct alignas(64) TensorMap { uint64_t opaque[16]; };   // mirrors CUtensorMap (driver type, 128 bytes)
 
 struct LayerW {
@@ -65,6 +66,10 @@ struct Buffers {
     act_t *ao = nullptr;                        // [2][pf_rows][H*64] attention output (GEMM operand, hi/lo)
     act_t *actb = nullptr;                      // [2][pf_rows][F] SwiGLU output (GEMM operand, hi/lo)
     act_t *hn_last = nullptr;                   // [2][32][d] normalised last rows (LM-head operand, hi/lo)
+    // verbatim-relay verification (HQ_FLAG_VERIFY)
+    float *verify_logits = nullptr;             // [kVerifyRows][V]
+    unsigned long long *verify_best = nullptr;  // [kVerifyRows] packed argmax per row
+    int *verify_out = nullptr;                  // accepted answer tokens
     int *err = nullptr;                         // device error flag (a lost cluster arrival / tagged word traps instead of hanging)
     unsigned long long *ab_ll = nullptr;        // attention block: tagged words of the attention vector [H * 64] (zeroed at create)
     unsigned int *ab_epoch = nullptr;           // attention block: tag of the next launch (starts at 1, never reset)
@@ -231,6 +236,9 @@ cudaError_t launch_flash_prefill(const LaunchCtx &c, const __half *q16, const kv
                                  size_t lo_offset, const int *pos, int batch, int Tc, int n_heads, int n_kv_heads, int max_seq);
 cudaError_t launch_attn_combine(const LaunchCtx &c, const float *part_o, const float2 *part_ml, act_t *out,
                                 size_t lo_offset, const int *pos, int batch, int n_heads);
+cudaError_t launch_verify_rows(const LaunchCtx &c, const float *logits, int vocab, int n_rows, const int *answer, int n_envelope,
+                               int *cur_tok, int *tok_hist, int *pos, unsigned int *counter, unsigned long long *best_rows,
+                               int *n_accepted);
 cudaError_t launch_argmax_rows(const LaunchCtx &c, const float *logits, int vocab, int batch, int *cur_tok,
                                int *tok_hist, int *pos, int pos_inc, unsigned int *counter, unsigned long long *best_rows);
 

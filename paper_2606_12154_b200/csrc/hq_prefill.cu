@@ -405,6 +405,61 @@ __global__ void __launch_bounds__(256) argmax_rows_kernel(const float *logits, i
     }
 }
 
+// =====================================================================================================
+// Verbatim-relay verification: row j of logits [n_rows][vocab] is the LM head at the position that
+// predicts answer token j (row n_answer = n_rows - 1: the token after the whole answer).  grid (slices, n_rows): per-slice
+// winner -> packed atomicMax per row; the last CTA counts the leading rows whose greedy token equals the answer token,
+// publishes the count, and leaves the step state as if envelope + accepted answer tokens had been fed: position,
+// and as "last emitted token" the model's own choice at the first mismatch (streaming decode continues from there).
+// =====================================================================================================
+__global__ void __launch_bounds__(256) verify_rows_kernel(const float *logits, int vocab, int n_rows, const int *answer,
+                                                          int n_envelope, int *cur_tok, int *tok_hist, int *pos,
+                                                          unsigned int *counter, unsigned long long *best_rows,
+                                                          int *n_accepted) {
+    pdl_launch_dependents();
+    pdl_wait();
+    __shared__ unsigned long long red[8];
+    __shared__ int last;
+    const int b = blockIdx.y;
+    const float *row = logits + (size_t)b * vocab;
+    const int per = ((vocab + (int)gridDim.x - 1) / (int)gridDim.x + 3) & ~3;
+    const int i0 = blockIdx.x * per, i1 = min(vocab, i0 + per);
+    unsigned long long best = 0ull;
+    for (int i = i0 + threadIdx.x; i < i1; i += blockDim.x) {
+        const unsigned long long k = pack_argmax(ld_act(row + i), i);
+        best = best > k ? best : k;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        const unsigned long long other = __shfl_xor_sync(0xffffffffu, best, o);
+        best = best > other ? best : other;
+    }
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = best;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int w = 1; w < 8; ++w) best = best > red[w] ? best : red[w];
+        if (best) atomicMax(best_rows + b, best);   // packed (ordered logit, ~index): lowest index wins ties
+        __threadfence();
+        const unsigned int ticket = atomicAdd(counter, 1u);
+        last = ticket == gridDim.x * gridDim.y - 1u;
+    }
+    __syncthreads();
+    if (last && threadIdx.x == 0) {   // every row's winner is final
+        __threadfence();
+        int j = 0;
+        while (j < n_rows - 1 && unpack_argmax_idx(__ldcg(best_rows + j)) == ld_act(answer + j)) ++j;
+        const int tok = unpack_argmax_idx(__ldcg(best_rows + j));
+        const int p = ld_act(pos) + n_envelope + j;
+        *n_accepted = j;
+        *cur_tok = tok;
+        tok_hist[p] = tok;
+        *pos = p;
+        for (int r = 0; r < n_rows; ++r) best_rows[r] = 0ull;
+        *counter = 0u;
+    }
+}
+
 // ---- launchers ------------------------------------------------------------------------------------------
 template <typename... KArgs, typename... Args>
 static cudaError_t launch_k(const LaunchCtx &c, void (*kernel)(KArgs...), dim3 grid, dim3 block, Args... args) {
@@ -458,6 +513,13 @@ cudaError_t launch_flash_prefill(const LaunchCtx &c, const __half *q16, const kv
 cudaError_t launch_attn_combine(const LaunchCtx &c, const float *part_o, const float2 *part_ml, act_t *out,
                                 size_t lo_offset, const int *pos, int batch, int n_heads) {
     return launch_k(c, attn_combine_kernel, dim3(batch), dim3(256), part_o, part_ml, out, lo_offset, pos, n_heads);
+}
+cudaError_t launch_verify_rows(const LaunchCtx &c, const float *logits, int vocab, int n_rows, const int *answer, int n_envelope,
+                               int *cur_tok, int *tok_hist, int *pos, unsigned int *counter, unsigned long long *best_rows,
+                               int *n_accepted) {
+    const int slices = vocab >= 32768 ? 16 : (vocab >= 4096 ? 4 : 1);
+    return launch_k(c, verify_rows_kernel, dim3(slices, n_rows), dim3(256), logits, vocab, n_rows, answer, n_envelope, cur_tok,
+                    tok_hist, pos, counter, best_rows, n_accepted);
 }
 cudaError_t launch_argmax_rows(const LaunchCtx &c, const float *logits, int vocab, int batch, int *cur_tok,
                                int *tok_hist, int *pos, int pos_inc, unsigned int *counter, unsigned long long *best_rows) {

@@ -332,6 +332,50 @@ def test_1b_config1_teacher_forced(one_b_weights, ref_config1, path):
 
 
 @pytest.mark.parametrize("path", PATHS)
+def test_1b_window_131072(one_b_weights, ref_config1, path):
+    """PAPER.md:L170 (section 6.6, "context length is free"): the largest window of the paper's sweep, 131,072 positions
+    (4 GiB of KV cache, a 32 MiB RoPE table), with the configs[1] query in it: same tolerances, first 16 decode steps."""
+    ref = dict(ref_config1)
+    ref["n_steps"] = 16
+    ref["sampled"] = {i: v for i, v in ref_config1["sampled"].items() if i <= 16}
+    gm = gpu_model(one_b_weights, max_seq=131072, path=path)
+    stats = {"argmax_checked": 0, "positions": 0}
+    tok = gm.prefill(ref["prompt"])
+    for i in range(17):
+        if i:
+            tok = gm.decode_step(tokens_in=[int(ref["tokens"][i - 1])])
+        if i in ref["sampled"]:
+            check_position(gm, ref["sampled"][i][0], ref["sampled"][i][1], f"step {i}", stats)
+            stats["positions"] += 1
+        if ref["margins"][i] > MARGIN:
+            assert int(tok[0]) == int(ref["tokens"][i])
+            stats["argmax_checked"] += 1
+    check_kv_rows(gm, ref_config1["om"], (0, 255, 256, 270), stats)
+    assert gm.seq_len() == 256 + 16 and stats["positions"] == 3
+    print("1b window 131,072 parity:", stats)
+
+
+def test_tiny_window_131072_high_positions(tiny_weights):
+    """Positions deep inside a 131,072 window: the tiny model's oracle walks 9,000 positions (RoPE angles up to 9,000 rad
+    at theta = 1e4), the GPU prefills them in 2,048-row passes and decodes at positions 9,000+ (kernel-per-row and
+    attention block: 1,126 cached positions per cluster CTA, 5 ring tiles)."""
+    n = 9000
+    toks = datagen.tokens(4244, datagen.TINY.vocab, n + 4)
+    om = oracle.Model.from_datagen(tiny_weights, max_seq=n + 8)
+    hid, lg = om.forward(toks, hidden="all", logits="all")
+    for path in (0, KERNEL_PER_ROW):
+        gm = gpu_model(tiny_weights, max_seq=131072, path=path)
+        gm.prefill(toks[:n])
+        stats = {}
+        check_position(gm, hid[n - 1], lg[n - 1], "prefill", stats)
+        for j in range(3):
+            gm.decode_step(tokens_in=[int(toks[n + j])])
+            check_position(gm, hid[n + j], lg[n + j], f"decode at position {n + j}", stats)
+        check_kv_rows(gm, om, (0, 4095, 8999, 9000, 9002), stats)
+        print("tiny window 131,072, positions 9,000+:", stats)
+
+
+@pytest.mark.parametrize("path", PATHS)
 def test_1b_config2_long_context(one_b_weights, ref_config2, path):
     """configs[2] at full size and full length: 2,048-token prompt (one tensor-core pass, causal flash attention over
     32 query tiles), then all 256 teacher-forced decode steps at contexts 2,049..2,304 — the attention block streams
@@ -529,3 +573,75 @@ def test_large_magnitude_activations(tiny_weights):
             lg = gm.decode_logits()[0].cpu().numpy()
             assert np.isfinite(lg).all()
             assert rel_l2(lg, ref["logits"][i]) <= TOL_LOGITS, (path, i, rel_l2(lg, ref["logits"][i]))
+
+
+# ---------------------------------------------------------------------------------------------------
+# verbatim-relay verification in one dense pass (hq_verify_relay)
+# ---------------------------------------------------------------------------------------------------
+def test_tiny_verify_relay(tiny_weights):
+    """The oracle's own greedy continuation is the 'answer line': one dense pass accepts all of it; a corrupted token
+    stops the acceptance exactly there, and streaming decode continues from the model's own token.  Envelope seed 2003:
+    every oracle margin of the continuation is > 0.6, so the argmax decisions are not rounding-sensitive."""
+    import paper_2606_12154_b200 as hq
+    V = datagen.TINY.vocab
+    env = datagen.tokens(2003, V, 24)
+    om = oracle.Model.from_datagen(tiny_weights, max_seq=64)
+    ref = om.greedy(env, 20)
+    assert ref["margins"].min() > MARGIN
+    answer = ref["tokens"][:16]
+    for path in (0, KERNEL_PER_ROW):
+        gm = gpu_model(tiny_weights, max_seq=64, flags=hq.FLAG_CAPTURE_HIDDEN | hq.FLAG_VERIFY, path=path)
+        # (a) everything accepted; the waiting token is the model's choice after the whole answer
+        assert gm.verify_relay(env, answer) == 16
+        assert gm.seq_len() == 24 + 16
+        lg = gm.decode_logits()[0].cpu().numpy()
+        assert rel_l2(lg, ref["logits"][16]) <= TOL_LOGITS and max_abs(lg, ref["logits"][16]) <= MAXABS_LOGIT
+        assert int(gm.decode_step()[0]) == int(ref["tokens"][17]) and int(gm.decode_step()[0]) == int(ref["tokens"][18])
+        # (b) a wrong token at answer position 5: five accepted, streaming resumes with the model's own token 5
+        bad = answer.copy()
+        bad[5] = (bad[5] + 1) % V
+        gm.kv_reset()
+        assert gm.verify_relay(env, bad) == 5
+        assert gm.seq_len() == 24 + 5
+        lg = gm.decode_logits()[0].cpu().numpy()
+        assert rel_l2(lg, ref["logits"][5]) <= TOL_LOGITS
+        out = [int(gm.decode_step()[0]) for _ in range(4)]
+        assert out == [int(t) for t in ref["tokens"][6:10]], (out, ref["tokens"][6:10])
+        assert gm.seq_len() == 24 + 5 + 4
+        # (c) appended to a cache that already holds the head of the envelope (chunked), first token wrong -> 0 accepted
+        gm.kv_reset()
+        gm.prefill(env[:10])
+        bad0 = answer.copy()
+        bad0[0] = (bad0[0] + 7) % V
+        assert gm.verify_relay(env[10:], bad0) == 0 and gm.seq_len() == 24
+        assert int(gm.decode_step()[0]) == int(ref["tokens"][1])
+        # the cached rows of envelope + accepted prefix are the oracle's
+        check_kv_rows(gm, om, (0, 9, 10, 23, 24), {})
+    with pytest.raises(hq.HQError) as e:
+        gpu_model(tiny_weights, max_seq=64).verify_relay(env, answer)
+    assert e.value.code == -3          # model created without HQ_FLAG_VERIFY
+
+
+def test_1b_verify_relay(one_b_weights, ref_config1):
+    """configs[1] shape: 256-token envelope + the oracle's first 100 greedy tokens as the answer line, verified in one
+    dense pass (356 rows through the tcgen05 GEMMs, LM head over 101 positions)."""
+    import paper_2606_12154_b200 as hq
+    ref = ref_config1
+    answer = ref["tokens"][:100]
+    wide = ref["margins"][:101] > MARGIN
+    first_narrow = int(np.argmin(wide)) if not wide.all() else 101      # first answer position the GPU may legitimately miss
+    gm = gpu_model(one_b_weights, max_seq=512, flags=hq.FLAG_VERIFY)
+    acc = gm.verify_relay(ref["prompt"], answer)
+    assert acc >= min(first_narrow, 100), (acc, first_narrow)
+    if acc in ref["sampled"]:
+        assert rel_l2(gm.decode_logits()[0].cpu().numpy(), ref["sampled"][acc][1]) <= TOL_LOGITS
+    # corrupt a position in front of the first narrow margin: acceptance stops exactly there
+    j = min(first_narrow, 100) - 1
+    if j >= 1:
+        bad = answer.copy()
+        bad[j] = (bad[j] + 1) % datagen.ONE_B.vocab
+        gm.kv_reset()
+        assert gm.verify_relay(ref["prompt"], bad) == j
+        assert gm.seq_len() == 256 + j
+        assert int(gm.decode_step()[0]) == int(ref["tokens"][j + 1]) or ref["margins"][j + 1] <= MARGIN
+    print("1b verify relay: accepted", acc, "of 100; first narrow margin at", first_narrow)
