@@ -247,7 +247,7 @@ def main():
 
     s = datagen.ONE_B
     weights = datagen.make_weights(s)
-    max_seq = PROMPT_LEN + DECODE_STEPS + 32
+    max_seq = 1024 if args.runtime else PROMPT_LEN + DECODE_STEPS + 32
     gm = hq.Model.from_bf16_bits(s, weights.embedding, weights.final_norm, weights.layers, max_seq=max_seq,
                                  device=str(dev))
     prompt = datagen.tokens(1001, s.vocab, PROMPT_LEN)
