@@ -22,9 +22,8 @@ WEIGHT_SEED = 20260612  # SURVEY.md §8(d) seed scheme
 
 def build(force: bool = False) -> str:
     if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
-        subprocess.check_call(
-            ["gcc", "-O2", "-fopenmp", "-shared", "-fPIC", "-o", _SO, _SRC, "-lm"]
-        )
+        extra = os.environ.get("HQO_EXTRA_CFLAGS", "").split()   # sanitizer run, see oracle/__init__.py
+        subprocess.check_call(["gcc", "-O2", "-fopenmp", "-shared", "-fPIC"] + extra + ["-o", _SO, _SRC, "-lm"])
     return _SO
 
 

@@ -34,8 +34,10 @@ class _Weights(ctypes.Structure):
 
 def build(force: bool = False) -> str:
     if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
-        subprocess.check_call(["gcc", "-O2", "-march=x86-64-v3", "-fopenmp", "-shared", "-fPIC",
-                               "-o", _SO, _SRC, "-lm"])
+        # HQO_EXTRA_CFLAGS: e.g. "-fsanitize=address,undefined -g" for the recorded sanitizer run (profiles/r02_sanitizers.md)
+        extra = os.environ.get("HQO_EXTRA_CFLAGS", "").split()
+        subprocess.check_call(["gcc", "-O2", "-march=x86-64-v3", "-fopenmp", "-shared", "-fPIC"] + extra +
+                              ["-o", _SO, _SRC, "-lm"])
     return _SO
 
 

@@ -151,7 +151,7 @@ class Model:
     """
 
     def __init__(self, cfg: Config, embedding, final_norm, layers: Sequence[Dict[str, "object"]],
-                 lm_head=None, stream=None):
+                 lm_head=None, stream=None, guard_bytes: int = 0):
         import torch
         if not torch.cuda.is_available():
             raise HQError(HQ_ERR_CUDA, "no CUDA device: hq has no CPU fallback")
@@ -169,7 +169,13 @@ class Model:
         nbytes = workspace_bytes(cfg)
         if nbytes == 0:
             _check(HQ_ERR_INVALID_ARG)
-        self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        # guard_bytes (a multiple of 256): canary regions in front of and behind the workspace (tests: guards_intact())
+        self._guard = int(guard_bytes)
+        self._ws_alloc = torch.empty(nbytes + 2 * self._guard, dtype=torch.uint8, device=self.device)
+        if self._guard:
+            self._ws_alloc[:self._guard] = 0xA5
+            self._ws_alloc[self._guard + nbytes:] = 0xA5
+        self.workspace = self._ws_alloc[self._guard:self._guard + nbytes]
         arrays = {}
         for k in LAYER_TENSORS:
             arr = (ctypes.c_void_p * cfg.n_layers)(*[layers[l][k].data_ptr() for l in range(cfg.n_layers)])
@@ -188,7 +194,7 @@ class Model:
     @classmethod
     def from_bf16_bits(cls, shape, embedding_bits: np.ndarray, final_norm_bits: np.ndarray,
                        layer_bits: List[Dict[str, np.ndarray]], *, max_batch=1, max_seq=4352, flags=0,
-                       device="cuda:0", stream=None) -> "Model":
+                       device="cuda:0", stream=None, guard_bytes: int = 0) -> "Model":
         import torch
 
         def up(a: np.ndarray):
@@ -200,7 +206,13 @@ class Model:
                           vocab=shape.vocab, rms_eps=shape.rms_eps, rope_theta=shape.rope_theta,
                           max_batch=max_batch, max_seq=max_seq, flags=flags)
         layers = [{k: up(l[k]) for k in LAYER_TENSORS} for l in layer_bits]
-        return cls(cfg, up(embedding_bits), up(final_norm_bits), layers, stream=stream)
+        return cls(cfg, up(embedding_bits), up(final_norm_bits), layers, stream=stream, guard_bytes=guard_bytes)
+
+    def guards_intact(self) -> bool:
+        """True when no byte of the canary regions around the workspace has been written (guard_bytes > 0)."""
+        self.sync()
+        g, n = self._guard, self.workspace.numel()
+        return bool((self._ws_alloc[:g] == 0xA5).all().item() and (self._ws_alloc[g + n:] == 0xA5).all().item())
 
     def cfg_with_flags(self, flags: int) -> "Config":
         """A copy of this model's config with other HQ_FLAG_* bits (for a second model over the same weights)."""

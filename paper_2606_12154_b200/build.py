@@ -51,7 +51,8 @@ def build_host(force: bool = False) -> str:
     """libhq_host.so: the host-side runtime path (include/hq_host.h), plain g++."""
     deps = [HOST_SRC, os.path.join(INCLUDE, "hq_host.h")]
     if force or not os.path.exists(HOST_LIB) or any(os.path.getmtime(p) > os.path.getmtime(HOST_LIB) for p in deps):
-        subprocess.check_call([os.environ.get("CXX", "g++"), "-O2", "-std=c++17", "-shared", "-fPIC", "-Wall", "-o", HOST_LIB, HOST_SRC])
+        extra = os.environ.get("HQ_HOST_EXTRA_CXXFLAGS", "").split()   # e.g. -fsanitize=address,undefined (profiles/r02_sanitizers.md)
+        subprocess.check_call([os.environ.get("CXX", "g++"), "-O2", "-std=c++17", "-shared", "-fPIC", "-Wall"] + extra + ["-o", HOST_LIB, HOST_SRC])
     return HOST_LIB
 
 

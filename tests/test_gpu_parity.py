@@ -518,6 +518,32 @@ def test_1b_config4_batch2_ctx4096(one_b_weights, ref_ctx4096):
     print("1b config[4] B=2 ctx=4096 parity:", stats)
 
 
+def test_workspace_guards(tiny_weights, tiny_tokens):
+    """compute-sanitizer is closed on this pool (profiles/r02_sanitizers.md), so out-of-bounds WRITES are looked for
+    directly: 1 MiB canary regions in front of and behind the workspace must survive every path — tensor-core prefill
+    (single and multi-pass), both batch-1 decode paths up to the last cache slot, batched decode at max_batch, the
+    dense verification pass."""
+    import paper_2606_12154_b200 as hq
+    w = tiny_weights
+    for path in (0, KERNEL_PER_ROW):
+        gm = hq.Model.from_bf16_bits(w.shape, w.embedding, w.final_norm, w.layers, max_seq=80, max_batch=4,
+                                     flags=hq.FLAG_CAPTURE_HIDDEN | hq.FLAG_VERIFY | path, guard_bytes=1 << 20)
+        gm.prefill(tiny_tokens)
+        gm.decode_run(48)                                   # fills the cache to its last slot (32 + 48 = 80)
+        assert gm.seq_len() == 80 and gm.guards_intact()
+        gm.kv_reset()
+        gm.prefill(np.stack([tiny_tokens] * 4))
+        gm.decode_run(48, batch=4)
+        assert gm.guards_intact()
+        gm.kv_reset()
+        gm.verify_relay(tiny_tokens[:20], tiny_tokens[20:])
+        assert gm.guards_intact()
+    big = hq.Model.from_bf16_bits(w.shape, w.embedding, w.final_norm, w.layers, max_seq=4200, max_batch=2, guard_bytes=1 << 20)
+    big.prefill(datagen.tokens(7, datagen.TINY.vocab, 2 * 4190).reshape(2, 4190))     # five tensor-core passes
+    big.decode_run(10, batch=2)
+    assert big.seq_len() == 4200 and big.guards_intact()
+
+
 def test_tiny_batch_invariance(tiny_weights):
     """Sequence 0's logits do not depend on its neighbours beyond rounding (reading 17)."""
     T = 20
