@@ -170,7 +170,7 @@ def run_reference(args):
     import oracle
     s = datagen.ONE_B
     w = datagen.make_weights(s)
-    prompt_len, steps = 8, 8  # bounded sample of the workload per bench step
+    prompt_len, steps = (PROMPT_LEN, DECODE_STEPS) if args.full_config1 else (8, 8)  # default: bounded sample of the workload per bench step
     om = oracle.Model.from_datagen(w, max_seq=prompt_len + steps + 1)
     prompt = datagen.tokens(1001, s.vocab, prompt_len)
 
@@ -194,7 +194,8 @@ def run_reference(args):
         td += b
     value = args.steps * steps / td
     sample = (f"per step: {prompt_len}-token prompt + {steps} greedy decode steps (context {prompt_len + 1}.."
-              f"{prompt_len + steps}) of the same 1B weights (bounded sample of configs[1], whose context is 257..384)")
+              f"{prompt_len + steps}) of the same 1B weights " +
+              ("(the whole of configs[1])" if args.full_config1 else "(bounded sample of configs[1], whose context is 257..384)"))
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": (tp + td) / args.steps * 1e3,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
@@ -214,6 +215,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="hq", choices=["hq", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg")
+    ap.add_argument("--full-config1", action="store_true",
+                    help="with --impl reference: time the oracle on the whole of configs[1] (256-token prompt + 128 steps) per step")
     ap.add_argument("--sweep", action="store_true",
                     help="configs[4]: batch {1,4,16,32} x context {512,4096}, 128 decode steps each; one JSON line per point")
     ap.add_argument("--runtime", action="store_true",
