@@ -45,7 +45,7 @@ typedef enum {
     HQ_ERR_UNSUPPORTED = -5  /* shape outside what the kernels implement (see hq_model_create) */
 } hq_status;
 
-enum { HQ_BF16 = 0 };
+enum { HQ_BF16 = 0, HQ_Q4 = 1 /* bf16 model whose FFN and LM-head matrices are additionally given in the 4-bit hq4 format (hq_model_create_q4) */ };
 enum {
     HQ_FLAG_CAPTURE_HIDDEN = 1u, /* keep the residual stream after every layer (parity tests) */
     HQ_FLAG_NO_GRAPH = 2u,       /* launch decode kernels directly instead of replaying a CUDA graph */
@@ -65,7 +65,7 @@ typedef struct {
     float rope_theta;   /* rotate-half pairing (i, i + head_dim/2), angle pos * theta^(-2i/head_dim) */
     int32_t max_batch;  /* KV capacity: sequences */
     int32_t max_seq;    /* KV capacity: positions per sequence */
-    int32_t weight_dtype; /* HQ_BF16 */
+    int32_t weight_dtype; /* HQ_BF16, or HQ_Q4 with hq_model_create_q4 */
     uint32_t flags;       /* HQ_FLAG_* */
 } hq_config;
 
@@ -109,6 +109,34 @@ size_t hq_workspace_bytes(const hq_config *cfg);
  * Defined by: BASELINE.json north_star ("hq_model_create from a shape config and device weight pointers"). */
 int32_t hq_model_create(const hq_config *cfg, const hq_weights *weights, void *workspace_dev,
                         size_t workspace_bytes, void *cuda_stream, hq_model **out);
+
+/* 4-bit weight-only decode.  The paper's mouth model runs at 4-bit quantisation ("A
+ * 1B-class model (MiniCPM5-1B, 4-bit) then streams the answer"; section 5); its runtime's format is not
+ * described and not used.  "hq4" is this library's own format: a weight row of K elements (K % 32 == 0) is cut into
+ * groups of 32 consecutive elements; group exponent e = the smallest integer with max|w| <= 7 * 2^e (-126 for an all-zero
+ * group, at most 120), stored as the byte e + 127; code q = round-half-to-even(w / 2^e) in [-8, 7], stored as the nibble
+ * q + 8, element 2j of a row in the low nibble of byte j and element 2j + 1 in the high nibble.  The weight computed with
+ * is w' = q * 2^e, exactly representable in bf16.
+ *   codes: DEVICE uint8 [n_rows][K / 2];  exponent bytes: DEVICE uint8 [n_rows][K / 32]
+ * hq_quantize_q4 / hq_dequantize_q4: bf16 [n_rows][k] -> hq4 -> bf16 (w'), asynchronous on cuda_stream, all DEVICE.
+ * hq_model_create_q4: like hq_model_create with weight_dtype = HQ_Q4.  `weights` must hold the DEQUANTISED bf16 matrices
+ * w' for w_gate, w_up, w_down of every layer and for tok_embedding / lm_head (the tensor-core paths — prefill, batched
+ * decode, hq_verify_relay — compute with them), `q4` the hq4 tensors of the same matrices: batch-1 decode streams those
+ * (4.25 bits per weight instead of 16) through the streaming GEMV.  Attention weights and norm gains stay bf16.  Keeping
+ * the two copies consistent is the caller's business (quantise, then dequantise).  Extra shape limits: hidden a multiple of
+ * 64 and <= 2048, ffn a multiple of 32 (of 1024 above 2048), vocab a multiple of 16. */
+typedef struct {
+    const void *const *w_gate_codes, *const *w_gate_exps; /* HOST arrays of n_layers DEVICE pointers */
+    const void *const *w_up_codes, *const *w_up_exps;
+    const void *const *w_down_codes, *const *w_down_exps;
+    const void *lm_head_codes, *lm_head_exps;
+} hq_weights_q4;
+int32_t hq_quantize_q4(void *cuda_stream, const void *w_dev, int64_t n_rows, int32_t k, void *codes_dev, void *exps_dev);
+/* Inverse of hq_quantize_q4 (same passage: PAPER.md:L70, L82): w' = q * 2^e as bf16, exact. */
+int32_t hq_dequantize_q4(void *cuda_stream, const void *codes_dev, const void *exps_dev, int64_t n_rows, int32_t k, void *w_dev);
+/* See the hq4 comment above. */
+int32_t hq_model_create_q4(const hq_config *cfg, const hq_weights *weights, const hq_weights_q4 *q4, void *workspace_dev,
+                           size_t workspace_bytes, void *cuda_stream, hq_model **out);
 
 /* Frees graphs/events/handles; never the borrowed memory.  NULL is a no-op.  (Counterpart of hq_model_create.) */
 void hq_model_destroy(hq_model *m);

@@ -18,6 +18,7 @@ FLAG_NO_GRAPH = 2
 FLAG_NO_PDL = 4
 FLAG_KERNEL_PER_ROW = 8
 FLAG_VERIFY = 16
+DTYPE_BF16, DTYPE_Q4 = 0, 1
 
 HQ_OK, HQ_ERR_INVALID_ARG, HQ_ERR_CAPACITY, HQ_ERR_STATE, HQ_ERR_CUDA, HQ_ERR_UNSUPPORTED = 0, -1, -2, -3, -4, -5
 _CODE_NAMES = {-1: "HQ_ERR_INVALID_ARG", -2: "HQ_ERR_CAPACITY", -3: "HQ_ERR_STATE", -4: "HQ_ERR_CUDA",
@@ -25,7 +26,7 @@ _CODE_NAMES = {-1: "HQ_ERR_INVALID_ARG", -2: "HQ_ERR_CAPACITY", -3: "HQ_ERR_STAT
 
 # every symbol include/hq.h and include/hq_debug.h declare (tests check the headers and the library against this list)
 DECLARED_SYMBOLS = (
-    "hq_workspace_bytes", "hq_model_create", "hq_model_destroy", "hq_prefill", "hq_decode_step",
+    "hq_workspace_bytes", "hq_model_create", "hq_model_create_q4", "hq_quantize_q4", "hq_dequantize_q4", "hq_model_destroy", "hq_prefill", "hq_decode_step",
     "hq_decode_run", "hq_verify_relay", "hq_decode_logits", "hq_get_hidden", "hq_sync", "hq_seq_len", "hq_kv_reset",
     "hq_kernel_count", "hq_decode_path", "hq_bench_kernel", "hq_debug_copy_probe", "hq_debug_gemm", "hq_debug_kv_row", "hq_debug_read_probe", "hq_debug_step_trace", "hq_debug_trace", "hq_last_error",
     "hq_version",
@@ -55,6 +56,12 @@ class Weights(ctypes.Structure):
                 ("w_down", _vpp), ("final_norm", ctypes.c_void_p), ("lm_head", ctypes.c_void_p)]
 
 
+class WeightsQ4(ctypes.Structure):
+    _fields_ = [("w_gate_codes", _vpp), ("w_gate_exps", _vpp), ("w_up_codes", _vpp), ("w_up_exps", _vpp),
+                ("w_down_codes", _vpp), ("w_down_exps", _vpp), ("lm_head_codes", ctypes.c_void_p),
+                ("lm_head_exps", ctypes.c_void_p)]
+
+
 _lib = None
 
 
@@ -74,6 +81,13 @@ def load_library(path: Optional[str] = None):
     l.hq_model_create.restype = i32
     l.hq_model_create.argtypes = [ctypes.POINTER(Config), ctypes.POINTER(Weights), vp, ctypes.c_size_t, vp,
                                   ctypes.POINTER(vp)]
+    l.hq_model_create_q4.restype = i32
+    l.hq_model_create_q4.argtypes = [ctypes.POINTER(Config), ctypes.POINTER(Weights), ctypes.POINTER(WeightsQ4), vp,
+                                     ctypes.c_size_t, vp, ctypes.POINTER(vp)]
+    l.hq_quantize_q4.restype = i32
+    l.hq_quantize_q4.argtypes = [vp, vp, i64, i32, vp, vp]
+    l.hq_dequantize_q4.restype = i32
+    l.hq_dequantize_q4.argtypes = [vp, vp, vp, i64, i32, vp]
     l.hq_model_destroy.restype = None
     l.hq_model_destroy.argtypes = [vp]
     l.hq_prefill.restype = i32
@@ -131,9 +145,30 @@ def version() -> str:
 
 
 def make_config(*, n_layers, hidden, n_heads, n_kv_heads, head_dim, ffn, vocab, rms_eps, rope_theta,
-                max_batch=1, max_seq=4352, flags=0) -> Config:
+                max_batch=1, max_seq=4352, flags=0, weight_dtype=DTYPE_BF16) -> Config:
     return Config(n_layers, hidden, n_heads, n_kv_heads, head_dim, ffn, vocab, rms_eps, rope_theta,
-                  max_batch, max_seq, 0, flags)
+                  max_batch, max_seq, weight_dtype, flags)
+
+
+def quantize_q4(w, stream=None):
+    """hq_quantize_q4 on a CUDA bf16 tensor [N, K]: returns (codes uint8 [N, K/2], exponent bytes uint8 [N, K/32])."""
+    import torch
+    st = stream if stream is not None else torch.cuda.current_stream(w.device)
+    n, k = w.shape
+    codes = torch.empty((n, k // 2), dtype=torch.uint8, device=w.device)
+    exps = torch.empty((n, k // 32), dtype=torch.uint8, device=w.device)
+    _check(load_library().hq_quantize_q4(st.cuda_stream, w.data_ptr(), n, k, codes.data_ptr(), exps.data_ptr()))
+    return codes, exps
+
+
+def dequantize_q4(codes, exps, stream=None):
+    """hq_dequantize_q4: (codes, exponent bytes) -> CUDA bf16 tensor [N, K] of w' = q * 2^e."""
+    import torch
+    st = stream if stream is not None else torch.cuda.current_stream(codes.device)
+    n, k = codes.shape[0], codes.shape[1] * 2
+    w = torch.empty((n, k), dtype=torch.bfloat16, device=codes.device)
+    _check(load_library().hq_dequantize_q4(st.cuda_stream, codes.data_ptr(), exps.data_ptr(), n, k, w.data_ptr()))
+    return w
 
 
 def workspace_bytes(cfg: Config) -> int:
@@ -151,7 +186,9 @@ class Model:
     """
 
     def __init__(self, cfg: Config, embedding, final_norm, layers: Sequence[Dict[str, "object"]],
-                 lm_head=None, stream=None, guard_bytes: int = 0):
+                 lm_head=None, stream=None, guard_bytes: int = 0, q4=None):
+        """q4 (HQ_Q4 models): dict with per-layer lists "w_gate", "w_up", "w_down" of (codes, exps) CUDA tensors and
+        "lm_head": (codes, exps); the bf16 tensors passed for those matrices must be their dequantised values."""
         import torch
         if not torch.cuda.is_available():
             raise HQError(HQ_ERR_CUDA, "no CUDA device: hq has no CPU fallback")
@@ -163,6 +200,7 @@ class Model:
             if t.dtype != torch.bfloat16 or not t.is_cuda or not t.is_contiguous():
                 raise HQError(HQ_ERR_INVALID_ARG, "weights must be contiguous CUDA bfloat16 tensors")
         self._keep = [embedding, final_norm, layers, lm_head]
+        self._q4 = q4
         # a dedicated stream: CUDA graphs cannot be captured on the legacy default stream
         self.stream = stream if stream is not None else torch.cuda.Stream(self.device)
         torch.cuda.synchronize(self.device)     # weight uploads on the current stream are done
@@ -185,8 +223,18 @@ class Model:
                     final_norm.data_ptr(), head.data_ptr())
         h = ctypes.c_void_p()
         with torch.cuda.device(self.device):     # the library creates the model on the CURRENT device
-            _check(self._lib.hq_model_create(ctypes.byref(cfg), ctypes.byref(w), self.workspace.data_ptr(),
-                                             nbytes, self.stream.cuda_stream, ctypes.byref(h)))
+            if q4 is None:
+                _check(self._lib.hq_model_create(ctypes.byref(cfg), ctypes.byref(w), self.workspace.data_ptr(),
+                                                 nbytes, self.stream.cuda_stream, ctypes.byref(h)))
+            else:
+                qa = {}
+                for name in ("w_gate", "w_up", "w_down"):
+                    for j, kind in enumerate(("codes", "exps")):
+                        qa[name + "_" + kind] = (ctypes.c_void_p * cfg.n_layers)(*[q4[name][l][j].data_ptr() for l in range(cfg.n_layers)])
+                wq = WeightsQ4(*[ctypes.cast(qa[n + "_" + k], _vpp) for n in ("w_gate", "w_up", "w_down") for k in ("codes", "exps")],
+                               q4["lm_head"][0].data_ptr(), q4["lm_head"][1].data_ptr())
+                _check(self._lib.hq_model_create_q4(ctypes.byref(cfg), ctypes.byref(w), ctypes.byref(wq), self.workspace.data_ptr(),
+                                                    nbytes, self.stream.cuda_stream, ctypes.byref(h)))
         self._h = h
         self.vocab, self.hidden, self.n_layers = cfg.vocab, cfg.hidden, cfg.n_layers
 
@@ -207,6 +255,34 @@ class Model:
                           max_batch=max_batch, max_seq=max_seq, flags=flags)
         layers = [{k: up(l[k]) for k in LAYER_TENSORS} for l in layer_bits]
         return cls(cfg, up(embedding_bits), up(final_norm_bits), layers, stream=stream, guard_bytes=guard_bytes)
+
+    @classmethod
+    def from_bf16_bits_q4(cls, shape, embedding_bits: np.ndarray, final_norm_bits: np.ndarray,
+                          layer_bits: List[Dict[str, np.ndarray]], *, max_batch=1, max_seq=4352, flags=0,
+                          device="cuda:0", guard_bytes: int = 0) -> "Model":
+        """HQ_Q4 model from bf16 bit patterns: FFN matrices and the (tied) embedding / LM head are quantised to hq4 on the
+        device (hq_quantize_q4) and replaced by their dequantised values (hq_dequantize_q4); attention weights stay."""
+        import torch
+
+        def up(a: np.ndarray):
+            return torch.from_numpy(np.ascontiguousarray(a).view(np.int16)).to(device).view(torch.bfloat16)
+
+        cfg = make_config(n_layers=shape.n_layers, hidden=shape.hidden, n_heads=shape.n_heads,
+                          n_kv_heads=shape.n_kv_heads, head_dim=shape.head_dim, ffn=shape.ffn,
+                          vocab=shape.vocab, rms_eps=shape.rms_eps, rope_theta=shape.rope_theta,
+                          max_batch=max_batch, max_seq=max_seq, flags=flags, weight_dtype=DTYPE_Q4)
+        layers = [{k: up(l[k]) for k in LAYER_TENSORS} for l in layer_bits]
+        q4 = {"w_gate": [], "w_up": [], "w_down": []}
+        for l in layers:
+            for name in ("w_gate", "w_up", "w_down"):
+                ce = quantize_q4(l[name])
+                q4[name].append(ce)
+                l[name] = dequantize_q4(*ce)
+        emb = up(embedding_bits)
+        q4["lm_head"] = quantize_q4(emb)
+        emb = dequantize_q4(*q4["lm_head"])
+        torch.cuda.synchronize()
+        return cls(cfg, emb, up(final_norm_bits), layers, guard_bytes=guard_bytes, q4=q4)
 
     def guards_intact(self) -> bool:
         """True when no byte of the canary regions around the workspace has been written (guard_bytes > 0)."""

@@ -49,7 +49,7 @@ static bool config_ok(const hq_config *c, const char **why) {
     if (c->n_layers <= 0 || c->hidden <= 0 || c->n_heads <= 0 || c->n_kv_heads <= 0 || c->ffn <= 0 ||
         c->vocab <= 0 || c->max_batch <= 0 || c->max_seq <= 0)
         BAD("non-positive dimension");
-    if (c->weight_dtype != HQ_BF16) BAD("weight_dtype must be HQ_BF16");
+    if (c->weight_dtype != HQ_BF16 && c->weight_dtype != HQ_Q4) BAD("weight_dtype must be HQ_BF16 or HQ_Q4");
     return true;
 #undef BAD
 }
@@ -167,6 +167,7 @@ static SgemvParams sgemv_gateup(const hq_model *m, int l) {
     p.trace = m->step_trace; p.trace_slot = 2 + 3 * l;
     if (m->use_attn_block) { p.n_early = m->n_sms - kAbCluster * c.n_kv_heads; p.late_deficit = kLateDeficit; }
     p.out_planes = reinterpret_cast<bf16 *>(m->b.act);
+    if (m->q4) { p.q0 = m->layers_q4[l].gate_q; p.e0 = m->layers_q4[l].gate_e; p.q1 = m->layers_q4[l].up_q; p.e1 = m->layers_q4[l].up_e; }
     return p;
 }
 static SgemvParams sgemv_down(const hq_model *m, int l) {
@@ -175,6 +176,7 @@ static SgemvParams sgemv_down(const hq_model *m, int l) {
     p.w0 = m->layers[l].w_down; p.xin = m->b.act; p.K = c.ffn; p.n_rows = c.hidden;
     p.trace = m->step_trace; p.trace_slot = 3 + 3 * l;
     p.mode = SGEMV_RESID; p.xin_mode = SGEMV_XIN_PLANES; p.out = m->b.x;
+    if (m->q4) { p.q0 = m->layers_q4[l].down_q; p.e0 = m->layers_q4[l].down_e; }
     return p;
 }
 // final norm + LM head + argmax over the residual row x; the position advances by pos_inc
@@ -187,6 +189,7 @@ static SgemvParams sgemv_lm_head(const hq_model *m, const float *x, int pos_inc)
     p.pos = b.pos; p.best = b.best; p.counter = b.counter; p.cur_tok = b.cur_tok; p.tok_hist = b.tok_hist;
     p.trace = m->step_trace; p.trace_slot = 1 + 3 * c.n_layers;
     p.pos_rw = b.pos; p.pos_inc = pos_inc;
+    if (m->q4) { p.q0 = m->lm_head_q; p.e0 = m->lm_head_e; }
     return p;
 }
 
@@ -454,8 +457,45 @@ static bool build_tensor_maps(hq_model *m) {
 }
 
 // ---- create / destroy ---------------------------------------------------------------------------------
+static int32_t model_create(const hq_config *cfg, const hq_weights *w, const hq_weights_q4 *q, void *workspace, size_t ws_bytes,
+                            void *cuda_stream, hq_model **out);
+
 extern "C" int32_t hq_model_create(const hq_config *cfg, const hq_weights *w, void *workspace, size_t ws_bytes,
                                    void *cuda_stream, hq_model **out) {
+    if (cfg && cfg->weight_dtype == HQ_Q4) return fail(HQ_ERR_INVALID_ARG, "hq_model_create: HQ_Q4 models are created with hq_model_create_q4");
+    return model_create(cfg, w, nullptr, workspace, ws_bytes, cuda_stream, out);
+}
+
+extern "C" int32_t hq_model_create_q4(const hq_config *cfg, const hq_weights *w, const hq_weights_q4 *q, void *workspace,
+                                      size_t ws_bytes, void *cuda_stream, hq_model **out) {
+    if (!cfg || cfg->weight_dtype != HQ_Q4 || !q) return fail(HQ_ERR_INVALID_ARG, "hq_model_create_q4: needs weight_dtype HQ_Q4 and the hq4 tensors");
+    if (!q->w_gate_codes || !q->w_gate_exps || !q->w_up_codes || !q->w_up_exps || !q->w_down_codes || !q->w_down_exps ||
+        !q->lm_head_codes || !q->lm_head_exps)
+        return fail(HQ_ERR_INVALID_ARG, "hq_model_create_q4: an hq4 pointer is NULL");
+    for (int l = 0; l < cfg->n_layers; ++l)
+        if (!q->w_gate_codes[l] || !q->w_gate_exps[l] || !q->w_up_codes[l] || !q->w_up_exps[l] || !q->w_down_codes[l] || !q->w_down_exps[l])
+            return fail(HQ_ERR_INVALID_ARG, "hq_model_create_q4: an hq4 pointer of layer %d is NULL", l);
+    if (!sgemv_q4_shape_supported(cfg->hidden) || !sgemv_q4_shape_supported(cfg->ffn) || cfg->hidden % 64 != 0 || cfg->ffn % 16 != 0 ||
+        cfg->hidden % 16 != 0 || cfg->vocab % 16 != 0 || cfg->hidden > 2048)
+        return fail(HQ_ERR_UNSUPPORTED, "hq_model_create_q4: hq4 needs hidden a multiple of 64 and <= 2048, ffn a multiple of 32 (of 1024 above 2048), "
+                                        "vocab a multiple of 16");
+    return model_create(cfg, w, q, workspace, ws_bytes, cuda_stream, out);
+}
+
+extern "C" int32_t hq_quantize_q4(void *cuda_stream, const void *w_dev, int64_t n_rows, int32_t k, void *codes_dev, void *exps_dev) {
+    if (!w_dev || !codes_dev || !exps_dev || n_rows <= 0 || k <= 0 || k % 32 != 0) return fail(HQ_ERR_INVALID_ARG, "hq_quantize_q4: bad argument (k must be a multiple of 32)");
+    HQ_CUDA(launch_q4_quantize((cudaStream_t)cuda_stream, (const bf16 *)w_dev, (size_t)n_rows, k, (uint8_t *)codes_dev, (uint8_t *)exps_dev));
+    return HQ_OK;
+}
+
+extern "C" int32_t hq_dequantize_q4(void *cuda_stream, const void *codes_dev, const void *exps_dev, int64_t n_rows, int32_t k, void *w_dev) {
+    if (!w_dev || !codes_dev || !exps_dev || n_rows <= 0 || k <= 0 || k % 32 != 0) return fail(HQ_ERR_INVALID_ARG, "hq_dequantize_q4: bad argument (k must be a multiple of 32)");
+    HQ_CUDA(launch_q4_dequantize((cudaStream_t)cuda_stream, (const uint8_t *)codes_dev, (const uint8_t *)exps_dev, (size_t)n_rows, k, (bf16 *)w_dev));
+    return HQ_OK;
+}
+
+static int32_t model_create(const hq_config *cfg, const hq_weights *w, const hq_weights_q4 *q, void *workspace, size_t ws_bytes,
+                            void *cuda_stream, hq_model **out) {
     const char *why = "";
     if (!out) return fail(HQ_ERR_INVALID_ARG, "hq_model_create: out is NULL");
     *out = nullptr;
@@ -484,6 +524,7 @@ extern "C" int32_t hq_model_create(const hq_config *cfg, const hq_weights *w, vo
 
     HQ_CUDA(gemm_prepare());
     HQ_CUDA(sgemv_prepare());
+    HQ_CUDA(sgemv_q4_prepare());
     hq_model *m = new (std::nothrow) hq_model();
     if (!m) return fail(HQ_ERR_INVALID_ARG, "hq_model_create: out of host memory");
     m->cfg = *cfg;
@@ -500,6 +541,15 @@ extern "C" int32_t hq_model_create(const hq_config *cfg, const hq_weights *w, vo
         lw.wk = (const bf16 *)w->wk[l]; lw.wv = (const bf16 *)w->wv[l]; lw.wo = (const bf16 *)w->wo[l];
         lw.ffn_norm = (const bf16 *)w->ffn_norm[l]; lw.w_gate = (const bf16 *)w->w_gate[l];
         lw.w_up = (const bf16 *)w->w_up[l]; lw.w_down = (const bf16 *)w->w_down[l];
+    }
+    if (q) {
+        m->q4 = true;
+        m->layers_q4.resize(cfg->n_layers);
+        for (int l = 0; l < cfg->n_layers; ++l)
+            m->layers_q4[l] = LayerQ4{(const uint8_t *)q->w_gate_codes[l], (const uint8_t *)q->w_gate_exps[l], (const uint8_t *)q->w_up_codes[l],
+                                      (const uint8_t *)q->w_up_exps[l], (const uint8_t *)q->w_down_codes[l], (const uint8_t *)q->w_down_exps[l]};
+        m->lm_head_q = (const uint8_t *)q->lm_head_codes;
+        m->lm_head_e = (const uint8_t *)q->lm_head_exps;
     }
     carve(cfg, (char *)workspace, &m->b);
     m->pf_rows = (int)pass_rows(cfg);
@@ -849,13 +899,13 @@ extern "C" int32_t hq_bench_kernel(hq_model *m, int32_t which, int32_t reps, int
                 SgemvParams pg = sgemv_gateup(m, l);
                 pg.n_early = 0;   // timed alone there is no attention block in front of it: even split
                 HQ_CUDA(launch_sgemv(lc, pg));
-                bytes = 2ll * 2 * c.ffn * c.hidden;
+                bytes = m->q4 ? 2ll * c.ffn * (c.hidden / 2 + c.hidden / 32) : 2ll * 2 * c.ffn * c.hidden;
                 break;
             }
             case 1: {
                 // LM head without state side effects: pos_inc = 0 (token / history writes repeat the current slot)
                 HQ_CUDA(launch_sgemv(lc, sgemv_lm_head(m, b.x, 0)));
-                bytes = 2ll * c.vocab * c.hidden;
+                bytes = m->q4 ? 1ll * c.vocab * (c.hidden / 2 + c.hidden / 32) : 2ll * c.vocab * c.hidden;
                 break;
             }
             case 2:
@@ -875,7 +925,7 @@ extern "C" int32_t hq_bench_kernel(hq_model *m, int32_t which, int32_t reps, int
                 break;
             case 4:
                 HQ_CUDA(launch_sgemv(lc, sgemv_down(m, l)));
-                bytes = 2ll * c.hidden * c.ffn;
+                bytes = m->q4 ? 1ll * c.hidden * (c.ffn / 2 + c.ffn / 32) : 2ll * c.hidden * c.ffn;
                 break;
             case 5: {
                 AttnDecodeParams a = {b.q, b.kcache + l * layer_kv, b.vcache + l * layer_kv, b.part_o, b.part_ml,

@@ -36,6 +36,10 @@ struct alignas(64) TensorMap { uint64_t opaque[16]; };   // mirrors CUtensorMap 
 struct LayerW {
     const bf16 *attn_norm, *wq, *wk, *wv, *wo, *ffn_norm, *w_gate, *w_up, *w_down;
 };
+// hq4 copies of the streamed matrices of a layer (HQ_Q4 models): codes and exponent bytes
+struct LayerQ4 {
+    const uint8_t *gate_q, *gate_e, *up_q, *up_e, *down_q, *down_e;
+};
 
 // Device buffers carved from the caller's workspace (see hq_api.cu carve()).
 struct Buffers {
@@ -81,6 +85,9 @@ struct LayerMaps { TensorMap wq, wk, wv, wo, w_gate, w_up, w_down; };
 struct hq_model_impl {
     hq_config cfg;
     std::vector<LayerW> layers;
+    bool q4 = false;                            // HQ_Q4: batch-1 decode streams gate/up/down/LM head as hq4
+    std::vector<LayerQ4> layers_q4;
+    const uint8_t *lm_head_q = nullptr, *lm_head_e = nullptr;
     const bf16 *emb = nullptr, *final_norm = nullptr, *lm_head = nullptr;
     cudaStream_t stream = nullptr;
     int device = 0;                             // CUDA device the model was created on (made current by every entry point)
@@ -133,6 +140,8 @@ enum SgemvMode { SGEMV_GATEUP = 0, SGEMV_RESID = 1, SGEMV_LMHEAD = 2 };
 enum SgemvInput { SGEMV_XIN_NORM = 0, SGEMV_XIN_PLANES = 1 };
 struct SgemvParams {
     const bf16 *w0, *w1;     // GATEUP: gate, up [n_rows][K] each; RESID / LMHEAD: w0 [n_rows][K]
+    const uint8_t *q0, *q1;  // hq4 weights instead (hq_stream_q4.cu): codes [n_rows][K / 2] ...
+    const uint8_t *e0, *e1;  // ... and exponent bytes [n_rows][K / 32]; q0 == NULL: bf16 weights
     const bf16 *gain;        // XIN_NORM: RMSNorm gains [K]
     const float *xin;        // XIN_NORM: fp32 residual stream [K]; XIN_PLANES: bf16 hi plane [K] then lo plane [K]
     int K, n_rows;
@@ -178,7 +187,12 @@ struct LaunchCtx {
 
 bool sgemv_shape_supported(int K);
 cudaError_t sgemv_prepare();
-cudaError_t launch_sgemv(const LaunchCtx &c, const SgemvParams &p);
+cudaError_t launch_sgemv(const LaunchCtx &c, const SgemvParams &p);   // dispatches to the hq4 kernel when p.q0 is set
+bool sgemv_q4_shape_supported(int K);
+cudaError_t sgemv_q4_prepare();
+cudaError_t launch_sgemv_q4(const LaunchCtx &c, const SgemvParams &p);
+cudaError_t launch_q4_quantize(cudaStream_t stream, const bf16 *w, size_t n_rows, int K, uint8_t *codes, uint8_t *exps);
+cudaError_t launch_q4_dequantize(cudaStream_t stream, const uint8_t *codes, const uint8_t *exps, size_t n_rows, int K, bf16 *w);
 
 // ---- attention block: A2-A6 of a layer in one cluster launch (hq_attn.cu) -----------------------------------
 constexpr int kAbCluster = 8;        // CTAs per cluster = per KV head (portable cluster size)

@@ -358,6 +358,7 @@ cudaError_t sgemv_prepare() {
 }
 
 cudaError_t launch_sgemv(const LaunchCtx &c, const SgemvParams &p) {
+    if (p.q0) return launch_sgemv_q4(c, p);
     if (!sgemv_shape_supported(p.K)) return cudaErrorInvalidValue;
     const int rps = sg_rows_per_stage(p.K, p.mode);
     const int n_stages = (p.n_rows + rps - 1) / rps;
