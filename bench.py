@@ -219,6 +219,8 @@ def main():
                     help="with --impl reference: time the oracle on the whole of configs[1] (256-token prompt + 128 steps) per step")
     ap.add_argument("--sweep", action="store_true",
                     help="configs[4]: batch {1,4,16,32} x context {512,4096}, 128 decode steps each; one JSON line per point")
+    ap.add_argument("--q4", action="store_true",
+                    help="SURVEY 8(f)-1: the configs[1] query with the FFN and LM-head matrices streamed as 4-bit hq4 (hq_model_create_q4)")
     ap.add_argument("--runtime", action="store_true",
                     help="SURVEY 8(f)-3: the whole runtime path per query on the synthetic 563-entry store (route, gate, render, "
                          "tokenise, prefill, streaming decode): e2e wall, e2e tok/s, TTFT, route p50 as PAPER.md:L109 defines them")
@@ -314,6 +316,56 @@ def main():
                 m.close()
                 del m
                 torch.cuda.empty_cache()
+        return
+
+    if args.q4:
+        # the paper's mouth runs at 4-bit.  Same query as the headline, FFN + LM head as hq4 (4.25 bits per
+        # weight), attention weights bf16: algorithmic bytes per token = hq4 bytes + bf16 attention / norm bytes + embedding row + KV
+        del gm
+        torch.cuda.empty_cache()
+        qm = hq.Model.from_bf16_bits_q4(s, weights.embedding, weights.final_norm, weights.layers, max_seq=max_seq, device=str(dev))
+        qd = s.n_heads * s.head_dim
+        attn_bytes = s.n_layers * 2 * (qd * s.hidden + 2 * s.n_kv_heads * s.head_dim * s.hidden + s.hidden * qd + 2 * s.hidden) + 2 * s.hidden
+        q4_weights = s.n_layers * 3 * s.ffn * s.hidden + s.vocab * s.hidden
+        q4_bytes = q4_weights // 2 + q4_weights // 32
+        kv_tok = 2 * s.n_kv_heads * s.head_dim * 2 * s.n_layers
+        bpt = attn_bytes + q4_bytes + 2 * s.hidden + (PROMPT_LEN + DECODE_STEPS // 2 + 1) * kv_tok
+        dec, pf = [], []
+        sampler = ClockSampler(local_rank)
+        sampler.start()
+        for it in range(3 + args.steps):
+            qm.kv_reset()
+            a, b, c2 = ev(), ev(), ev()
+            a.record(qm.stream)
+            qm.prefill(prompt, want_token=False)
+            b.record(qm.stream)
+            qm.decode_run(DECODE_STEPS, want_tokens=False)
+            c2.record(qm.stream)
+            torch.cuda.synchronize(dev)
+            if it >= 3:
+                pf.append(a.elapsed_time(b))
+                dec.append(b.elapsed_time(c2))
+        clk = sampler.stop()
+        kernels = {}
+        qm.kv_reset(); qm.prefill(prompt, want_token=False); qm.sync()
+        for which, name in ((0, "gate_up"), (1, "lm_head"), (4, "down"), (6, "attn_block")):
+            r = 16 if which == 1 else 128
+            qm.bench_kernel(which, 8)
+            a, b = ev(), ev()
+            a.record(qm.stream)
+            nbytes = qm.bench_kernel(which, r)
+            b.record(qm.stream)
+            torch.cuda.synchronize(dev)
+            ms = a.elapsed_time(b) / r
+            kernels[name] = {"us": ms * 1e3, "GBps": nbytes / ms / 1e6, "bytes_per_launch": nbytes}
+        peak, _ = measured_peak()
+        ms_tok = float(np.mean(dec)) / DECODE_STEPS
+        print(json.dumps({"q4": True, "workload": WORKLOAD + "; FFN and LM head as hq4 (4.25 bits per weight), attention weights bf16",
+                          "tokens_per_s": 1e3 / ms_tok, "ms_per_token": ms_tok, "ttft_ms": float(np.mean(pf)),
+                          "bytes_per_token": bpt, "achieved_GBps": bpt / (ms_tok * 1e-3) / 1e9,
+                          "frac_of_measured_peak": bpt / (ms_tok * 1e-3) / 1e9 / peak,
+                          "weight_bytes_q4_model": attn_bytes + q4_bytes, "weight_bytes_bf16_model": weight_bytes(s),
+                          "kernels_alone": kernels, "clocks": clk, "decode_path": qm.decode_path()}), flush=True)
         return
 
     if args.runtime:
