@@ -5,8 +5,9 @@
 // keeps the stream independent of everything else the CTA does:
 //   * grid = one CTA per SM; one producer thread copies weights with cp.async.bulk (TMA bulk copy, mbarrier complete_tx,
 //     L2 evict-first) into a ring of 3 x 64 KB shared-memory stages.  A stage is ONE copy of 64 KB of consecutive weight
-//     rows (two of 32 KB for gate | up): measured on B200, an SM pulls ~58 GB/s through 4 KB bulk copies, ~135 GB/s
-//     through 16 KB ones and ~160 GB/s through 64 KB ones, and the chip-wide LM-head stream rises from 6.6 to 6.85 TB/s.
+//     rows (two of 32 KB for gate | up): measured on B200 (bench.py --probes, profiles/r02_copy_size.md), an SM pulls
+//     33 GB/s through 1 KB bulk copies, ~105 through 4 KB ones (58 next to busy consumer warps) and ~180 through >= 16 KB
+//     ones, and the chip-wide stream rises from 6.85 to 7.26 TB/s.
 //     The high per-SM rate matters behind the attention block: its 64 SMs join the following gate/up stream ~11 us
 //     late and have to catch up with the 84 SMs whose CTAs were resident — and pre-filled their rings — meanwhile.
 //   * weights are immutable, so the ring is filled BEFORE griddepcontrol.wait: under programmatic dependent launch the
