@@ -110,9 +110,9 @@ static size_t carve(const hq_config *c, char *base, Buffers *b) {
     o.pf_tok = (int *)take(R * sizeof(int));
     o.last_idx = (int *)take(B * sizeof(int));
     o.xs = (float *)take(R * d * sizeof(float));
-    o.delta = (float *)take(R * d * sizeof(float));
+    o.delta = (float *)take(kPrefillSplits * R * d * sizeof(float));
     o.hn = (act_t *)take(2 * R * d * sizeof(act_t));
-    o.qkv = (float *)take(R * qkvd * sizeof(float));
+    o.qkv = (float *)take(kPrefillSplits * R * qkvd * sizeof(float));
     o.q16 = (__half *)take(R * qdim * sizeof(__half));
     o.ao = (act_t *)take(2 * R * qdim * sizeof(act_t));
     o.actb = (act_t *)take(2 * R * F * sizeof(act_t));
@@ -274,6 +274,28 @@ static int tile_index(int rows) { return rows <= 32 ? 0 : rows <= 64 ? 1 : rows 
 struct TilePlan { int ti, NT, splits; };
 static TilePlan plan_gemm(const hq_model *m, int n_rows, int rows, int K, int max_splits) {
     const int n_tiles = (n_rows + 127) / 128;
+    if (rows > 32 && max_splits > 1) {
+        // Prefill pass with split-K partial buffers (no atomics).  At these sizes a GEMM is bound by moving its operands from L2
+        // into shared memory (profiles/r02_ncu_full_summary.md: DRAM 9-21 %, tensor pipe 20-49 %): a CTA pulls ~65 GB/s of
+        // tiles (~40 with 256-token tiles: two stages only), the chip ~8.5 TB/s.  Pick the (token tile, splits) with the
+        // least modelled time: the slower of the per-CTA stream (times the number of waves) and the chip-wide one.
+        const int kb = (K + 63) / 64;
+        TilePlan best{1, 64, 1};
+        double best_t = 1e30;
+        for (int ti = 1; ti <= 3; ++ti) {
+            const int NT = kTokenTiles[ti];
+            if (ti > 1 && NT > ((rows + 63) / 64) * 64) continue;   // no tile wider than the pass (rounded to 64)
+            const int t_tiles = (rows + NT - 1) / NT;
+            for (int sp = 1; sp <= max_splits; sp *= 2) {
+                if (sp > 1 && kb / sp < 8) break;
+                const double ctas = (double)n_tiles * t_tiles * sp, waves = ceil(ctas / m->n_sms);
+                const double per_cta = (double)((kb + sp - 1) / sp) * (16384.0 + 2.0 * NT * 128.0);
+                const double t = fmax(waves * per_cta / (NT == 256 ? 40e9 : 65e9), ctas * per_cta / 8.5e12) + 2e-6 * (sp - 1) / 4;
+                if (t < best_t) { best_t = t; best = TilePlan{ti, NT, sp}; }
+            }
+        }
+        return best;
+    }
     const int ti_max = tile_index(rows);
     int ti = ti_max;
     while (ti > 1 && n_tiles * ((rows + kTokenTiles[ti] - 1) / kTokenTiles[ti]) < (m->n_sms * 3) / 4) --ti;
@@ -309,33 +331,34 @@ static cudaError_t enqueue_rows_layers(hq_model *m, int batch, int Tc, bool deco
     // Prefill passes defer the residual adds of the O and down projections (bit-reproducible split-K, see
     // rmsnorm_rows_kernel); decode steps add atomically into the residual.
     const bool defer = !decode;
-    if (defer) {
-        e = cudaMemsetAsync(b.delta, 0, (size_t)rows * d * sizeof(float), m->stream);
-        if (e != cudaSuccess) return e;
-    }
+    // split-K partials of the O / down projection not yet added to xs (prefill passes): buffers R * d floats apart
+    const size_t d_stride = (size_t)R * d, q_stride = (size_t)R * qkvd;
+    int pending = 0;
     for (int l = 0; l < c.n_layers; ++l) {
         const LayerW &w = m->layers[l];
         const LayerMaps &mp = m->maps[l];
         kv_t *kc = b.kcache + l * layer_kv, *vc = b.vcache + l * layer_kv;
-        STEP(launch_rmsnorm_rows(lc, b.xs, defer ? b.delta : nullptr, w.attn_norm, b.hn, lo_d, d, c.rms_eps, rows, nullptr, d));
+        STEP(launch_rmsnorm_rows(lc, b.xs, b.delta, pending, d_stride, w.attn_norm, b.hn, lo_d, d, c.rms_eps, rows, nullptr, d));
+        pending = 0;
         // P1: Q, K, V projections (three weight pointers, no repack) into one fp32 [rows][qkvd] buffer
         const bool stacked = qdim % 128 == 0 && kvdim % 128 == 0;
-        const int split_store = decode ? 16 : 2, split_resid = decode ? 16 : 2;
+        const int split_store = decode ? 16 : kPrefillSplits, split_resid = decode ? 16 : kPrefillSplits;
         const TilePlan pq = plan_gemm(m, stacked ? qkvd : qdim, rows, d, split_store);
-        if (pq.splits > 1) {
+        const size_t qs = defer ? q_stride : 0;   // prefill: one partial buffer per split; batched decode: atomics into a zeroed buffer
+        if (pq.splits > 1 && !defer) {
             e = cudaMemsetAsync(b.qkv, 0, (size_t)rows * qkvd * sizeof(float), m->stream);
             if (e != cudaSuccess) return e;
         }
         if (stacked) {
-            STEP(launch_gemm_qkv(lc, mp.wq, mp.wk, mp.wv, m->map_hn[pq.ti], R, qdim, kvdim, kvdim, d, rows, pq.NT, pq.splits, b.qkv, qkvd));
+            STEP(launch_gemm_qkv(lc, mp.wq, mp.wk, mp.wv, m->map_hn[pq.ti], R, qdim, kvdim, kvdim, d, rows, pq.NT, pq.splits, b.qkv, qkvd, qs));
         } else {
-            STEP(launch_gemm(lc, EPI_STORE, mp.wq, nullptr, m->map_hn[pq.ti], R, qdim, d, rows, pq.NT, pq.splits, b.qkv, nullptr, 0, qkvd));
-            STEP(launch_gemm(lc, EPI_STORE, mp.wk, nullptr, m->map_hn[pq.ti], R, kvdim, d, rows, pq.NT, pq.splits, b.qkv + qdim, nullptr, 0, qkvd));
-            STEP(launch_gemm(lc, EPI_STORE, mp.wv, nullptr, m->map_hn[pq.ti], R, kvdim, d, rows, pq.NT, pq.splits, b.qkv + qdim + kvdim, nullptr, 0, qkvd));
+            STEP(launch_gemm(lc, EPI_STORE, mp.wq, nullptr, m->map_hn[pq.ti], R, qdim, d, rows, pq.NT, pq.splits, b.qkv, nullptr, 0, qkvd, qs));
+            STEP(launch_gemm(lc, EPI_STORE, mp.wk, nullptr, m->map_hn[pq.ti], R, kvdim, d, rows, pq.NT, pq.splits, b.qkv + qdim, nullptr, 0, qkvd, qs));
+            STEP(launch_gemm(lc, EPI_STORE, mp.wv, nullptr, m->map_hn[pq.ti], R, kvdim, d, rows, pq.NT, pq.splits, b.qkv + qdim + kvdim, nullptr, 0, qkvd, qs));
         }
-        // P4: RoPE + KV append
-        STEP(launch_rope_append(lc, b.qkv, b.q16, decode ? b.q : nullptr, kc, vc, b.rope, b.pos, rows, Tc, c.n_heads,
-                                c.n_kv_heads, c.max_seq));
+        // P4: RoPE + KV append (adds the split-K partials of the projection in order)
+        STEP(launch_rope_append(lc, b.qkv, defer ? pq.splits : 1, q_stride, b.q16, decode ? b.q : nullptr, kc, vc, b.rope, b.pos, rows, Tc,
+                                c.n_heads, c.n_kv_heads, c.max_seq));
         if (decode) {
             // B2: split-KV decode attention per sequence, then merge
             AttnDecodeParams a = {b.q, kc, vc, b.part_o, b.part_ml, b.pos, c.n_heads, c.n_kv_heads, c.max_seq};
@@ -347,15 +370,21 @@ static cudaError_t enqueue_rows_layers(hq_model *m, int batch, int Tc, bool deco
         }
         const TilePlan po = plan_gemm(m, d, rows, qdim, split_resid);
         STEP(launch_gemm(lc, defer ? EPI_STORE : EPI_RESID, mp.wo, nullptr, m->map_ao[po.ti], R, d, qdim, rows, po.NT, po.splits,
-                         defer ? b.delta : b.xs, nullptr, 0, d));
-        STEP(launch_rmsnorm_rows(lc, b.xs, defer ? b.delta : nullptr, w.ffn_norm, b.hn, lo_d, d, c.rms_eps, rows, nullptr, d));
+                         defer ? b.delta : b.xs, nullptr, 0, d, defer ? d_stride : 0));
+        if (defer) pending = po.splits;
+        STEP(launch_rmsnorm_rows(lc, b.xs, b.delta, pending, d_stride, w.ffn_norm, b.hn, lo_d, d, c.rms_eps, rows, nullptr, d));
+        pending = 0;
         const TilePlan pg = plan_gemm(m, c.ffn, rows, d, 1);
         STEP(launch_gemm(lc, EPI_SWIGLU, mp.w_gate, &mp.w_up, m->map_hn[pg.ti], R, c.ffn, d, rows, pg.NT, 1, nullptr, b.actb,
                          lo_f, c.ffn));
         const TilePlan pd = plan_gemm(m, d, rows, c.ffn, split_resid);
         STEP(launch_gemm(lc, defer ? EPI_STORE : EPI_RESID, mp.w_down, nullptr, m->map_actb[pd.ti], R, d, c.ffn, rows, pd.NT, pd.splits,
-                         defer ? b.delta : b.xs, nullptr, 0, d));
-        if (defer && capture_hidden) STEP(launch_add_delta_rows(lc, b.xs, b.delta, (size_t)rows * d));
+                         defer ? b.delta : b.xs, nullptr, 0, d, defer ? d_stride : 0));
+        if (defer) pending = pd.splits;
+        if (defer && capture_hidden) {
+            STEP(launch_add_delta_rows(lc, b.xs, b.delta, pending, d_stride, (size_t)rows * d));
+            pending = 0;
+        }
         if (capture_hidden) {
             // residual of the last position of every sequence -> hidden[l][b]
             e = cudaMemcpy2DAsync(b.hidden + (size_t)l * c.max_batch * d, d * sizeof(float),
@@ -365,6 +394,7 @@ static cudaError_t enqueue_rows_layers(hq_model *m, int batch, int Tc, bool deco
         }
     }
 #undef STEP
+    m->delta_pending = pending;   // consumed by the head / verification pass that follows
     if (n_launched) *n_launched += n;
     return cudaSuccess;
 }
@@ -382,14 +412,15 @@ static cudaError_t enqueue_rows_head(hq_model *m, int batch, int Tc, int pos_inc
         // one sequence: the batch-1 LM-head GEMV (A9: final norm, 6.4 TB/s weight stream, fused argmax and bookkeeping) on the
         // last row of the pass instead of norm + 32-token-tile GEMM + argmax (116 + 10 us -> 85 us)
         float *xl = b.xs + (size_t)(Tc - 1) * c.hidden;
-        if (deferred) STEP(launch_add_delta_rows(lc, xl, b.delta + (size_t)(Tc - 1) * c.hidden, (size_t)c.hidden));
+        if (deferred && m->delta_pending) STEP(launch_add_delta_rows(lc, xl, b.delta + (size_t)(Tc - 1) * c.hidden, m->delta_pending, (size_t)m->pf_rows * c.hidden, (size_t)c.hidden));
         STEP(launch_sgemv(lc, sgemv_lm_head(m, xl, pos_inc)));
         if (n_launched) *n_launched += n;
         return cudaSuccess;
     }
     // rows (Tc-1), (2Tc-1), ... : stride Tc rows starting at row Tc-1
-    STEP(launch_rmsnorm_rows(lc, b.xs + (size_t)(Tc - 1) * c.hidden, deferred ? b.delta + (size_t)(Tc - 1) * c.hidden : nullptr, m->final_norm, b.hn_last, (size_t)32 * c.hidden,
-                             c.hidden, c.rms_eps, batch, nullptr, Tc * c.hidden));
+    STEP(launch_rmsnorm_rows(lc, b.xs + (size_t)(Tc - 1) * c.hidden, b.delta + (size_t)(Tc - 1) * c.hidden, deferred ? m->delta_pending : 0,
+                             (size_t)m->pf_rows * c.hidden, m->final_norm, b.hn_last, (size_t)32 * c.hidden, c.hidden, c.rms_eps, batch, nullptr,
+                             Tc * c.hidden));
     STEP(launch_gemm(lc, EPI_STORE, m->map_lm_head, nullptr, m->map_hn_last, 32, c.vocab, c.hidden, batch, 32, 1, b.logits,
                      nullptr, 0, c.vocab));
     STEP(launch_argmax_rows(lc, b.logits, c.vocab, batch, b.cur_tok, b.tok_hist, b.pos, pos_inc, b.counter, b.best));
@@ -756,8 +787,8 @@ extern "C" int32_t hq_verify_relay(hq_model *m, const int32_t *tokens_host, int3
     // LM head at the n_answer + 1 positions n_envelope - 1 .. T - 1: final norm (folds the deferred residual of the last
     // layer in) -> one GEMM over the vocabulary (weights read once per 256-token tile) -> per-row argmax against the answer
     const int r0 = n_envelope - 1;
-    HQ_CUDA(launch_rmsnorm_rows(lc, b.xs + (size_t)r0 * d, b.delta + (size_t)r0 * d, m->final_norm, b.hn, (size_t)m->pf_rows * d, d,
-                                c.rms_eps, nv, nullptr, d));
+    HQ_CUDA(launch_rmsnorm_rows(lc, b.xs + (size_t)r0 * d, b.delta + (size_t)r0 * d, m->delta_pending, (size_t)m->pf_rows * d, m->final_norm, b.hn,
+                                (size_t)m->pf_rows * d, d, c.rms_eps, nv, nullptr, d));
     const TilePlan pv = plan_gemm(m, c.vocab, nv, d, 1);
     HQ_CUDA(launch_gemm(lc, EPI_STORE, m->map_lm_head, nullptr, m->map_hn[pv.ti], m->pf_rows, c.vocab, d, nv, pv.NT, 1,
                         b.verify_logits, nullptr, 0, c.vocab));
@@ -767,8 +798,6 @@ extern "C" int32_t hq_verify_relay(hq_model *m, const int32_t *tokens_host, int3
     int accepted = 0;
     HQ_CUDA(cudaMemcpyAsync(&accepted, b.verify_out, sizeof(int), cudaMemcpyDeviceToHost, m->stream));
     HQ_CUDA(cudaStreamSynchronize(m->stream));
-    // the rows of the pass that were not consumed by the final norm still carry a deferred residual: clear it for the next pass
-    HQ_CUDA(cudaMemsetAsync(b.delta, 0, (size_t)T * d * sizeof(float), m->stream));
     // hq_decode_logits: the logits that chose the token now waiting to be fed
     HQ_CUDA(cudaMemcpyAsync(b.logits, b.verify_logits + (size_t)accepted * c.vocab, (size_t)c.vocab * sizeof(float),
                             cudaMemcpyDeviceToDevice, m->stream));

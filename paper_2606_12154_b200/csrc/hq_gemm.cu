@@ -257,7 +257,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap map_w, const __grid_constant_
                 for (int j = 0; j < 32; ++j) {
                     const int t = t0 + c + j;
                     if (t < p.T) {
-                        float *dst = p.out_f32 + (size_t)t * p.ld_out + n;
+                        float *dst = p.out_f32 + (size_t)blockIdx.z * p.split_stride + (size_t)t * p.ld_out + n;
                         const float val = __uint_as_float(v[j]);
                         if (p.atomic) atomicAdd(dst, val);
                         else if (MODE == EPI_RESID) *dst = __ldcg(dst) + val;
@@ -340,7 +340,7 @@ static cudaError_t launch_mode(const LaunchCtx &c, const TensorMap &w, const Ten
 // zeroed buffer, EPI_RESID always legal).
 cudaError_t launch_gemm(const LaunchCtx &c, GemmEpilogue mode, const TensorMap &w, const TensorMap *w2,
                         const TensorMap &x, int x_lo_row, int n_rows, int K, int T, int NT, int splits, float *out_f32,
-                        act_t *out_act, size_t out_lo_offset, int ld_out) {
+                        act_t *out_act, size_t out_lo_offset, int ld_out, size_t split_stride) {
     // K need not be a multiple of 64: TMA zero-fills the out-of-range tail of the last K block
     if (K % 8 != 0 || NT % 32 != 0 || NT < 32 || NT > 256 || T <= 0) return cudaErrorInvalidValue;
     const int kblocks = (K + kBlockK - 1) / kBlockK;
@@ -350,7 +350,9 @@ cudaError_t launch_gemm(const LaunchCtx &c, GemmEpilogue mode, const TensorMap &
     p.K = K; p.n_rows = n_rows; p.T = T; p.NT = NT; p.k_blocks = kblocks;
     p.k_blocks_per_split = (kblocks + splits - 1) / splits;
     splits = (kblocks + p.k_blocks_per_split - 1) / p.k_blocks_per_split;
-    p.out_f32 = out_f32; p.out_act = out_act; p.out_lo_offset = out_lo_offset; p.x_lo_row = x_lo_row; p.ld_out = ld_out; p.atomic = splits > 1 ? 1 : 0;
+    p.out_f32 = out_f32; p.out_act = out_act; p.out_lo_offset = out_lo_offset; p.x_lo_row = x_lo_row; p.ld_out = ld_out;
+    p.split_stride = mode == EPI_STORE ? split_stride : 0;
+    p.atomic = (splits > 1 && p.split_stride == 0) ? 1 : 0;
     const int n_tiles = (n_rows + kBlockM - 1) / kBlockM, t_tiles = (T + NT - 1) / NT;
     switch (mode) {
         case EPI_STORE: return launch_mode<EPI_STORE>(c, w, w, w, x, p, n_tiles, t_tiles, splits);
@@ -365,7 +367,8 @@ cudaError_t launch_gemm(const LaunchCtx &c, GemmEpilogue mode, const TensorMap &
 // Q, K and V projections in ONE launch: three weight matrices with n1, n2, n3 rows (multiples of 128) stacked along
 // the output dimension of out_f32 [T][n1 + n2 + n3].
 cudaError_t launch_gemm_qkv(const LaunchCtx &c, const TensorMap &wq, const TensorMap &wk, const TensorMap &wv, const TensorMap &x,
-                            int x_lo_row, int n1, int n2, int n3, int K, int T, int NT, int splits, float *out_f32, int ld_out) {
+                            int x_lo_row, int n1, int n2, int n3, int K, int T, int NT, int splits, float *out_f32, int ld_out,
+                            size_t split_stride) {
     if (K % 8 != 0 || NT % 32 != 0 || NT < 32 || NT > 256 || T <= 0 || n1 % kBlockM || n2 % kBlockM || n3 % kBlockM)
         return cudaErrorInvalidValue;
     const int kblocks = (K + kBlockK - 1) / kBlockK;
@@ -375,7 +378,8 @@ cudaError_t launch_gemm_qkv(const LaunchCtx &c, const TensorMap &wq, const Tenso
     p.K = K; p.n_rows = n1 + n2 + n3; p.T = T; p.NT = NT; p.k_blocks = kblocks;
     p.k_blocks_per_split = (kblocks + splits - 1) / splits;
     splits = (kblocks + p.k_blocks_per_split - 1) / p.k_blocks_per_split;
-    p.out_f32 = out_f32; p.x_lo_row = x_lo_row; p.ld_out = ld_out; p.atomic = splits > 1 ? 1 : 0;
+    p.out_f32 = out_f32; p.x_lo_row = x_lo_row; p.ld_out = ld_out; p.split_stride = split_stride;
+    p.atomic = (splits > 1 && split_stride == 0) ? 1 : 0;
     p.tiles_w1 = n1 / kBlockM; p.tiles_w2 = n2 / kBlockM;
     return launch_mode<EPI_STORE>(c, wq, wk, wv, x, p, p.n_rows / kBlockM, (T + NT - 1) / NT, splits);
 }

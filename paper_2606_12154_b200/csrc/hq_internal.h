@@ -30,6 +30,7 @@ constexpr int kHeadDim = 64;        // only head_dim the kernels implement
 constexpr int kMaxSplits = 16;      // split-KV partials per head (decode attention)
 constexpr int kMinSplitLen = 64;    // do not split contexts shorter than this per split
 constexpr int kGemvThreads = 256;
+constexpr int kPrefillSplits = 4;   // split-K partial buffers of a prefill pass (qkv, delta): each split stores its own, consumers add in order
 constexpr int kVerifyRows = 256;    // answer tokens + 1 of one hq_verify_relay call (the paper's rule: answer lines of at most ~230 tokens)
 struct alignas(64) TensorMap { uint64_t opaque[16]; };   // mirrors CUtensorMap (driver type, 128 bytes)
 
@@ -107,6 +108,7 @@ struct hq_model_impl {
     TensorMap map_hn[4], map_ao[4], map_actb[4], map_hn_last;   // activation maps per token tile
     cudaGraphExec_t batch_graph = nullptr;      // batched decode step (captured for batch_graph_b)
     int batch_graph_b = 0, batch_graph_kernels = 0, batch_eager_b = 0;
+    int delta_pending = 0;                      // split-K partials of the last O / down projection of a pass not yet added to xs
     bool use_attn_block = false;                // per-step path: QKV + attention + O of a layer in one cluster launch (hq_attn.cu)
     unsigned long long *trace = nullptr;        // hq_debug_trace: device buffer [n_sms][trace_cap] or NULL
     unsigned long long *step_trace = nullptr;   // hq_debug_step_trace: device buffer [slots][4] or NULL
@@ -227,24 +229,26 @@ struct GemmParams {
     int ld_out;
     int atomic;
     int x_lo_row;       // row offset of the lo plane inside the activation tensor map
+    size_t split_stride;      // > 0: K split z stores its partial at out_f32 + z * split_stride (no atomics; the consumer adds them in order)
     int tiles_w1, tiles_w2;   // EPI_STORE over three stacked weight matrices: 128-row tiles of the first and second (0 = one matrix)
 };
 bool make_tensor_map_16b(TensorMap *out, const void *base, uint64_t rows, uint64_t cols, uint32_t box_rows);
 cudaError_t gemm_prepare();   // shared-memory opt-in on the current device
 cudaError_t launch_gemm(const LaunchCtx &c, GemmEpilogue mode, const TensorMap &w, const TensorMap *w2,
                         const TensorMap &x, int x_lo_row, int n_rows, int K, int T, int NT, int splits, float *out_f32,
-                        act_t *out_act, size_t out_lo_offset, int ld_out);
+                        act_t *out_act, size_t out_lo_offset, int ld_out, size_t split_stride = 0);
 
 cudaError_t launch_gemm_qkv(const LaunchCtx &c, const TensorMap &wq, const TensorMap &wk, const TensorMap &wv, const TensorMap &x,
-                            int x_lo_row, int n1, int n2, int n3, int K, int T, int NT, int splits, float *out_f32, int ld_out);
+                            int x_lo_row, int n1, int n2, int n3, int K, int T, int NT, int splits, float *out_f32, int ld_out,
+                            size_t split_stride = 0);
 
 // ---- row-batched kernels (hq_prefill.cu) -------------------------------------------------------------
 cudaError_t launch_embed_rows(const LaunchCtx &c, const bf16 *emb, const int *tok, float *x, int hidden, int rows);
-cudaError_t launch_rmsnorm_rows(const LaunchCtx &c, float *x, float *delta, const bf16 *gain, act_t *out, size_t lo_offset,
-                                int hidden, float eps, int rows, const int *row_index, int x_stride_rows);
-cudaError_t launch_add_delta_rows(const LaunchCtx &c, float *x, float *delta, size_t n);
-cudaError_t launch_rope_append(const LaunchCtx &c, const float *qkv, __half *q16, float *q32, kv_t *kc, kv_t *vc,
-                               const float2 *rope, const int *pos, int rows, int Tc, int n_heads, int n_kv_heads,
+cudaError_t launch_rmsnorm_rows(const LaunchCtx &c, float *x, const float *delta, int n_parts, size_t part_stride, const bf16 *gain,
+                                act_t *out, size_t lo_offset, int hidden, float eps, int rows, const int *row_index, int x_stride_rows);
+cudaError_t launch_add_delta_rows(const LaunchCtx &c, float *x, const float *delta, int n_parts, size_t part_stride, size_t n);
+cudaError_t launch_rope_append(const LaunchCtx &c, const float *qkv, int n_parts, size_t part_stride, __half *q16, float *q32, kv_t *kc,
+                               kv_t *vc, const float2 *rope, const int *pos, int rows, int Tc, int n_heads, int n_kv_heads,
                                int max_seq);
 cudaError_t launch_flash_prefill(const LaunchCtx &c, const __half *q16, const kv_t *kc, const kv_t *vc, act_t *out,
                                  size_t lo_offset, const int *pos, int batch, int Tc, int n_heads, int n_kv_heads, int max_seq);

@@ -27,10 +27,10 @@ __global__ void __launch_bounds__(256) embed_rows_kernel(const bf16 *__restrict_
 }
 
 // one CTA per row; x row stays in L1/L2 between the two passes
-// delta (optional): the deferred output of the previous residual projection, x += delta first (written back, delta
-// zeroed for its next use).  Keeps split-K of those projections bit-reproducible: two splits add into a zeroed buffer
-// (0 + a + b in either order) instead of into the residual (x + a + b is order-dependent).
-__global__ void __launch_bounds__(256) rmsnorm_rows_kernel(float *x, float *delta, const bf16 *__restrict__ gain,
+// delta (n_parts > 0): the deferred output of the previous residual projection as n_parts split-K partial buffers,
+// part_stride floats apart: x += delta[0] + delta[1] + ... first, in that order, written back.  Keeps split-K of those
+// projections bit-reproducible without atomics: every split stores its own partial, the consumer adds them in order.
+__global__ void __launch_bounds__(256) rmsnorm_rows_kernel(float *x, const float *delta, int n_parts, size_t part_stride, const bf16 *__restrict__ gain,
                                                            act_t *__restrict__ out, size_t lo_offset, int hidden,
                                                            float eps, const int *row_index, int x_stride_rows) {
     pdl_launch_dependents();
@@ -40,15 +40,16 @@ __global__ void __launch_bounds__(256) rmsnorm_rows_kernel(float *x, float *delt
     // row_index (optional) gathers rows (e.g. last position of every sequence)
     const size_t src = row_index ? (size_t)row_index[m] : (size_t)m;
     float *xr = x + src * x_stride_rows;
-    float *dr = delta ? delta + src * x_stride_rows : nullptr;
+    const float *dr = (delta && n_parts > 0) ? delta + src * x_stride_rows : nullptr;
     float ss = 0.f;
     for (int c = threadIdx.x; c < (hidden >> 2); c += blockDim.x) {
         float4 v = ld_act4(xr + c * 4);
         if (dr) {
-            const float4 dv = ld_act4(dr + c * 4);
-            v.x += dv.x; v.y += dv.y; v.z += dv.z; v.w += dv.w;
+            for (int sp = 0; sp < n_parts; ++sp) {
+                const float4 dv = ld_act4(dr + (size_t)sp * part_stride + c * 4);
+                v.x += dv.x; v.y += dv.y; v.z += dv.z; v.w += dv.w;
+            }
             *reinterpret_cast<float4 *>(xr + c * 4) = v;
-            *reinterpret_cast<float4 *>(dr + c * 4) = make_float4(0.f, 0.f, 0.f, 0.f);
         }
         ss += v.x * v.x + v.y * v.y + v.z * v.z + v.w * v.w;
     }
@@ -72,7 +73,7 @@ __global__ void __launch_bounds__(256) rmsnorm_rows_kernel(float *x, float *delt
 
 // qkv fp32 [M][(H + 2 Hkv) * 64] -> q (fp16 [M][H*64], optional fp32 copy), K/V cache rows.
 // grid (M), block 256: thread handles (head-any hh, i) pairs in a loop.
-__global__ void __launch_bounds__(256) rope_append_kernel(const float *qkv, __half *q16, float *q32, kv_t *kc, kv_t *vc,
+__global__ void __launch_bounds__(256) rope_append_kernel(const float *qkv, int n_parts, size_t part_stride, __half *q16, float *q32, kv_t *kc, kv_t *vc,
                                                           const float2 *__restrict__ rope, const int *pos_ptr, int Tc,
                                                           int n_heads, int n_kv_heads, int max_seq) {
     pdl_launch_dependents();
@@ -84,7 +85,11 @@ __global__ void __launch_bounds__(256) rope_append_kernel(const float *qkv, __ha
     const float *src = qkv + (size_t)m * nh * kHeadDim;
     for (int idx = threadIdx.x; idx < nh * 32; idx += blockDim.x) {
         const int hh = idx >> 5, i = idx & 31;
-        const float a = ld_act(src + hh * kHeadDim + i), c = ld_act(src + hh * kHeadDim + i + 32);
+        float a = ld_act(src + hh * kHeadDim + i), c = ld_act(src + hh * kHeadDim + i + 32);
+        for (int sp = 1; sp < n_parts; ++sp) {   // split-K partials of the projection, fixed order
+            a += ld_act(src + (size_t)sp * part_stride + hh * kHeadDim + i);
+            c += ld_act(src + (size_t)sp * part_stride + hh * kHeadDim + i + 32);
+        }
         if (hh < n_heads + n_kv_heads) {
             const float2 cs = rope[(size_t)pos * 32 + i];
             const float ra = a * cs.x - c * cs.y, rc = c * cs.x + a * cs.y;
@@ -478,30 +483,31 @@ static cudaError_t launch_k(const LaunchCtx &c, void (*kernel)(KArgs...), dim3 g
 cudaError_t launch_embed_rows(const LaunchCtx &c, const bf16 *emb, const int *tok, float *x, int hidden, int rows) {
     return launch_k(c, embed_rows_kernel, dim3(rows), dim3(256), emb, tok, x, hidden);
 }
-cudaError_t launch_rmsnorm_rows(const LaunchCtx &c, float *x, float *delta, const bf16 *gain, act_t *out, size_t lo_offset,
-                                int hidden, float eps, int rows, const int *row_index, int x_stride_rows) {
-    return launch_k(c, rmsnorm_rows_kernel, dim3(rows), dim3(256), x, delta, gain, out, lo_offset, hidden, eps, row_index,
-                    x_stride_rows);
+cudaError_t launch_rmsnorm_rows(const LaunchCtx &c, float *x, const float *delta, int n_parts, size_t part_stride, const bf16 *gain,
+                                act_t *out, size_t lo_offset, int hidden, float eps, int rows, const int *row_index, int x_stride_rows) {
+    return launch_k(c, rmsnorm_rows_kernel, dim3(rows), dim3(256), x, delta, n_parts, part_stride, gain, out, lo_offset, hidden, eps,
+                    row_index, x_stride_rows);
 }
 // x += delta, delta = 0 (parity capture needs the residual itself after every layer)
-__global__ void __launch_bounds__(256) add_delta_rows_kernel(float *x, float *delta, size_t n4) {
+__global__ void __launch_bounds__(256) add_delta_rows_kernel(float *x, const float *delta, int n_parts, size_t part_stride, size_t n4) {
     pdl_launch_dependents();
     pdl_wait();
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += (size_t)gridDim.x * blockDim.x) {
         float4 v = ld_act4(x + i * 4);
-        const float4 dv = ld_act4(delta + i * 4);
-        v.x += dv.x; v.y += dv.y; v.z += dv.z; v.w += dv.w;
+        for (int sp = 0; sp < n_parts; ++sp) {   // the split-K partials in fixed order
+            const float4 dv = ld_act4(delta + (size_t)sp * part_stride + i * 4);
+            v.x += dv.x; v.y += dv.y; v.z += dv.z; v.w += dv.w;
+        }
         *reinterpret_cast<float4 *>(x + i * 4) = v;
-        *reinterpret_cast<float4 *>(delta + i * 4) = make_float4(0.f, 0.f, 0.f, 0.f);
     }
 }
-cudaError_t launch_add_delta_rows(const LaunchCtx &c, float *x, float *delta, size_t n) {
-    return launch_k(c, add_delta_rows_kernel, dim3(296), dim3(256), x, delta, n / 4);
+cudaError_t launch_add_delta_rows(const LaunchCtx &c, float *x, const float *delta, int n_parts, size_t part_stride, size_t n) {
+    return launch_k(c, add_delta_rows_kernel, dim3(296), dim3(256), x, delta, n_parts, part_stride, n / 4);
 }
-cudaError_t launch_rope_append(const LaunchCtx &c, const float *qkv, __half *q16, float *q32, kv_t *kc, kv_t *vc,
-                               const float2 *rope, const int *pos, int rows, int Tc, int n_heads, int n_kv_heads,
+cudaError_t launch_rope_append(const LaunchCtx &c, const float *qkv, int n_parts, size_t part_stride, __half *q16, float *q32, kv_t *kc,
+                               kv_t *vc, const float2 *rope, const int *pos, int rows, int Tc, int n_heads, int n_kv_heads,
                                int max_seq) {
-    return launch_k(c, rope_append_kernel, dim3(rows), dim3(256), qkv, q16, q32, kc, vc, rope, pos, Tc, n_heads,
+    return launch_k(c, rope_append_kernel, dim3(rows), dim3(256), qkv, n_parts, part_stride, q16, q32, kc, vc, rope, pos, Tc, n_heads,
                     n_kv_heads, max_seq);
 }
 cudaError_t launch_flash_prefill(const LaunchCtx &c, const __half *q16, const kv_t *kc, const kv_t *vc, act_t *out,
