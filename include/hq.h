@@ -16,14 +16,20 @@
  *  - All GPU work is enqueued on the one CUDA stream given at create time, in call order.  Calls
  *    that hand a result to a HOST pointer synchronise that stream before returning; all others
  *    are asynchronous.  Asynchronous CUDA faults surface at the next synchronising call.
- *  - Every call returns HQ_OK (0) or a negative hq_status; on error the model state (KV cache
- *    length, last token) is unchanged and hq_last_error() describes the failure.  No exceptions,
- *    no abort().  There is NO CPU fallback: without a CUDA device the calls return HQ_ERR_CUDA.
+ *  - Every call returns HQ_OK (0) or a negative hq_status and hq_last_error() describes the failure.
+ *    HQ_ERR_INVALID_ARG / CAPACITY / STATE / UNSUPPORTED are detected before any work is enqueued: the
+ *    model state (KV cache length, last token) is unchanged.  After HQ_ERR_CUDA (a runtime call or a
+ *    kernel failed, possibly midway through a multi-launch call) the device-side position may be ahead of
+ *    the host's: call hq_kv_reset (or destroy the model) before using it again.  No exceptions, no
+ *    abort().  There is NO CPU fallback: without a CUDA device the calls return HQ_ERR_CUDA.
  *  - Weight matrices are bf16, nn.Linear layout [out_features, in_features], row-major, rows
  *    16-byte aligned.  Norm gains are bf16 [hidden].  Activations inside the library: fp32
  *    residual stream, fp32 accumulators/softmax/norm statistics, fp16 KV cache (2 bytes per element,
- *    32,768 B per cached token for the 1B shape), on the tensor cores (prefill / batched decode only) bf16
- *    weight operands x activation operands split into two bf16 planes hi + lo (16 mantissa bits).
+ *    32,768 B per cached token for the 1B shape; K/V magnitudes beyond 65,504 would overflow it).  Every
+ *    matrix product runs on the tensor cores with bf16 weight operands x activation operands split into two
+ *    bf16 planes hi + lo (16 mantissa bits, bf16 range): mma.sync in the batch-1 decode kernels, tcgen05 in
+ *    prefill / batched decode; the vectors between kernels (SwiGLU output, normalised hidden state, attention
+ *    output) are stored as those two planes or as fp32.  Prefill attention computes in fp16 mma.sync.
  *  - Sequences of a batch advance in lock step (equal lengths), as in every BASELINE.json config.
  */
 #ifndef HQ_H_
