@@ -177,6 +177,11 @@ static SgemvParams sgemv_down(const hq_model *m, int l) {
     p.trace = m->step_trace; p.trace_slot = 3 + 3 * l;
     p.mode = SGEMV_RESID; p.xin_mode = SGEMV_XIN_PLANES; p.out = m->b.x;
     if (m->q4) { p.q0 = m->layers_q4[l].down_q; p.e0 = m->layers_q4[l].down_e; }
+    // Three quarters of the SMs stream the down projection as fast as all of them (HBM is the limit from ~64 streaming SMs
+    // on, profiles/r02_copy_size.md); the others are free for the clusters of the next layer's attention block, which become
+    // resident — barriers, cluster sync, first weight stages — under this kernel instead of after it (measured: 104-124 CTAs
+    // all -2 % of the step, 84 and 128-148 none)
+    if (m->use_attn_block) p.max_ctas = (m->n_sms * 3) / 4;
     return p;
 }
 // final norm + LM head + argmax over the residual row x; the position advances by pos_inc

@@ -157,6 +157,7 @@ struct SgemvParams {
     unsigned int *counter;
     int *cur_tok, *tok_hist, *pos_rw;
     int pos_inc;
+    int max_ctas;            // > 0: launch at most this many CTAs (leave the other SMs to the kernel that follows)
     int n_early;             // CTAs expected to start (and pre-fill their rings) while the previous kernel holds the other SMs
     float late_deficit;      // ... and how many stages more than the others each of them takes
     unsigned long long *trace;   // NULL or step timeline [slots][4] (hq_debug_step_trace)

@@ -363,7 +363,8 @@ cudaError_t launch_sgemv(const LaunchCtx &c, const SgemvParams &p) {
     if (!sgemv_shape_supported(p.K)) return cudaErrorInvalidValue;
     const int rps = sg_rows_per_stage(p.K, p.mode);
     const int n_stages = (p.n_rows + rps - 1) / rps;
-    const int grid = c.n_sms < n_stages ? c.n_sms : n_stages;
+    int grid = c.n_sms < n_stages ? c.n_sms : n_stages;
+    if (p.max_ctas > 0 && p.max_ctas < grid) grid = p.max_ctas;
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(grid);
     cfg.blockDim = dim3(kSgThreads);

@@ -461,7 +461,8 @@ cudaError_t launch_sgemv_q4(const LaunchCtx &c, const SgemvParams &p) {
     const int rps = q4_rows_per_stage(p.K, p.mode);
     if ((size_t)(p.mode == SGEMV_GATEUP ? 16 : rps) * (p.K / 2) > (size_t)kQ4CodeBytes) return cudaErrorInvalidValue;
     const int n_stages = (p.n_rows + rps - 1) / rps;
-    const int grid = c.n_sms < n_stages ? c.n_sms : n_stages;
+    int grid = c.n_sms < n_stages ? c.n_sms : n_stages;
+    if (p.max_ctas > 0 && p.max_ctas < grid) grid = p.max_ctas;
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(grid);
     cfg.blockDim = dim3(kQ4Threads);
