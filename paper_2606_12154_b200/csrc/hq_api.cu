@@ -294,7 +294,8 @@ static TilePlan plan_gemm(const hq_model *m, int n_rows, int rows, int K, int ma
             for (int sp = 1; sp <= max_splits; sp *= 2) {
                 if (sp > 1 && kb / sp < 8) break;
                 const double ctas = (double)n_tiles * t_tiles * sp, waves = ceil(ctas / m->n_sms);
-                const double per_cta = (double)((kb + sp - 1) / sp) * (16384.0 + 2.0 * NT * 128.0);
+                // tile bytes per K block: the weight tile + the token tile's planes (CTA pairs, token tile <= 128: one plane each)
+                const double per_cta = (double)((kb + sp - 1) / sp) * (16384.0 + (NT <= 128 ? 1.0 : 2.0) * NT * 128.0);
                 const double t = fmax(waves * per_cta / (NT == 256 ? 40e9 : 65e9), ctas * per_cta / 8.5e12) + 2e-6 * (sp - 1) / 4;
                 if (t < best_t) { best_t = t; best = TilePlan{ti, NT, sp}; }
             }

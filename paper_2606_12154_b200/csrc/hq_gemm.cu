@@ -60,6 +60,31 @@ __device__ __forceinline__ void umma_bf16(uint32_t tmem_d, uint64_t desc_a, uint
         "l"(desc_a), "l"(desc_b), "r"(idesc), "r"(accumulate)
         : "memory");
 }
+// ---- CTA pair (cta_group::2): two CTAs of a cluster run ONE MMA of M = 256: each holds 128 rows of A (weights) and half of
+// the rows of B (here: one of the two activation planes); both TMA-load into their own shared memory and credit the bytes to
+// the LEADER's (even rank's) mbarrier; the leader issues the MMA and its commit arrives on the barriers of both CTAs.
+constexpr uint32_t kPeerBitMask = 0xFEFFFFFFu;   // clears the peer bit of a shared-window address: the even CTA of the pair
+__device__ __forceinline__ void tma_load_2d_pair(const CUtensorMap *map, uint64_t *leader_bar, void *smem_dst, int c0, int c1) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];" ::"r"(
+            smem_u32(smem_dst)),
+        "l"(map), "r"(smem_u32(leader_bar) & kPeerBitMask), "r"(c0), "r"(c1)
+        : "memory");
+}
+__device__ __forceinline__ void umma_bf16_pair(uint32_t tmem_d, uint64_t desc_a, uint64_t desc_b, uint32_t idesc, uint32_t accumulate) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, {%5, %5, %5, %5, %5, %5, %5, %5}, p;\n\t}" ::"r"(tmem_d),
+        "l"(desc_a), "l"(desc_b), "r"(idesc), "r"(accumulate), "r"(0u)
+        : "memory");
+}
+// arrives (once the MMAs issued so far have retired) on the barrier at the same shared-memory offset in BOTH CTAs of the pair
+__device__ __forceinline__ void tcgen05_commit_pair(uint64_t *bar) {
+    asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;" ::"r"(smem_u32(bar)),
+                 "h"((unsigned short)3)
+                 : "memory");
+}
+
 // 32 lanes x 32 columns of fp32: thread (lane) gets 32 consecutive columns of its own TMEM lane
 __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
     asm volatile(
@@ -86,11 +111,11 @@ __device__ __forceinline__ uint64_t make_smem_desc(uint32_t smem_addr) {
 // kind::f16 instruction descriptor: D fp32 (bits 4-5 = 1), A and B bf16 (bits 7-9 and 10-12 = 1; the two
 // formats must match: a bf16 x fp16 descriptor raises an illegal-instruction fault on sm_100a), both K-major
 // (bits 15, 16 = 0), N >> 3 at bits 17-22, M >> 4 at bits 24-28
-__host__ __device__ inline uint32_t make_idesc(int n) {
-    return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(kBlockM >> 4) << 24);
+__host__ __device__ inline uint32_t make_idesc(int n, int m = kBlockM) {
+    return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(m >> 4) << 24);
 }
 
-template <int MODE>
+template <int MODE, int CTAS>
 __global__ void __launch_bounds__(kGemmThreads, 1)
 gemm_tc_kernel(const __grid_constant__ CUtensorMap map_w, const __grid_constant__ CUtensorMap map_w2,
                const __grid_constant__ CUtensorMap map_w3, const __grid_constant__ CUtensorMap map_x, const GemmParams p) {
@@ -99,7 +124,9 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap map_w, const __grid_constant_
     const int NT = p.NT;
     const uint32_t a_bytes = kBlockM * kBlockK * 2;          // 16 KB per weight tile
     const uint32_t b_bytes = (uint32_t)NT * kBlockK * 2;      // one plane (hi or lo) of the token tile
-    const uint32_t stage_bytes = NACC * a_bytes + 2 * b_bytes;
+    // CTA pair: this CTA holds ONE plane (rank 0 hi, rank 1 lo): together the B operand of 2 NT rows of the pair's MMA
+    const uint32_t stage_bytes = NACC * a_bytes + (CTAS == 2 ? 1 : 2) * b_bytes;
+    const uint32_t pair_rank = CTAS == 2 ? cluster_ctarank() : 0;
     const int stages = p.stages;
 
     uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
@@ -117,7 +144,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap map_w, const __grid_constant_
     // NT <= 128: the hi and lo activation planes of a stage lie back to back and are ONE B operand of 2 NT rows: one MMA per
     // K step fills D columns [0, NT) with W x_hi and [NT, 2 NT) with W x_lo (half the MMA instructions, a quarter less
     // operand traffic from shared memory than two MMAs into the same columns); the epilogue adds the two halves
-    const bool stacked = NT <= 128;
+    const bool stacked = NT <= 128;   // always true for CTA pairs (launch_mode)
     const int acc_cols = stacked ? 2 * NT : NT;          // TMEM columns of one accumulator
     const uint32_t need_cols = (uint32_t)(NACC * acc_cols);
     const uint32_t tmem_cols = need_cols <= 32 ? 32 : need_cols <= 64 ? 64 : need_cols <= 128 ? 128 : need_cols <= 256 ? 256 : 512;
@@ -133,9 +160,15 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap map_w, const __grid_constant_
         mbarrier_init(acc_bar, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
+    if (CTAS == 2) cluster_sync_all();   // the barriers of both CTAs exist before either allocates, loads or commits
     if (warp == 1) {
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "r"(tmem_cols) : "memory");
-        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+        if (CTAS == 2) {
+            asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "r"(tmem_cols) : "memory");
+            asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+        } else {
+            asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "r"(tmem_cols) : "memory");
+            asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+        }
     }
     tcgen05_fence_before();
     __syncthreads();
@@ -157,13 +190,20 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap map_w, const __grid_constant_
             // Weights do not depend on the previous kernel: the first ring of weight tiles is requested BEFORE the
             // programmatic-dependency wait, so the launch and the first HBM round trip overlap the previous kernel's tail.
             const int pre = nkb < stages ? nkb : stages;
-            for (int i = 0; i < pre; ++i) {
-                uint8_t *st = smem + (size_t)i * stage_bytes;
-                mbarrier_expect_tx(&full_bar[i], stage_bytes);
-                const int kc = (kb0 + i) * kBlockK;
-                tma_load_2d(mw, &full_bar[i], st, kc, nw);
-                if (NACC == 2) tma_load_2d(&map_w2, &full_bar[i], st + a_bytes, kc, n0);
-            }
+            // CTA pair: every load of both CTAs is credited to the leader's barrier, which expects both CTAs' stage bytes
+            auto load_w = [&](int s, int kc) {
+                uint8_t *st = smem + (size_t)s * stage_bytes;
+                if (CTAS == 2) {
+                    if (pair_rank == 0) mbarrier_expect_tx(&full_bar[s], 2 * stage_bytes);
+                    tma_load_2d_pair(mw, &full_bar[s], st, kc, nw);
+                    if (NACC == 2) tma_load_2d_pair(&map_w2, &full_bar[s], st + a_bytes, kc, n0);
+                } else {
+                    mbarrier_expect_tx(&full_bar[s], stage_bytes);
+                    tma_load_2d(mw, &full_bar[s], st, kc, nw);
+                    if (NACC == 2) tma_load_2d(&map_w2, &full_bar[s], st + a_bytes, kc, n0);
+                }
+            };
+            for (int i = 0; i < pre; ++i) load_w(i, (kb0 + i) * kBlockK);
             pdl_wait();   // activations come from earlier kernels
             for (int i = 0; i < nkb; ++i) {
                 const int s = i % stages;
@@ -172,17 +212,40 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap map_w, const __grid_constant_
                 const int kc = (kb0 + i) * kBlockK;
                 if (i >= pre) {
                     mbarrier_wait(&empty_bar[s], ph ^ 1);
-                    mbarrier_expect_tx(&full_bar[s], stage_bytes);
-                    tma_load_2d(mw, &full_bar[s], st, kc, nw);
-                    if (NACC == 2) tma_load_2d(&map_w2, &full_bar[s], st + a_bytes, kc, n0);
+                    load_w(s, kc);
                 }
-                tma_load_2d(&map_x, &full_bar[s], st + NACC * a_bytes, kc, t0);
-                tma_load_2d(&map_x, &full_bar[s], st + NACC * a_bytes + b_bytes, kc, p.x_lo_row + t0);
+                if (CTAS == 2) {
+                    tma_load_2d_pair(&map_x, &full_bar[s], st + NACC * a_bytes, kc, (pair_rank ? p.x_lo_row : 0) + t0);
+                } else {
+                    tma_load_2d(&map_x, &full_bar[s], st + NACC * a_bytes, kc, t0);
+                    tma_load_2d(&map_x, &full_bar[s], st + NACC * a_bytes + b_bytes, kc, p.x_lo_row + t0);
+                }
             }
         }
     } else if (warp == 1) {
         // ===== MMA issuer (one elected thread) =====
-        if (lane == 0) {
+        if (lane == 0 && CTAS == 2) {
+            // leader of the pair only: M = 256 (128 rows of A from each CTA), N = 2 NT (the hi plane from rank 0, the lo plane from rank 1)
+            if (pair_rank == 0) {
+                const uint32_t idesc = make_idesc(2 * NT, 2 * kBlockM);
+                for (int i = 0; i < nkb; ++i) {
+                    const int s = i % stages;
+                    const uint32_t ph = (i / stages) & 1;
+                    mbarrier_wait(&full_bar[s], ph);
+                    tcgen05_fence_after();
+                    const uint32_t a_addr = smem_u32(smem + (size_t)s * stage_bytes);
+                    const uint64_t da = make_smem_desc(a_addr), da2 = make_smem_desc(a_addr + a_bytes), db = make_smem_desc(a_addr + NACC * a_bytes);
+#pragma unroll
+                    for (int k = 0; k < kBlockK / 16; ++k) {
+                        const uint32_t acc = (i > 0 || k > 0) ? 1u : 0u;
+                        umma_bf16_pair(tmem_base, da + 2 * k, db + 2 * k, idesc, acc);
+                        if (NACC == 2) umma_bf16_pair(tmem_base + acc_cols, da2 + 2 * k, db + 2 * k, idesc, acc);
+                    }
+                    tcgen05_commit_pair(&empty_bar[s]);   // frees the stage in BOTH CTAs when these MMAs retire
+                }
+                tcgen05_commit_pair(acc_bar);             // accumulators of both CTAs complete
+            }
+        } else if (lane == 0) {
             const uint32_t idesc = make_idesc(stacked ? 2 * NT : NT);
             for (int i = 0; i < nkb; ++i) {
                 const int s = i % stages;
@@ -269,9 +332,11 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap map_w, const __grid_constant_
         tcgen05_fence_before();
     }
     __syncthreads();
+    if (CTAS == 2) cluster_sync_all();   // neither CTA frees tensor memory or exits while the pair's MMAs / loads may still touch it
     if (warp == 1) {
         tcgen05_fence_after();
-        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(tmem_cols) : "memory");
+        if (CTAS == 2) asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(tmem_cols) : "memory");
+        else asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(tmem_cols) : "memory");
     }
 }
 
@@ -314,23 +379,42 @@ template <int MODE>
 static cudaError_t launch_mode(const LaunchCtx &c, const TensorMap &w, const TensorMap &w2, const TensorMap &w3,
                                const TensorMap &x, GemmParams p, int n_tiles, int t_tiles, int splits) {
     const int nacc = (MODE == EPI_SWIGLU) ? 2 : 1;
-    const int stage_bytes = nacc * kBlockM * kBlockK * 2 + 2 * p.NT * kBlockK * 2;
+    // CTA pairs (cta_group::2, M = 256) for prefill-sized passes: the activation tile is shared by two weight tiles, each CTA
+    // loads one of its two planes (a third less operand traffic from L2, the bound of these GEMMs).  Needs the stacked-plane
+    // form (token tile <= 128); batched-decode steps (<= 32 rows) keep single CTAs.
+    const bool pair = p.NT <= 128 && p.T > 32;
+    const int stage_bytes = nacc * kBlockM * kBlockK * 2 + (pair ? 1 : 2) * p.NT * kBlockK * 2;
     int stages = kSmemBudget / stage_bytes;
     if (stages > 8) stages = 8;
     if (stages > p.k_blocks_per_split) stages = p.k_blocks_per_split < 2 ? 2 : p.k_blocks_per_split;
     p.stages = stages;
     const size_t smem = (size_t)stages * stage_bytes + 1024 + (2 * stages + 1) * 8 + 16;
     cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3(n_tiles, t_tiles, splits);
+    cfg.gridDim = dim3(pair ? (n_tiles + 1) / 2 * 2 : n_tiles, t_tiles, splits);   // a pair's odd tile past the end loads zeros (TMA) and stores nothing
     cfg.blockDim = dim3(kGemmThreads);
     cfg.dynamicSmemBytes = smem;
     cfg.stream = c.stream;
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cudaLaunchAttribute attr[2];
+    int na = 0;
+    if (c.pdl) {
+        attr[na].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[na].val.programmaticStreamSerializationAllowed = 1;
+        ++na;
+    }
+    if (pair) {
+        attr[na].id = cudaLaunchAttributeClusterDimension;
+        attr[na].val.clusterDim.x = 2;
+        attr[na].val.clusterDim.y = 1;
+        attr[na].val.clusterDim.z = 1;
+        ++na;
+    }
     cfg.attrs = attr;
-    cfg.numAttrs = c.pdl ? 1 : 0;
-    return cudaLaunchKernelEx(&cfg, gemm_tc_kernel<MODE>, *reinterpret_cast<const CUtensorMap *>(&w),
+    cfg.numAttrs = na;
+    if (pair)
+        return cudaLaunchKernelEx(&cfg, gemm_tc_kernel<MODE, 2>, *reinterpret_cast<const CUtensorMap *>(&w),
+                                  *reinterpret_cast<const CUtensorMap *>(&w2), *reinterpret_cast<const CUtensorMap *>(&w3),
+                                  *reinterpret_cast<const CUtensorMap *>(&x), p);
+    return cudaLaunchKernelEx(&cfg, gemm_tc_kernel<MODE, 1>, *reinterpret_cast<const CUtensorMap *>(&w),
                               *reinterpret_cast<const CUtensorMap *>(&w2), *reinterpret_cast<const CUtensorMap *>(&w3),
                               *reinterpret_cast<const CUtensorMap *>(&x), p);
 }
@@ -387,9 +471,12 @@ cudaError_t launch_gemm_qkv(const LaunchCtx &c, const TensorMap &wq, const Tenso
 // Shared-memory opt-in of every instantiation on the CURRENT device (the attribute is per device: hq_model_create and
 // hq_debug_gemm call this, not a process-wide once-flag).
 cudaError_t gemm_prepare() {
-    cudaError_t e = cudaFuncSetAttribute(gemm_tc_kernel<EPI_STORE>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(gemm_tc_kernel<EPI_RESID>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(gemm_tc_kernel<EPI_SWIGLU>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    cudaError_t e = cudaFuncSetAttribute(gemm_tc_kernel<EPI_STORE, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(gemm_tc_kernel<EPI_RESID, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(gemm_tc_kernel<EPI_SWIGLU, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(gemm_tc_kernel<EPI_STORE, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(gemm_tc_kernel<EPI_RESID, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(gemm_tc_kernel<EPI_SWIGLU, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     return e;
 }
 

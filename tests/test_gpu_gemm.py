@@ -41,6 +41,9 @@ def _case(N, K, T, seed):
     (256, 688, 33, 64, 2),       # ragged K (688 = 10*64 + 48): TMA zero fill
     (2048, 8192, 300, 256, 9),   # down-proj shape, two token tiles
     (384, 512, 8, 32, 2),        # batched-decode shape: 8 sequences padded to a 32-token tile
+    (384, 512, 100, 64, 1),      # CTA pairs (token tile <= 128, more than 32 tokens) with an odd number of weight tiles
+    (3072, 2048, 256, 128, 2),   # the 1B Q|K|V shape as the prefill pass runs it: CTA pairs, 128-token tiles, 2 K splits
+    (2048, 8192, 256, 128, 4),   # the 1B down-projection shape: CTA pairs, 4 K splits
 ])
 def test_gemm_store_matches_oracle_matmul(N, K, T, tile, splits):
     import torch
