@@ -230,6 +230,8 @@ def main():
                     help="memory-system probes behind the kernel design: bulk-copy size vs per-SM rate, read-only stream; JSON lines")
     ap.add_argument("--profile", type=int, default=0, metavar="N",
                     help="ncu helper: one prefill + N decode steps of the bench workload, no timing")
+    ap.add_argument("--profile-batch", type=int, default=1, metavar="B",
+                    help="with --profile: B sequences of the configs[3] shape (192-token prompts) instead of the batch-1 query")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -499,6 +501,19 @@ def main():
             b.record(stream)
             torch.cuda.synchronize(dev)
             print(json.dumps({"probe": "read_only_ldg", "GBps": 5 * buf.numel() / (a.elapsed_time(b) * 1e-3) / 1e9}), flush=True)
+        return
+
+    if args.profile and args.profile_batch > 1:
+        B = args.profile_batch
+        bm = hq.Model(hq.binding.make_config(n_layers=s.n_layers, hidden=s.hidden, n_heads=s.n_heads, n_kv_heads=s.n_kv_heads,
+                                             head_dim=s.head_dim, ffn=s.ffn, vocab=s.vocab, rms_eps=s.rms_eps,
+                                             rope_theta=s.rope_theta, max_batch=B, max_seq=512, flags=0), *gm.weight_tensors())
+        bm.prefill(datagen.tokens(1003, s.vocab, B * 192).reshape(B, 192), want_token=False)
+        bm.sync()
+        before = bm.kernel_count()
+        bm.decode_run(args.profile, want_tokens=False, batch=B)
+        bm.sync()
+        print(json.dumps({"profile": True, "batch": B, "decode_launches": bm.kernel_count() - before}), flush=True)
         return
 
     if args.profile:

@@ -32,6 +32,7 @@ int32_t hq_bench_kernel(hq_model *m, int32_t which, int32_t reps, int64_t *bytes
  *   mode 0: out fp32 [n_tokens][n_rows]  = x w^T   (splits > 1: out must be zeroed, partials add atomically)
  *   mode 1: out fp32 [n_tokens][n_rows] += x w^T   (residual epilogue)
  *   mode 2: out bf16 [2][n_tokens][n_rows] = hi/lo planes of silu(x w^T) * (x w2^T)   (SwiGLU epilogue)
+ *   mode 3: the result of mode 2 computed from 64-row weight tiles (the batched-decode form; n_rows % 64 == 0)
  * Asynchronous on cuda_stream. */
 int32_t hq_debug_gemm(void *cuda_stream, int32_t mode, const void *w_dev, const void *w2_dev, const void *x_dev,
                       void *out_dev, int32_t n_rows, int32_t k, int32_t n_tokens, int32_t token_tile, int32_t splits);

@@ -381,8 +381,10 @@ static cudaError_t enqueue_rows_layers(hq_model *m, int batch, int Tc, bool deco
         STEP(launch_rmsnorm_rows(lc, b.xs, b.delta, pending, d_stride, w.ffn_norm, b.hn, lo_d, d, c.rms_eps, rows, nullptr, d));
         pending = 0;
         const TilePlan pg = plan_gemm(m, c.ffn, rows, d, 1);
-        STEP(launch_gemm(lc, EPI_SWIGLU, mp.w_gate, &mp.w_up, m->map_hn[pg.ti], R, c.ffn, d, rows, pg.NT, 1, nullptr, b.actb,
-                         lo_f, c.ffn));
+        // batched decode (one token tile): 64-row weight tiles, so that ffn / 64 CTAs stream gate/up instead of ffn / 128
+        const bool half_tiles = decode && c.ffn % 64 == 0 && (c.ffn / 128) * ((rows + pg.NT - 1) / pg.NT) < m->n_sms;
+        STEP(launch_gemm(lc, half_tiles ? EPI_SWIGLU64 : EPI_SWIGLU, half_tiles ? mp.w_gate64 : mp.w_gate, half_tiles ? &mp.w_up64 : &mp.w_up,
+                         m->map_hn[pg.ti], R, c.ffn, d, rows, pg.NT, 1, nullptr, b.actb, lo_f, c.ffn));
         const TilePlan pd = plan_gemm(m, d, rows, c.ffn, split_resid);
         STEP(launch_gemm(lc, defer ? EPI_STORE : EPI_RESID, mp.w_down, nullptr, m->map_actb[pd.ti], R, d, c.ffn, rows, pd.NT, pd.splits,
                          defer ? b.delta : b.xs, nullptr, 0, d, defer ? d_stride : 0));
@@ -480,7 +482,8 @@ static bool build_tensor_maps(hq_model *m) {
         ok = ok && make_tensor_map_16b(&mp.wq, w.wq, qdim, d, 128) && make_tensor_map_16b(&mp.wk, w.wk, kvdim, d, 128) &&
              make_tensor_map_16b(&mp.wv, w.wv, kvdim, d, 128) && make_tensor_map_16b(&mp.wo, w.wo, d, qdim, 128) &&
              make_tensor_map_16b(&mp.w_gate, w.w_gate, F, d, 128) && make_tensor_map_16b(&mp.w_up, w.w_up, F, d, 128) &&
-             make_tensor_map_16b(&mp.w_down, w.w_down, d, F, 128);
+             make_tensor_map_16b(&mp.w_down, w.w_down, d, F, 128) && make_tensor_map_16b(&mp.w_gate64, w.w_gate, F, d, 64) &&
+             make_tensor_map_16b(&mp.w_up64, w.w_up, F, d, 64);
     }
     ok = ok && make_tensor_map_16b(&m->map_lm_head, m->lm_head, c.vocab, d, 128);
     for (int i = 0; i < 4; ++i) {
@@ -1040,19 +1043,21 @@ extern "C" int32_t hq_debug_gemm(void *cuda_stream, int32_t mode, const void *w_
                                  int32_t token_tile, int32_t splits) {
     if (!w_dev || !x_dev || !out_dev || n_rows <= 0 || k <= 0 || n_tokens <= 0)
         return fail(HQ_ERR_INVALID_ARG, "hq_debug_gemm: bad argument");
-    if (mode < 0 || mode > 2 || (mode == 2 && !w2_dev)) return fail(HQ_ERR_INVALID_ARG, "hq_debug_gemm: bad mode");
+    if (mode < 0 || mode > 3 || (mode >= 2 && !w2_dev)) return fail(HQ_ERR_INVALID_ARG, "hq_debug_gemm: bad mode");
+    if (mode == 3 && n_rows % 64 != 0) return fail(HQ_ERR_UNSUPPORTED, "hq_debug_gemm: mode 3 needs n_rows % 64 == 0");
     if (token_tile != 32 && token_tile != 64 && token_tile != 128 && token_tile != 256)
         return fail(HQ_ERR_INVALID_ARG, "hq_debug_gemm: token_tile must be 32, 64, 128 or 256");
     if (k % 8 != 0) return fail(HQ_ERR_UNSUPPORTED, "hq_debug_gemm: k must be a multiple of 8");
     TensorMap mw, mw2, mx;
     // x_dev holds the hi plane [n_tokens][k] followed by the lo plane [n_tokens][k]
-    if (!make_tensor_map_16b(&mw, w_dev, n_rows, k, 128) || !make_tensor_map_16b(&mx, x_dev, 2 * (uint64_t)n_tokens, k, token_tile) ||
-        (mode == 2 && !make_tensor_map_16b(&mw2, w2_dev, n_rows, k, 128)))
+    const uint32_t wbox = mode == 3 ? 64 : 128;
+    if (!make_tensor_map_16b(&mw, w_dev, n_rows, k, wbox) || !make_tensor_map_16b(&mx, x_dev, 2 * (uint64_t)n_tokens, k, token_tile) ||
+        (mode >= 2 && !make_tensor_map_16b(&mw2, w2_dev, n_rows, k, wbox)))
         return fail(HQ_ERR_CUDA, "hq_debug_gemm: cuTensorMapEncodeTiled failed");
     const LaunchCtx lc{(cudaStream_t)cuda_stream, false, 148};
     HQ_CUDA(gemm_prepare());
-    HQ_CUDA(launch_gemm(lc, (GemmEpilogue)mode, mw, mode == 2 ? &mw2 : nullptr, mx, n_tokens, n_rows, k, n_tokens, token_tile,
-                        mode == 2 ? 1 : splits, mode == 2 ? nullptr : (float *)out_dev, mode == 2 ? (act_t *)out_dev : nullptr,
+    HQ_CUDA(launch_gemm(lc, (GemmEpilogue)mode, mw, mode >= 2 ? &mw2 : nullptr, mx, n_tokens, n_rows, k, n_tokens, token_tile,
+                        mode >= 2 ? 1 : splits, mode >= 2 ? nullptr : (float *)out_dev, mode >= 2 ? (act_t *)out_dev : nullptr,
                         (size_t)n_tokens * n_rows, n_rows));
     return HQ_OK;
 }

@@ -11,6 +11,10 @@
 //   EPI_STORE   out_f32[t][n]  = D            (split-K: atomic add into a zeroed buffer)
 //   EPI_RESID   x[t][n]       += D            (residual add; split-K partials add atomically)
 //   EPI_SWIGLU  act[t][f]      = hi/lo bf16 of silu(D_gate) * D_up   two accumulators, two weight maps
+//   EPI_SWIGLU64  the same result from 64-row weight tiles: one CTA takes 64 gate rows AND the 64 up rows of the same
+//               features as the two halves of ONE 128-row A tile (one accumulator; the epilogue warps of the up half
+//               hand their values to the gate half through shared memory).  Twice the CTAs of EPI_SWIGLU: the form
+//               batched decode uses, where ffn / 128 tiles leave more than half of the SMs idle.
 // Warp roles (192 threads): warp 0 TMA producer, warp 1 TMEM owner + MMA issuer, warps 2-5 epilogue.
 #include <cuda.h>
 
@@ -121,6 +125,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap map_w, const __grid_constant_
                const __grid_constant__ CUtensorMap map_w3, const __grid_constant__ CUtensorMap map_x, const GemmParams p) {
     extern __shared__ __align__(1024) uint8_t smem_raw[];
     constexpr int NACC = (MODE == EPI_SWIGLU) ? 2 : 1;
+    constexpr bool HALF = MODE == EPI_SWIGLU64;
     const int NT = p.NT;
     const uint32_t a_bytes = kBlockM * kBlockK * 2;          // 16 KB per weight tile
     const uint32_t b_bytes = (uint32_t)NT * kBlockK * 2;      // one plane (hi or lo) of the token tile
@@ -136,7 +141,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap map_w, const __grid_constant_
     uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(acc_bar + 1);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int n0 = blockIdx.x * kBlockM;           // first weight row of this CTA
+    const int n0 = blockIdx.x * (HALF ? kBlockM / 2 : kBlockM);   // first weight row of this CTA
     const int t0 = blockIdx.y * NT;                // first token of this CTA
     const int kb0 = blockIdx.z * p.k_blocks_per_split;
     const int kb1 = min(kb0 + p.k_blocks_per_split, p.k_blocks);
@@ -152,7 +157,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap map_w, const __grid_constant_
     if (warp == 0 && lane == 0) {
         asm volatile("prefetch.tensormap [%0];" ::"l"(&map_w) : "memory");
         asm volatile("prefetch.tensormap [%0];" ::"l"(&map_x) : "memory");
-        if (NACC == 2) asm volatile("prefetch.tensormap [%0];" ::"l"(&map_w2) : "memory");
+        if (NACC == 2 || HALF) asm volatile("prefetch.tensormap [%0];" ::"l"(&map_w2) : "memory");
         for (int s = 0; s < stages; ++s) {
             mbarrier_init(&full_bar[s], 1);
             mbarrier_init(&empty_bar[s], 1);
@@ -199,8 +204,9 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap map_w, const __grid_constant_
                     if (NACC == 2) tma_load_2d_pair(&map_w2, &full_bar[s], st + a_bytes, kc, n0);
                 } else {
                     mbarrier_expect_tx(&full_bar[s], stage_bytes);
-                    tma_load_2d(mw, &full_bar[s], st, kc, nw);
+                    tma_load_2d(mw, &full_bar[s], st, kc, nw);   // HALF: a 64-row box (rows 0..63 of the A tile: gate)
                     if (NACC == 2) tma_load_2d(&map_w2, &full_bar[s], st + a_bytes, kc, n0);
+                    if (HALF) tma_load_2d(&map_w2, &full_bar[s], st + a_bytes / 2, kc, n0);   // rows 64..127: up
                 }
             };
             for (int i = 0; i < pre; ++i) load_w(i, (kb0 + i) * kBlockK);
@@ -279,7 +285,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap map_w, const __grid_constant_
     } else {
         // ===== epilogue: warp w owns TMEM lanes 32*(w%4) .. +31 =====
         const int q = warp & 3;
-        const int n = n0 + 32 * q + lane;
+        const int n = n0 + 32 * (HALF ? (q & 1) : q) + lane;
         pdl_wait();   // the output buffer (residual, zeroed split-K target) belongs to earlier kernels until now
         mbarrier_wait(acc_bar, 0);
         tcgen05_fence_after();
@@ -294,7 +300,30 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap map_w, const __grid_constant_
 #pragma unroll
                 for (int j = 0; j < 32; ++j) v[j] = __float_as_uint(__uint_as_float(v[j]) + __uint_as_float(w[j]));
             }
-            if (MODE == EPI_SWIGLU) {
+            if (HALF) {
+                // lanes 64..127 of the accumulator (warps q = 2, 3) hold the up projection of the features whose gate
+                // projection is in lanes 0..63 (q = 0, 1): hand it over through stage 0 of the ring (every load has been
+                // consumed and every MMA has retired once acc_bar completes), [token][feature] so that lanes do not conflict
+                float *xch = reinterpret_cast<float *>(smem);
+                if (q >= 2) {
+#pragma unroll
+                    for (int j = 0; j < 32; ++j) xch[j * 64 + 32 * (q - 2) + lane] = __uint_as_float(v[j]);
+                }
+                asm volatile("bar.sync 1, 128;" ::: "memory");
+                if (q < 2 && row_ok) {
+#pragma unroll
+                    for (int j = 0; j < 32; ++j) {
+                        const int t = t0 + c + j;
+                        if (t < p.T) {
+                            act_t hi, lo;
+                            split_bf16(silu_f(__uint_as_float(v[j])) * xch[j * 64 + 32 * q + lane], hi, lo);
+                            p.out_act[(size_t)t * p.ld_out + n] = hi;
+                            p.out_act[p.out_lo_offset + (size_t)t * p.ld_out + n] = lo;
+                        }
+                    }
+                }
+                if (c + 32 < NT) asm volatile("bar.sync 1, 128;" ::: "memory");
+            } else if (MODE == EPI_SWIGLU) {
                 uint32_t u[32];
                 tmem_ld32(lane_addr + acc_cols + c, u);
                 if (stacked) {
@@ -382,7 +411,7 @@ static cudaError_t launch_mode(const LaunchCtx &c, const TensorMap &w, const Ten
     // CTA pairs (cta_group::2, M = 256) for prefill-sized passes: the activation tile is shared by two weight tiles, each CTA
     // loads one of its two planes (a third less operand traffic from L2, the bound of these GEMMs).  Needs the stacked-plane
     // form (token tile <= 128); batched-decode steps (<= 32 rows) keep single CTAs.
-    const bool pair = p.NT <= 128 && p.T > 32;
+    const bool pair = MODE != EPI_SWIGLU64 && p.NT <= 128 && p.T > 32;
     const int stage_bytes = nacc * kBlockM * kBlockK * 2 + (pair ? 1 : 2) * p.NT * kBlockK * 2;
     int stages = kSmemBudget / stage_bytes;
     if (stages > 8) stages = 8;
@@ -410,7 +439,8 @@ static cudaError_t launch_mode(const LaunchCtx &c, const TensorMap &w, const Ten
     }
     cfg.attrs = attr;
     cfg.numAttrs = na;
-    if (pair)
+    if constexpr (MODE != EPI_SWIGLU64)
+      if (pair)
         return cudaLaunchKernelEx(&cfg, gemm_tc_kernel<MODE, 2>, *reinterpret_cast<const CUtensorMap *>(&w),
                                   *reinterpret_cast<const CUtensorMap *>(&w2), *reinterpret_cast<const CUtensorMap *>(&w3),
                                   *reinterpret_cast<const CUtensorMap *>(&x), p);
@@ -444,6 +474,9 @@ cudaError_t launch_gemm(const LaunchCtx &c, GemmEpilogue mode, const TensorMap &
         case EPI_SWIGLU:
             if (splits != 1 || !w2) return cudaErrorInvalidValue;
             return launch_mode<EPI_SWIGLU>(c, w, *w2, w, x, p, n_tiles, t_tiles, 1);
+        case EPI_SWIGLU64:   // w, w2: tensor maps with 64-ROW boxes
+            if (splits != 1 || !w2 || n_rows % (kBlockM / 2) != 0) return cudaErrorInvalidValue;
+            return launch_mode<EPI_SWIGLU64>(c, w, *w2, w, x, p, n_rows / (kBlockM / 2), t_tiles, 1);
     }
     return cudaErrorInvalidValue;
 }
@@ -474,6 +507,7 @@ cudaError_t gemm_prepare() {
     cudaError_t e = cudaFuncSetAttribute(gemm_tc_kernel<EPI_STORE, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(gemm_tc_kernel<EPI_RESID, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(gemm_tc_kernel<EPI_SWIGLU, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(gemm_tc_kernel<EPI_SWIGLU64, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(gemm_tc_kernel<EPI_STORE, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(gemm_tc_kernel<EPI_RESID, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(gemm_tc_kernel<EPI_SWIGLU, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);

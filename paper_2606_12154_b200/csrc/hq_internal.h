@@ -81,7 +81,7 @@ struct Buffers {
 };
 
 constexpr int kTokenTiles[4] = {32, 64, 128, 256};
-struct LayerMaps { TensorMap wq, wk, wv, wo, w_gate, w_up, w_down; };
+struct LayerMaps { TensorMap wq, wk, wv, wo, w_gate, w_up, w_down, w_gate64, w_up64; };   // *64: 64-row boxes (EPI_SWIGLU64)
 
 struct hq_model_impl {
     hq_config cfg;
@@ -221,7 +221,7 @@ cudaError_t attn_block_prepare(int n_kv_heads, bool *co_resident);
 cudaError_t launch_attn_block(const LaunchCtx &c, const AttnBlockParams &p);
 
 // ---- tensor-core GEMM (hq_gemm.cu) -------------------------------------------------------------------
-enum GemmEpilogue { EPI_STORE = 0, EPI_RESID = 1, EPI_SWIGLU = 2 };
+enum GemmEpilogue { EPI_STORE = 0, EPI_RESID = 1, EPI_SWIGLU = 2, EPI_SWIGLU64 = 3 };   // 3: SwiGLU from 64-row tiles (tensor maps with 64-row boxes)
 struct GemmParams {
     int K, n_rows, T, NT, k_blocks, k_blocks_per_split, stages;
     float *out_f32;

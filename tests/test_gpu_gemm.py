@@ -81,17 +81,22 @@ def test_gemm_residual_accumulates():
         assert np.abs(out.cpu().numpy() - want).max() <= 3e-5 * np.abs(want).max()
 
 
-def test_gemm_swiglu_epilogue():
+@pytest.mark.parametrize("mode,N,K,T,tile", [
+    (2, 688, 256, 100, 128),    # two accumulators per 128-row tile, ragged weight rows
+    (3, 704, 256, 8, 32),       # 64-row tiles (batched decode), an odd number of them, 8 sequences in a 32-token tile
+    (3, 8192, 2048, 32, 32),    # the 1B gate/up shape at batch 32
+    (3, 256, 512, 70, 64),      # 64-row tiles, two exchange rounds per token tile, ragged tokens
+])
+def test_gemm_swiglu_epilogue(mode, N, K, T, tile):
     import torch
     import paper_2606_12154_b200 as hq
-    N, K, T = 688, 256, 100
     wg, x = _case(N, K, T, 11)
     wu, _ = _case(N, K, T, 12)
     wgt, wgr = _bf16_tensor(wg)
     wut, wur = _bf16_tensor(wu)
     xt, xr = _hilo_tensor(x)
     out = torch.zeros((2, T, N), dtype=torch.bfloat16, device="cuda")
-    hq.debug_gemm(2, wgt, xt, out, w2=wut, token_tile=128)
+    hq.debug_gemm(mode, wgt, xt, out, w2=wut, token_tile=tile)
     torch.cuda.synchronize()
     g = oracle.matmul(wgr, xr.astype(np.float64))
     u = oracle.matmul(wur, xr.astype(np.float64))
