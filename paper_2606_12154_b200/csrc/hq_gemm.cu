@@ -119,6 +119,44 @@ __host__ __device__ inline uint32_t make_idesc(int n, int m = kBlockM) {
     return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(m >> 4) << 24);
 }
 
+// ---- epilogue helpers.  The epilogue runs after the last MMA with nothing left to overlap it (one tile per CTA), and all
+// CTAs reach it together: its length is pure instruction count (measured with globaltimer stamps: 0.85 us per 32-token
+// chunk of plain stores with a bounds branch and a mode branch per element, 2.9 us per chunk of the SwiGLU form; after
+// the rewrite below ~0.3 / ~1 us).  So: no per-element branches (a chunk is either complete or takes the predicated
+// copy of the loop), reciprocal and exponential from the SFU, and bf16 outputs leave as 32-bit pairs.
+__device__ __forceinline__ float silu_fast(float z) { return z * __frcp_rn(1.0f + __expf(-z)); }   // <= 2 ulp from z / (1 + exp(-z))
+
+// a[j]: this lane's feature n, token j of the chunk (32 tokens).  Writes the hi / lo bf16 planes out[t][n]: lanes exchange
+// with their neighbour so that an even lane stores features (n, n + 1) of an even token and an odd lane those of the
+// next token, as one 32-bit word per plane (half the store instructions; 64 B per token row and instruction).
+// Needs even n0, ld and n_rows (pairs never straddle the end of a row or of the matrix).
+__device__ __forceinline__ void store_act_pairs(const float (&a)[32], act_t *out, size_t lo_offset, size_t ld, int n, bool row_ok, int nvalid, int lane) {
+    const bool odd = lane & 1;
+    act_t *dst = out + (size_t)(odd ? 1 : 0) * ld + (n - (odd ? 1 : 0));
+#pragma unroll
+    for (int j = 0; j < 32; j += 2) {
+        const float other = __shfl_xor_sync(0xffffffffu, odd ? a[j] : a[j + 1], 1);
+        const float x0 = odd ? other : a[j], x1 = odd ? a[j + 1] : other;   // features (n even, n even + 1) of token j + odd
+        uint32_t hi, lo;
+        split_bf16x2(x0, x1, hi, lo);
+        if (row_ok && j + (odd ? 1 : 0) < nvalid) {
+            *reinterpret_cast<uint32_t *>(dst + (size_t)j * ld) = hi;
+            *reinterpret_cast<uint32_t *>(dst + lo_offset + (size_t)j * ld) = lo;
+        }
+    }
+}
+__device__ __forceinline__ void store_act_scalar(const float (&a)[32], act_t *out, size_t lo_offset, size_t ld, bool row_ok, int nvalid) {
+#pragma unroll
+    for (int j = 0; j < 32; ++j) {
+        act_t hi, lo;
+        split_bf16(a[j], hi, lo);
+        if (row_ok && j < nvalid) {
+            out[(size_t)j * ld] = hi;
+            out[lo_offset + (size_t)j * ld] = lo;
+        }
+    }
+}
+
 template <int MODE, int CTAS>
 __global__ void __launch_bounds__(kGemmThreads, 1)
 gemm_tc_kernel(const __grid_constant__ CUtensorMap map_w, const __grid_constant__ CUtensorMap map_w2,
@@ -291,7 +329,9 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap map_w, const __grid_constant_
         tcgen05_fence_after();
         const uint32_t lane_addr = tmem_base + ((uint32_t)(32 * q) << 16);
         const bool row_ok = n < p.n_rows;
+        const bool pairable = (p.n_rows & 1) == 0 && (p.ld_out & 1) == 0;   // bf16 outputs as 32-bit pairs
         for (int c = 0; c < NT; c += 32) {
+            const int nvalid = p.T - (t0 + c);   // tokens of this chunk that exist (>= 32: all)
             uint32_t v[32];
             tmem_ld32(lane_addr + c, v);
             if (stacked) {
@@ -300,61 +340,58 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap map_w, const __grid_constant_
 #pragma unroll
                 for (int j = 0; j < 32; ++j) v[j] = __float_as_uint(__uint_as_float(v[j]) + __uint_as_float(w[j]));
             }
-            if (HALF) {
-                // lanes 64..127 of the accumulator (warps q = 2, 3) hold the up projection of the features whose gate
-                // projection is in lanes 0..63 (q = 0, 1): hand it over through stage 0 of the ring (every load has been
-                // consumed and every MMA has retired once acc_bar completes), [token][feature] so that lanes do not conflict
-                float *xch = reinterpret_cast<float *>(smem);
-                if (q >= 2) {
+            if (HALF || MODE == EPI_SWIGLU) {
+                float a[32];
+                if (HALF) {
+                    // lanes 64..127 of the accumulator (warps q = 2, 3) hold the up projection of the features whose gate
+                    // projection is in lanes 0..63 (q = 0, 1): hand it over through stage 0 of the ring (every load has been
+                    // consumed and every MMA has retired once acc_bar completes), [token][feature] so that lanes do not conflict
+                    float *xch = reinterpret_cast<float *>(smem);
+                    if (q >= 2) {
 #pragma unroll
-                    for (int j = 0; j < 32; ++j) xch[j * 64 + 32 * (q - 2) + lane] = __uint_as_float(v[j]);
-                }
-                asm volatile("bar.sync 1, 128;" ::: "memory");
-                if (q < 2 && row_ok) {
-#pragma unroll
-                    for (int j = 0; j < 32; ++j) {
-                        const int t = t0 + c + j;
-                        if (t < p.T) {
-                            act_t hi, lo;
-                            split_bf16(silu_f(__uint_as_float(v[j])) * xch[j * 64 + 32 * q + lane], hi, lo);
-                            p.out_act[(size_t)t * p.ld_out + n] = hi;
-                            p.out_act[p.out_lo_offset + (size_t)t * p.ld_out + n] = lo;
-                        }
+                        for (int j = 0; j < 32; ++j) xch[j * 64 + 32 * (q - 2) + lane] = __uint_as_float(v[j]);
                     }
-                }
-                if (c + 32 < NT) asm volatile("bar.sync 1, 128;" ::: "memory");
-            } else if (MODE == EPI_SWIGLU) {
-                uint32_t u[32];
-                tmem_ld32(lane_addr + acc_cols + c, u);
-                if (stacked) {
-                    uint32_t w[32];
-                    tmem_ld32(lane_addr + acc_cols + NT + c, w);
+                    asm volatile("bar.sync 1, 128;" ::: "memory");
+                    if (q < 2) {
 #pragma unroll
-                    for (int j = 0; j < 32; ++j) u[j] = __float_as_uint(__uint_as_float(u[j]) + __uint_as_float(w[j]));
-                }
-                if (row_ok) {
-#pragma unroll
-                    for (int j = 0; j < 32; ++j) {
-                        const int t = t0 + c + j;
-                        if (t < p.T) {
-                            act_t hi, lo;
-                            split_bf16(silu_f(__uint_as_float(v[j])) * __uint_as_float(u[j]), hi, lo);
-                            p.out_act[(size_t)t * p.ld_out + n] = hi;
-                            p.out_act[p.out_lo_offset + (size_t)t * p.ld_out + n] = lo;
-                        }
+                        for (int j = 0; j < 32; ++j) a[j] = silu_fast(__uint_as_float(v[j])) * xch[j * 64 + 32 * q + lane];
                     }
-                }
-            } else if (row_ok) {
+                } else {
+                    uint32_t u[32];
+                    tmem_ld32(lane_addr + acc_cols + c, u);
+                    if (stacked) {
+                        uint32_t w[32];
+                        tmem_ld32(lane_addr + acc_cols + NT + c, w);
 #pragma unroll
-                for (int j = 0; j < 32; ++j) {
-                    const int t = t0 + c + j;
-                    if (t < p.T) {
-                        float *dst = p.out_f32 + (size_t)blockIdx.z * p.split_stride + (size_t)t * p.ld_out + n;
-                        const float val = __uint_as_float(v[j]);
-                        if (p.atomic) atomicAdd(dst, val);
-                        else if (MODE == EPI_RESID) *dst = __ldcg(dst) + val;
-                        else *dst = val;
+                        for (int j = 0; j < 32; ++j) u[j] = __float_as_uint(__uint_as_float(u[j]) + __uint_as_float(w[j]));
                     }
+#pragma unroll
+                    for (int j = 0; j < 32; ++j) a[j] = silu_fast(__uint_as_float(v[j])) * __uint_as_float(u[j]);
+                }
+                if ((!HALF || q < 2) && nvalid > 0) {   // warp-uniform
+                    act_t *out = p.out_act + (size_t)(t0 + c) * p.ld_out;
+                    if (pairable) store_act_pairs(a, out, p.out_lo_offset, (size_t)p.ld_out, n, row_ok, nvalid, lane);
+                    else store_act_scalar(a, out + n, p.out_lo_offset, (size_t)p.ld_out, row_ok, nvalid);
+                }
+                if (HALF && c + 32 < NT) asm volatile("bar.sync 1, 128;" ::: "memory");
+            } else if (row_ok && nvalid > 0) {
+                float *dst = p.out_f32 + (size_t)blockIdx.z * p.split_stride + (size_t)(t0 + c) * p.ld_out + n;
+                const size_t ld = (size_t)p.ld_out;
+                if (p.atomic) {
+#pragma unroll
+                    for (int j = 0; j < 32; ++j)
+                        if (j < nvalid) atomicAdd(dst + j * ld, __uint_as_float(v[j]));
+                } else if (MODE == EPI_RESID) {
+#pragma unroll
+                    for (int j = 0; j < 32; ++j)
+                        if (j < nvalid) dst[j * ld] = __ldcg(dst + j * ld) + __uint_as_float(v[j]);
+                } else if (nvalid >= 32) {
+#pragma unroll
+                    for (int j = 0; j < 32; ++j) dst[j * ld] = __uint_as_float(v[j]);
+                } else {
+#pragma unroll
+                    for (int j = 0; j < 32; ++j)
+                        if (j < nvalid) dst[j * ld] = __uint_as_float(v[j]);
                 }
             }
         }
