@@ -41,7 +41,52 @@ __global__ void __launch_bounds__(256) rmsnorm_rows_kernel(float *x, const float
     const size_t src = row_index ? (size_t)row_index[m] : (size_t)m;
     float *xr = x + src * x_stride_rows;
     const float *dr = (delta && n_parts > 0) ? delta + src * x_stride_rows : nullptr;
+    // Every load of a thread is issued before the first value is used (4 float4 of x and up to 4 partials of each: 20 L2
+    // round trips in flight instead of one after the other -- the row kernels are latency, not bandwidth), and the summed
+    // row stays in registers for the second pass.  Rows longer than 4 x 1024 floats take the plain loop below.
+    constexpr int kChunks = 4, kParts = 4;
     float ss = 0.f;
+    if (hidden <= kChunks * 1024 && blockDim.x == 256 && n_parts <= kParts) {
+        const int n4 = hidden >> 2;
+        float4 v[kChunks], dv[kChunks][kParts];
+#pragma unroll
+        for (int k = 0; k < kChunks; ++k) {
+            const int c = threadIdx.x + k * 256;
+            v[k] = c < n4 ? ld_act4(xr + c * 4) : make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+            for (int sp = 0; sp < kParts; ++sp)
+                dv[k][sp] = (dr && sp < n_parts && c < n4) ? ld_act4(dr + (size_t)sp * part_stride + c * 4) : make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+#pragma unroll
+        for (int k = 0; k < kChunks; ++k) {
+            const int c = threadIdx.x + k * 256;
+#pragma unroll
+            for (int sp = 0; sp < kParts; ++sp)
+                if (dr && sp < n_parts) { v[k].x += dv[k][sp].x; v[k].y += dv[k][sp].y; v[k].z += dv[k][sp].z; v[k].w += dv[k][sp].w; }   // fixed order
+            if (dr && c < n4) *reinterpret_cast<float4 *>(xr + c * 4) = v[k];
+            ss += v[k].x * v[k].x + v[k].y * v[k].y + v[k].z * v[k].z + v[k].w * v[k].w;
+        }
+        ss = warp_sum(ss);
+        if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = ss;
+        __syncthreads();
+        float tot = 0.f;
+#pragma unroll
+        for (int w = 0; w < 8; ++w) tot += red[w];
+        const float inv = 1.0f / sqrtf(tot / (float)hidden + eps);
+#pragma unroll
+        for (int k = 0; k < kChunks; ++k) {
+            const int c = threadIdx.x + k * 256;
+            if (c < n4) {
+                const uint2 g = *reinterpret_cast<const uint2 *>(gain + c * 4);
+                uint2 oh, ol;
+                split_bf16x2(v[k].x * inv * bf16lo(g.x), v[k].y * inv * bf16hi(g.x), oh.x, ol.x);
+                split_bf16x2(v[k].z * inv * bf16lo(g.y), v[k].w * inv * bf16hi(g.y), oh.y, ol.y);
+                *reinterpret_cast<uint2 *>(out + (size_t)m * hidden + c * 4) = oh;
+                *reinterpret_cast<uint2 *>(out + lo_offset + (size_t)m * hidden + c * 4) = ol;
+            }
+        }
+        return;
+    }
     for (int c = threadIdx.x; c < (hidden >> 2); c += blockDim.x) {
         float4 v = ld_act4(xr + c * 4);
         if (dr) {
@@ -83,30 +128,59 @@ __global__ void __launch_bounds__(256) rope_append_kernel(const float *qkv, int 
     const int pos = ld_act(pos_ptr) + t;
     const int nh = n_heads + 2 * n_kv_heads;
     const float *src = qkv + (size_t)m * nh * kHeadDim;
-    for (int idx = threadIdx.x; idx < nh * 32; idx += blockDim.x) {
-        const int hh = idx >> 5, i = idx & 31;
-        float a = ld_act(src + hh * kHeadDim + i), c = ld_act(src + hh * kHeadDim + i + 32);
-        for (int sp = 1; sp < n_parts; ++sp) {   // split-K partials of the projection, fixed order
-            a += ld_act(src + (size_t)sp * part_stride + hh * kHeadDim + i);
-            c += ld_act(src + (size_t)sp * part_stride + hh * kHeadDim + i + 32);
+    // three (head, pair) units per thread and round, every load of the round (and of every split-K partial) issued before
+    // the first use: the kernel is a chain of L2 round trips otherwise (6 units x 2 partials one after the other)
+    constexpr int kU = 3;
+    const int lim = nh * 32;
+    for (int idx0 = threadIdx.x; idx0 < lim; idx0 += kU * blockDim.x) {
+        float a[kU], c[kU];
+#pragma unroll
+        for (int u = 0; u < kU; ++u) {
+            const int idx = idx0 + u * (int)blockDim.x, hh = idx >> 5, i = idx & 31;
+            const bool ok = idx < lim;
+            a[u] = ok ? ld_act(src + hh * kHeadDim + i) : 0.f;
+            c[u] = ok ? ld_act(src + hh * kHeadDim + i + 32) : 0.f;
         }
-        if (hh < n_heads + n_kv_heads) {
-            const float2 cs = rope[(size_t)pos * 32 + i];
-            const float ra = a * cs.x - c * cs.y, rc = c * cs.x + a * cs.y;
-            if (hh < n_heads) {
-                const size_t o = ((size_t)m * n_heads + hh) * kHeadDim + i;
-                q16[o] = __float2half_rn(ra);
-                q16[o + 32] = __float2half_rn(rc);
-                if (q32) { q32[o] = ra; q32[o + 32] = rc; }
+        for (int sp = 1; sp < n_parts; sp += 2) {   // split-K partials of the projection, fixed order, two at a time
+            float pa[2][kU], pc[2][kU];
+#pragma unroll
+            for (int s2 = 0; s2 < 2; ++s2)
+#pragma unroll
+                for (int u = 0; u < kU; ++u) {
+                    const int idx = idx0 + u * (int)blockDim.x, hh = idx >> 5, i = idx & 31;
+                    const bool ok = idx < lim && sp + s2 < n_parts;
+                    pa[s2][u] = ok ? ld_act(src + (size_t)(sp + s2) * part_stride + hh * kHeadDim + i) : 0.f;
+                    pc[s2][u] = ok ? ld_act(src + (size_t)(sp + s2) * part_stride + hh * kHeadDim + i + 32) : 0.f;
+                }
+#pragma unroll
+            for (int s2 = 0; s2 < 2; ++s2)
+                if (sp + s2 < n_parts) {
+#pragma unroll
+                    for (int u = 0; u < kU; ++u) { a[u] += pa[s2][u]; c[u] += pc[s2][u]; }
+                }
+        }
+#pragma unroll
+        for (int u = 0; u < kU; ++u) {
+            const int idx = idx0 + u * (int)blockDim.x, hh = idx >> 5, i = idx & 31;
+            if (idx >= lim) continue;
+            if (hh < n_heads + n_kv_heads) {
+                const float2 cs = rope[(size_t)pos * 32 + i];
+                const float ra = a[u] * cs.x - c[u] * cs.y, rc = c[u] * cs.x + a[u] * cs.y;
+                if (hh < n_heads) {
+                    const size_t o = ((size_t)m * n_heads + hh) * kHeadDim + i;
+                    q16[o] = __float2half_rn(ra);
+                    q16[o + 32] = __float2half_rn(rc);
+                    if (q32) { q32[o] = ra; q32[o + 32] = rc; }
+                } else {
+                    kv_t *dst = kc + (((size_t)b * n_kv_heads + (hh - n_heads)) * max_seq + pos) * kHeadDim;
+                    dst[i] = __float2half_rn(ra);
+                    dst[i + 32] = __float2half_rn(rc);
+                }
             } else {
-                kv_t *dst = kc + (((size_t)b * n_kv_heads + (hh - n_heads)) * max_seq + pos) * kHeadDim;
-                dst[i] = __float2half_rn(ra);
-                dst[i + 32] = __float2half_rn(rc);
+                kv_t *dst = vc + (((size_t)b * n_kv_heads + (hh - n_heads - n_kv_heads)) * max_seq + pos) * kHeadDim;
+                dst[i] = __float2half_rn(a[u]);
+                dst[i + 32] = __float2half_rn(c[u]);
             }
-        } else {
-            kv_t *dst = vc + (((size_t)b * n_kv_heads + (hh - n_heads - n_kv_heads)) * max_seq + pos) * kHeadDim;
-            dst[i] = __float2half_rn(a);
-            dst[i + 32] = __float2half_rn(c);
         }
     }
 }
