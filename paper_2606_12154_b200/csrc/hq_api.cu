@@ -280,10 +280,10 @@ struct TilePlan { int ti, NT, splits; };
 static TilePlan plan_gemm(const hq_model *m, int n_rows, int rows, int K, int max_splits) {
     const int n_tiles = (n_rows + 127) / 128;
     if (rows > 32 && max_splits > 1) {
-        // Prefill pass with split-K partial buffers (no atomics).  At these sizes a GEMM is bound by moving its operands from L2
-        // into shared memory (profiles/r02_ncu_full_summary.md: DRAM 9-21 %, tensor pipe 20-49 %): a CTA pulls ~65 GB/s of
-        // tiles (~40 with 256-token tiles: two stages only), the chip ~8.5 TB/s.  Pick the (token tile, splits) with the
-        // least modelled time: the slower of the per-CTA stream (times the number of waves) and the chip-wide one.
+        // Prefill pass with split-K partial buffers (no atomics).  Pick the (token tile, splits) with the least modelled time:
+        // the slower of a per-CTA tile stream (times the number of waves) and a chip-wide one.  A heuristic fitted to
+        // measured launches: the main loops themselves run at the tensor-core rate (profiles/r02_launches.md), what the
+        // model really ranks is CTA count (waves) against K blocks per CTA and partial buffers to write.
         const int kb = (K + 63) / 64;
         TilePlan best{1, 64, 1};
         double best_t = 1e30;
