@@ -395,17 +395,36 @@ __global__ void __launch_bounds__(256) attn_combine_kernel(const float *part_o, 
         const int head = chunk >> 3, d0 = (chunk & 7) * 8;
         const size_t hb = (size_t)b * n_heads + head;
         const float2 *ml = part_ml + hb * kMaxSplits;
+        // every (m, l) pair in one round trip, then the partial outputs four splits at a time (this kernel is a chain of L2
+        // round trips: 8 CTAs, a few hundred bytes each)
+        float2 mls[kMaxSplits];
+#pragma unroll
+        for (int s = 0; s < kMaxSplits; ++s) mls[s] = s < ns ? __ldcg(&ml[s]) : make_float2(-INFINITY, 0.f);
         float M = -INFINITY;
-        for (int s = 0; s < ns; ++s) M = fmaxf(M, __ldcg(&ml[s]).x);
+#pragma unroll
+        for (int s = 0; s < kMaxSplits; ++s) M = fmaxf(M, mls[s].x);
         float acc[8] = {0, 0, 0, 0, 0, 0, 0, 0}, denom = 0.f;
-        for (int s = 0; s < ns; ++s) {
-            const float2 v = __ldcg(&ml[s]);
-            const float w = __expf(v.x - M);
-            denom += w * v.y;
-            const float *po = part_o + (hb * kMaxSplits + s) * kHeadDim + d0;
-            const float4 a = ld_act4(po), c = ld_act4(po + 4);
-            acc[0] += w * a.x; acc[1] += w * a.y; acc[2] += w * a.z; acc[3] += w * a.w;
-            acc[4] += w * c.x; acc[5] += w * c.y; acc[6] += w * c.z; acc[7] += w * c.w;
+#pragma unroll
+        for (int s4 = 0; s4 < kMaxSplits; s4 += 4) {
+            if (s4 < ns) {   // uniform over the CTA
+                float4 a[4], c[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const float *po = part_o + (hb * kMaxSplits + s4 + u) * kHeadDim + d0;
+                    const bool ok = s4 + u < ns;
+                    a[u] = ok ? ld_act4(po) : make_float4(0.f, 0.f, 0.f, 0.f);
+                    c[u] = ok ? ld_act4(po + 4) : make_float4(0.f, 0.f, 0.f, 0.f);
+                }
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    if (s4 + u < ns) {   // same order and arithmetic as one split after the other
+                        const float w = __expf(mls[s4 + u].x - M);
+                        denom += w * mls[s4 + u].y;
+                        acc[0] += w * a[u].x; acc[1] += w * a[u].y; acc[2] += w * a[u].z; acc[3] += w * a[u].w;
+                        acc[4] += w * c[u].x; acc[5] += w * c[u].y; acc[6] += w * c[u].z; acc[7] += w * c[u].w;
+                    }
+                }
+            }
         }
         const float inv = 1.0f / denom;
         act_t *dst = out + hb * kHeadDim + d0;
