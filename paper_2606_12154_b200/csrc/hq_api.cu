@@ -181,7 +181,8 @@ static SgemvParams sgemv_down(const hq_model *m, int l) {
     // on, profiles/r02_copy_size.md); the others are free for the clusters of the next layer's attention block, which become
     // resident — barriers, cluster sync, first weight stages — under this kernel instead of after it (measured: 104-124 CTAs
     // all -2 % of the step, 84 and 128-148 none)
-    if (m->use_attn_block) p.max_ctas = (m->n_sms * 3) / 4;
+    // (bf16 only: the hq4 kernel is bound by expanding nibbles, not by HBM, and wants every SM: 0.431 -> 0.424 ms per token)
+    if (m->use_attn_block && !m->q4) p.max_ctas = (m->n_sms * 3) / 4;
     return p;
 }
 // final norm + LM head + argmax over the residual row x; the position advances by pos_inc
