@@ -226,6 +226,8 @@ def main():
                          "tokenise, prefill, streaming decode): e2e wall, e2e tok/s, TTFT, route p50 as PAPER.md:L109 defines them")
     ap.add_argument("--window-sweep", action="store_true",
                     help="PAPER.md:L170 (section 6.6): context WINDOW 4,096 -> 131,072 with the configs[1] query; one JSON line per window")
+    ap.add_argument("--gemm-timeline", action="store_true",
+                    help="globaltimer stamps inside the tcgen05 GEMM (hq_debug_gemm_timeline) for the 1B prefill and batched-decode shapes; JSON lines")
     ap.add_argument("--probes", action="store_true",
                     help="memory-system probes behind the kernel design: bulk-copy size vs per-SM rate, read-only stream; JSON lines")
     ap.add_argument("--profile", type=int, default=0, metavar="N",
@@ -470,6 +472,43 @@ def main():
             m.close()
             del m
             torch.cuda.empty_cache()
+        return
+
+    if args.gemm_timeline:
+        # Where a GEMM launch spends its time (profiles/r02_launches.md): each shape launched alone over fresh weights (three
+        # sets cycled so that they come from HBM), stamps of the CTAs of the first token tile / K split, medians over CTAs.
+        shapes = [("prefill gate/up", 2, s.ffn, s.hidden, 256, 128, 1), ("prefill Q|K|V", 0, 3072, s.hidden, 256, 128, 2),
+                  ("prefill O", 0, s.hidden, s.hidden, 256, 128, 4), ("prefill down", 0, s.hidden, s.ffn, 256, 128, 4),
+                  ("decode B=8 gate/up", 3, s.ffn, s.hidden, 8, 32, 1), ("decode B=8 down", 0, s.hidden, s.ffn, 8, 32, 9),
+                  ("decode B=8 LM head", 0, s.vocab, s.hidden, 8, 32, 1)]
+        g = torch.Generator(device=dev).manual_seed(7)
+        with torch.cuda.stream(stream):
+            for name, mode, N, K, T, tile, splits in shapes:
+                nset = 2 if N > 100000 else 3
+                ws = [torch.randn(N, K, device=dev, generator=g).mul_(0.02).bfloat16() for _ in range(nset)]
+                w2 = [torch.randn(N, K, device=dev, generator=g).mul_(0.02).bfloat16() for _ in range(nset)] if mode >= 2 else [None] * nset
+                x = torch.randn(2, T, K, device=dev, generator=g).bfloat16()
+                out = (torch.zeros((2, T, N), dtype=torch.bfloat16, device=dev) if mode >= 2
+                       else torch.zeros((T, N), dtype=torch.float32, device=dev))
+                n_ctas = (N // 64 if mode == 3 else (N + 127) // 128)
+                n_ctas += n_ctas & 1 if T > 32 else 0
+                tr = torch.zeros((n_ctas, 8), dtype=torch.int64, device=dev)
+                for i in range(nset + 1):
+                    hq.debug_gemm(mode, ws[i % nset], x, out, w2=w2[i % nset], token_tile=tile, splits=splits, stream=stream, trace=tr)
+                torch.cuda.synchronize(dev)
+                t = tr.cpu().numpy().astype(np.float64)
+                t = t[(t[:, 4] > 0) & (t[:, 1] > 0)]   # CTA pairs: only the leader issues MMAs and stamps [1], [2]
+                rel = (t[:, 1:5] - t[:, 0:1]) / 1e3
+                kb = ((K + 63) // 64 + splits - 1) // splits
+                med = np.median(rel, axis=0)
+                print(json.dumps({"gemm_timeline": name, "mode": mode, "n_rows": N, "k": K, "tokens": T, "token_tile": tile, "splits": splits,
+                                  "ctas_stamped": int(t.shape[0]), "k_blocks_per_cta": kb,
+                                  "first_stage_landed_us": round(float(med[0]), 2), "last_stage_landed_us": round(float(med[1]), 2),
+                                  "us_per_k_block": round(float((med[1] - med[0]) / max(kb - 1, 1)), 3),
+                                  "accumulator_complete_us": round(float(med[2]), 2), "epilogue_us": round(float(med[3] - med[2]), 2),
+                                  "note": "us since the CTA had its barriers and tensor memory; medians over the stamped CTAs"}), flush=True)
+                del ws, w2
+                torch.cuda.empty_cache()
         return
 
     if args.probes:

@@ -37,6 +37,15 @@ int32_t hq_bench_kernel(hq_model *m, int32_t which, int32_t reps, int64_t *bytes
 int32_t hq_debug_gemm(void *cuda_stream, int32_t mode, const void *w_dev, const void *w2_dev, const void *x_dev,
                       void *out_dev, int32_t n_rows, int32_t k, int32_t n_tokens, int32_t token_tile, int32_t splits);
 
+/* Measurement: hq_debug_gemm with a timeline (profiles/r02_launches.md).  trace_dev: DEVICE uint64
+ * [CTAs along the weight rows][8] (ceil(n_rows / 128) CTAs, n_rows / 64 for mode 3, rounded up to even for CTA pairs);
+ * every CTA of the first token tile and K split writes GPU globaltimer values (ns): [0] barriers and tensor memory set up,
+ * [1] first stage of operands landed, [2] last stage landed, [3] accumulator complete (all MMAs retired),
+ * [4] epilogue of the stamping warp issued.  Same arguments, result and asynchrony as hq_debug_gemm. */
+int32_t hq_debug_gemm_timeline(void *cuda_stream, int32_t mode, const void *w_dev, const void *w2_dev, const void *x_dev,
+                               void *out_dev, int32_t n_rows, int32_t k, int32_t n_tokens, int32_t token_tile,
+                               int32_t splits, uint64_t *trace_dev);
+
 /* Measurement: read-only streaming probe: one launch sums the 32-bit words of src_dev[0, bytes) into
  * *sum_dev (atomicAdd, wraps; DEVICE uint32, caller-zeroed).  Time it with CUDA events on cuda_stream over a buffer much
  * larger than L2: bytes / time is what a kernel that only reads HBM reaches on this box.  Asynchronous. */

@@ -28,7 +28,7 @@ _CODE_NAMES = {-1: "HQ_ERR_INVALID_ARG", -2: "HQ_ERR_CAPACITY", -3: "HQ_ERR_STAT
 DECLARED_SYMBOLS = (
     "hq_workspace_bytes", "hq_model_create", "hq_model_create_q4", "hq_quantize_q4", "hq_dequantize_q4", "hq_model_destroy", "hq_prefill", "hq_decode_step",
     "hq_decode_run", "hq_verify_relay", "hq_decode_logits", "hq_get_hidden", "hq_sync", "hq_seq_len", "hq_kv_reset",
-    "hq_kernel_count", "hq_decode_path", "hq_bench_kernel", "hq_debug_copy_probe", "hq_debug_gemm", "hq_debug_kv_row", "hq_debug_read_probe", "hq_debug_step_trace", "hq_debug_trace", "hq_last_error",
+    "hq_kernel_count", "hq_decode_path", "hq_bench_kernel", "hq_debug_copy_probe", "hq_debug_gemm", "hq_debug_gemm_timeline", "hq_debug_kv_row", "hq_debug_read_probe", "hq_debug_step_trace", "hq_debug_trace", "hq_last_error",
     "hq_version",
 )
 
@@ -116,6 +116,8 @@ def load_library(path: Optional[str] = None):
     l.hq_bench_kernel.argtypes = [vp, i32, i32, ctypes.POINTER(i64)]
     l.hq_debug_gemm.restype = i32
     l.hq_debug_gemm.argtypes = [vp, i32, vp, vp, vp, vp, i32, i32, i32, i32, i32]
+    l.hq_debug_gemm_timeline.restype = i32
+    l.hq_debug_gemm_timeline.argtypes = [vp, i32, vp, vp, vp, vp, i32, i32, i32, i32, i32, vp]
     l.hq_debug_copy_probe.restype = i32
     l.hq_debug_copy_probe.argtypes = [vp, vp, ctypes.c_size_t, i32, i32]
     l.hq_debug_read_probe.restype = i32
@@ -430,11 +432,15 @@ def copy_probe(buf, copy_bytes: int, n_ctas: int, stream=None) -> int:
     return n_ctas * (nbytes // 65536 // n_ctas) * 65536
 
 
-def debug_gemm(mode: int, w, x, out, *, w2=None, token_tile: int = 128, splits: int = 1, stream=None):
+def debug_gemm(mode: int, w, x, out, *, w2=None, token_tile: int = 128, splits: int = 1, stream=None, trace=None):
     """hq_debug_gemm on torch CUDA tensors: bf16 w [N,K], bf16 x planes [2,T,K] (hi, lo); out fp32 [T,N],
-    or bf16 planes [2,T,N] for mode 2."""
+    or bf16 planes [2,T,N] for modes 2 and 3.  trace: int64 CUDA tensor [CTAs, 8] -> hq_debug_gemm_timeline."""
     import torch
     st = stream if stream is not None else torch.cuda.current_stream(w.device)
     n_rows, k = w.shape
-    _check(load_library().hq_debug_gemm(st.cuda_stream, mode, w.data_ptr(), w2.data_ptr() if w2 is not None else None,
-                                        x.data_ptr(), out.data_ptr(), n_rows, k, x.shape[1], token_tile, splits))
+    args = (st.cuda_stream, mode, w.data_ptr(), w2.data_ptr() if w2 is not None else None,
+            x.data_ptr(), out.data_ptr(), n_rows, k, x.shape[1], token_tile, splits)
+    if trace is None:
+        _check(load_library().hq_debug_gemm(*args))
+    else:
+        _check(load_library().hq_debug_gemm_timeline(*args, trace.data_ptr()))

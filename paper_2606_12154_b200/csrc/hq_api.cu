@@ -1039,9 +1039,8 @@ extern "C" int32_t hq_debug_trace(hq_model *m, uint64_t *trace_dev, int32_t cap)
 }
 
 // ---- diagnostics: the tensor-core GEMM on its own ------------------------------------------------------
-extern "C" int32_t hq_debug_gemm(void *cuda_stream, int32_t mode, const void *w_dev, const void *w2_dev,
-                                 const void *x_dev, void *out_dev, int32_t n_rows, int32_t k, int32_t n_tokens,
-                                 int32_t token_tile, int32_t splits) {
+static int32_t debug_gemm_impl(void *cuda_stream, int32_t mode, const void *w_dev, const void *w2_dev, const void *x_dev, void *out_dev,
+                               int32_t n_rows, int32_t k, int32_t n_tokens, int32_t token_tile, int32_t splits, uint64_t *trace_dev) {
     if (!w_dev || !x_dev || !out_dev || n_rows <= 0 || k <= 0 || n_tokens <= 0)
         return fail(HQ_ERR_INVALID_ARG, "hq_debug_gemm: bad argument");
     if (mode < 0 || mode > 3 || (mode >= 2 && !w2_dev)) return fail(HQ_ERR_INVALID_ARG, "hq_debug_gemm: bad mode");
@@ -1059,6 +1058,18 @@ extern "C" int32_t hq_debug_gemm(void *cuda_stream, int32_t mode, const void *w_
     HQ_CUDA(gemm_prepare());
     HQ_CUDA(launch_gemm(lc, (GemmEpilogue)mode, mw, mode >= 2 ? &mw2 : nullptr, mx, n_tokens, n_rows, k, n_tokens, token_tile,
                         mode >= 2 ? 1 : splits, mode >= 2 ? nullptr : (float *)out_dev, mode >= 2 ? (act_t *)out_dev : nullptr,
-                        (size_t)n_tokens * n_rows, n_rows));
+                        (size_t)n_tokens * n_rows, n_rows, 0, (unsigned long long *)trace_dev));
     return HQ_OK;
+}
+
+extern "C" int32_t hq_debug_gemm(void *cuda_stream, int32_t mode, const void *w_dev, const void *w2_dev, const void *x_dev, void *out_dev,
+                                 int32_t n_rows, int32_t k, int32_t n_tokens, int32_t token_tile, int32_t splits) {
+    return debug_gemm_impl(cuda_stream, mode, w_dev, w2_dev, x_dev, out_dev, n_rows, k, n_tokens, token_tile, splits, nullptr);
+}
+
+extern "C" int32_t hq_debug_gemm_timeline(void *cuda_stream, int32_t mode, const void *w_dev, const void *w2_dev, const void *x_dev,
+                                          void *out_dev, int32_t n_rows, int32_t k, int32_t n_tokens, int32_t token_tile, int32_t splits,
+                                          uint64_t *trace_dev) {
+    if (!trace_dev) return fail(HQ_ERR_INVALID_ARG, "hq_debug_gemm_timeline: trace_dev is NULL");
+    return debug_gemm_impl(cuda_stream, mode, w_dev, w2_dev, x_dev, out_dev, n_rows, k, n_tokens, token_tile, splits, trace_dev);
 }

@@ -119,6 +119,12 @@ __host__ __device__ inline uint32_t make_idesc(int n, int m = kBlockM) {
     return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(m >> 4) << 24);
 }
 
+__device__ __forceinline__ unsigned long long gemm_time() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+
 // ---- epilogue helpers.  The epilogue runs after the last MMA with nothing left to overlap it (one tile per CTA), and all
 // CTAs reach it together: its length is pure instruction count (measured with globaltimer stamps: 0.85 us per 32-token
 // chunk of plain stores with a bounds branch and a mode branch per element, 2.9 us per chunk of the SwiGLU form; after
@@ -170,7 +176,9 @@ __device__ __forceinline__ void store_act_scalar(const float (&a)[32], act_t *ou
     }
 }
 
-template <int MODE, int CTAS>
+// TRACE: the timeline instantiations (hq_debug_gemm_timeline) are separate kernels: the stamps cost the batched-decode
+// step 3 % when they were run-time branches in the product kernels.
+template <int MODE, int CTAS, bool TRACE = false>
 __global__ void __launch_bounds__(kGemmThreads, 1)
 gemm_tc_kernel(const __grid_constant__ CUtensorMap map_w, const __grid_constant__ CUtensorMap map_w2,
                const __grid_constant__ CUtensorMap map_w3, const __grid_constant__ CUtensorMap map_x, const GemmParams p) {
@@ -231,6 +239,9 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap map_w, const __grid_constant_
     tcgen05_fence_after();
     const uint32_t tmem_base = *tmem_slot;
 
+    // optional timeline (hq_debug_gemm_timeline): five globaltimer stamps per CTA of the first token tile / K split
+    unsigned long long *tr = (TRACE && p.trace && blockIdx.y == 0 && blockIdx.z == 0) ? p.trace + (size_t)blockIdx.x * kGemmTraceLen : nullptr;
+    if (TRACE && tr && threadIdx.x == 0) tr[0] = gemm_time();   // barriers and tensor memory are up
     pdl_launch_dependents();
 
     if (warp == 0) {
@@ -290,6 +301,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap map_w, const __grid_constant_
                     const uint32_t ph = (i / stages) & 1;
                     mbarrier_wait(&full_bar[s], ph);
                     tcgen05_fence_after();
+                    if (TRACE && tr && (i == 0 || i == nkb - 1)) tr[i == 0 ? 1 : 2] = gemm_time();   // first / last stage landed
                     const uint32_t a_addr = smem_u32(smem + (size_t)s * stage_bytes);
                     const uint64_t da = make_smem_desc(a_addr), da2 = make_smem_desc(a_addr + a_bytes), db = make_smem_desc(a_addr + NACC * a_bytes);
 #pragma unroll
@@ -304,11 +316,14 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap map_w, const __grid_constant_
             }
         } else if (lane == 0) {
             const uint32_t idesc = make_idesc(stacked ? 2 * NT : NT);
+            unsigned long long t_first = 0, t_last = 0;
             for (int i = 0; i < nkb; ++i) {
                 const int s = i % stages;
                 const uint32_t ph = (i / stages) & 1;
                 mbarrier_wait(&full_bar[s], ph);
                 tcgen05_fence_after();
+                if (TRACE && tr && i == 0) t_first = gemm_time();        // first stage landed
+                if (TRACE && tr && i == nkb - 1) t_last = gemm_time();   // last stage landed
                 const uint32_t a_addr = smem_u32(smem + (size_t)s * stage_bytes);
                 const uint32_t b_addr = a_addr + NACC * a_bytes;
                 const uint64_t da = make_smem_desc(a_addr), db = make_smem_desc(b_addr);
@@ -332,6 +347,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap map_w, const __grid_constant_
                 tcgen05_commit(&empty_bar[s]);   // frees the smem stage when these MMAs retire
             }
             tcgen05_commit(acc_bar);             // accumulator complete
+            if (TRACE && tr) { tr[1] = t_first; tr[2] = t_last; }
         }
     } else {
         // ===== epilogue: warp w owns TMEM lanes 32*(w%4) .. +31 =====
@@ -340,6 +356,8 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap map_w, const __grid_constant_
         pdl_wait();   // the output buffer (residual, zeroed split-K target) belongs to earlier kernels until now
         mbarrier_wait(acc_bar, 0);
         tcgen05_fence_after();
+        if (TRACE && tr && warp == 2 && lane == 0) tr[3] = gemm_time();   // accumulator complete
+        if (TRACE) __syncwarp();   // the tensor-memory loads below are warp-aligned instructions
         const uint32_t lane_addr = tmem_base + ((uint32_t)(32 * q) << 16);
         const bool row_ok = n < p.n_rows;
         const bool pairable = (p.n_rows & 1) == 0 && (p.ld_out & 1) == 0;   // bf16 outputs as 32-bit pairs
@@ -413,6 +431,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap map_w, const __grid_constant_
             }
         }
         tcgen05_fence_before();
+        if (TRACE && tr && warp == 2 && lane == 0) tr[4] = gemm_time();   // this warp's share of the epilogue issued
     }
     __syncthreads();
     if (CTAS == 2) cluster_sync_all();   // neither CTA frees tensor memory or exits while the pair's MMAs / loads may still touch it
@@ -493,14 +512,16 @@ static cudaError_t launch_mode(const LaunchCtx &c, const TensorMap &w, const Ten
     }
     cfg.attrs = attr;
     cfg.numAttrs = na;
+    typedef void (*kernel_t)(const CUtensorMap, const CUtensorMap, const CUtensorMap, const CUtensorMap, const GemmParams);
+    kernel_t k = p.trace ? gemm_tc_kernel<MODE, 1, true> : gemm_tc_kernel<MODE, 1, false>;
     if constexpr (MODE != EPI_SWIGLU64)
-      if (pair)
-        return cudaLaunchKernelEx(&cfg, gemm_tc_kernel<MODE, 2>, *reinterpret_cast<const CUtensorMap *>(&w),
-                                  *reinterpret_cast<const CUtensorMap *>(&w2), *reinterpret_cast<const CUtensorMap *>(&w3),
-                                  *reinterpret_cast<const CUtensorMap *>(&x), p);
-    return cudaLaunchKernelEx(&cfg, gemm_tc_kernel<MODE, 1>, *reinterpret_cast<const CUtensorMap *>(&w),
-                              *reinterpret_cast<const CUtensorMap *>(&w2), *reinterpret_cast<const CUtensorMap *>(&w3),
-                              *reinterpret_cast<const CUtensorMap *>(&x), p);
+        if (pair) k = p.trace ? gemm_tc_kernel<MODE, 2, true> : gemm_tc_kernel<MODE, 2, false>;
+    if (p.trace) {   // diagnostics only: opt in here instead of in gemm_prepare
+        cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+        if (e != cudaSuccess) return e;
+    }
+    return cudaLaunchKernelEx(&cfg, k, *reinterpret_cast<const CUtensorMap *>(&w), *reinterpret_cast<const CUtensorMap *>(&w2),
+                              *reinterpret_cast<const CUtensorMap *>(&w3), *reinterpret_cast<const CUtensorMap *>(&x), p);
 }
 
 // n_rows: weight rows (output features; for EPI_SWIGLU the ffn size), K: reduction size (multiple of 64),
@@ -508,7 +529,7 @@ static cudaError_t launch_mode(const LaunchCtx &c, const TensorMap &w, const Ten
 // zeroed buffer, EPI_RESID always legal).
 cudaError_t launch_gemm(const LaunchCtx &c, GemmEpilogue mode, const TensorMap &w, const TensorMap *w2,
                         const TensorMap &x, int x_lo_row, int n_rows, int K, int T, int NT, int splits, float *out_f32,
-                        act_t *out_act, size_t out_lo_offset, int ld_out, size_t split_stride) {
+                        act_t *out_act, size_t out_lo_offset, int ld_out, size_t split_stride, unsigned long long *trace) {
     // K need not be a multiple of 64: TMA zero-fills the out-of-range tail of the last K block
     if (K % 8 != 0 || NT % 32 != 0 || NT < 32 || NT > 256 || T <= 0) return cudaErrorInvalidValue;
     const int kblocks = (K + kBlockK - 1) / kBlockK;
@@ -520,6 +541,7 @@ cudaError_t launch_gemm(const LaunchCtx &c, GemmEpilogue mode, const TensorMap &
     splits = (kblocks + p.k_blocks_per_split - 1) / p.k_blocks_per_split;
     p.out_f32 = out_f32; p.out_act = out_act; p.out_lo_offset = out_lo_offset; p.x_lo_row = x_lo_row; p.ld_out = ld_out;
     p.split_stride = mode == EPI_STORE ? split_stride : 0;
+    p.trace = trace;
     p.atomic = (splits > 1 && p.split_stride == 0) ? 1 : 0;
     const int n_tiles = (n_rows + kBlockM - 1) / kBlockM, t_tiles = (T + NT - 1) / NT;
     switch (mode) {

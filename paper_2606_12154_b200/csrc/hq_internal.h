@@ -221,6 +221,7 @@ cudaError_t attn_block_prepare(int n_kv_heads, bool *co_resident);
 cudaError_t launch_attn_block(const LaunchCtx &c, const AttnBlockParams &p);
 
 // ---- tensor-core GEMM (hq_gemm.cu) -------------------------------------------------------------------
+constexpr int kGemmTraceLen = 8;   // stamps per CTA: 0 set up, 1 first stage landed, 2 last stage landed, 3 accumulator complete, 4 epilogue issued
 enum GemmEpilogue { EPI_STORE = 0, EPI_RESID = 1, EPI_SWIGLU = 2, EPI_SWIGLU64 = 3 };   // 3: SwiGLU from 64-row tiles (tensor maps with 64-row boxes)
 struct GemmParams {
     int K, n_rows, T, NT, k_blocks, k_blocks_per_split, stages;
@@ -231,13 +232,14 @@ struct GemmParams {
     int atomic;
     int x_lo_row;       // row offset of the lo plane inside the activation tensor map
     size_t split_stride;      // > 0: K split z stores its partial at out_f32 + z * split_stride (no atomics; the consumer adds them in order)
+    unsigned long long *trace;   // NULL, or [CTAs along the weight rows][kGemmTraceLen] globaltimer stamps (hq_debug_gemm_timeline)
     int tiles_w1, tiles_w2;   // EPI_STORE over three stacked weight matrices: 128-row tiles of the first and second (0 = one matrix)
 };
 bool make_tensor_map_16b(TensorMap *out, const void *base, uint64_t rows, uint64_t cols, uint32_t box_rows);
 cudaError_t gemm_prepare();   // shared-memory opt-in on the current device
 cudaError_t launch_gemm(const LaunchCtx &c, GemmEpilogue mode, const TensorMap &w, const TensorMap *w2,
                         const TensorMap &x, int x_lo_row, int n_rows, int K, int T, int NT, int splits, float *out_f32,
-                        act_t *out_act, size_t out_lo_offset, int ld_out, size_t split_stride = 0);
+                        act_t *out_act, size_t out_lo_offset, int ld_out, size_t split_stride = 0, unsigned long long *trace = nullptr);
 
 cudaError_t launch_gemm_qkv(const LaunchCtx &c, const TensorMap &wq, const TensorMap &wk, const TensorMap &wv, const TensorMap &x,
                             int x_lo_row, int n1, int n2, int n3, int K, int T, int NT, int splits, float *out_f32, int ld_out,
