@@ -29,7 +29,7 @@ DECLARED_SYMBOLS = (
     "hq_workspace_bytes", "hq_model_create", "hq_model_create_q4", "hq_quantize_q4", "hq_dequantize_q4", "hq_model_destroy", "hq_prefill", "hq_decode_step",
     "hq_decode_run", "hq_verify_relay", "hq_decode_logits", "hq_get_hidden", "hq_sync", "hq_seq_len", "hq_kv_reset",
     "hq_kernel_count", "hq_decode_path", "hq_bench_kernel", "hq_debug_copy_probe", "hq_debug_gemm", "hq_debug_gemm_timeline", "hq_debug_kv_row", "hq_debug_read_probe", "hq_debug_step_trace", "hq_debug_trace", "hq_last_error",
-    "hq_version",
+    "hq_version", "hq_noalloc_scratch_bytes", "hq_noalloc_setup", "hq_gemm_noalloc",
 )
 
 
@@ -116,6 +116,12 @@ def load_library(path: Optional[str] = None):
     l.hq_bench_kernel.argtypes = [vp, i32, i32, ctypes.POINTER(i64)]
     l.hq_debug_gemm.restype = i32
     l.hq_debug_gemm.argtypes = [vp, i32, vp, vp, vp, vp, i32, i32, i32, i32, i32]
+    l.hq_noalloc_scratch_bytes.restype = ctypes.c_size_t
+    l.hq_noalloc_scratch_bytes.argtypes = []
+    l.hq_noalloc_setup.restype = i32
+    l.hq_noalloc_setup.argtypes = []
+    l.hq_gemm_noalloc.restype = i32
+    l.hq_gemm_noalloc.argtypes = [vp, vp, vp, vp, i32, i32, i32, i32, i32]
     l.hq_debug_gemm_timeline.restype = i32
     l.hq_debug_gemm_timeline.argtypes = [vp, i32, vp, vp, vp, vp, i32, i32, i32, i32, i32, vp]
     l.hq_debug_copy_probe.restype = i32
@@ -413,6 +419,28 @@ class Model:
         b = ctypes.c_int64()
         _check(self._lib.hq_bench_kernel(self._h, which, reps, ctypes.byref(b)))
         return b.value
+
+
+def noalloc_scratch_bytes() -> int:
+    """hq_noalloc_scratch_bytes: size of the library's static scratch array (include/hq_noalloc.h)."""
+    return int(load_library().hq_noalloc_scratch_bytes())
+
+
+def noalloc_setup(device=None):
+    """hq_noalloc_setup for `device` (default: torch's current device): once per device, before any no-allocation region."""
+    import torch
+    with torch.cuda.device(device if device is not None else torch.cuda.current_device()):
+        _check(load_library().hq_noalloc_setup())
+
+
+def gemm_noalloc(w, x, out, *, token_tile: int = 128, splits: int = 1, stream=None):
+    """hq_gemm_noalloc on torch CUDA tensors: bf16 w [N,K], bf16 x planes [2,T,K] (hi, lo), fp32 out [T,N]; allocates nothing."""
+    import torch
+    st = stream if stream is not None else torch.cuda.current_stream(w.device)
+    n_rows, k = w.shape
+    with torch.cuda.device(w.device):
+        _check(load_library().hq_gemm_noalloc(st.cuda_stream, w.data_ptr(), x.data_ptr(), out.data_ptr(), n_rows, k, x.shape[1],
+                                              token_tile, splits))
 
 
 def read_probe(buf, result, stream=None):

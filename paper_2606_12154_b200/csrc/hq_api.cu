@@ -35,6 +35,17 @@ static int32_t fail(int32_t code, const char *fmt, ...) {
 
 extern "C" const char *hq_last_error(void) { return g_err; }
 
+// the same message buffer for entry points that live in other files (hq_noalloc.cu)
+namespace hq {
+int32_t set_error(int32_t code, const char *fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+}  // namespace hq
+
 // Every entry point that touches the GPU makes the model's device current first (a caller may have switched devices
 // between calls; kernel attributes and launches are per device).
 #define HQ_ON_DEVICE(m) HQ_CUDA(cudaSetDevice((m)->device))

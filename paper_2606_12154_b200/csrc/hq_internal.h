@@ -9,6 +9,7 @@
 #include <vector>
 
 #include "../../include/hq_debug.h"
+#include "../../include/hq_noalloc.h"
 
 namespace hq {
 
@@ -181,6 +182,9 @@ __host__ __device__ inline int attn_split_len(int n_ctx, int n_splits) {
     int c = (n_ctx + n_splits - 1) / n_splits;
     return (c + 15) & ~15;  // 16-position granules
 }
+
+// records the message hq_last_error() returns and hands the code back (for entry points outside hq_api.cu)
+int32_t set_error(int32_t code, const char *fmt, ...);
 
 struct LaunchCtx {
     cudaStream_t stream;

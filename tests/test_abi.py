@@ -22,7 +22,7 @@ def hq():
 
 def header_functions():
     names = set()
-    for h in ("hq.h", "hq_debug.h"):
+    for h in ("hq.h", "hq_debug.h", "hq_noalloc.h"):
         src = open(os.path.join(ROOT, "include", h)).read()
         src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
         names |= set(re.findall(r"\b(hq_[a-z_0-9]+)\s*\(", src))
