@@ -109,6 +109,7 @@ static size_t carve(const hq_config *c, char *base, Buffers *b) {
     o.tok_hist = (int *)take((T + 1) * B * sizeof(int));
     o.best = (unsigned long long *)take(B * sizeof(unsigned long long));
     o.counter = (unsigned int *)take(sizeof(unsigned int));
+    o.attn_tickets = (unsigned int *)take(B * Hkv * sizeof(unsigned int));
     o.x = (float *)take(B * d * sizeof(float));
     o.q = (float *)take(B * H * kHeadDim * sizeof(float));
     o.part_o = (float *)take(B * H * kMaxSplits * kHeadDim * sizeof(float));
@@ -374,15 +375,14 @@ static cudaError_t enqueue_rows_layers(hq_model *m, int batch, int Tc, bool deco
             STEP(launch_gemm(lc, EPI_STORE, mp.wk, nullptr, m->map_hn[pq.ti], R, kvdim, d, rows, pq.NT, pq.splits, b.qkv + qdim, nullptr, 0, qkvd, qs));
             STEP(launch_gemm(lc, EPI_STORE, mp.wv, nullptr, m->map_hn[pq.ti], R, kvdim, d, rows, pq.NT, pq.splits, b.qkv + qdim + kvdim, nullptr, 0, qkvd, qs));
         }
-        // P4: RoPE + KV append (adds the split-K partials of the projection in order)
-        STEP(launch_rope_append(lc, b.qkv, defer ? pq.splits : 1, q_stride, b.q16, decode ? b.q : nullptr, kc, vc, b.rope, b.pos, rows, Tc,
-                                c.n_heads, c.n_kv_heads, c.max_seq));
         if (decode) {
-            // B2: split-KV decode attention per sequence, then merge
-            AttnDecodeParams a = {b.q, kc, vc, b.part_o, b.part_ml, b.pos, c.n_heads, c.n_kv_heads, c.max_seq};
-            STEP(launch_attn_decode(lc, a, batch));
-            STEP(launch_attn_combine(lc, b.part_o, b.part_ml, b.ao, lo_q, b.pos, batch, c.n_heads));
+            // P4 + B2 in one launch: RoPE, KV append, split-KV decode attention per sequence, split merge
+            AttnFusedParams a = {b.qkv, kc, vc, b.rope, b.part_o, b.part_ml, b.attn_tickets, b.ao, lo_q, b.pos, c.n_heads, c.n_kv_heads, c.max_seq};
+            STEP(launch_attn_decode_fused(lc, a, batch));
         } else {
+            // P4: RoPE + KV append (adds the split-K partials of the projection in order)
+            STEP(launch_rope_append(lc, b.qkv, pq.splits, q_stride, b.q16, nullptr, kc, vc, b.rope, b.pos, rows, Tc,
+                                    c.n_heads, c.n_kv_heads, c.max_seq));
             // P2: causal flash attention
             STEP(launch_flash_prefill(lc, b.q16, kc, vc, b.ao, lo_q, b.pos, batch, Tc, c.n_heads, c.n_kv_heads, c.max_seq));
         }
@@ -645,6 +645,7 @@ static int32_t model_create(const hq_config *cfg, const hq_weights *w, const hq_
         if (e == cudaSuccess) e = launch_set_state(LaunchCtx{m->stream, false, m->n_sms}, m->b.pos, 0, m->b.best,
                                                    m->b.counter, cfg->max_batch, m->b.err);
         if (e == cudaSuccess) e = launch_zero_tokens(LaunchCtx{m->stream, false, m->n_sms}, m->b.cur_tok, cfg->max_batch);
+        if (e == cudaSuccess) e = cudaMemsetAsync(m->b.attn_tickets, 0, (size_t)cfg->max_batch * cfg->n_kv_heads * sizeof(unsigned int), m->stream);
         if (e == cudaSuccess) e = cudaStreamSynchronize(m->stream);
         if (e != cudaSuccess) {
             delete m;
@@ -706,6 +707,8 @@ extern "C" int32_t hq_kv_reset(hq_model *m) {
     HQ_ON_DEVICE(m);
     HQ_CUDA(launch_set_state(LaunchCtx{m->stream, false, m->n_sms}, m->b.pos, 0, m->b.best, m->b.counter,
                              m->cfg.max_batch, m->b.err));
+    // the split tickets of the batched decode attention are zero between launches unless a launch was cut short (HQ_ERR_CUDA)
+    HQ_CUDA(cudaMemsetAsync(m->b.attn_tickets, 0, (size_t)m->cfg.max_batch * m->cfg.n_kv_heads * sizeof(unsigned int), m->stream));
     m->kernel_count += 1;
     m->seq_len = 0;
     m->batch = 0;

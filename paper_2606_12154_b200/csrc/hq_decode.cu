@@ -265,6 +265,54 @@ __global__ void __launch_bounds__(kGemvThreads) gemv_kernel(const __grid_constan
 // =====================================================================================================
 constexpr int kAttnTile = 128;  // positions per staged tile (16 KB of K + 16 KB of V)
 
+// One staged tile of nt positions for one query head (one warp): online softmax over the tile, state (m, l, o0, o1) =
+// running max, denominator and this lane's two output dims.  q: the head's query, pre-scaled, in shared memory.
+__device__ __forceinline__ void attn_tile(const kv_t *Ks, const kv_t *Vs, int nt, const float *q, int lane, float &m, float &l, float &o0,
+                                          float &o1) {
+    for (int r0 = 0; r0 < nt; r0 += 32) {
+        const int nr = min(32, nt - r0);
+        // scores of up to 32 positions: lane i computes the whole dot product of position r0 + i (one warp reduction
+        // per position made this loop a chain of 5 dependent shuffles x 32: 2.6 us per 32 positions).  Lane i walks the
+        // eight 16-byte chunks of its K row starting at chunk i & 7, so that the 8 lanes of a quarter-warp read 8
+        // different bank groups of K and of q: conflict free.
+        float s_mine = -INFINITY;
+        if (lane < nr) {
+            const uint4 *krow = reinterpret_cast<const uint4 *>(Ks + (r0 + lane) * kHeadDim);
+            float acc4[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+            for (int c = 0; c < 8; ++c) {
+                const int cc = (c + lane) & 7;
+                const uint4 kk = krow[cc];
+                const float4 qa = *reinterpret_cast<const float4 *>(&q[cc * 8]);
+                const float4 qb = *reinterpret_cast<const float4 *>(&q[cc * 8 + 4]);
+                const float2 k0 = __half22float2(*reinterpret_cast<const __half2 *>(&kk.x));
+                const float2 k1 = __half22float2(*reinterpret_cast<const __half2 *>(&kk.y));
+                const float2 k2 = __half22float2(*reinterpret_cast<const __half2 *>(&kk.z));
+                const float2 k3 = __half22float2(*reinterpret_cast<const __half2 *>(&kk.w));
+                acc4[0] = fmaf(qa.x, k0.x, fmaf(qa.y, k0.y, acc4[0]));
+                acc4[1] = fmaf(qa.z, k1.x, fmaf(qa.w, k1.y, acc4[1]));
+                acc4[2] = fmaf(qb.x, k2.x, fmaf(qb.y, k2.y, acc4[2]));
+                acc4[3] = fmaf(qb.z, k3.x, fmaf(qb.w, k3.y, acc4[3]));
+            }
+            s_mine = (acc4[0] + acc4[1]) + (acc4[2] + acc4[3]);
+        }
+        const float m_new = fmaxf(m, warp_max(s_mine));
+        const float corr = __expf(m - m_new);   // m = -inf first time -> 0
+        const float pr = (lane < nr) ? __expf(s_mine - m_new) : 0.f;
+        l = l * corr + warp_sum(pr);
+        o0 *= corr;
+        o1 *= corr;
+        for (int r = 0; r < nr; ++r) {
+            const float pb = __shfl_sync(0xffffffffu, pr, r);
+            const float2 vv = __half22float2(*reinterpret_cast<const __half2 *>(Vs + (r0 + r) * kHeadDim + 2 * lane));
+            o0 = fmaf(pb, vv.x, o0);
+            o1 = fmaf(pb, vv.y, o1);
+        }
+        m = m_new;
+    }
+}
+
+
 __global__ void __launch_bounds__(256) attn_decode_kernel(const __grid_constant__ AttnDecodeParams p) {
     __shared__ __align__(128) kv_t Ks[kAttnTile * kHeadDim];
     __shared__ __align__(128) kv_t Vs[kAttnTile * kHeadDim];
@@ -313,52 +361,163 @@ __global__ void __launch_bounds__(256) attn_decode_kernel(const __grid_constant_
         }
         mbar_wait(&bar, parity);
         parity ^= 1;
-        for (int r0 = 0; r0 < nt; r0 += 32) {
-            const int nr = min(32, nt - r0);
-            // scores of up to 32 positions: lane i computes the whole dot product of position r0 + i (one warp reduction
-            // per position made this loop a chain of 5 dependent shuffles x 32: 2.6 us per 32 positions).  Lane i walks the
-            // eight 16-byte chunks of its K row starting at chunk i & 7, so that the 8 lanes of a quarter-warp read 8
-            // different bank groups of K and of q: conflict free.
-            float s_mine = -INFINITY;
-            if (lane < nr) {
-                const uint4 *krow = reinterpret_cast<const uint4 *>(Ks + (r0 + lane) * kHeadDim);
-                float acc4[4] = {0.f, 0.f, 0.f, 0.f};
-#pragma unroll
-                for (int c = 0; c < 8; ++c) {
-                    const int cc = (c + lane) & 7;
-                    const uint4 kk = krow[cc];
-                    const float4 qa = *reinterpret_cast<const float4 *>(&qs[warp][cc * 8]);
-                    const float4 qb = *reinterpret_cast<const float4 *>(&qs[warp][cc * 8 + 4]);
-                    const float2 k0 = __half22float2(*reinterpret_cast<const __half2 *>(&kk.x));
-                    const float2 k1 = __half22float2(*reinterpret_cast<const __half2 *>(&kk.y));
-                    const float2 k2 = __half22float2(*reinterpret_cast<const __half2 *>(&kk.z));
-                    const float2 k3 = __half22float2(*reinterpret_cast<const __half2 *>(&kk.w));
-                    acc4[0] = fmaf(qa.x, k0.x, fmaf(qa.y, k0.y, acc4[0]));
-                    acc4[1] = fmaf(qa.z, k1.x, fmaf(qa.w, k1.y, acc4[1]));
-                    acc4[2] = fmaf(qb.x, k2.x, fmaf(qb.y, k2.y, acc4[2]));
-                    acc4[3] = fmaf(qb.z, k3.x, fmaf(qb.w, k3.y, acc4[3]));
-                }
-                s_mine = (acc4[0] + acc4[1]) + (acc4[2] + acc4[3]);
-            }
-            const float m_new = fmaxf(m, warp_max(s_mine));
-            const float corr = __expf(m - m_new);   // m = -inf first time -> 0
-            const float pr = (lane < nr) ? __expf(s_mine - m_new) : 0.f;
-            l = l * corr + warp_sum(pr);
-            o0 *= corr;
-            o1 *= corr;
-            for (int r = 0; r < nr; ++r) {
-                const float pb = __shfl_sync(0xffffffffu, pr, r);
-                const float2 vv = __half22float2(*reinterpret_cast<const __half2 *>(Vs + (r0 + r) * kHeadDim + 2 * lane));
-                o0 = fmaf(pb, vv.x, o0);
-                o1 = fmaf(pb, vv.y, o1);
-            }
-            m = m_new;
-        }
+        attn_tile(Ks, Vs, nt, qs[warp], lane, m, l, o0, o1);
         __syncthreads();  // everyone done with the tile before it is overwritten
     }
     const size_t pidx = ((size_t)b * p.n_heads + head) * kMaxSplits + split;
     reinterpret_cast<float2 *>(p.part_o + pidx * kHeadDim)[lane] = make_float2(o0, o1);
     if (lane == 0) p.part_ml[pidx] = make_float2(m, l);
+}
+
+// =====================================================================================================
+// Batched decode, rows P4 + B2 of SURVEY.md 8(a) in ONE launch (was three: rope_append, attn_decode, attn_combine):
+// RoPE of this step's q and k, KV append, split-KV attention, split merge.  Same grid and warp roles as
+// attn_decode_kernel.  Per (sequence, KV head):
+//   * every split CTA rotates the q of its G heads itself (64 values per head from the fp32 Q|K|V row);
+//   * the split that holds the current position rotates k, rounds k and v to the cache type, appends the row to the
+//     cache AND patches it into its staged tile (the bulk copy stops one row short: it must not race the append);
+//   * the splits publish their states; the one that draws the last ticket (atomic counter per (sequence, KV head),
+//     reset by that CTA for the next launch) merges them in split order and writes the attention vector as bf16 planes.
+// Values and summation order are those of the three kernels it replaces.
+// =====================================================================================================
+__global__ void __launch_bounds__(256) attn_decode_fused_kernel(const __grid_constant__ AttnFusedParams p) {
+    __shared__ __align__(128) kv_t Ks[kAttnTile * kHeadDim];
+    __shared__ __align__(128) kv_t Vs[kAttnTile * kHeadDim];
+    __shared__ __align__(8) uint64_t bar;
+    __shared__ __align__(16) float qs[8][kHeadDim];
+    __shared__ __align__(16) kv_t new_k[kHeadDim], new_v[kHeadDim];
+    __shared__ int is_last;
+
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int G = p.n_heads / p.n_kv_heads;
+    const int kvh = blockIdx.y, b = blockIdx.z;
+    const int head = kvh * G + warp;
+
+    if (threadIdx.x == 0) {
+        mbar_init(&bar, 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    pdl_launch_dependents();
+    pdl_wait();
+
+    // the Q|K|V row of this sequence: RoPE pair (lane, lane + 32) of this warp's head, requested with the position
+    const int nh = p.n_heads + 2 * p.n_kv_heads;
+    const float *row = p.qkv + (size_t)b * nh * kHeadDim;
+    const float qa = ld_act(row + head * kHeadDim + lane), qc = ld_act(row + head * kHeadDim + lane + 32);
+    const int pos = ld_act(p.pos);
+    const int n_ctx = pos + 1;
+    const int ns = attn_num_splits(n_ctx);
+    const int split = blockIdx.x;
+    if (split >= ns) return;
+    const int len = attn_split_len(n_ctx, ns);
+    const int s0 = split * len;
+    const int s1 = min(n_ctx, s0 + len);
+    const bool has_new = pos >= s0 && pos < s1;
+
+    const size_t seq_base = ((size_t)b * p.n_kv_heads + kvh) * p.max_seq * kHeadDim;
+    kv_t *kg = p.kc + seq_base, *vg = p.vc + seq_base;
+    const float2 cs = p.rope[(size_t)pos * 32 + lane];
+    qs[warp][lane] = (qa * cs.x - qc * cs.y) * 0.125f;        // pre-scaled by 1/sqrt(64) (exact)
+    qs[warp][lane + 32] = (qc * cs.x + qa * cs.y) * 0.125f;
+    if (has_new && warp == 0) {
+        // this step's k (rotated) and v, rounded exactly as the cache row later steps will read
+        const float *kr = row + (p.n_heads + kvh) * kHeadDim, *vr = row + (p.n_heads + p.n_kv_heads + kvh) * kHeadDim;
+        const float ka = ld_act(kr + lane), kc2 = ld_act(kr + lane + 32), va = ld_act(vr + lane), vc2 = ld_act(vr + lane + 32);
+        const kv_t k0 = __float2half_rn(ka * cs.x - kc2 * cs.y), k1 = __float2half_rn(kc2 * cs.x + ka * cs.y);
+        const kv_t v0 = __float2half_rn(va), v1 = __float2half_rn(vc2);
+        new_k[lane] = k0; new_k[lane + 32] = k1; new_v[lane] = v0; new_v[lane + 32] = v1;
+        kv_t *dk = kg + (size_t)pos * kHeadDim, *dv = vg + (size_t)pos * kHeadDim;
+        dk[lane] = k0; dk[lane + 32] = k1; dv[lane] = v0; dv[lane + 32] = v1;
+    }
+    __syncthreads();
+
+    float m = -INFINITY, l = 0.f, o0 = 0.f, o1 = 0.f;
+    uint32_t parity = 0;
+    for (int t0 = s0; t0 < s1; t0 += kAttnTile) {
+        const int nt = min(kAttnTile, s1 - t0);
+        const bool patch = has_new && pos < t0 + nt;          // the current position is the last row of this tile
+        const int n_cached = patch ? nt - 1 : nt;
+        if (n_cached > 0) {
+            if (threadIdx.x == 0) {
+                const uint32_t bytes = (uint32_t)n_cached * kHeadDim * sizeof(kv_t);
+                mbar_expect_tx(&bar, 2 * bytes);
+                bulk_g2s(Ks, kg + (size_t)t0 * kHeadDim, bytes, &bar);
+                bulk_g2s(Vs, vg + (size_t)t0 * kHeadDim, bytes, &bar);
+            }
+            mbar_wait(&bar, parity);
+            parity ^= 1;
+        }
+        if (patch) {
+            for (int i = threadIdx.x; i < kHeadDim; i += blockDim.x) {
+                Ks[(nt - 1) * kHeadDim + i] = new_k[i];
+                Vs[(nt - 1) * kHeadDim + i] = new_v[i];
+            }
+            __syncthreads();
+        }
+        attn_tile(Ks, Vs, nt, qs[warp], lane, m, l, o0, o1);
+        __syncthreads();  // everyone done with the tile before it is overwritten
+    }
+    const size_t hb = (size_t)b * p.n_heads + head;
+    const size_t pidx = hb * kMaxSplits + split;
+    reinterpret_cast<float2 *>(p.part_o + pidx * kHeadDim)[lane] = make_float2(o0, o1);
+    if (lane == 0) p.part_ml[pidx] = make_float2(m, l);
+
+    // ticket: the CTA that finds ns - 1 earlier arrivals merges (its own stores and the others' are fenced before the draw)
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        unsigned int *ticket = p.tickets + (size_t)b * p.n_kv_heads + kvh;
+        const unsigned int old = atomicAdd(ticket, 1u);
+        is_last = old == (unsigned int)(ns - 1);
+        if (is_last) *ticket = 0u;       // for the next launch (kernel boundary orders it)
+    }
+    __syncthreads();
+    if (!is_last) return;
+    __threadfence();
+    if (lane < 8) {
+        // lanes 0-7 of warp w: 8 output dims each of head kvh * G + w; arithmetic and order of attn_combine_kernel
+        const int d0 = lane * 8;
+        const float2 *ml = p.part_ml + hb * kMaxSplits;
+        float2 mls[kMaxSplits];
+#pragma unroll
+        for (int s = 0; s < kMaxSplits; ++s) mls[s] = s < ns ? __ldcg(&ml[s]) : make_float2(-INFINITY, 0.f);
+        float M = -INFINITY;
+#pragma unroll
+        for (int s = 0; s < kMaxSplits; ++s) M = fmaxf(M, mls[s].x);
+        float acc[8] = {0, 0, 0, 0, 0, 0, 0, 0}, denom = 0.f;
+#pragma unroll
+        for (int s4 = 0; s4 < kMaxSplits; s4 += 4) {
+            if (s4 < ns) {
+                float4 a[4], c[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const float *po = p.part_o + (hb * kMaxSplits + s4 + u) * kHeadDim + d0;
+                    const bool ok = s4 + u < ns;
+                    a[u] = ok ? ld_act4(po) : make_float4(0.f, 0.f, 0.f, 0.f);
+                    c[u] = ok ? ld_act4(po + 4) : make_float4(0.f, 0.f, 0.f, 0.f);
+                }
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    if (s4 + u < ns) {
+                        const float w = __expf(mls[s4 + u].x - M);
+                        denom += w * mls[s4 + u].y;
+                        acc[0] += w * a[u].x; acc[1] += w * a[u].y; acc[2] += w * a[u].z; acc[3] += w * a[u].w;
+                        acc[4] += w * c[u].x; acc[5] += w * c[u].y; acc[6] += w * c[u].z; acc[7] += w * c[u].w;
+                    }
+                }
+            }
+        }
+        const float inv = 1.0f / denom;
+        act_t *dst = p.out + hb * kHeadDim + d0;
+#pragma unroll
+        for (int i = 0; i < 8; i += 2) {
+            uint32_t vh, vl;
+            split_bf16x2(acc[i] * inv, acc[i + 1] * inv, vh, vl);
+            *reinterpret_cast<uint32_t *>(dst + i) = vh;
+            *reinterpret_cast<uint32_t *>(dst + p.lo_offset + i) = vl;
+        }
+    }
 }
 
 // =====================================================================================================
@@ -424,6 +583,11 @@ cudaError_t launch_gemv(const LaunchCtx &c, GemvMode mode, GemvInput xin, const 
     if (mode == GEMV_QKV && xin == XIN_NORM) return launch_gemv_mx<GEMV_QKV, XIN_NORM>(c, p);
     if (mode == GEMV_RESID && xin == XIN_ATTN) return launch_gemv_mx<GEMV_RESID, XIN_ATTN>(c, p);
     return cudaErrorInvalidValue;
+}
+
+cudaError_t launch_attn_decode_fused(const LaunchCtx &c, const AttnFusedParams &p, int batch) {
+    const int G = p.n_heads / p.n_kv_heads;
+    return launch_k(c, attn_decode_fused_kernel, dim3(kMaxSplits, p.n_kv_heads, batch), dim3(32 * G), p);
 }
 
 cudaError_t launch_attn_decode(const LaunchCtx &c, const AttnDecodeParams &p, int batch) {

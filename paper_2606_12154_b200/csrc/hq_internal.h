@@ -53,6 +53,7 @@ struct Buffers {
     int *tok_hist = nullptr;                    // [Tmax+1][B] emitted tokens, index = pos at emission
     unsigned long long *best = nullptr;         // [B] packed argmax
     unsigned int *counter = nullptr;            // last-CTA ticket
+    unsigned int *attn_tickets = nullptr;       // [B][Hkv] last-split tickets of attn_decode_fused_kernel (zero between launches)
     float *x = nullptr;                         // [B][d] residual stream
     float *q = nullptr;                         // [B][H*64]
     float *part_o = nullptr;                    // [B][H][kMaxSplits][64]
@@ -173,6 +174,20 @@ struct AttnDecodeParams {
     int n_heads, n_kv_heads, max_seq;
 };
 
+// batched decode: RoPE + KV append + split-KV attention + split merge in one launch (attn_decode_fused_kernel)
+struct AttnFusedParams {
+    const float *qkv;        // fp32 [batch][(H + 2 Hkv) * 64]: this step's projections, complete (not rotated)
+    kv_t *kc, *vc;           // layer base; row pos of every sequence is appended
+    const float2 *rope;      // [max_seq][32] (cos, sin)
+    float *part_o;
+    float2 *part_ml;
+    unsigned int *tickets;   // [batch][Hkv], zero between launches
+    act_t *out;              // attention vector as bf16 planes: hi [batch][H * 64], lo at + lo_offset
+    size_t lo_offset;
+    const int *pos;
+    int n_heads, n_kv_heads, max_seq;
+};
+
 // split policy shared by the attention kernel and the O-proj prologue (host + device)
 __host__ __device__ inline int attn_num_splits(int n_ctx) {
     int s = (n_ctx + kMinSplitLen - 1) / kMinSplitLen;
@@ -275,6 +290,7 @@ cudaError_t launch_copy_probe(cudaStream_t stream, const void *src, size_t bytes
 cudaError_t launch_embed(const LaunchCtx &c, const bf16 *emb, const int *tok, float *x, int hidden, int batch);
 cudaError_t launch_gemv(const LaunchCtx &c, GemvMode mode, GemvInput xin, const GemvParams &p);
 cudaError_t launch_attn_decode(const LaunchCtx &c, const AttnDecodeParams &p, int batch);
+cudaError_t launch_attn_decode_fused(const LaunchCtx &c, const AttnFusedParams &p, int batch);
 cudaError_t launch_advance(const LaunchCtx &c, int *pos, int inc);
 cudaError_t launch_set_state(const LaunchCtx &c, int *pos, int pos_value, unsigned long long *best,
                              unsigned int *counter, int batch, int *err);
