@@ -357,17 +357,20 @@ static cudaError_t enqueue_rows_layers(hq_model *m, int batch, int Tc, bool deco
         const LayerW &w = m->layers[l];
         const LayerMaps &mp = m->maps[l];
         kv_t *kc = b.kcache + l * layer_kv, *vc = b.vcache + l * layer_kv;
-        STEP(launch_rmsnorm_rows(lc, b.xs, b.delta, pending, d_stride, w.attn_norm, b.hn, lo_d, d, c.rms_eps, rows, nullptr, d));
-        pending = 0;
         // P1: Q, K, V projections (three weight pointers, no repack) into one fp32 [rows][qkvd] buffer
         const bool stacked = qdim % 128 == 0 && kvdim % 128 == 0;
         const int split_store = decode ? 16 : kPrefillSplits, split_resid = decode ? 16 : kPrefillSplits;
         const TilePlan pq = plan_gemm(m, stacked ? qkvd : qdim, rows, d, split_store);
         const size_t qs = defer ? q_stride : 0;   // prefill: one partial buffer per split; batched decode: atomics into a zeroed buffer
-        if (pq.splits > 1 && !defer) {
+        // batched decode: the norm kernel clears the rows the split-K projections add into (no memset node between the two)
+        const bool zero_qkv = pq.splits > 1 && !defer;
+        if (zero_qkv && qkvd % 4 != 0) {
             e = cudaMemsetAsync(b.qkv, 0, (size_t)rows * qkvd * sizeof(float), m->stream);
             if (e != cudaSuccess) return e;
         }
+        STEP(launch_rmsnorm_rows(lc, b.xs, b.delta, pending, d_stride, w.attn_norm, b.hn, lo_d, d, c.rms_eps, rows, nullptr, d,
+                                 zero_qkv && qkvd % 4 == 0 ? b.qkv : nullptr, qkvd));
+        pending = 0;
         if (stacked) {
             STEP(launch_gemm_qkv(lc, mp.wq, mp.wk, mp.wv, m->map_hn[pq.ti], R, qdim, kvdim, kvdim, d, rows, pq.NT, pq.splits, b.qkv, qkvd, qs));
         } else {

@@ -267,7 +267,8 @@ cudaError_t launch_gemm_qkv(const LaunchCtx &c, const TensorMap &wq, const Tenso
 // ---- row-batched kernels (hq_prefill.cu) -------------------------------------------------------------
 cudaError_t launch_embed_rows(const LaunchCtx &c, const bf16 *emb, const int *tok, float *x, int hidden, int rows);
 cudaError_t launch_rmsnorm_rows(const LaunchCtx &c, float *x, const float *delta, int n_parts, size_t part_stride, const bf16 *gain,
-                                act_t *out, size_t lo_offset, int hidden, float eps, int rows, const int *row_index, int x_stride_rows);
+                                act_t *out, size_t lo_offset, int hidden, float eps, int rows, const int *row_index, int x_stride_rows,
+                                float *zero = nullptr, int zero_per_row = 0);
 cudaError_t launch_add_delta_rows(const LaunchCtx &c, float *x, const float *delta, int n_parts, size_t part_stride, size_t n);
 cudaError_t launch_rope_append(const LaunchCtx &c, const float *qkv, int n_parts, size_t part_stride, __half *q16, float *q32, kv_t *kc,
                                kv_t *vc, const float2 *rope, const int *pos, int rows, int Tc, int n_heads, int n_kv_heads,

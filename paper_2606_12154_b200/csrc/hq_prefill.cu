@@ -32,11 +32,16 @@ __global__ void __launch_bounds__(256) embed_rows_kernel(const bf16 *__restrict_
 // projections bit-reproducible without atomics: every split stores its own partial, the consumer adds them in order.
 __global__ void __launch_bounds__(256) rmsnorm_rows_kernel(float *x, const float *delta, int n_parts, size_t part_stride, const bf16 *__restrict__ gain,
                                                            act_t *__restrict__ out, size_t lo_offset, int hidden,
-                                                           float eps, const int *row_index, int x_stride_rows) {
+                                                           float eps, const int *row_index, int x_stride_rows, float *zero, int zero_per_row) {
     pdl_launch_dependents();
     pdl_wait();
     __shared__ float red[8];
     const int m = blockIdx.x;
+    // zero (optional): row m of a buffer the NEXT kernel accumulates into with atomics (the Q|K|V projections of a batched
+    // decode step).  Cleared here instead of by a memset node, which would cut the programmatic launch edge to that kernel.
+    if (zero)
+        for (int c = threadIdx.x; c < (zero_per_row >> 2); c += blockDim.x)
+            reinterpret_cast<float4 *>(zero + (size_t)m * zero_per_row)[c] = make_float4(0.f, 0.f, 0.f, 0.f);
     // row_index (optional) gathers rows (e.g. last position of every sequence)
     const size_t src = row_index ? (size_t)row_index[m] : (size_t)m;
     float *xr = x + src * x_stride_rows;
@@ -577,9 +582,11 @@ cudaError_t launch_embed_rows(const LaunchCtx &c, const bf16 *emb, const int *to
     return launch_k(c, embed_rows_kernel, dim3(rows), dim3(256), emb, tok, x, hidden);
 }
 cudaError_t launch_rmsnorm_rows(const LaunchCtx &c, float *x, const float *delta, int n_parts, size_t part_stride, const bf16 *gain,
-                                act_t *out, size_t lo_offset, int hidden, float eps, int rows, const int *row_index, int x_stride_rows) {
+                                act_t *out, size_t lo_offset, int hidden, float eps, int rows, const int *row_index, int x_stride_rows,
+                                float *zero, int zero_per_row) {
+    if (zero && zero_per_row % 4 != 0) return cudaErrorInvalidValue;
     return launch_k(c, rmsnorm_rows_kernel, dim3(rows), dim3(256), x, delta, n_parts, part_stride, gain, out, lo_offset, hidden, eps,
-                    row_index, x_stride_rows);
+                    row_index, x_stride_rows, zero, zero_per_row);
 }
 // x += delta, delta = 0 (parity capture needs the residual itself after every layer)
 __global__ void __launch_bounds__(256) add_delta_rows_kernel(float *x, const float *delta, int n_parts, size_t part_stride, size_t n4) {
