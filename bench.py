@@ -479,8 +479,10 @@ def main():
         # sets cycled so that they come from HBM), stamps of the CTAs of the first token tile / K split, medians over CTAs.
         shapes = [("prefill gate/up", 2, s.ffn, s.hidden, 256, 128, 1), ("prefill Q|K|V", 0, 3072, s.hidden, 256, 128, 2),
                   ("prefill O", 0, s.hidden, s.hidden, 256, 128, 4), ("prefill down", 0, s.hidden, s.ffn, 256, 128, 4),
-                  ("decode B=8 gate/up", 3, s.ffn, s.hidden, 8, 32, 1), ("decode B=8 down", 0, s.hidden, s.ffn, 8, 32, 9),
-                  ("decode B=8 LM head", 0, s.vocab, s.hidden, 8, 32, 1)]
+                  ("decode B=8 gate/up", 3, s.ffn, s.hidden, 8, 8, 1), ("decode B=8 down", 0, s.hidden, s.ffn, 8, 8, 9),
+                  ("decode B=8 LM head", 0, s.vocab, s.hidden, 8, 8, 1),
+                  ("decode B=8 gate/up, 32-token tile", 3, s.ffn, s.hidden, 8, 32, 1), ("decode B=8 down, 32-token tile", 0, s.hidden, s.ffn, 8, 32, 9),
+                  ("decode B=32 LM head", 0, s.vocab, s.hidden, 32, 32, 1)]
         g = torch.Generator(device=dev).manual_seed(7)
         with torch.cuda.stream(stream):
             for name, mode, N, K, T, tile, splits in shapes:

@@ -28,7 +28,8 @@ int32_t hq_bench_kernel(hq_model *m, int32_t which, int32_t reps, int64_t *bytes
 
 /* Diagnostics: the tcgen05 GEMM of the prefill / batched-decode path on its own (unit tests).
  * All pointers DEVICE.  w, w2: bf16 [n_rows][k]; x: bf16 [2][n_tokens][k], the activation as two planes
- * x = hi + lo (hi = bf16(x), lo = bf16(x - hi)); token_tile in {32,64,128,256}.
+ * x = hi + lo (hi = bf16(x), lo = bf16(x - hi)); token_tile in {32,64,128,256}, or 8 / 16 (the batched-decode
+ * tiles for <= 8 / <= 16 sequences; not in mode 2).
  *   mode 0: out fp32 [n_tokens][n_rows]  = x w^T   (splits > 1: out must be zeroed, partials add atomically)
  *   mode 1: out fp32 [n_tokens][n_rows] += x w^T   (residual epilogue)
  *   mode 2: out bf16 [2][n_tokens][n_rows] = hi/lo planes of silu(x w^T) * (x w2^T)   (SwiGLU epilogue)

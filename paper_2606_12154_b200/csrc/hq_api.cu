@@ -333,6 +333,14 @@ static TilePlan plan_gemm(const hq_model *m, int n_rows, int rows, int K, int ma
     return p;
 }
 
+// Batched decode steps of <= 16 sequences: token tiles of 8 / 16 rows instead of 32.  The main loop of these GEMMs pays
+// for every shared-memory byte (profiles/r02_batched_decode.md, item 10): a 32-row tile that is 3/4 padding is 8 KB of TMA
+// writes and 8 KB of operand reads per 16 KB of weights, an 8-row tile 2 KB of each.
+static void small_token_tile(TilePlan &p, int rows) {
+    if (rows <= 8) { p.ti = 4; p.NT = 8; }
+    else if (rows <= 16) { p.ti = 5; p.NT = 16; }
+}
+
 // All layers for `rows` = batch * Tc token rows already embedded in b.xs; positions start at *b.pos.
 // decode = true: Tc == 1, attention over the cache with the split-KV decode kernel.
 static cudaError_t enqueue_rows_layers(hq_model *m, int batch, int Tc, bool decode, bool capture_hidden, int *n_launched) {
@@ -360,7 +368,8 @@ static cudaError_t enqueue_rows_layers(hq_model *m, int batch, int Tc, bool deco
         // P1: Q, K, V projections (three weight pointers, no repack) into one fp32 [rows][qkvd] buffer
         const bool stacked = qdim % 128 == 0 && kvdim % 128 == 0;
         const int split_store = decode ? 16 : kPrefillSplits, split_resid = decode ? 16 : kPrefillSplits;
-        const TilePlan pq = plan_gemm(m, stacked ? qkvd : qdim, rows, d, split_store);
+        TilePlan pq = plan_gemm(m, stacked ? qkvd : qdim, rows, d, split_store);
+        if (decode) small_token_tile(pq, rows);
         const size_t qs = defer ? q_stride : 0;   // prefill: one partial buffer per split; batched decode: atomics into a zeroed buffer
         // batched decode: the norm kernel clears the rows the split-K projections add into (no memset node between the two)
         const bool zero_qkv = pq.splits > 1 && !defer;
@@ -389,18 +398,21 @@ static cudaError_t enqueue_rows_layers(hq_model *m, int batch, int Tc, bool deco
             // P2: causal flash attention
             STEP(launch_flash_prefill(lc, b.q16, kc, vc, b.ao, lo_q, b.pos, batch, Tc, c.n_heads, c.n_kv_heads, c.max_seq));
         }
-        const TilePlan po = plan_gemm(m, d, rows, qdim, split_resid);
+        TilePlan po = plan_gemm(m, d, rows, qdim, split_resid);
+        if (decode) small_token_tile(po, rows);
         STEP(launch_gemm(lc, defer ? EPI_STORE : EPI_RESID, mp.wo, nullptr, m->map_ao[po.ti], R, d, qdim, rows, po.NT, po.splits,
                          defer ? b.delta : b.xs, nullptr, 0, d, defer ? d_stride : 0));
         if (defer) pending = po.splits;
         STEP(launch_rmsnorm_rows(lc, b.xs, b.delta, pending, d_stride, w.ffn_norm, b.hn, lo_d, d, c.rms_eps, rows, nullptr, d));
         pending = 0;
-        const TilePlan pg = plan_gemm(m, c.ffn, rows, d, 1);
+        TilePlan pg = plan_gemm(m, c.ffn, rows, d, 1);
         // batched decode (one token tile): 64-row weight tiles, so that ffn / 64 CTAs stream gate/up instead of ffn / 128
         const bool half_tiles = decode && c.ffn % 64 == 0 && (c.ffn / 128) * ((rows + pg.NT - 1) / pg.NT) < m->n_sms;
+        if (half_tiles) small_token_tile(pg, rows);   // (the two-accumulator form keeps 32-row tiles)
         STEP(launch_gemm(lc, half_tiles ? EPI_SWIGLU64 : EPI_SWIGLU, half_tiles ? mp.w_gate64 : mp.w_gate, half_tiles ? &mp.w_up64 : &mp.w_up,
                          m->map_hn[pg.ti], R, c.ffn, d, rows, pg.NT, 1, nullptr, b.actb, lo_f, c.ffn));
-        const TilePlan pd = plan_gemm(m, d, rows, c.ffn, split_resid);
+        TilePlan pd = plan_gemm(m, d, rows, c.ffn, split_resid);
+        if (decode) small_token_tile(pd, rows);
         STEP(launch_gemm(lc, defer ? EPI_STORE : EPI_RESID, mp.w_down, nullptr, m->map_actb[pd.ti], R, d, c.ffn, rows, pd.NT, pd.splits,
                          defer ? b.delta : b.xs, nullptr, 0, d, defer ? d_stride : 0));
         if (defer) pending = pd.splits;
@@ -444,7 +456,9 @@ static cudaError_t enqueue_rows_head(hq_model *m, int batch, int Tc, int pos_inc
     STEP(launch_rmsnorm_rows(lc, b.xs + (size_t)(Tc - 1) * c.hidden, b.delta + (size_t)(Tc - 1) * c.hidden, deferred ? m->delta_pending : 0,
                              (size_t)m->pf_rows * c.hidden, m->final_norm, b.hn_last, (size_t)32 * c.hidden, c.hidden, c.rms_eps, batch, nullptr,
                              Tc * c.hidden));
-    STEP(launch_gemm(lc, EPI_STORE, m->map_lm_head, nullptr, m->map_hn_last, 32, c.vocab, c.hidden, batch, 32, 1, b.logits,
+    TilePlan ph{0, 32, 1};
+    small_token_tile(ph, batch);
+    STEP(launch_gemm(lc, EPI_STORE, m->map_lm_head, nullptr, m->map_hn_last[ph.ti], 32, c.vocab, c.hidden, batch, ph.NT, 1, b.logits,
                      nullptr, 0, c.vocab));
     STEP(launch_argmax_rows(lc, b.logits, c.vocab, batch, b.cur_tok, b.tok_hist, b.pos, pos_inc, b.counter, b.best));
 #undef STEP
@@ -501,13 +515,13 @@ static bool build_tensor_maps(hq_model *m) {
              make_tensor_map_16b(&mp.w_up64, w.w_up, F, d, 64);
     }
     ok = ok && make_tensor_map_16b(&m->map_lm_head, m->lm_head, c.vocab, d, 128);
-    for (int i = 0; i < 4; ++i) {
+    for (int i = 0; i < 6; ++i) {
         const uint32_t nt = kTokenTiles[i];
         ok = ok && make_tensor_map_16b(&m->map_hn[i], b.hn, 2 * (uint64_t)m->pf_rows, d, nt) &&
              make_tensor_map_16b(&m->map_ao[i], b.ao, 2 * (uint64_t)m->pf_rows, qdim, nt) &&
              make_tensor_map_16b(&m->map_actb[i], b.actb, 2 * (uint64_t)m->pf_rows, F, nt);
     }
-    ok = ok && make_tensor_map_16b(&m->map_hn_last, b.hn_last, 64, d, 32);
+    for (int i : {0, 4, 5}) ok = ok && make_tensor_map_16b(&m->map_hn_last[i], b.hn_last, 64, d, kTokenTiles[i]);
     return ok;
 }
 
@@ -1062,8 +1076,8 @@ static int32_t debug_gemm_impl(void *cuda_stream, int32_t mode, const void *w_de
         return fail(HQ_ERR_INVALID_ARG, "hq_debug_gemm: bad argument");
     if (mode < 0 || mode > 3 || (mode >= 2 && !w2_dev)) return fail(HQ_ERR_INVALID_ARG, "hq_debug_gemm: bad mode");
     if (mode == 3 && n_rows % 64 != 0) return fail(HQ_ERR_UNSUPPORTED, "hq_debug_gemm: mode 3 needs n_rows % 64 == 0");
-    if (token_tile != 32 && token_tile != 64 && token_tile != 128 && token_tile != 256)
-        return fail(HQ_ERR_INVALID_ARG, "hq_debug_gemm: token_tile must be 32, 64, 128 or 256");
+    if (token_tile != 32 && token_tile != 64 && token_tile != 128 && token_tile != 256 && !((token_tile == 8 || token_tile == 16) && mode != 2))
+        return fail(HQ_ERR_INVALID_ARG, "hq_debug_gemm: token_tile must be 32, 64, 128 or 256 (8 or 16 too, except in mode 2)");
     if (k % 8 != 0) return fail(HQ_ERR_UNSUPPORTED, "hq_debug_gemm: k must be a multiple of 8");
     TensorMap mw, mw2, mx;
     // x_dev holds the hi plane [n_tokens][k] followed by the lo plane [n_tokens][k]

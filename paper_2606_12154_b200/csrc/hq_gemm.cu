@@ -362,10 +362,20 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap map_w, const __grid_constant_
         const bool row_ok = n < p.n_rows;
         const bool pairable = (p.n_rows & 1) == 0 && (p.ld_out & 1) == 0;   // bf16 outputs as 32-bit pairs
         for (int c = 0; c < NT; c += 32) {
-            const int nvalid = p.T - (t0 + c);   // tokens of this chunk that exist (>= 32: all)
+            const int nvalid = min(p.T - (t0 + c), NT - c);   // tokens of this chunk that exist and belong to this tile (>= 32: all)
             uint32_t v[32];
             tmem_ld32(lane_addr + c, v);
-            if (stacked) {
+            if (NT < 32) {
+                // small token tiles (batched decode with <= 16 sequences): the hi and lo halves of the accumulator are columns
+                // [0, NT) and [NT, 2 NT) of the 32 just read (the allocation is 32 columns: nothing beyond them may be read)
+                if (NT == 8) {
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) v[j] = __float_as_uint(__uint_as_float(v[j]) + __uint_as_float(v[8 + j]));
+                } else {
+#pragma unroll
+                    for (int j = 0; j < 16; ++j) v[j] = __float_as_uint(__uint_as_float(v[j]) + __uint_as_float(v[16 + j]));
+                }
+            } else if (stacked) {
                 uint32_t w[32];
                 tmem_ld32(lane_addr + NT + c, w);
 #pragma unroll
@@ -484,7 +494,7 @@ static cudaError_t launch_mode(const LaunchCtx &c, const TensorMap &w, const Ten
     // CTA pairs (cta_group::2, M = 256) for prefill-sized passes: the activation tile is shared by two weight tiles, each CTA
     // loads one of its two planes (a third less operand traffic from L2, the bound of these GEMMs).  Needs the stacked-plane
     // form (token tile <= 128); batched-decode steps (<= 32 rows) keep single CTAs.
-    const bool pair = MODE != EPI_SWIGLU64 && p.NT <= 128 && p.T > 32;
+    const bool pair = MODE != EPI_SWIGLU64 && p.NT >= 32 && p.NT <= 128 && p.T > 32;
     const int stage_bytes = nacc * kBlockM * kBlockK * 2 + (pair ? 1 : 2) * p.NT * kBlockK * 2;
     int stages = kSmemBudget / stage_bytes;
     if (stages > 8) stages = 8;
@@ -524,6 +534,13 @@ static cudaError_t launch_mode(const LaunchCtx &c, const TensorMap &w, const Ten
                               *reinterpret_cast<const CUtensorMap *>(&w3), *reinterpret_cast<const CUtensorMap *>(&x), p);
 }
 
+// token tiles: 32, 64, 128, 256, and 8 / 16 for passes of <= 16 rows (not for the two-accumulator SwiGLU form, whose second
+// accumulator the epilogue reads with a 32-column load of its own)
+static bool gemm_token_tile_ok(int NT, int mode) {
+    if (NT == 8 || NT == 16) return mode != EPI_SWIGLU;
+    return NT % 32 == 0 && NT >= 32 && NT <= 256;
+}
+
 // n_rows: weight rows (output features; for EPI_SWIGLU the ffn size), K: reduction size (multiple of 64),
 // T: valid tokens, NT: token tile (32/64/128/256).  splits > 1 requires atomic accumulation (EPI_STORE into a
 // zeroed buffer, EPI_RESID always legal).
@@ -531,7 +548,7 @@ cudaError_t launch_gemm(const LaunchCtx &c, GemmEpilogue mode, const TensorMap &
                         const TensorMap &x, int x_lo_row, int n_rows, int K, int T, int NT, int splits, float *out_f32,
                         act_t *out_act, size_t out_lo_offset, int ld_out, size_t split_stride, unsigned long long *trace) {
     // K need not be a multiple of 64: TMA zero-fills the out-of-range tail of the last K block
-    if (K % 8 != 0 || NT % 32 != 0 || NT < 32 || NT > 256 || T <= 0) return cudaErrorInvalidValue;
+    if (K % 8 != 0 || !gemm_token_tile_ok(NT, mode) || T <= 0) return cudaErrorInvalidValue;
     const int kblocks = (K + kBlockK - 1) / kBlockK;
     if (splits < 1) splits = 1;
     if (splits > kblocks) splits = kblocks;
@@ -562,7 +579,7 @@ cudaError_t launch_gemm(const LaunchCtx &c, GemmEpilogue mode, const TensorMap &
 cudaError_t launch_gemm_qkv(const LaunchCtx &c, const TensorMap &wq, const TensorMap &wk, const TensorMap &wv, const TensorMap &x,
                             int x_lo_row, int n1, int n2, int n3, int K, int T, int NT, int splits, float *out_f32, int ld_out,
                             size_t split_stride) {
-    if (K % 8 != 0 || NT % 32 != 0 || NT < 32 || NT > 256 || T <= 0 || n1 % kBlockM || n2 % kBlockM || n3 % kBlockM)
+    if (K % 8 != 0 || !gemm_token_tile_ok(NT, EPI_STORE) || T <= 0 || n1 % kBlockM || n2 % kBlockM || n3 % kBlockM)
         return cudaErrorInvalidValue;
     const int kblocks = (K + kBlockK - 1) / kBlockK;
     if (splits < 1) splits = 1;

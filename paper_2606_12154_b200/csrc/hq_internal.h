@@ -82,7 +82,7 @@ struct Buffers {
     unsigned int *ab_epoch = nullptr;           // attention block: tag of the next launch (starts at 1, never reset)
 };
 
-constexpr int kTokenTiles[4] = {32, 64, 128, 256};
+constexpr int kTokenTiles[6] = {32, 64, 128, 256, 8, 16};   // indices 4, 5: batched decode steps of <= 8 / <= 16 sequences
 struct LayerMaps { TensorMap wq, wk, wv, wo, w_gate, w_up, w_down, w_gate64, w_up64; };   // *64: 64-row boxes (EPI_SWIGLU64)
 
 struct hq_model_impl {
@@ -107,7 +107,7 @@ struct hq_model_impl {
     int pf_rows = 0;                            // row capacity of one pass
     std::vector<LayerMaps> maps;
     TensorMap map_lm_head;
-    TensorMap map_hn[4], map_ao[4], map_actb[4], map_hn_last;   // activation maps per token tile
+    TensorMap map_hn[6], map_ao[6], map_actb[6], map_hn_last[6];   // activation maps per token tile (map_hn_last: tiles <= 32 only)
     cudaGraphExec_t batch_graph = nullptr;      // batched decode step (captured for batch_graph_b)
     int batch_graph_b = 0, batch_graph_kernels = 0, batch_eager_b = 0;
     int delta_pending = 0;                      // split-K partials of the last O / down projection of a pass not yet added to xs

@@ -41,6 +41,11 @@ def _case(N, K, T, seed):
     (256, 688, 33, 64, 2),       # ragged K (688 = 10*64 + 48): TMA zero fill
     (2048, 8192, 300, 256, 9),   # down-proj shape, two token tiles
     (384, 512, 8, 32, 2),        # batched-decode shape: 8 sequences padded to a 32-token tile
+    (384, 512, 8, 8, 2),         # the same in an 8-token tile (batched decode with <= 8 sequences)
+    (2048, 8192, 5, 8, 9),       # down-projection shape, 5 sequences, 8-token tile, 9 K splits
+    (3072, 2048, 16, 16, 6),     # Q|K|V shape, 16 sequences, 16-token tile
+    (640, 256, 13, 16, 1),       # ragged tokens inside a 16-token tile
+    (256, 512, 40, 8, 1),        # several 8-token tiles, ragged last one
     (384, 512, 100, 64, 1),      # CTA pairs (token tile <= 128, more than 32 tokens) with an odd number of weight tiles
     (3072, 2048, 256, 128, 2),   # the 1B Q|K|V shape as the prefill pass runs it: CTA pairs, 128-token tiles, 2 K splits
     (2048, 8192, 256, 128, 4),   # the 1B down-projection shape: CTA pairs, 4 K splits
@@ -84,6 +89,9 @@ def test_gemm_residual_accumulates():
 @pytest.mark.parametrize("mode,N,K,T,tile", [
     (2, 688, 256, 100, 128),    # two accumulators per 128-row tile, ragged weight rows
     (3, 704, 256, 8, 32),       # 64-row tiles (batched decode), an odd number of them, 8 sequences in a 32-token tile
+    (3, 704, 256, 8, 8),        # the same in an 8-token tile
+    (3, 8192, 2048, 16, 16),    # the 1B gate/up shape at batch 16, 16-token tile
+    (3, 256, 512, 11, 16),
     (3, 8192, 2048, 32, 32),    # the 1B gate/up shape at batch 32
     (3, 256, 512, 70, 64),      # 64-row tiles, two exchange rounds per token tile, ragged tokens
 ])
