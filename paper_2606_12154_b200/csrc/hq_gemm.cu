@@ -210,7 +210,12 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap map_w, const __grid_constant_
     // operand traffic from shared memory than two MMAs into the same columns); the epilogue adds the two halves
     const bool stacked = NT <= 128;   // always true for CTA pairs (launch_mode)
     const int acc_cols = stacked ? 2 * NT : NT;          // TMEM columns of one accumulator
-    const uint32_t need_cols = (uint32_t)(NACC * acc_cols);
+    // Token tiles of <= 32 rows, one accumulator, single CTA (batched decode): the four K = 16 MMAs of a K block go to FOUR
+    // accumulators (summed by the epilogue) instead of one.  Consecutive MMAs into the same tensor-memory columns are a
+    // dependent chain, and at N <= 64 an MMA is far shorter than its latency: one chain cost 0.43 us per K block, four
+    // independent ones 0.35 (bench.py --gemm-timeline; profiles/r02_batched_decode.md).
+    const bool quad = CTAS == 1 && NACC == 1 && NT <= 32;
+    const uint32_t need_cols = (uint32_t)(NACC * acc_cols) * (quad ? 4u : 1u);
     const uint32_t tmem_cols = need_cols <= 32 ? 32 : need_cols <= 64 ? 64 : need_cols <= 128 ? 128 : need_cols <= 256 ? 256 : 512;
 
     if (warp == 0 && lane == 0) {
@@ -332,7 +337,9 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap map_w, const __grid_constant_
                 for (int k = 0; k < kBlockK / 16; ++k) {
                     const uint32_t acc = (i > 0 || k > 0) ? 1u : 0u;
                     // advance 16 elements = 32 bytes inside the 128-byte swizzle row: +2 in the >>4 address field
-                    if (stacked) {
+                    if (quad) {
+                        umma_bf16(tmem_base + k * acc_cols, da + 2 * k, db + 2 * k, idesc, i > 0 ? 1u : 0u);   // chain k of four
+                    } else if (stacked) {
                         umma_bf16(tmem_base, da + 2 * k, db + 2 * k, idesc, acc);       // W * [x_hi ; x_lo]
                         if (NACC == 2) umma_bf16(tmem_base + acc_cols, da2 + 2 * k, db + 2 * k, idesc, acc);
                     } else {
@@ -365,13 +372,25 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap map_w, const __grid_constant_
             const int nvalid = min(p.T - (t0 + c), NT - c);   // tokens of this chunk that exist and belong to this tile (>= 32: all)
             uint32_t v[32];
             tmem_ld32(lane_addr + c, v);
-            if (NT < 32) {
-                // small token tiles (batched decode with <= 16 sequences): the hi and lo halves of the accumulator are columns
-                // [0, NT) and [NT, 2 NT) of the 32 just read (the allocation is 32 columns: nothing beyond them may be read)
+            if (quad) {
+                // four accumulators of 2 NT columns ([hi | lo] each) = NT / 4 loads of 32 columns, added column-wise; then the
+                // 32 columns fold to NT tokens (8: four groups of 8; 16: two groups of 16; 32: the loads already alternate
+                // hi and lo of the same tokens)
+                const int n_loads = NT >> 2;
+#pragma unroll
+                for (int ql = 1; ql < 8; ++ql) {
+                    if (ql < n_loads) {   // warp-uniform
+                        uint32_t w[32];
+                        tmem_ld32(lane_addr + 32 * ql, w);
+#pragma unroll
+                        for (int j = 0; j < 32; ++j) v[j] = __float_as_uint(__uint_as_float(v[j]) + __uint_as_float(w[j]));
+                    }
+                }
                 if (NT == 8) {
 #pragma unroll
-                    for (int j = 0; j < 8; ++j) v[j] = __float_as_uint(__uint_as_float(v[j]) + __uint_as_float(v[8 + j]));
-                } else {
+                    for (int j = 0; j < 8; ++j)
+                        v[j] = __float_as_uint((__uint_as_float(v[j]) + __uint_as_float(v[8 + j])) + (__uint_as_float(v[16 + j]) + __uint_as_float(v[24 + j])));
+                } else if (NT == 16) {
 #pragma unroll
                     for (int j = 0; j < 16; ++j) v[j] = __float_as_uint(__uint_as_float(v[j]) + __uint_as_float(v[16 + j]));
                 }
