@@ -405,6 +405,13 @@ __global__ void __launch_bounds__(256) attn_decode_fused_kernel(const __grid_con
     const int nh = p.n_heads + 2 * p.n_kv_heads;
     const float *row = p.qkv + (size_t)b * nh * kHeadDim;
     const float qa = ld_act(row + head * kHeadDim + lane), qc = ld_act(row + head * kHeadDim + lane + 32);
+    // warp 0 also requests this step's k and v now (needed only by the split that holds the current position, but the
+    // loads do not depend on the position: one L2 round trip instead of a third one later)
+    float ka = 0.f, kc2 = 0.f, va = 0.f, vc2 = 0.f;
+    if (warp == 0) {
+        const float *kr = row + (p.n_heads + kvh) * kHeadDim, *vr = row + (p.n_heads + p.n_kv_heads + kvh) * kHeadDim;
+        ka = ld_act(kr + lane); kc2 = ld_act(kr + lane + 32); va = ld_act(vr + lane); vc2 = ld_act(vr + lane + 32);
+    }
     const int pos = ld_act(p.pos);
     const int n_ctx = pos + 1;
     const int ns = attn_num_splits(n_ctx);
@@ -418,12 +425,19 @@ __global__ void __launch_bounds__(256) attn_decode_fused_kernel(const __grid_con
     const size_t seq_base = ((size_t)b * p.n_kv_heads + kvh) * p.max_seq * kHeadDim;
     kv_t *kg = p.kc + seq_base, *vg = p.vc + seq_base;
     const float2 cs = p.rope[(size_t)pos * 32 + lane];
+    // the cached rows of the first tile are requested before the RoPE arithmetic (they depend on the position only)
+    const int nt_first = min(kAttnTile, s1 - s0);
+    const int nc_first = (has_new && pos < s0 + nt_first) ? nt_first - 1 : nt_first;
+    if (threadIdx.x == 0 && nc_first > 0) {
+        const uint32_t bytes = (uint32_t)nc_first * kHeadDim * sizeof(kv_t);
+        mbar_expect_tx(&bar, 2 * bytes);
+        bulk_g2s(Ks, kg + (size_t)s0 * kHeadDim, bytes, &bar);
+        bulk_g2s(Vs, vg + (size_t)s0 * kHeadDim, bytes, &bar);
+    }
     qs[warp][lane] = (qa * cs.x - qc * cs.y) * 0.125f;        // pre-scaled by 1/sqrt(64) (exact)
     qs[warp][lane + 32] = (qc * cs.x + qa * cs.y) * 0.125f;
     if (has_new && warp == 0) {
         // this step's k (rotated) and v, rounded exactly as the cache row later steps will read
-        const float *kr = row + (p.n_heads + kvh) * kHeadDim, *vr = row + (p.n_heads + p.n_kv_heads + kvh) * kHeadDim;
-        const float ka = ld_act(kr + lane), kc2 = ld_act(kr + lane + 32), va = ld_act(vr + lane), vc2 = ld_act(vr + lane + 32);
         const kv_t k0 = __float2half_rn(ka * cs.x - kc2 * cs.y), k1 = __float2half_rn(kc2 * cs.x + ka * cs.y);
         const kv_t v0 = __float2half_rn(va), v1 = __float2half_rn(vc2);
         new_k[lane] = k0; new_k[lane + 32] = k1; new_v[lane] = v0; new_v[lane + 32] = v1;
@@ -439,7 +453,7 @@ __global__ void __launch_bounds__(256) attn_decode_fused_kernel(const __grid_con
         const bool patch = has_new && pos < t0 + nt;          // the current position is the last row of this tile
         const int n_cached = patch ? nt - 1 : nt;
         if (n_cached > 0) {
-            if (threadIdx.x == 0) {
+            if (threadIdx.x == 0 && t0 > s0) {   // (the first tile was requested above)
                 const uint32_t bytes = (uint32_t)n_cached * kHeadDim * sizeof(kv_t);
                 mbar_expect_tx(&bar, 2 * bytes);
                 bulk_g2s(Ks, kg + (size_t)t0 * kHeadDim, bytes, &bar);
