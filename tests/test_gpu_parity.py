@@ -444,6 +444,21 @@ def test_tiny_batch32(tiny_weights):
     assert stats["positions"] == B * (steps + 1)
 
 
+@pytest.mark.parametrize("B", [8, 9, 16])
+def test_tiny_batch_token_tiles(tiny_weights, B):
+    """Batched decode with <= 8 / <= 16 sequences runs its GEMMs on 8- / 16-row token tiles (a full 8-row tile, a ragged and a
+    full 16-row tile; tiny ffn = 688 keeps the two-accumulator SwiGLU form on 32 rows); every sequence checked, and the K/V
+    rows that the one-launch decode attention appends."""
+    T, steps = 30, 6
+    prompts = datagen.tokens(1010 + B, datagen.TINY.vocab, B * T).reshape(B, T)
+    gm = gpu_model(tiny_weights, max_seq=64, max_batch=B)
+    refs, stats = run_batched(gm, tiny_weights, prompts, steps, 64)
+    for b in (0, B - 1):
+        check_kv_rows(gm, refs[b]["om"], range(T - 2, T + steps), stats, seq=b)
+    print(f"tiny batch-{B} parity:", stats)
+    assert stats["positions"] == B * (steps + 1)
+
+
 def test_1b_config3_batch8(one_b_weights):
     """configs[3] at full size and full length: 8 sequences x 192-token prompts in one tensor-core pass (1,536 rows),
     then all 192 batched decode steps (tcgen05 GEMMs with a 32-token tile); hidden/logits every 16th step, argmax at
