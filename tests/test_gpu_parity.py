@@ -459,6 +459,25 @@ def test_tiny_batch_token_tiles(tiny_weights, B):
     assert stats["positions"] == B * (steps + 1)
 
 
+@pytest.mark.parametrize("n_heads,n_kv_heads", [(4, 4), (8, 1), (6, 2)])
+def test_gqa_group_sizes_batched(n_heads, n_kv_heads):
+    """Group sizes other than the models' (G = 1: plain multi-head attention, one warp per CTA of the decode attention;
+    G = 8: the widest CTA; G = 3): batched prefill + decode against the oracle, every sequence, and the appended K/V rows."""
+    import dataclasses
+    import paper_2606_12154_b200 as hq
+    shape = dataclasses.replace(datagen.TINY, name=f"tiny-h{n_heads}-kv{n_kv_heads}", n_heads=n_heads, n_kv_heads=n_kv_heads)
+    weights = datagen.make_weights(shape, seed=datagen.WEIGHT_SEED + n_heads)
+    B, T, steps = 3, 20, 5
+    prompts = datagen.tokens(1020 + n_heads, shape.vocab, B * T).reshape(B, T)
+    gm = hq.Model.from_bf16_bits(shape, weights.embedding, weights.final_norm, weights.layers, max_seq=64, max_batch=4,
+                                 flags=hq.FLAG_CAPTURE_HIDDEN)
+    refs, stats = run_batched(gm, weights, prompts, steps, 64)
+    for b in range(B):
+        check_kv_rows(gm, refs[b]["om"], range(T - 1, T + steps), stats, seq=b)
+    print(f"GQA {n_heads}/{n_kv_heads} batched parity:", stats)
+    assert stats["positions"] == B * (steps + 1)
+
+
 def test_1b_config3_batch8(one_b_weights):
     """configs[3] at full size and full length: 8 sequences x 192-token prompts in one tensor-core pass (1,536 rows),
     then all 192 batched decode steps (tcgen05 GEMMs with a 32-token tile); hidden/logits every 16th step, argmax at
