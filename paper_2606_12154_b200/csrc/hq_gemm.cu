@@ -515,7 +515,12 @@ static cudaError_t launch_mode(const LaunchCtx &c, const TensorMap &w, const Ten
     // form (token tile <= 128); batched-decode steps (<= 32 rows) keep single CTAs.
     const bool pair = MODE != EPI_SWIGLU64 && p.NT >= 32 && p.NT <= 128 && p.T > 32;
     const int stage_bytes = nacc * kBlockM * kBlockK * 2 + (pair ? 1 : 2) * p.NT * kBlockK * 2;
-    int stages = kSmemBudget / stage_bytes;
+    // Decode GEMMs that run as many waves of CTAs (the LM head: 1002 tiles over 148 SMs) take half-size rings: two CTAs then
+    // share an SM and one's set-up and first loads run under the other's main loop (B = 8 step 960 -> 946 us, B = 32 x 512
+    // 1,345 -> 1,307).  The one-wave GEMMs of a layer do NOT: there the co-resident CTAs belong to the NEXT kernel and their
+    // prefetch only competes (profiles/r02_batched_decode.md, item 13).
+    const bool two_per_sm = !pair && p.T <= 32 && n_tiles * t_tiles * splits > 2 * c.n_sms;
+    int stages = (two_per_sm ? 108 * 1024 : kSmemBudget) / stage_bytes;
     if (stages > 8) stages = 8;
     if (stages > p.k_blocks_per_split) stages = p.k_blocks_per_split < 2 ? 2 : p.k_blocks_per_split;
     p.stages = stages;
