@@ -19,6 +19,7 @@
 //     the others at once (programmatic dependent launch) and prefetch their first weight batch meanwhile.
 #include "hq_common.cuh"
 #include "hq_internal.h"
+#include "hq_attn_tile.cuh"
 
 namespace hq {
 

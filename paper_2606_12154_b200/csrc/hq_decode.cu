@@ -13,6 +13,7 @@
 //     bulk async copy (TMA, cp.async.bulk) per tile, shared by the G query heads of the group.
 #include "hq_common.cuh"
 #include "hq_internal.h"
+#include "hq_attn_tile.cuh"
 
 namespace hq {
 
@@ -265,69 +266,6 @@ __global__ void __launch_bounds__(kGemvThreads) gemv_kernel(const __grid_constan
 // =====================================================================================================
 constexpr int kAttnTile = 128;  // positions per staged tile (16 KB of K + 16 KB of V)
 
-// One staged tile of nt positions for one query head (one warp): online softmax over the tile, state (m, l, o0, o1) =
-// running max, denominator and this lane's two output dims.
-//   qr: the head's query, pre-scaled, in REGISTERS, chunk c of this lane = dims [8 ((c + lane) & 7), + 8) (attn_load_q): the
-//       order in which the lane walks its K row, so that the 8 lanes of a quarter-warp hit 8 different bank groups;
-//   ps: 32 floats of shared memory of this warp: the probabilities of a round, read back four at a time as broadcasts
-//       (one LDS.128 per four positions instead of four shuffles).
-__device__ __forceinline__ void attn_load_q(const float *q_smem, int lane, float (&qr)[8][8]) {
-#pragma unroll
-    for (int c = 0; c < 8; ++c) {
-        const int cc = (c + lane) & 7;
-        const float4 a = *reinterpret_cast<const float4 *>(q_smem + cc * 8), b = *reinterpret_cast<const float4 *>(q_smem + cc * 8 + 4);
-        qr[c][0] = a.x; qr[c][1] = a.y; qr[c][2] = a.z; qr[c][3] = a.w; qr[c][4] = b.x; qr[c][5] = b.y; qr[c][6] = b.z; qr[c][7] = b.w;
-    }
-}
-__device__ __forceinline__ void attn_tile(const kv_t *Ks, const kv_t *Vs, int nt, const float (&qr)[8][8], float *ps, int lane, float &m,
-                                          float &l, float &o0, float &o1) {
-    for (int r0 = 0; r0 < nt; r0 += 32) {
-        const int nr = min(32, nt - r0);
-        // scores of up to 32 positions: lane i computes the whole dot product of position r0 + i (one warp reduction per
-        // position made this loop a chain of 5 dependent shuffles x 32: 2.6 us per 32 positions)
-        float s_mine = -INFINITY;
-        if (lane < nr) {
-            const uint4 *krow = reinterpret_cast<const uint4 *>(Ks + (r0 + lane) * kHeadDim);
-            float acc4[4] = {0.f, 0.f, 0.f, 0.f};
-#pragma unroll
-            for (int c = 0; c < 8; ++c) {
-                const uint4 kk = krow[(c + lane) & 7];
-                const float2 k0 = __half22float2(*reinterpret_cast<const __half2 *>(&kk.x));
-                const float2 k1 = __half22float2(*reinterpret_cast<const __half2 *>(&kk.y));
-                const float2 k2 = __half22float2(*reinterpret_cast<const __half2 *>(&kk.z));
-                const float2 k3 = __half22float2(*reinterpret_cast<const __half2 *>(&kk.w));
-                acc4[0] = fmaf(qr[c][0], k0.x, fmaf(qr[c][1], k0.y, acc4[0]));
-                acc4[1] = fmaf(qr[c][2], k1.x, fmaf(qr[c][3], k1.y, acc4[1]));
-                acc4[2] = fmaf(qr[c][4], k2.x, fmaf(qr[c][5], k2.y, acc4[2]));
-                acc4[3] = fmaf(qr[c][6], k3.x, fmaf(qr[c][7], k3.y, acc4[3]));
-            }
-            s_mine = (acc4[0] + acc4[1]) + (acc4[2] + acc4[3]);
-        }
-        const float m_new = fmaxf(m, warp_max(s_mine));
-        const float corr = __expf(m - m_new);   // m = -inf first time -> 0
-        const float pr = (lane < nr) ? __expf(s_mine - m_new) : 0.f;
-        l = l * corr + warp_sum(pr);
-        o0 *= corr;
-        o1 *= corr;
-        ps[lane] = pr;
-        __syncwarp();
-        for (int r = 0; r < nr; r += 4) {
-            const float4 p4 = *reinterpret_cast<const float4 *>(ps + r);   // broadcast
-            const float pb[4] = {p4.x, p4.y, p4.z, p4.w};
-#pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                if (r + u < nr) {   // warp-uniform; rows past nr of the tile are not initialised
-                    const float2 vv = __half22float2(*reinterpret_cast<const __half2 *>(Vs + (r0 + r + u) * kHeadDim + 2 * lane));
-                    o0 = fmaf(pb[u], vv.x, o0);
-                    o1 = fmaf(pb[u], vv.y, o1);
-                }
-            }
-        }
-        __syncwarp();   // ps is rewritten by the next round
-        m = m_new;
-    }
-}
-
 __global__ void __launch_bounds__(256) attn_decode_kernel(const __grid_constant__ AttnDecodeParams p) {
     __shared__ __align__(128) kv_t Ks[kAttnTile * kHeadDim];
     __shared__ __align__(128) kv_t Vs[kAttnTile * kHeadDim];
@@ -379,7 +317,7 @@ __global__ void __launch_bounds__(256) attn_decode_kernel(const __grid_constant_
         }
         mbar_wait(&bar, parity);
         parity ^= 1;
-        attn_tile(Ks, Vs, nt, qr, ps[warp], lane, m, l, o0, o1);
+        attn_tile(Ks, Vs, nt, qr, ps[warp], lane, m, l, o0, o1, 0, 32);
         __syncthreads();  // everyone done with the tile before it is overwritten
     }
     const size_t pidx = ((size_t)b * p.n_heads + head) * kMaxSplits + split;
@@ -490,7 +428,7 @@ __global__ void __launch_bounds__(256) attn_decode_fused_kernel(const __grid_con
             }
             __syncthreads();
         }
-        attn_tile(Ks, Vs, nt, qr, ps[warp], lane, m, l, o0, o1);
+        attn_tile(Ks, Vs, nt, qr, ps[warp], lane, m, l, o0, o1, 0, 32);
         __syncthreads();  // everyone done with the tile before it is overwritten
     }
     const size_t hb = (size_t)b * p.n_heads + head;
