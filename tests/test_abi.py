@@ -83,6 +83,14 @@ def test_workspace_bytes_is_host_arithmetic(hq):
     assert b"non-positive" in hq.load_library().hq_last_error()
 
 
+def test_noalloc_scratch_size_is_the_header_constant(hq):
+    """include/hq_noalloc.h states the size of the static scratch array; the library reports the same (host arithmetic)."""
+    src = open(os.path.join(ROOT, "include", "hq_noalloc.h")).read()
+    m = re.search(r"#define\s+HQ_NOALLOC_SCRATCH_BYTES\s+\((\d+)u\s*<<\s*(\d+)\)", src)
+    assert m, "HQ_NOALLOC_SCRATCH_BYTES not found"
+    assert hq.noalloc_scratch_bytes() == int(m.group(1)) << int(m.group(2)) == 16 << 20
+
+
 def test_create_rejects_bad_arguments_before_touching_cuda(hq):
     from paper_2606_12154_b200.binding import Weights, make_config
     lib = hq.load_library()
